@@ -1,0 +1,186 @@
+/* gm.h -- C ABI of libgm: the batched galaxy-profile chi^2 + gradient + update
+ * hot path of arxiv 2404.07780 (Galmoss) on NVIDIA B200 (sm_100a).
+ *
+ * Citations "P:<line>" are lines of the paper text; "R:<id>" are the
+ * readings of silent / garbled passages listed in DESIGN.md.
+ *
+ * What the library computes, per galaxy (Fig. 1):
+ *   S   = sum of the PSF-convolved components, evaluated at pixel centres
+ *         x = j + 0.5, y = H - 0.5 - i (R:G1) from the elliptical
+ *         radius of Eq. 2-4 (R:G2) and the radial laws Eq. 1, 7, 9, 11,
+ *         12, 13;
+ *   M   = PSF (*) S + unconvolved components + sky (Eq. 16), true convolution,
+ *         PSF centre (K-1)/2, zero fill outside the cutout, same size (R:C1);
+ *   chi2 = sum_ij Omega_ij (D_ij - M_ij)^2 / sigma_ij^2            (Eq. 18);
+ *   grad = d chi2 / d p for every entry of the parameter vector (the paper uses
+ *         autograd; here the analytic adjoint: flipped-PSF correlation
+ *         of G = -2 w (D - M), then a reduction against dS/dp);
+ *   fit  = n_iter steps of Adam on u = p or log10 p with projection onto the
+ *         parameter ranges (R:O1-O5).
+ *
+ * Conventions
+ *   - Pointers marked "dev" are DEVICE pointers owned by the caller (e.g. torch
+ *     allocations); pointers marked "host" are host pointers.  The library never
+ *     frees or keeps a caller pointer past the call.
+ *   - All images are row-major, [B,H,W] contiguous, float32; row 0 is the TOP row
+ *     (largest y).  Angles are radians, lengths pixels, amplitudes intensities.
+ *   - Device entry points are asynchronous on `cuda_stream` (a cudaStream_t; NULL =
+ *     the legacy default stream), allocate nothing, and never synchronise.  Scratch
+ *     comes from the caller: `workspace` (dev, 256-byte aligned) of at least
+ *     gm_workspace_bytes(model, batch) bytes.
+ *   - Return value: GM_OK or a negative gm_status; nothing is launched when the
+ *     arguments fail validation.  There is no CPU fallback: without a CUDA device
+ *     every compute entry point returns GM_ECUDA.
+ */
+#ifndef GM_H_
+#define GM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GM_VERSION   100     /* major*10000 + minor*100 + patch */
+#define GM_MAX_COMP  8       /* components per model                               */
+#define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
+#define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
+
+typedef enum {
+  GM_OK = 0,
+  GM_EINVAL = -1,    /* NULL pointer, even / oversize K, P or C over the maximum,
+                        slot index out of range, non-positive size               */
+  GM_ENOTSUP = -2,   /* valid request that this build has no kernel for          */
+  GM_ECUDA = -3,     /* CUDA launch / runtime error (see gm_last_cuda_error)      */
+  GM_EWORKSPACE = -4 /* workspace NULL, misaligned or too small                   */
+} gm_status;
+
+/* radial laws: Sec. 4.1, 4.2.1 - 4.2.6 */
+typedef enum {
+  GM_SERSIC = 0, GM_EXPDISK = 1, GM_FERRER = 2, GM_KING = 3,
+  GM_GAUSSIAN = 4, GM_MOFFAT = 5, GM_SKY = 6
+} gm_kind;
+
+/* index of each quantity inside gm_component.slot[] */
+enum { GM_SLOT_XC = 0, GM_SLOT_YC, GM_SLOT_THETA, GM_SLOT_Q, GM_SLOT_AMP,
+       GM_SLOT_S0, GM_SLOT_S1, GM_SLOT_S2, GM_SLOT_BOX, GM_NSLOT };
+
+/* One summed component (host memory, POD).  slot[k] is the index, inside the
+ * galaxy's parameter vector, of the k-th quantity, or -1 when unused:
+ *   Sersic   amp=Ie  s0=re    s1=n            Eq. 1
+ *   ExpDisk  amp=I0  s0=rs                    Eq. 7
+ *   Ferrer   amp=I0  s0=r_out s1=a   s2=b     Eq. 9   (0 for r >= r_out)
+ *   King     amp=I0  s0=rc    s1=rt  s2=alpha Eq. 11  (0 for r >= rt, R:K1)
+ *   Gaussian amp=I0  s0=FWHM                  Eq. 12  (FWHM = 2 sqrt(2 ln 2) sigma, R:F1)
+ *   Moffat   amp=I0  s0=FWHM  s1=n            Eq. 13-14
+ *   Sky      amp=I_sky                        Eq. 16  (never convolved)
+ * Unused q means 1 (circular), unused theta means 0, unused box means B = 0.
+ * Two components naming the same index are TIED: their gradients add.
+ * convolve = 1: the component goes through the PSF; 0: added after it.
+ * A boxiness slot (Eq. 2 with B != 0) is accepted by the ABI; kernels for it
+ * are not built yet and the call returns GM_ENOTSUP. */
+typedef struct {
+  int32_t kind;
+  int32_t convolve;
+  int32_t slot[GM_NSLOT];
+} gm_component;
+
+typedef struct {
+  int32_t n_comp;              /* 1..GM_MAX_COMP                                  */
+  int32_t n_par;               /* P, 1..GM_MAX_PAR                                */
+  const gm_component* comp;    /* host [n_comp]                                   */
+} gm_model;
+
+/* One batch of equally sized cutouts.  Mixed sizes = one gm_batch
+ * per size, called one after the other (or on different streams). */
+typedef struct {
+  int32_t B, H, W, K;          /* K odd, 1..GM_MAX_K                               */
+  const float*   data;         /* dev [B,H,W]  D_ij          (NULL for gm_render)  */
+  const float*   sigma;        /* dev [B,H,W]  sigma_ij > 0 wherever mask != 0     */
+  const uint8_t* mask;         /* dev [B,H,W]  Omega: 1 used, 0 ignored (R:X1);
+                                  NULL = every pixel used                          */
+  const float*   psf;          /* dev [B,K,K] or [K,K]; used as given (R:C1)       */
+  int64_t        psf_stride;   /* elements between galaxies; 0 = one shared PSF    */
+} gm_batch;
+
+/* Update rule (R:O1-O5).  For every free parameter k, per galaxy, t = 1..n_iter:
+ *   u = p or log10 p;  g = dchi2/dp * dp/du
+ *   m <- beta1 m + (1-beta1) g ;  s <- beta2 s + (1-beta2) g^2
+ *   u <- u - lr[k] lr_decay^(t-1) [m/(1-beta1^t)] / (sqrt(s/(1-beta2^t)) + eps)
+ *   u <- min(max(u, T(lo[k])), T(hi[k]))                         (projection)
+ * A galaxy stops early once |chi2_t - chi2_(t-1)| <= tol chi2_t held for `patience`
+ * consecutive iterations (tol <= 0: never).  All arrays are HOST arrays of n_par. */
+typedef struct {
+  int32_t n_iter;
+  float   beta1, beta2, eps;
+  float   lr_decay;
+  const float*   lr;
+  const float*   lo;
+  const float*   hi;           /* +-INFINITY allowed                               */
+  const uint8_t* log10_space;  /* 1: optimise u = log10 p; NULL = all 0    */
+  const uint8_t* free_mask;    /* 0: parameter held fixed;    NULL = all free      */
+  float   tol;
+  int32_t patience;
+} gm_fit_opts;
+
+/* per-galaxy status written by gm_fit */
+enum { GM_FIT_OK = 0, GM_FIT_CONVERGED = 1, GM_FIT_NONFINITE = 2 };
+
+/* ---- device entry points (asynchronous) ---------------------------------- */
+
+/* Bytes of device scratch gm_render / gm_loss_grad / gm_fit need for this model
+ * and batch shape (only B, H, W, K and the model are read).  0 on invalid input. */
+size_t gm_workspace_bytes(const gm_model* model, const gm_batch* batch);
+
+/* Render the model image M (App. C "initial_model").
+ * params: dev [B,P].  model_out: dev [B,H,W].  batch->data/sigma/mask ignored. */
+int gm_render(const gm_model* model, const gm_batch* batch, const float* params,
+              float* model_out, void* workspace, size_t workspace_bytes,
+              void* cuda_stream);
+
+/* chi^2 (Eq. 18) and its gradient with respect to the PHYSICAL parameters.
+ * chi2: dev [B].  grad: dev [B,P] (NULL = not wanted).
+ * jtj: dev [B,P,P], jtr: dev [B,P] = J^T W J and J^T W (D-M), or NULL;
+ * requesting them returns GM_ENOTSUP until the covariance row is built. */
+int gm_loss_grad(const gm_model* model, const gm_batch* batch, const float* params,
+                 float* chi2, float* grad, float* jtj, float* jtr,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Fixed-iteration batched fit.  params: dev [B,P], in/out.
+ * chi2_out: dev [B], chi^2 AT the returned parameters.  iters_used: dev [B] number
+ * of updates applied, or NULL.  status: dev [B] GM_FIT_*, or NULL.
+ * A galaxy whose chi^2 turns non-finite gets GM_FIT_NONFINITE and keeps the last
+ * parameters that had a finite chi^2. */
+int gm_fit(const gm_model* model, const gm_batch* batch, float* params,
+           const gm_fit_opts* opts, float* chi2_out, int32_t* iters_used,
+           int32_t* status, void* workspace, size_t workspace_bytes,
+           void* cuda_stream);
+
+/* ---- host-buffer entry points (synchronous, end to end) -------------------- */
+/* Same operations with every pointer of `batch` and every array argument in HOST
+ * memory (pinned memory makes the copies faster, pageable works).  The call
+ * allocates device memory, copies the inputs in, runs the device entry point,
+ * copies the results out, frees, and returns after the device is idle. */
+int gm_render_host(const gm_model* model, const gm_batch* host_batch,
+                   const float* params, float* model_out);
+int gm_loss_grad_host(const gm_model* model, const gm_batch* host_batch,
+                      const float* params, float* chi2, float* grad);
+int gm_fit_host(const gm_model* model, const gm_batch* host_batch, float* params,
+                const gm_fit_opts* opts, float* chi2_out, int32_t* iters_used,
+                int32_t* status);
+
+/* ---- misc ------------------------------------------------------------------ */
+const char* gm_strerror(int status);
+int         gm_version(void);
+/* cudaError_t of the most recent GM_ECUDA on this thread (0 = none) and its text */
+int         gm_last_cuda_error(void);
+const char* gm_last_cuda_error_string(void);
+/* number of kernels launched by this thread's last device entry point; lets a
+ * caller (bench.py "gpu_launches") count launches without a profiler */
+int64_t     gm_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GM_H_ */

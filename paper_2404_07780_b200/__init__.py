@@ -1,0 +1,20 @@
+"""B200-native batched galaxy-profile fitting hot path (arxiv 2404.07780).
+
+Thin Python binding over the C-ABI library ``libgm.so`` (``include/gm.h``):
+argument marshalling only -- every step of the path runs in the CUDA kernels
+under ``csrc/``.  PyTorch supplies device memory and streams.
+"""
+from .binding import (  # noqa: F401
+    GmError,
+    gm_fit,
+    gm_fit_host,
+    gm_last_launch_count,
+    gm_loss_grad,
+    gm_loss_grad_host,
+    gm_render,
+    gm_render_host,
+    gm_strerror,
+    gm_version,
+    gm_workspace_bytes,
+    library_path,
+)

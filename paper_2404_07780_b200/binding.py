@@ -1,0 +1,290 @@
+"""ctypes binding of libgm.so: same names as the C entry points of include/gm.h.
+
+Only marshals arguments (torch tensors -> device pointers, dict model ->
+gm_component array).  There is NO fallback: a missing library, a missing CUDA
+device or a non-zero status raises.
+
+A model is plain data (see gen.models / include/gm.h gm_component):
+``{"n_par": P, "components": [{"kind": "sersic", "convolve": 1,
+"slots": {"xc": 0, "yc": 1, "amp": 2, "s0": 3, "s1": 4, "q": 5, "theta": 6}}]}``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+import torch
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libgm.so"
+
+GM_MAX_COMP, GM_MAX_PAR, GM_MAX_K, GM_NSLOT = 8, 32, 41, 9
+_KINDS = {"sersic": 0, "expdisk": 1, "ferrer": 2, "king": 3, "gaussian": 4, "moffat": 5, "sky": 6}
+_SLOTS = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box")
+
+
+class GmError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = _lib().gm_strerror(status).decode()
+        if status == -3:
+            msg += ": " + _lib().gm_last_cuda_error_string().decode()
+        super().__init__(f"{where} failed with status {status} ({msg})")
+
+
+class _Component(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("convolve", C.c_int32), ("slot", C.c_int32 * GM_NSLOT)]
+
+
+class _Model(C.Structure):
+    _fields_ = [("n_comp", C.c_int32), ("n_par", C.c_int32), ("comp", C.POINTER(_Component))]
+
+
+class _Batch(C.Structure):
+    _fields_ = [("B", C.c_int32), ("H", C.c_int32), ("W", C.c_int32), ("K", C.c_int32),
+                ("data", C.c_void_p), ("sigma", C.c_void_p), ("mask", C.c_void_p),
+                ("psf", C.c_void_p), ("psf_stride", C.c_int64)]
+
+
+class _FitOpts(C.Structure):
+    _fields_ = [("n_iter", C.c_int32), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
+                ("lr_decay", C.c_float), ("lr", C.c_void_p), ("lo", C.c_void_p), ("hi", C.c_void_p),
+                ("log10_space", C.c_void_p), ("free_mask", C.c_void_p), ("tol", C.c_float),
+                ("patience", C.c_int32)]
+
+
+_handle = None
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+def _lib():
+    global _handle
+    if _handle is None:
+        if not _LIB_PATH.exists():
+            raise ImportError(
+                f"{_LIB_PATH} is missing: build the CUDA extension first "
+                "(python -m paper_2404_07780_b200.build, or __graft_entry__.build()); "
+                "there is no CPU fallback")
+        L = C.CDLL(str(_LIB_PATH))
+        vp, sz, i = C.c_void_p, C.c_size_t, C.c_int
+        mp, bp, op = C.POINTER(_Model), C.POINTER(_Batch), C.POINTER(_FitOpts)
+        L.gm_workspace_bytes.restype = sz; L.gm_workspace_bytes.argtypes = [mp, bp]
+        L.gm_render.restype = i; L.gm_render.argtypes = [mp, bp, vp, vp, vp, sz, vp]
+        L.gm_loss_grad.restype = i; L.gm_loss_grad.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.gm_fit.restype = i; L.gm_fit.argtypes = [mp, bp, vp, op, vp, vp, vp, vp, sz, vp]
+        L.gm_render_host.restype = i; L.gm_render_host.argtypes = [mp, bp, vp, vp]
+        L.gm_loss_grad_host.restype = i; L.gm_loss_grad_host.argtypes = [mp, bp, vp, vp, vp]
+        L.gm_fit_host.restype = i; L.gm_fit_host.argtypes = [mp, bp, vp, op, vp, vp, vp]
+        L.gm_strerror.restype = C.c_char_p; L.gm_strerror.argtypes = [i]
+        L.gm_version.restype = i; L.gm_version.argtypes = []
+        L.gm_last_cuda_error.restype = i; L.gm_last_cuda_error.argtypes = []
+        L.gm_last_cuda_error_string.restype = C.c_char_p; L.gm_last_cuda_error_string.argtypes = []
+        L.gm_last_launch_count.restype = C.c_int64; L.gm_last_launch_count.argtypes = []
+        _handle = L
+    return _handle
+
+
+# ---- marshalling ---------------------------------------------------------------
+def _model_struct(model: dict):
+    comps = model["components"]
+    arr = (_Component * len(comps))()
+    for c, comp in enumerate(comps):
+        arr[c].kind = _KINDS[comp["kind"]]
+        arr[c].convolve = int(comp.get("convolve", 1))
+        for k in range(GM_NSLOT):
+            arr[c].slot[k] = -1
+        for name, idx in comp["slots"].items():
+            arr[c].slot[_SLOTS.index(name)] = int(idx)
+    m = _Model(len(comps), int(model["n_par"]), arr)
+    m._keep = arr
+    return m
+
+
+def _dev(t, dtype, name):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}")
+    return t.data_ptr()
+
+
+def _batch_struct(B, H, W, psf, data=None, sigma=None, mask=None, host=False):
+    if host:
+        ptr = lambda a: None if a is None else a.ctypes.data
+        K = psf.shape[-1]
+        shared = psf.ndim == 2
+        return _Batch(B, H, W, K, ptr(data), ptr(sigma), ptr(mask), ptr(psf), 0 if shared else K * K)
+    K = psf.shape[-1]
+    if psf.ndim == 2:
+        stride = 0
+    else:
+        if psf.shape[0] != B:
+            raise ValueError("per-galaxy psf must be [B,K,K]")
+        stride = K * K
+    return _Batch(B, H, W, K, _dev(data, torch.float32, "data"), _dev(sigma, torch.float32, "sigma"),
+                  _dev(mask, torch.uint8, "mask"), _dev(psf, torch.float32, "psf"), stride)
+
+
+def _stream_ptr(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _workspace(m, b, workspace):
+    need = _lib().gm_workspace_bytes(C.byref(m), C.byref(b))
+    if need == 0:
+        raise GmError(-1, "gm_workspace_bytes")
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+    off = (-workspace.data_ptr()) % 256
+    return workspace, workspace.data_ptr() + off, workspace.numel() - off
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise GmError(rc, where)
+
+
+def _opts_struct(opts: dict, P: int):
+    lr = np.ascontiguousarray(opts["lr"], dtype=np.float32)
+    lo = np.ascontiguousarray(opts["lo"], dtype=np.float32)
+    hi = np.ascontiguousarray(opts["hi"], dtype=np.float32)
+    lg = np.ascontiguousarray(opts.get("log10_space", np.zeros(P)), dtype=np.uint8)
+    fm = np.ascontiguousarray(opts.get("free_mask", np.ones(P)), dtype=np.uint8)
+    for a in (lr, lo, hi, lg, fm):
+        if a.shape != (P,):
+            raise ValueError("fit option arrays must have n_par entries")
+    o = _FitOpts(int(opts["n_iter"]), float(opts.get("beta1", 0.9)), float(opts.get("beta2", 0.999)),
+                 float(opts.get("eps", 1e-8)), float(opts.get("lr_decay", 1.0)), lr.ctypes.data,
+                 lo.ctypes.data, hi.ctypes.data, lg.ctypes.data, fm.ctypes.data,
+                 float(opts.get("tol", 0.0)), int(opts.get("patience", 10)))
+    o._keep = (lr, lo, hi, lg, fm)
+    return o
+
+
+# ---- entry points (same names as include/gm.h) ---------------------------------
+def gm_version() -> int:
+    return _lib().gm_version()
+
+
+def gm_strerror(status: int) -> str:
+    return _lib().gm_strerror(int(status)).decode()
+
+
+def gm_last_launch_count() -> int:
+    return int(_lib().gm_last_launch_count())
+
+
+def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) -> int:
+    m = _model_struct(model)
+    b = _Batch(B, H, W, K, None, None, None, None, 0)
+    return int(_lib().gm_workspace_bytes(C.byref(m), C.byref(b)))
+
+
+def gm_render(model, params, H, W, psf, out=None, workspace=None, stream=None):
+    """M[B,H,W] for params[B,P].  Asynchronous on the stream."""
+    B = params.shape[0]
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf)
+    if out is None:
+        out = torch.empty((B, H, W), dtype=torch.float32, device=params.device)
+    ws, wp, wn = _workspace(m, b, workspace)
+    rc = _lib().gm_render(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"),
+                          _dev(out, torch.float32, "out"), wp, wn, _stream_ptr(stream))
+    _check(rc, "gm_render")
+    out._gm_ws = ws
+    return out
+
+
+def gm_loss_grad(model, params, data, sigma, mask, psf, want_grad=True, chi2=None, grad=None,
+                 workspace=None, stream=None):
+    """chi^2[B] (Eq. 18) and d chi^2 / d p [B,P].  Asynchronous on the stream."""
+    B, P = params.shape
+    _, H, W = data.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, data, sigma, mask)
+    if chi2 is None:
+        chi2 = torch.empty(B, dtype=torch.float32, device=params.device)
+    if want_grad and grad is None:
+        grad = torch.empty((B, P), dtype=torch.float32, device=params.device)
+    ws, wp, wn = _workspace(m, b, workspace)
+    rc = _lib().gm_loss_grad(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"),
+                             _dev(chi2, torch.float32, "chi2"),
+                             _dev(grad, torch.float32, "grad") if want_grad else None,
+                             None, None, wp, wn, _stream_ptr(stream))
+    _check(rc, "gm_loss_grad")
+    chi2._gm_ws = ws
+    return (chi2, grad) if want_grad else chi2
+
+
+def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=None):
+    """Batched fixed-iteration fit; params[B,P] is updated IN PLACE.  Asynchronous."""
+    B, P = params.shape
+    _, H, W = data.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, data, sigma, mask)
+    o = _opts_struct(opts, P)
+    chi2 = torch.empty(B, dtype=torch.float32, device=params.device)
+    iters = torch.empty(B, dtype=torch.int32, device=params.device)
+    status = torch.empty(B, dtype=torch.int32, device=params.device)
+    ws, wp, wn = _workspace(m, b, workspace)
+    rc = _lib().gm_fit(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"), C.byref(o),
+                       chi2.data_ptr(), iters.data_ptr(), status.data_ptr(), wp, wn, _stream_ptr(stream))
+    _check(rc, "gm_fit")
+    return {"params": params, "chi2": chi2, "iters_used": iters, "status": status, "_ws": ws}
+
+
+# ---- host-buffer entry points (numpy in, numpy out; copies inside the call) ------
+def _np(a, dtype, name):
+    if a is None:
+        return None
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous:
+        raise TypeError(f"{name} must be a C-contiguous numpy array of {dtype}")
+    return a
+
+
+def gm_render_host(model, params, H, W, psf):
+    params = _np(params, np.float32, "params"); psf = _np(psf, np.float32, "psf")
+    B = params.shape[0]
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, host=True)
+    out = np.empty((B, H, W), dtype=np.float32)
+    _check(_lib().gm_render_host(C.byref(m), C.byref(b), params.ctypes.data, out.ctypes.data), "gm_render_host")
+    return out
+
+
+def gm_loss_grad_host(model, params, data, sigma, mask, psf):
+    params = _np(params, np.float32, "params"); psf = _np(psf, np.float32, "psf")
+    data = _np(data, np.float32, "data"); sigma = _np(sigma, np.float32, "sigma")
+    mask = _np(mask, np.uint8, "mask")
+    B, P = params.shape
+    _, H, W = data.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, data, sigma, mask, host=True)
+    chi2 = np.empty(B, dtype=np.float32); grad = np.empty((B, P), dtype=np.float32)
+    _check(_lib().gm_loss_grad_host(C.byref(m), C.byref(b), params.ctypes.data, chi2.ctypes.data,
+                                    grad.ctypes.data), "gm_loss_grad_host")
+    return chi2, grad
+
+
+def gm_fit_host(model, params, data, sigma, mask, psf, opts):
+    """params (numpy [B,P]) is updated in place; returns dict of numpy arrays."""
+    params = _np(params, np.float32, "params"); psf = _np(psf, np.float32, "psf")
+    data = _np(data, np.float32, "data"); sigma = _np(sigma, np.float32, "sigma")
+    mask = _np(mask, np.uint8, "mask")
+    B, P = params.shape
+    _, H, W = data.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, data, sigma, mask, host=True)
+    o = _opts_struct(opts, P)
+    chi2 = np.empty(B, dtype=np.float32)
+    iters = np.empty(B, dtype=np.int32); status = np.empty(B, dtype=np.int32)
+    _check(_lib().gm_fit_host(C.byref(m), C.byref(b), params.ctypes.data, C.byref(o), chi2.ctypes.data,
+                              iters.ctypes.data, status.ctypes.data), "gm_fit_host")
+    return {"params": params, "chi2": chi2, "iters_used": iters, "status": status}

@@ -1,0 +1,657 @@
+// gm_api.cu -- C ABI of libgm (include/gm.h): validation, workspace carving,
+// launch sequences for gm_render / gm_loss_grad / gm_fit, the per-galaxy prologue
+// (a0), gradient assembly and Adam update (a5 tail, a6), and the host-buffer
+// end-to-end variants.  No CPU fallback: every compute entry point needs a CUDA
+// device and returns GM_ECUDA without one.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <mutex>
+
+#include "gm_kernels.cuh"
+
+namespace gm {
+
+static thread_local cudaError_t t_last_err = cudaSuccess;
+static thread_local int64_t t_launches = 0;
+
+#define GM_CUDA(expr)                                         \
+  do {                                                        \
+    cudaError_t e__ = (expr);                                 \
+    if (e__ != cudaSuccess) { t_last_err = e__; return GM_ECUDA; } \
+  } while (0)
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------
+// small kernels: PSF padding, prologue, gradient assembly, fit state
+// ---------------------------------------------------------------------------
+__global__ void k_pad_psf(const float* __restrict__ psf, long long stride, int n_psf, int K, int KP,
+                          float* __restrict__ out) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int per = KP * KP;
+  if (idx >= n_psf * per) return;
+  const int p = idx / per, r = idx - p * per;
+  const int a = r / KP, b = r - a * KP;
+  const int off = (KP - K) / 2;
+  const int aa = a - off, bb = b - off;
+  float v = 0.0f;
+  if (aa >= 0 && aa < K && bb >= 0 && bb < K) v = psf[(long long)p * stride + aa * K + bb];
+  out[idx] = v;
+}
+
+__global__ void k_prologue(const ModelDesc md, int B, const float* __restrict__ params,
+                           CompConst* __restrict__ cc, const int* __restrict__ frozen) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= B * md.n_comp) return;
+  const int b = idx / md.n_comp, c = idx - b * md.n_comp;
+  if (frozen && frozen[b]) return;
+  make_comp_const(md, c, params + (size_t)b * md.n_par, cc + idx);
+}
+
+struct FitOptsDev {
+  float lr[GM_MAX_PAR], ulo[GM_MAX_PAR], uhi[GM_MAX_PAR];
+  uint8_t lg[GM_MAX_PAR], fr[GM_MAX_PAR];
+  float beta1, beta2, eps, tol;
+  int patience;
+};
+
+struct FitState {
+  float *u, *m, *s, *p_prev, *chi2_prev;
+  int *calm, *frozen;
+};
+
+struct FinArgs {
+  ModelDesc md;
+  int B, tiles;
+  const CompConst* cc;
+  const float* chi2_part;
+  const float* grad_part;
+  float* chi2;      // [B] out (loss_grad) / chi2_out (fit)
+  float* grad;      // [B,P] out or nullptr
+};
+
+// chi2 and d chi2 / d p of galaxy b from the per-tile partials; one warp per galaxy.
+// Returns chi2 to every lane; lane k < P gets grad_k in *gk.
+__device__ __forceinline__ float assemble(const FinArgs& a, int b, int lane, float* sh /*[n_comp*8]*/,
+                                          float* gk) {
+  float c2 = 0.0f;
+  for (int t = lane; t < a.tiles; t += 32) c2 += a.chi2_part[(size_t)b * a.tiles + t];
+  c2 = warp_sum(c2);
+  const int nsum = a.md.n_comp * kNSum;
+  if (a.grad_part) {
+    for (int idx = lane; idx < nsum; idx += 32) {
+      float s = 0.0f;
+      for (int t = 0; t < a.tiles; ++t) s += a.grad_part[((size_t)b * a.tiles + t) * nsum + idx];
+      sh[idx] = s;
+    }
+  }
+  __syncwarp();
+  float g = 0.0f;
+  if (a.grad_part && lane < a.md.n_par) {
+    for (int c = 0; c < a.md.n_comp; ++c) {
+      const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
+      const float* s = sh + c * kNSum;
+#pragma unroll
+      for (int k = 0; k < GM_NSLOT; ++k) {
+        if (a.md.slot[c][k] != lane) continue;
+        float v = 0.0f;
+        switch (k) {
+          case GM_SLOT_XC: v = -cc.ct * s[0] + cc.st * cc.iq * s[1]; break;
+          case GM_SLOT_YC: v = -cc.st * s[0] - cc.ct * cc.iq * s[1]; break;
+          case GM_SLOT_THETA: v = (cc.q - cc.iq) * s[2]; break;
+          case GM_SLOT_Q: v = -cc.iq * s[3]; break;
+          case GM_SLOT_AMP: v = s[4]; break;
+          case GM_SLOT_S0: v = s[5]; break;
+          case GM_SLOT_S1: v = s[6]; break;
+          case GM_SLOT_S2: v = s[7]; break;
+          default: break;
+        }
+        g += v;
+      }
+    }
+  }
+  __syncwarp();
+  *gk = g;
+  return c2;
+}
+
+constexpr int kFinWarps = 4;
+
+__global__ void __launch_bounds__(kFinWarps * 32) k_finalize(const FinArgs a) {
+  __shared__ float sh[kFinWarps][GM_MAX_COMP * kNSum];
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int b = blockIdx.x * kFinWarps + wid;
+  if (b >= a.B) return;
+  float g;
+  const float c2 = assemble(a, b, lane, sh[wid], &g);
+  if (lane == 0) a.chi2[b] = c2;
+  if (a.grad && lane < a.md.n_par) a.grad[(size_t)b * a.md.n_par + lane] = g;
+}
+
+__global__ void k_fit_init(int B, int P, const float* __restrict__ params, FitOptsDev o, FitState st,
+                           int* iters, int* status) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= B * P) return;
+  const int k = idx % P;
+  const float p = params[idx];
+  st.u[idx] = o.lg[k] ? log10f(p) : p;
+  st.m[idx] = 0.0f;
+  st.s[idx] = 0.0f;
+  st.p_prev[idx] = p;
+  if (k == 0) {
+    const int b = idx / P;
+    st.calm[b] = 0; st.frozen[b] = 0; st.chi2_prev[b] = 0.0f;
+    if (iters) iters[b] = 0;
+    if (status) status[b] = GM_FIT_OK;
+  }
+}
+
+// a6: one warp per galaxy, lane k = parameter k.  t = 1..n_iter are update steps,
+// t = n_iter + 1 is the closing evaluation (last != 0, no update).
+__global__ void __launch_bounds__(kFinWarps * 32)
+k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* __restrict__ params, int t, int last,
+           float c1 /*1-b1^t*/, float c2 /*1-b2^t*/, float dec /*decay^(t-1)*/, int* iters, int* status) {
+  __shared__ float sh[kFinWarps][GM_MAX_COMP * kNSum];
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int b = blockIdx.x * kFinWarps + wid;
+  if (b >= a.B) return;
+  if (st.frozen[b]) return;
+  const int P = a.md.n_par;
+  float g;
+  const float chi2 = assemble(a, b, lane, sh[wid], &g);
+  const size_t pk = (size_t)b * P + lane;
+  const bool mine = lane < P;
+  if (!isfinite(chi2)) {                                   // GM_FIT_NONFINITE
+    if (t > 1 && mine) params[pk] = st.p_prev[pk];
+    if (lane == 0) {
+      a.chi2[b] = (t > 1) ? st.chi2_prev[b] : chi2;
+      st.frozen[b] = 1;
+      if (status) status[b] = GM_FIT_NONFINITE;
+      if (iters) iters[b] = t > 1 ? t - 1 : 0;
+    }
+    return;
+  }
+  if (last) {
+    if (lane == 0) a.chi2[b] = chi2;
+    return;
+  }
+  if (o.tol > 0.0f && t > 1) {
+    int calm = st.calm[b];
+    calm = (fabsf(chi2 - st.chi2_prev[b]) <= o.tol * chi2) ? calm + 1 : 0;
+    __syncwarp();
+    if (lane == 0) st.calm[b] = calm;
+    if (calm >= o.patience) {                              // GM_FIT_CONVERGED
+      if (lane == 0) {
+        a.chi2[b] = chi2;
+        st.frozen[b] = 1;
+        if (status) status[b] = GM_FIT_CONVERGED;
+        if (iters) iters[b] = t - 1;
+      }
+      return;
+    }
+  }
+  if (lane == 0) {
+    st.chi2_prev[b] = chi2;
+    if (iters) iters[b] = t;
+  }
+  if (mine) {
+    const float p = params[pk];
+    st.p_prev[pk] = p;
+    if (o.fr[lane]) {
+      const float gu = o.lg[lane] ? g * p * 2.302585092994046f : g;
+      const float m = o.beta1 * st.m[pk] + (1.0f - o.beta1) * gu;
+      const float s = o.beta2 * st.s[pk] + (1.0f - o.beta2) * gu * gu;
+      st.m[pk] = m;
+      st.s[pk] = s;
+      float u = st.u[pk] - o.lr[lane] * dec * (m / c1) / (sqrtf(s / c2) + o.eps);
+      u = fminf(fmaxf(u, o.ulo[lane]), o.uhi[lane]);
+      st.u[pk] = u;
+      params[pk] = o.lg[lane] ? exp10f(u) : u;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------
+static const int kCompiledK[] = {5, 9, 15, 21, 25, 33, 41};
+
+static int padded_K(int K) {
+  for (int kp : kCompiledK)
+    if (K <= kp) return kp;
+  return -1;
+}
+
+static int validate(const gm_model* m, const gm_batch* bt, bool need_data, ModelDesc* md) {
+  if (!m || !bt || !m->comp) return GM_EINVAL;
+  if (m->n_comp < 1 || m->n_comp > GM_MAX_COMP || m->n_par < 1 || m->n_par > GM_MAX_PAR) return GM_EINVAL;
+  if (bt->B < 1 || bt->H < 1 || bt->W < 1) return GM_EINVAL;
+  if (bt->K < 1 || bt->K > GM_MAX_K || (bt->K & 1) == 0) return GM_EINVAL;
+  if (!bt->psf || bt->psf_stride < 0) return GM_EINVAL;
+  if (need_data && (!bt->data || !bt->sigma)) return GM_EINVAL;
+  if ((long long)bt->B * m->n_comp > (1ll << 30)) return GM_EINVAL;
+  md->n_comp = m->n_comp;
+  md->n_par = m->n_par;
+  for (int c = 0; c < GM_MAX_COMP; ++c) {
+    md->kind[c] = GM_SKY; md->conv[c] = 0;
+    for (int k = 0; k < GM_NSLOT; ++k) md->slot[c][k] = -1;
+  }
+  for (int c = 0; c < m->n_comp; ++c) {
+    const gm_component& gc = m->comp[c];
+    if (gc.kind < GM_SERSIC || gc.kind > GM_SKY) return GM_EINVAL;
+    md->kind[c] = gc.kind;
+    md->conv[c] = (gc.kind != GM_SKY && gc.convolve != 0) ? 1 : 0;
+    for (int k = 0; k < GM_NSLOT; ++k) {
+      const int s = gc.slot[k];
+      if (s < -1 || s >= m->n_par) return GM_EINVAL;
+      md->slot[c][k] = (int8_t)s;
+    }
+    if (gc.slot[GM_SLOT_AMP] < 0) return GM_EINVAL;
+    if (gc.kind != GM_SKY && gc.slot[GM_SLOT_S0] < 0) return GM_EINVAL;
+    if (gc.slot[GM_SLOT_BOX] >= 0) return GM_ENOTSUP;     // Eq. 2 with B != 0: not built yet
+  }
+  return GM_OK;
+}
+
+static void tile_for(int D, int* T, int* n) {
+  const int nt = (D + 127) / 128;
+  const int per = (D + nt - 1) / nt;
+  *T = (per + 7) / 8 * 8;
+  *n = (D + *T - 1) / *T;
+}
+
+static TileGeom make_geom(int H, int W, int KP) {
+  TileGeom tg;
+  tg.H = H; tg.W = W;
+  tile_for(H, &tg.TH, &tg.tiles_y);
+  tile_for(W, &tg.TW, &tg.tiles_x);
+  tg.ntx = tg.TW / kTC;
+  tg.nty = tg.TH / kTR;
+  const int win = ((kTC + KP - 1) + 3) / 4 * 4;            // floats read per thread window row
+  tg.pitch = (tg.TW - kTC + win + 3) / 4 * 4;
+  tg.rows = tg.TH + KP - 1;
+  return tg;
+}
+
+struct Workspace {
+  CompConst* cc;
+  float* G;
+  float* chi2_part;
+  float* grad_part;
+  float* psf_pad;
+  float *u, *m, *s, *p_prev, *chi2_prev;
+  int *calm, *frozen;
+  size_t total;
+};
+
+static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int KP, const TileGeom& tg) {
+  Workspace w;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    void* p = base ? (void*)((char*)base + off) : nullptr;
+    off += align_up(bytes, 256);
+    return p;
+  };
+  const size_t B = bt->B, P = md.n_par, tiles = (size_t)tg.tiles_x * tg.tiles_y;
+  w.cc = (CompConst*)take(B * md.n_comp * sizeof(CompConst));
+  w.G = (float*)take(B * bt->H * bt->W * 4);
+  w.chi2_part = (float*)take(B * tiles * 4);
+  w.grad_part = (float*)take(B * tiles * md.n_comp * kNSum * 4);
+  const size_t n_psf = bt->psf_stride == 0 ? 1 : B;
+  w.psf_pad = (float*)take(KP != bt->K ? n_psf * KP * KP * 4 : 0);
+  w.u = (float*)take(B * P * 4);
+  w.m = (float*)take(B * P * 4);
+  w.s = (float*)take(B * P * 4);
+  w.p_prev = (float*)take(B * P * 4);
+  w.chi2_prev = (float*)take(B * 4);
+  w.calm = (int*)take(B * 4);
+  w.frozen = (int*)take(B * 4);
+  w.total = off;
+  return w;
+}
+
+// per-K launchers live in gm_tiles.cu, compiled once per PSF side (-DGM_K=..)
+#define GM_DECL_K(K)                                                                          \
+  int launch_forward_##K(const FwdArgs& a, bool render, int B, cudaStream_t st, cudaError_t* err); \
+  int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);
+GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
+#undef GM_DECL_K
+
+static int dispatch_forward(int KP, const FwdArgs& a, bool render, int B, cudaStream_t st) {
+  int rc;
+  cudaError_t err = cudaSuccess;
+  switch (KP) {
+    case 5: rc = launch_forward_5(a, render, B, st, &err); break;
+    case 9: rc = launch_forward_9(a, render, B, st, &err); break;
+    case 15: rc = launch_forward_15(a, render, B, st, &err); break;
+    case 21: rc = launch_forward_21(a, render, B, st, &err); break;
+    case 25: rc = launch_forward_25(a, render, B, st, &err); break;
+    case 33: rc = launch_forward_33(a, render, B, st, &err); break;
+    case 41: rc = launch_forward_41(a, render, B, st, &err); break;
+    default: return GM_ENOTSUP;
+  }
+  if (rc == GM_OK) ++t_launches;
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+
+static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
+  int rc;
+  cudaError_t err = cudaSuccess;
+  switch (KP) {
+    case 5: rc = launch_backward_5(a, B, st, &err); break;
+    case 9: rc = launch_backward_9(a, B, st, &err); break;
+    case 15: rc = launch_backward_15(a, B, st, &err); break;
+    case 21: rc = launch_backward_21(a, B, st, &err); break;
+    case 25: rc = launch_backward_25(a, B, st, &err); break;
+    case 33: rc = launch_backward_33(a, B, st, &err); break;
+    case 41: rc = launch_backward_41(a, B, st, &err); break;
+    default: return GM_ENOTSUP;
+  }
+  if (rc == GM_OK) ++t_launches;
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+
+// everything a call needs after validation
+struct Plan {
+  ModelDesc md;
+  TileGeom tg;
+  Workspace ws;
+  int KP;
+  const float* psf; long long psf_stride;
+  int tiles;
+};
+
+static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, void* workspace,
+                     size_t workspace_bytes, cudaStream_t st, Plan* pl) {
+  int rc = validate(model, bt, need_data, &pl->md);
+  if (rc != GM_OK) return rc;
+  pl->KP = padded_K(bt->K);
+  if (pl->KP < 0) return GM_ENOTSUP;
+  pl->tg = make_geom(bt->H, bt->W, pl->KP);
+  pl->tiles = pl->tg.tiles_x * pl->tg.tiles_y;
+  if ((size_t)bt->B * pl->tiles > 0x7fffffffull) return GM_EINVAL;
+  pl->ws = carve(workspace, pl->md, bt, pl->KP, pl->tg);
+  if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < pl->ws.total) return GM_EWORKSPACE;
+  pl->psf = bt->psf;
+  pl->psf_stride = bt->psf_stride;
+  if (pl->KP != bt->K) {
+    const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
+    const int n = n_psf * pl->KP * pl->KP;
+    k_pad_psf<<<(n + 255) / 256, 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, pl->KP, pl->ws.psf_pad);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+    pl->psf = pl->ws.psf_pad;
+    pl->psf_stride = bt->psf_stride == 0 ? 0 : (long long)pl->KP * pl->KP;
+  }
+  return GM_OK;
+}
+
+static int run_prologue(const Plan& pl, int B, const float* params, const int* frozen, cudaStream_t st) {
+  const int n = B * pl.md.n_comp;
+  k_prologue<<<(n + 127) / 128, 128, 0, st>>>(pl.md, B, params, pl.ws.cc, frozen);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  return GM_OK;
+}
+
+static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const int* frozen) {
+  FwdArgs a;
+  a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
+  a.psf = pl.psf; a.psf_stride = pl.psf_stride;
+  a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
+  a.G = out; a.chi2_part = pl.ws.chi2_part; a.frozen = frozen;
+  return a;
+}
+
+static BwdArgs bwd_args(const Plan& pl, const int* frozen) {
+  BwdArgs a;
+  a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
+  a.psf = pl.psf; a.psf_stride = pl.psf_stride;
+  a.G = pl.ws.G; a.grad_part = pl.ws.grad_part; a.frozen = frozen;
+  return a;
+}
+
+static FinArgs fin_args(const Plan& pl, int B, bool with_grad, float* chi2, float* grad) {
+  FinArgs a;
+  a.md = pl.md; a.B = B; a.tiles = pl.tiles; a.cc = pl.ws.cc;
+  a.chi2_part = pl.ws.chi2_part;
+  a.grad_part = with_grad ? pl.ws.grad_part : nullptr;
+  a.chi2 = chi2; a.grad = grad;
+  return a;
+}
+
+}  // namespace gm
+
+using namespace gm;
+
+extern "C" {
+
+size_t gm_workspace_bytes(const gm_model* model, const gm_batch* bt) {
+  ModelDesc md;
+  if (!model || !bt) return 0;
+  gm_batch tmp = *bt;
+  static const float dummy = 0.0f;
+  if (!tmp.psf) tmp.psf = &dummy;
+  if (validate(model, &tmp, false, &md) != GM_OK) return 0;
+  const int KP = padded_K(bt->K);
+  if (KP < 0) return 0;
+  const TileGeom tg = make_geom(bt->H, bt->W, KP);
+  return carve(nullptr, md, bt, KP, tg).total;
+}
+
+int gm_render(const gm_model* model, const gm_batch* bt, const float* params, float* model_out,
+              void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  if (!params || !model_out) return GM_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Plan pl;
+  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
+  if (rc != GM_OK) return rc;
+  if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
+  return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, nullptr), true, bt->B, st);
+}
+
+int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params, float* chi2,
+                 float* grad, float* jtj, float* jtr, void* workspace, size_t workspace_bytes,
+                 void* cuda_stream) {
+  t_launches = 0;
+  if (!params || !chi2) return GM_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Plan pl;
+  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl);
+  if (rc != GM_OK) return rc;
+  if (jtj || jtr) return GM_ENOTSUP;
+  if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
+  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, nullptr), false, bt->B, st)) != GM_OK) return rc;
+  if (grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, nullptr), bt->B, st)) != GM_OK) return rc;
+  k_finalize<<<(bt->B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(
+      fin_args(pl, bt->B, grad != nullptr, chi2, grad));
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  return GM_OK;
+}
+
+int gm_fit(const gm_model* model, const gm_batch* bt, float* params, const gm_fit_opts* opts,
+           float* chi2_out, int32_t* iters_used, int32_t* status, void* workspace,
+           size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  if (!params || !chi2_out || !opts || !opts->lr || !opts->lo || !opts->hi) return GM_EINVAL;
+  if (opts->n_iter < 0 || opts->patience < 0) return GM_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Plan pl;
+  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl);
+  if (rc != GM_OK) return rc;
+  const int B = bt->B, P = pl.md.n_par;
+
+  FitOptsDev o;
+  memset(&o, 0, sizeof(o));
+  for (int k = 0; k < P; ++k) {
+    const bool lg = opts->log10_space && opts->log10_space[k];
+    o.lg[k] = lg;
+    o.fr[k] = opts->free_mask ? (opts->free_mask[k] != 0) : 1;
+    o.lr[k] = opts->lr[k];
+    const double lo = opts->lo[k], hi = opts->hi[k];
+    o.ulo[k] = lg ? (lo > 0.0 ? (float)std::log10(lo) : -std::numeric_limits<float>::infinity()) : (float)lo;
+    o.uhi[k] = lg ? (float)std::log10(hi) : (float)hi;
+  }
+  o.beta1 = opts->beta1; o.beta2 = opts->beta2; o.eps = opts->eps; o.tol = opts->tol;
+  o.patience = opts->patience;
+  FitState fs{pl.ws.u, pl.ws.m, pl.ws.s, pl.ws.p_prev, pl.ws.chi2_prev, pl.ws.calm, pl.ws.frozen};
+
+  k_fit_init<<<(B * P + 127) / 128, 128, 0, st>>>(B, P, params, o, fs, iters_used, status);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+
+  const FwdArgs fa = fwd_args(pl, bt, pl.ws.G, fs.frozen);
+  const BwdArgs ba = bwd_args(pl, fs.frozen);
+  const int fin_grid = (B + kFinWarps - 1) / kFinWarps;
+  for (int t = 1; t <= opts->n_iter + 1; ++t) {
+    const int last = (t == opts->n_iter + 1);
+    if ((rc = run_prologue(pl, B, params, fs.frozen, st)) != GM_OK) return rc;
+    if ((rc = dispatch_forward(pl.KP, fa, false, B, st)) != GM_OK) return rc;
+    if (!last && (rc = dispatch_backward(pl.KP, ba, B, st)) != GM_OK) return rc;
+    const float c1 = (float)(1.0 - std::pow((double)opts->beta1, (double)t));
+    const float c2 = (float)(1.0 - std::pow((double)opts->beta2, (double)t));
+    const float dec = (float)std::pow((double)opts->lr_decay, (double)(t - 1));
+    k_fit_step<<<fin_grid, kFinWarps * 32, 0, st>>>(fin_args(pl, B, !last, chi2_out, nullptr), o, fs, params,
+                                                   t, last, c1, c2, dec, iters_used, status);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+  }
+  return GM_OK;
+}
+
+// ---- host-buffer variants ----------------------------------------------------
+namespace {
+struct DevBuf {
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  cudaError_t alloc(size_t n) { return cudaMalloc(&p, n ? n : 1); }
+};
+struct StreamGuard {
+  cudaStream_t s = nullptr;
+  ~StreamGuard() { if (s) cudaStreamDestroy(s); }
+};
+
+struct HostCall {
+  DevBuf data, sigma, mask, psf, params, ws;
+  StreamGuard sg;
+  gm_batch dev;
+  size_t ws_bytes = 0;
+};
+
+int stage_in(const gm_model* model, const gm_batch* hb, const float* params, bool need_data, HostCall* hc) {
+  if (!model || !hb || !params || !hb->psf) return GM_EINVAL;
+  if (need_data && (!hb->data || !hb->sigma)) return GM_EINVAL;
+  hc->ws_bytes = gm_workspace_bytes(model, hb);
+  if (hc->ws_bytes == 0) return GM_EINVAL;
+  GM_CUDA(cudaStreamCreateWithFlags(&hc->sg.s, cudaStreamNonBlocking));
+  cudaStream_t st = hc->sg.s;
+  const size_t npx = (size_t)hb->B * hb->H * hb->W;
+  const size_t npsf = (hb->psf_stride == 0 ? 1 : (size_t)hb->B) * hb->K * hb->K;
+  hc->dev = *hb;
+  hc->dev.data = nullptr; hc->dev.sigma = nullptr; hc->dev.mask = nullptr;
+  GM_CUDA(hc->psf.alloc(npsf * 4));
+  GM_CUDA(cudaMemcpyAsync(hc->psf.p, hb->psf, npsf * 4, cudaMemcpyHostToDevice, st));
+  hc->dev.psf = (const float*)hc->psf.p;
+  if (hb->psf_stride != 0) hc->dev.psf_stride = (int64_t)hb->K * hb->K;
+  if (hb->psf_stride != 0 && hb->psf_stride != (int64_t)hb->K * hb->K) return GM_EINVAL;
+  if (need_data) {
+    GM_CUDA(hc->data.alloc(npx * 4));
+    GM_CUDA(hc->sigma.alloc(npx * 4));
+    GM_CUDA(cudaMemcpyAsync(hc->data.p, hb->data, npx * 4, cudaMemcpyHostToDevice, st));
+    GM_CUDA(cudaMemcpyAsync(hc->sigma.p, hb->sigma, npx * 4, cudaMemcpyHostToDevice, st));
+    hc->dev.data = (const float*)hc->data.p;
+    hc->dev.sigma = (const float*)hc->sigma.p;
+    if (hb->mask) {
+      GM_CUDA(hc->mask.alloc(npx));
+      GM_CUDA(cudaMemcpyAsync(hc->mask.p, hb->mask, npx, cudaMemcpyHostToDevice, st));
+      hc->dev.mask = (const uint8_t*)hc->mask.p;
+    }
+  }
+  const size_t npar = (size_t)hb->B * model->n_par * 4;
+  GM_CUDA(hc->params.alloc(npar));
+  GM_CUDA(cudaMemcpyAsync(hc->params.p, params, npar, cudaMemcpyHostToDevice, st));
+  GM_CUDA(hc->ws.alloc(hc->ws_bytes));
+  return GM_OK;
+}
+}  // namespace
+
+int gm_render_host(const gm_model* model, const gm_batch* hb, const float* params, float* model_out) {
+  if (!model_out) return GM_EINVAL;
+  HostCall hc;
+  int rc = stage_in(model, hb, params, false, &hc);
+  if (rc != GM_OK) return rc;
+  const size_t npx = (size_t)hb->B * hb->H * hb->W;
+  DevBuf out;
+  GM_CUDA(out.alloc(npx * 4));
+  rc = gm_render(model, &hc.dev, (const float*)hc.params.p, (float*)out.p, hc.ws.p, hc.ws_bytes, hc.sg.s);
+  if (rc != GM_OK) return rc;
+  const int64_t n = t_launches;
+  GM_CUDA(cudaMemcpyAsync(model_out, out.p, npx * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  GM_CUDA(cudaStreamSynchronize(hc.sg.s));
+  t_launches = n;
+  return GM_OK;
+}
+
+int gm_loss_grad_host(const gm_model* model, const gm_batch* hb, const float* params, float* chi2, float* grad) {
+  if (!chi2) return GM_EINVAL;
+  HostCall hc;
+  int rc = stage_in(model, hb, params, true, &hc);
+  if (rc != GM_OK) return rc;
+  const size_t B = hb->B, P = model->n_par;
+  DevBuf dchi2, dgrad;
+  GM_CUDA(dchi2.alloc(B * 4));
+  GM_CUDA(dgrad.alloc(B * P * 4));
+  rc = gm_loss_grad(model, &hc.dev, (const float*)hc.params.p, (float*)dchi2.p, grad ? (float*)dgrad.p : nullptr,
+                    nullptr, nullptr, hc.ws.p, hc.ws_bytes, hc.sg.s);
+  if (rc != GM_OK) return rc;
+  GM_CUDA(cudaMemcpyAsync(chi2, dchi2.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  if (grad) GM_CUDA(cudaMemcpyAsync(grad, dgrad.p, B * P * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  GM_CUDA(cudaStreamSynchronize(hc.sg.s));
+  return GM_OK;
+}
+
+int gm_fit_host(const gm_model* model, const gm_batch* hb, float* params, const gm_fit_opts* opts,
+                float* chi2_out, int32_t* iters_used, int32_t* status) {
+  if (!chi2_out) return GM_EINVAL;
+  HostCall hc;
+  int rc = stage_in(model, hb, params, true, &hc);
+  if (rc != GM_OK) return rc;
+  const size_t B = hb->B, P = model->n_par;
+  DevBuf dchi2, dit, dst;
+  GM_CUDA(dchi2.alloc(B * 4));
+  GM_CUDA(dit.alloc(B * 4));
+  GM_CUDA(dst.alloc(B * 4));
+  rc = gm_fit(model, &hc.dev, (float*)hc.params.p, opts, (float*)dchi2.p, (int32_t*)dit.p, (int32_t*)dst.p,
+              hc.ws.p, hc.ws_bytes, hc.sg.s);
+  if (rc != GM_OK) return rc;
+  GM_CUDA(cudaMemcpyAsync(params, hc.params.p, B * P * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  GM_CUDA(cudaMemcpyAsync(chi2_out, dchi2.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  if (iters_used) GM_CUDA(cudaMemcpyAsync(iters_used, dit.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  if (status) GM_CUDA(cudaMemcpyAsync(status, dst.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
+  GM_CUDA(cudaStreamSynchronize(hc.sg.s));
+  return GM_OK;
+}
+
+const char* gm_strerror(int status) {
+  switch (status) {
+    case GM_OK: return "ok";
+    case GM_EINVAL: return "invalid argument";
+    case GM_ENOTSUP: return "not supported by this build";
+    case GM_ECUDA: return "CUDA error (see gm_last_cuda_error_string)";
+    case GM_EWORKSPACE: return "workspace missing, misaligned or too small";
+    default: return "unknown status";
+  }
+}
+
+int gm_version(void) { return GM_VERSION; }
+int gm_last_cuda_error(void) { return (int)t_last_err; }
+const char* gm_last_cuda_error_string(void) { return cudaGetErrorString(t_last_err); }
+int64_t gm_last_launch_count(void) { return t_launches; }
+
+}  // extern "C"

@@ -1,0 +1,373 @@
+// gm_kernels.cuh -- the per-tile kernels of the hot path (steps a1-a5 of
+// SURVEY.md section 8(a)), templated on the PSF side K.
+//
+// One CTA owns a TH x TW tile of one galaxy's cutout.  Each thread owns an
+// 8 x 8 block of output pixels and runs the direct PSF convolution as packed
+// FP32 FMAs (FFMA2 on sm_100a): an accumulator pair holds two vertically adjacent
+// output pixels, the multiplicand pair holds two vertically adjacent PSF taps,
+// and the input sample is the scalar-broadcast operand, so one instruction does
+// two of the 2 K^2 multiply-adds per pixel and half of the issue slots stay free
+// for the shared-memory loads that feed it.
+//
+//   k_forward<K, RENDER>  a1 render S on tile + halo (shared memory)
+//                         a2 M = PSF (*) S          (R:C1, flipped-tap correlation)
+//                         a3 rho, chi2 partial, G = -2 w rho -> workspace
+//                         (RENDER: write M instead; gm_render)
+//   k_backward<K>         a4 A = PSF (star) G        (R:C2) from the G tile + halo
+//                         a5 per-tile partial sums of A dS/dp (8 per component)
+//
+// Reductions are fixed-order (thread -> warp shuffle tree -> warps in order ->
+// tiles in order in k_finalize); no floating-point atomics anywhere.
+#pragma once
+#include "gm_device.cuh"
+
+namespace gm {
+
+constexpr int kTR = 8, kTC = 8;            // thread tile (rows x cols)
+constexpr int kNSum = 8;                   // partial sums per component
+
+struct TileGeom {
+  int H, W;                // cutout
+  int TH, TW;              // CTA tile (multiples of 8)
+  int tiles_x, tiles_y;    // tiles per cutout
+  int ntx, nty;            // thread tiles per CTA tile
+  int pitch;               // shared row pitch (floats), multiple of 4
+  int rows;                // TH + K - 1
+};
+
+struct FwdArgs {
+  ModelDesc md;
+  TileGeom tg;
+  const CompConst* cc;     // [B, n_comp]
+  const float* psf; long long psf_stride;
+  const float* data; const float* sigma; const uint8_t* mask;
+  float* G;                // [B,H,W] workspace (or model_out when RENDER)
+  float* chi2_part;        // [B, tiles]
+  const int* frozen;       // [B] or nullptr: skip galaxies that stopped
+};
+
+struct BwdArgs {
+  ModelDesc md;
+  TileGeom tg;
+  const CompConst* cc;
+  const float* psf; long long psf_stride;
+  const float* G;          // [B,H,W]
+  float* grad_part;        // [B, tiles, n_comp, 8]
+  const int* frozen;
+};
+
+template <int K> struct ConvCfg {
+  static constexpr int kWin = ((kTC + K - 1) + 3) / 4;   // float4 chunks per input row window
+  static constexpr int kTapPitch = K + 1;                // float2 per tap-pair row (even)
+  static constexpr int kTapRows = K + 1;
+  static constexpr int kInRows = kTR + K - 1;
+};
+
+// paired taps: T2[a][t] = (P[a][t], P[a-1][t]), a = 0..K, P[-1] = P[K] = 0.
+// FLIP selects the flipped PSF (true convolution) or the PSF itself (adjoint).
+template <int K, bool FLIP>
+__device__ __forceinline__ void load_tap_pairs(float2* taps, const float* __restrict__ psf, int tid,
+                                               int nthreads) {
+  constexpr int TP = ConvCfg<K>::kTapPitch;
+  for (int idx = tid; idx < (K + 1) * TP; idx += nthreads) {
+    const int a = idx / TP, t = idx - a * TP;
+    float lo = 0.0f, hi = 0.0f;
+    if (t < K) {
+      const int tt = FLIP ? (K - 1 - t) : t;
+      if (a < K) lo = psf[(FLIP ? (K - 1 - a) : a) * K + tt];
+      if (a >= 1) hi = psf[(FLIP ? (K - a) : (a - 1)) * K + tt];
+    }
+    taps[idx] = make_float2(lo, hi);
+  }
+}
+
+// 8x8 outputs per thread.  win points at the thread's window origin in the shared
+// tile (row 0 of its 8 + K - 1 input rows, first of its 8 + K - 1 input columns).
+// acc[rp][c] = (out[2rp][c], out[2rp+1][c]).
+template <int K>
+__device__ __forceinline__ void conv8x8(const float* __restrict__ win, int pitch,
+                                        const float2* __restrict__ taps, float2 (&acc)[4][kTC]) {
+  constexpr int NW = ConvCfg<K>::kWin;
+  constexpr int TP = ConvCfg<K>::kTapPitch;
+#pragma unroll 1
+  for (int y = 0; y < ConvCfg<K>::kInRows; ++y) {
+    float in[NW * 4];
+    const float4* row = reinterpret_cast<const float4*>(win + y * pitch);
+#pragma unroll
+    for (int j = 0; j < NW; ++j) {
+      const float4 v = row[j];
+      in[4 * j + 0] = v.x; in[4 * j + 1] = v.y; in[4 * j + 2] = v.z; in[4 * j + 3] = v.w;
+    }
+#pragma unroll
+    for (int rp = 0; rp < 4; ++rp) {
+      const int a = y - 2 * rp;
+      if (a >= 0 && a <= K) {
+        const float4* tp = reinterpret_cast<const float4*>(taps + a * TP);
+#pragma unroll
+        for (int t2 = 0; t2 < (K + 1) / 2; ++t2) {
+          const float4 w = tp[t2];                      // two tap pairs
+#pragma unroll
+          for (int c = 0; c < kTC; ++c)
+            acc[rp][c] = __ffma2_rn(make_float2(in[c + 2 * t2], in[c + 2 * t2]),
+                                    make_float2(w.x, w.y), acc[rp][c]);
+          if (2 * t2 + 1 < K) {
+#pragma unroll
+            for (int c = 0; c < kTC; ++c)
+              acc[rp][c] = __ffma2_rn(make_float2(in[c + 2 * t2 + 1], in[c + 2 * t2 + 1]),
+                                      make_float2(w.z, w.w), acc[rp][c]);
+          }
+        }
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// acc -> 8x8 block of the shared tile (rows 2rp, 2rp+1), two float4 per row
+__device__ __forceinline__ void store_acc(float* dst, int pitch, const float2 (&acc)[4][kTC]) {
+#pragma unroll
+  for (int rp = 0; rp < 4; ++rp) {
+    float4* r0 = reinterpret_cast<float4*>(dst + (size_t)(2 * rp) * pitch);
+    float4* r1 = reinterpret_cast<float4*>(dst + (size_t)(2 * rp + 1) * pitch);
+    r0[0] = make_float4(acc[rp][0].x, acc[rp][1].x, acc[rp][2].x, acc[rp][3].x);
+    r0[1] = make_float4(acc[rp][4].x, acc[rp][5].x, acc[rp][6].x, acc[rp][7].x);
+    r1[0] = make_float4(acc[rp][0].y, acc[rp][1].y, acc[rp][2].y, acc[rp][3].y);
+    r1[1] = make_float4(acc[rp][4].y, acc[rp][5].y, acc[rp][6].y, acc[rp][7].y);
+  }
+}
+
+// dynamic shared memory: [ tile: rows x pitch floats | taps: (K+1) x (K+1) float2 | red ]
+template <int K>
+__host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int n_red) {
+  return (size_t)tg.rows * tg.pitch * 4 + (size_t)(K + 1) * ConvCfg<K>::kTapPitch * 8 +
+         (size_t)nwarps * n_red * 4 + 64;
+}
+
+// ---------------------------------------------------------------------------
+// forward: render + convolve + residual
+// ---------------------------------------------------------------------------
+template <int K, bool RENDER>
+__global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const TileGeom& tg = a.tg;
+  const int tiles = tg.tiles_x * tg.tiles_y;
+  const int b = blockIdx.x / tiles;
+  const int tile = blockIdx.x - b * tiles;
+  if (a.frozen && a.frozen[b]) return;
+  const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
+  const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;     // tile origin in the cutout
+  constexpr int h = (K - 1) / 2;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  const int lane = tid & 31, wid = tid >> 5, nwarps = nthr >> 5;
+
+  float* tilebuf = reinterpret_cast<float*>(smem_raw);
+  float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
+  float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
+
+  load_tap_pairs<K, true>(taps, a.psf + (long long)b * a.psf_stride, tid, nthr);
+
+  // a1: S on the tile plus its halo; zero outside the cutout (R:C1) and in the pad
+  const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+  const int cols = tg.TW + K - 1;
+  for (int yy = wid; yy < tg.rows; yy += nwarps) {
+    const int i = i0 - h + yy;
+    float* rowp = tilebuf + (size_t)yy * tg.pitch;
+    const bool row_in = (i >= 0 && i < tg.H);
+    const float y = (float)tg.H - 0.5f - (float)i;       // R:G1
+    for (int xx = lane; xx < tg.pitch; xx += 32) {
+      const int j = j0 - h + xx;
+      float s = 0.0f;
+      if (row_in && xx < cols && j >= 0 && j < tg.W) {
+        const float x = (float)j + 0.5f;
+        for (int c = 0; c < a.md.n_comp; ++c) {
+          if (a.md.conv[c]) {
+            const CompConst cc = ccb[c];
+            const Geo g = geometry(cc, x, y);
+            s = fmaf(cc.amp, profile_value(a.md.kind[c], cc, g.r), s);
+          }
+        }
+      }
+      rowp[xx] = s;
+    }
+  }
+  __syncthreads();
+
+  // a2: M = PSF (*) S on this thread's 8x8 block
+  const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
+  const bool active = ty < tg.nty;
+  float2 acc[4][kTC];
+#pragma unroll
+  for (int rp = 0; rp < 4; ++rp)
+#pragma unroll
+    for (int c = 0; c < kTC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
+  if (active) conv8x8<K>(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, taps, acc);
+
+  // park M in the (now dead) tile buffer so that the epilogue can walk the tile
+  // row-major with coalesced global accesses
+  __syncthreads();
+  if (active) store_acc(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, acc);
+  __syncthreads();
+
+  // a3: unconvolved components, residual, chi2, back-seed G
+  float chi2 = 0.0f;
+  const size_t img = (size_t)b * tg.H * tg.W;
+  for (int yy = wid; yy < tg.TH; yy += nwarps) {
+    const int i = i0 + yy;
+    if (i >= tg.H) break;
+    const float y = (float)tg.H - 0.5f - (float)i;
+    for (int xx = lane; xx < tg.TW; xx += 32) {
+      const int j = j0 + xx;
+      if (j >= tg.W) break;
+      float m = tilebuf[(size_t)yy * tg.pitch + xx];
+      const float x = (float)j + 0.5f;
+      for (int c = 0; c < a.md.n_comp; ++c) {
+        if (a.md.conv[c]) continue;
+        const CompConst cc = ccb[c];
+        const int kind = a.md.kind[c];
+        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
+        m = fmaf(cc.amp, U, m);
+      }
+      const size_t off = img + (size_t)i * tg.W + j;
+      if (RENDER) {
+        a.G[off] = m;
+      } else {
+        const bool used = a.mask ? (a.mask[off] != 0) : true;
+        float g = 0.0f;
+        if (used) {                                      // select, never multiply by 0 (R:X1)
+          const float sg = a.sigma[off];
+          const float w = __frcp_rn(sg * sg);
+          const float rho = a.data[off] - m;
+          chi2 = fmaf(w * rho, rho, chi2);
+          g = -2.0f * w * rho;
+        }
+        a.G[off] = g;
+      }
+    }
+  }
+  if (!RENDER) {
+    chi2 = warp_sum(chi2);
+    if (lane == 0) red[wid] = chi2;
+    __syncthreads();
+    if (tid == 0) {
+      float s = 0.0f;
+      for (int w = 0; w < nwarps; ++w) s += red[w];
+      a.chi2_part[(size_t)b * tiles + tile] = s;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// backward: adjoint convolution + parameter-gradient partial sums
+// per component: s0 = sum c u, s1 = sum c v/q, s2 = sum c u v/q, s3 = sum c (v/q)^2
+//   with c = seed amp dU/dr / rg ; s4 = sum seed U ; s5..s7 = sum seed amp dU/ds
+// ---------------------------------------------------------------------------
+template <int K>
+__global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const TileGeom& tg = a.tg;
+  const int tiles = tg.tiles_x * tg.tiles_y;
+  const int b = blockIdx.x / tiles;
+  const int tile = blockIdx.x - b * tiles;
+  if (a.frozen && a.frozen[b]) return;
+  const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
+  const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;
+  constexpr int h = (K - 1) / 2;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  const int lane = tid & 31, wid = tid >> 5, nwarps = nthr >> 5;
+
+  float* tilebuf = reinterpret_cast<float*>(smem_raw);
+  float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
+  float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
+
+  load_tap_pairs<K, false>(taps, a.psf + (long long)b * a.psf_stride, tid, nthr);
+
+  // G tile + halo, zero outside the cutout
+  const float* Gb = a.G + (size_t)b * tg.H * tg.W;
+  const int cols = tg.TW + K - 1;
+  for (int yy = wid; yy < tg.rows; yy += nwarps) {
+    const int i = i0 - h + yy;
+    float* rowp = tilebuf + (size_t)yy * tg.pitch;
+    const bool row_in = (i >= 0 && i < tg.H);
+    for (int xx = lane; xx < tg.pitch; xx += 32) {
+      const int j = j0 - h + xx;
+      float s = 0.0f;
+      if (row_in && xx < cols && j >= 0 && j < tg.W) s = Gb[(size_t)i * tg.W + j];
+      rowp[xx] = s;
+    }
+  }
+  __syncthreads();
+
+  const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
+  const bool active = ty < tg.nty;
+  float2 acc[4][kTC];
+#pragma unroll
+  for (int rp = 0; rp < 4; ++rp)
+#pragma unroll
+    for (int c = 0; c < kTC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
+  if (active) conv8x8<K>(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, taps, acc);
+
+  // park A in the tile buffer (G itself stays in global memory for the
+  // unconvolved components), then walk the tile row-major
+  __syncthreads();
+  if (active) store_acc(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, acc);
+  __syncthreads();
+
+  // a5: partial sums per component
+  const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+  float* outp = a.grad_part + ((size_t)b * tiles + tile) * a.md.n_comp * kNSum;
+  for (int c = 0; c < a.md.n_comp; ++c) {
+    float s[kNSum];
+#pragma unroll
+    for (int k = 0; k < kNSum; ++k) s[k] = 0.0f;
+    const CompConst cc = ccb[c];
+    const int kind = a.md.kind[c];
+    const bool conv = a.md.conv[c] != 0;
+    for (int yy = wid; yy < tg.TH; yy += nwarps) {
+      const int i = i0 + yy;
+      if (i >= tg.H) break;
+      const float y = (float)tg.H - 0.5f - (float)i;
+      for (int xx = lane; xx < tg.TW; xx += 32) {
+        const int j = j0 + xx;
+        if (j >= tg.W) break;
+        const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
+        if (kind == GM_SKY) { s[4] += seed; continue; }
+        const float x = (float)j + 0.5f;
+        const Geo g = geometry(cc, x, y);
+        const float rg = fmaxf(g.r, kRGuard);
+        float U, dUdr, d0, d1, d2;
+        profile_grad(kind, cc, rg, U, dUdr, d0, d1, d2);
+        // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
+        const float Uv = (g.r < kRGuard) ? profile_value(kind, cc, g.r) : U;
+        const float sa = seed * cc.amp;
+        const float cgeo = __fdividef(sa * dUdr, rg);
+        s[0] = fmaf(cgeo, g.u, s[0]);
+        s[1] = fmaf(cgeo, g.vq, s[1]);
+        s[2] = fmaf(cgeo * g.u, g.vq, s[2]);
+        s[3] = fmaf(cgeo * g.vq, g.vq, s[3]);
+        s[4] = fmaf(seed, Uv, s[4]);
+        s[5] = fmaf(sa, d0, s[5]);
+        s[6] = fmaf(sa, d1, s[6]);
+        s[7] = fmaf(sa, d2, s[7]);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < kNSum; ++k) {
+      const float v = warp_sum(s[k]);
+      if (lane == 0) red[wid * kNSum + k] = v;
+    }
+    __syncthreads();
+    if (tid < kNSum) {
+      float t = 0.0f;
+      for (int w = 0; w < nwarps; ++w) t += red[w * kNSum + tid];
+      outp[c * kNSum + tid] = t;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace gm

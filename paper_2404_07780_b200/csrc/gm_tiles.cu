@@ -1,0 +1,53 @@
+// gm_tiles.cu -- instantiates the tile kernels for one PSF side, -DGM_K=<odd>.
+// Compiled once per supported K (see build.py) so the builds run in parallel.
+#include "gm_kernels.cuh"
+
+#ifndef GM_K
+#error "compile with -DGM_K=<PSF side>"
+#endif
+#define GM_CAT_(a, b) a##b
+#define GM_CAT(a, b) GM_CAT_(a, b)
+
+namespace gm {
+
+#define GM_TRY(expr)                                   \
+  do {                                                 \
+    cudaError_t e__ = (expr);                          \
+    if (e__ != cudaSuccess) { *err = e__; return GM_ECUDA; } \
+  } while (0)
+
+template <typename Kern>
+static cudaError_t set_smem(Kern kern, size_t bytes) {
+  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, bool render, int B, cudaStream_t st, cudaError_t* err) {
+  constexpr int K = GM_K;
+  const int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
+  if (nthr > 256) return GM_ENOTSUP;
+  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
+  const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
+  if (render) {
+    GM_TRY(set_smem(k_forward<K, true>, sm));
+    k_forward<K, true><<<grid, nthr, sm, st>>>(a);
+  } else {
+    GM_TRY(set_smem(k_forward<K, false>, sm));
+    k_forward<K, false><<<grid, nthr, sm, st>>>(a);
+  }
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
+int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err) {
+  constexpr int K = GM_K;
+  const int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
+  if (nthr > 256) return GM_ENOTSUP;
+  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum);
+  const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
+  GM_TRY(set_smem(k_backward<K>, sm));
+  k_backward<K><<<grid, nthr, sm, st>>>(a);
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
+}  // namespace gm

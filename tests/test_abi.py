@@ -1,0 +1,64 @@
+"""The C-ABI library loads and exports every symbol include/gm.h declares; argument
+validation returns the documented codes.  No compute call needs a GPU here."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2404_07780_b200 import build as gm_build
+    return C.CDLL(str(gm_build.build()))
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "gm.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gm_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    names = declared_symbols()
+    assert {"gm_render", "gm_loss_grad", "gm_fit", "gm_workspace_bytes", "gm_strerror", "gm_version",
+            "gm_render_host", "gm_loss_grad_host", "gm_fit_host"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_version_and_strerror(lib):
+    lib.gm_version.restype = C.c_int
+    lib.gm_strerror.restype = C.c_char_p
+    assert lib.gm_version() == 100
+    assert b"invalid" in lib.gm_strerror(-1) and b"ok" == lib.gm_strerror(0)
+
+
+def test_validation_codes_without_gpu():
+    import numpy as np
+    import paper_2404_07780_b200 as gm
+    from paper_2404_07780_b200 import binding as bd
+    from gen import models
+    model = models.single_sersic()
+    assert gm.gm_workspace_bytes(model, 16, 64, 64, 15) > 16 * 64 * 64 * 4
+    assert gm.gm_workspace_bytes(model, 16, 64, 64, 14) == 0        # even K
+    assert gm.gm_workspace_bytes(model, 16, 64, 64, 43) == 0        # K over GM_MAX_K
+    assert gm.gm_workspace_bytes(model, 0, 64, 64, 15) == 0
+    bad = {"n_par": 7, "components": [{"kind": "sersic", "convolve": 1, "slots": {"amp": 2, "s0": 9}}]}
+    assert gm.gm_workspace_bytes(bad, 4, 32, 32, 5) == 0           # slot index out of range
+    # null pointers are rejected before anything is launched (no GPU needed)
+    m = bd._model_struct(model)
+    b = bd._Batch(4, 32, 32, 5, None, None, None, None, 0)
+    L = bd._lib()
+    assert L.gm_render(C.byref(m), C.byref(b), None, None, None, 0, None) == -1
+    assert L.gm_fit(C.byref(m), C.byref(b), None, None, None, None, None, None, 0, None) == -1
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    import paper_2404_07780_b200 as gm
+    from gen import models
+    with pytest.raises(TypeError):
+        gm.gm_render(models.single_sersic(), torch.zeros(2, 7), 16, 16, torch.zeros(5, 5))

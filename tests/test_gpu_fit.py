@@ -1,0 +1,121 @@
+"""-m gpu: gm_fit against the oracle's fit on the same seeded inputs and options."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2404_07780_b200 as gm
+from gen import configs, models
+from gen.psf import gaussian_psf
+from gpu_util import PAR_RTOL, assert_chi2, dev, oracle_render
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_fit(b, opts, start=None):
+    p = dev(b["start"] if start is None else start).clone()
+    out = gm.gm_fit(b["model"], p, dev(b["data"]), dev(b["sigma"]), dev(b["mask"]), dev(b["psf"]), opts)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items() if not k.startswith("_")}
+
+
+def theta_close(a, b, rtol):
+    d = np.abs(((a - b) + np.pi / 2) % np.pi - np.pi / 2)      # theta is defined modulo pi (reading M1)
+    return d <= rtol * np.maximum(np.abs(b), 1.0)
+
+
+def compare_params(model, gpu, orc, rtol=PAR_RTOL):
+    ok = np.ones(gpu.shape, dtype=bool)
+    for k, role in enumerate(model["roles"]):
+        if role == "theta":
+            ok[:, k] = theta_close(gpu[:, k], orc[:, k], rtol)
+            ok[:, k] |= orc[:, [i for i, r in enumerate(model["roles"]) if r == "q"][0]] > 0.95
+        else:
+            ok[:, k] = np.abs(gpu[:, k] - orc[:, k]) <= rtol * np.abs(orc[:, k])
+    return ok
+
+
+def test_first_steps_match_oracle_closely():
+    # 3 iterations: every intermediate quantity is still well conditioned
+    b = configs.make_batch(0, range(8), oracle_render)
+    opts = configs.fit_options(b["model"], 64, 64, 3)
+    g = gpu_fit(b, opts)
+    o = oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
+    assert np.allclose(g["params"], o["params"], rtol=2e-5, atol=1e-6)
+    assert_chi2(g["chi2"], o["chi2"], rtol=5e-5)
+    assert (g["iters_used"] == 3).all() and (g["status"] == 0).all()
+
+
+def test_fit_c0_like_fixed_iterations():
+    b = configs.make_batch(0, range(16), oracle_render)
+    opts = configs.fit_options(b["model"], 64, 64, 150)
+    g = gpu_fit(b, opts)
+    o = oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
+    ok = compare_params(b["model"], g["params"], o["params"])
+    assert ok.mean() >= 0.97, f"parameter pass rate {ok.mean():.3f}\n{ok}"
+    assert_chi2(g["chi2"], o["chi2"], rtol=1e-4)
+    # chi2_out is chi^2 at the returned parameters
+    c, _ = gm.gm_loss_grad(b["model"], dev(g["params"]), dev(b["data"]), dev(b["sigma"]), None, dev(b["psf"]))
+    assert_chi2(g["chi2"], c.cpu().numpy().astype(np.float64), rtol=1e-6)
+
+
+def test_fit_bulge_disk_small():
+    def render(model, p, H, W, psf):
+        return oracle.render(model, p, H, W, psf)
+    cfg = configs.CONFIGS[3]
+    model = configs.get_model(cfg)
+    H = W = 48
+    gal = range(6)
+    truth = configs.truth_params(cfg, gal, H, W).astype(np.float32)
+    psf = gaussian_psf(9, 2.5).astype(np.float32)
+    M = oracle.render(model, truth, H, W, psf)
+    rng = np.random.default_rng(1)
+    sigma = np.full(M.shape, 0.02, dtype=np.float32)
+    data = (M + 0.02 * rng.normal(size=M.shape)).astype(np.float32)
+    start = configs.start_params(cfg, model, truth.astype(np.float64), gal, H, W).astype(np.float32)
+    b = {"model": model, "start": start, "data": data, "sigma": sigma, "mask": None, "psf": psf}
+    opts = configs.fit_options(model, H, W, 100)
+    g = gpu_fit(b, opts)
+    o = oracle.fit(model, start, data, sigma, None, psf, opts)
+    assert_chi2(g["chi2"], o["chi2"], rtol=1e-3)
+    ok = compare_params(model, g["params"], o["params"], rtol=5e-3)
+    assert ok.mean() >= 0.9, f"{ok.mean()}\n{ok}"
+
+
+def test_early_stop_fixed_parameter_and_nonfinite():
+    b = configs.make_batch(0, range(6), oracle_render)
+    data = b["data"].copy()
+    data[5, 10, 10] = np.nan                                   # galaxy 5: non-finite chi2 at once
+    b = dict(b, data=data)
+    opts = configs.fit_options(b["model"], 64, 64, 300, tol=1e-5, patience=5)
+    opts["free_mask"] = np.array([1, 1, 1, 1, 0, 1, 1], dtype=np.uint8)
+    g = gpu_fit(b, opts)
+    o = oracle.fit(b["model"], b["start"], data, b["sigma"], b["mask"], b["psf"], opts)
+    assert np.array_equal(g["status"], o["status"])
+    assert g["status"][5] == 2 and g["iters_used"][5] == 0
+    assert np.array_equal(g["params"][5], b["start"][5]) and not np.isfinite(g["chi2"][5])
+    assert np.array_equal(g["params"][:, 4], b["start"][:, 4])      # n held fixed, bit-identical
+    # early-stop iteration counts may differ by a few (reading O5); results must agree
+    assert np.all(np.abs(g["iters_used"][:5] - o["iters_used"][:5]) <= 15)
+    assert_chi2(g["chi2"][:5], o["chi2"][:5], rtol=1e-4)
+
+
+def test_bounds_are_respected():
+    b = configs.make_batch(0, range(4), oracle_render)
+    opts = configs.fit_options(b["model"], 64, 64, 30)
+    opts["lo"] = opts["lo"].copy(); opts["hi"] = opts["hi"].copy()
+    opts["hi"][3] = 3.0                                        # re <= 3 px: most truths are above
+    opts["lo"][5] = 0.5                                        # q >= 0.5
+    g = gpu_fit(b, opts)
+    o = oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
+    assert np.all(g["params"][:, 3] <= 3.0 * (1 + 1e-6)) and np.all(g["params"][:, 5] >= 0.5)
+    assert np.allclose(g["params"], o["params"], rtol=2e-3, atol=1e-4)
+
+
+def test_fit_host_matches_device():
+    b = configs.make_batch(0, range(4), oracle_render)
+    opts = configs.fit_options(b["model"], 64, 64, 20)
+    g = gpu_fit(b, opts)
+    p = b["start"].copy()
+    h = gm.gm_fit_host(b["model"], p, b["data"], b["sigma"], None, b["psf"], opts)
+    assert np.array_equal(h["params"], g["params"]) and np.array_equal(h["chi2"], g["chi2"])

@@ -1,0 +1,171 @@
+"""-m gpu: the CUDA path (through the C ABI) against the fp64 oracle, element by
+element, on the same seeded inputs.  Shapes span several tiles and ragged tails."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2404_07780_b200 as gm
+from gen import configs, models
+from gen.psf import asymmetric_psf, gaussian_psf, moffat_psf
+from gpu_util import (assert_chi2, assert_grad, assert_pixels, dev, oracle_render)
+from test_oracle_lossgrad import sample_params
+
+pytestmark = pytest.mark.gpu
+
+
+def synth(model, B, H, W, K, seed, masked=True, per_galaxy_psf=False):
+    rng = np.random.default_rng(seed)
+    truth = np.stack([sample_params(model, H, W, rng) for _ in range(B)]).astype(np.float32)
+    if per_galaxy_psf:
+        psf = np.stack([asymmetric_psf(K, seed=100 + g) for g in range(B)]).astype(np.float32)
+    else:
+        psf = asymmetric_psf(K).astype(np.float32)
+    M = oracle.render(model, truth, H, W, psf)
+    sigma = (0.05 + 0.1 * rng.random((B, H, W))).astype(np.float32)
+    data = (M + sigma * rng.normal(size=M.shape)).astype(np.float32)
+    mask = (rng.random((B, H, W)) > 0.15).astype(np.uint8) if masked else None
+    par = (truth * (1 + 0.05 * rng.uniform(-1, 1, size=truth.shape))).astype(np.float32)
+    return par, data, sigma, mask, psf
+
+
+def run_loss_grad(model, par, data, sigma, mask, psf):
+    chi2, grad = gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(psf))
+    torch.cuda.synchronize()
+    return chi2.cpu().numpy(), grad.cpu().numpy()
+
+
+# ---- config C0 exactly as BASELINE.json states it -------------------------------
+def test_c0_render_chi2_gradient():
+    b = configs.make_batch(0, range(16), oracle_render)
+    model = b["model"]
+    img = gm.gm_render(model, dev(b["start"]), b["H"], b["W"], dev(b["psf"]))
+    assert_pixels(img.cpu().numpy(), oracle.render(model, b["start"], b["H"], b["W"], b["psf"]))
+    chi2, grad = run_loss_grad(model, b["start"], b["data"], b["sigma"], b["mask"], b["psf"])
+    oc, og = oracle.loss_grad(model, b["start"], b["data"], b["sigma"], b["mask"], b["psf"])
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+
+
+# ---- every profile, tied parameters, unconvolved point source, sky -------------------
+@pytest.mark.parametrize("H,W,K,per_psf", [(40, 48, 9, False), (37, 45, 7, True), (21, 19, 5, False)])
+def test_all_profiles_render_and_gradient(H, W, K, per_psf):
+    model = models.all_profiles()
+    par, data, sigma, mask, psf = synth(model, 3, H, W, K, seed=H * W + K, per_galaxy_psf=per_psf)
+    img = gm.gm_render(model, dev(par), H, W, dev(psf))
+    assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+    # parameter by parameter too: each within 1e-3 of the gradient norm
+    scale = np.linalg.norm(og, axis=1, keepdims=True)
+    assert np.all(np.abs(grad - og) <= 1e-3 * scale)
+
+
+@pytest.mark.parametrize("kind", ["sersic", "expdisk", "ferrer", "king", "gaussian", "moffat"])
+@pytest.mark.parametrize("convolve", [1, 0])
+def test_each_profile_alone(kind, convolve):
+    model = models.one_component(kind, convolve)
+    H, W, K = 33, 30, 9
+    par, data, sigma, mask, psf = synth(model, 4, H, W, K, seed=len(kind) * 7 + convolve)
+    img = gm.gm_render(model, dev(par), H, W, dev(psf))
+    assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+
+
+# ---- several tiles per cutout, ragged tails, every compiled PSF side ------------------
+@pytest.mark.parametrize("H,W,K", [(150, 140, 25), (131, 70, 15), (64, 200, 21), (96, 96, 25),
+                                   (50, 50, 41), (40, 40, 33), (9, 300, 5), (5, 7, 3), (1, 1, 1),
+                                   (130, 129, 11)])
+def test_multi_tile_and_ragged(H, W, K):
+    model = models.bulge_disk()
+    par, data, sigma, mask, psf = synth(model, 2, H, W, K, seed=H + W + K)
+    img = gm.gm_render(model, dev(par), H, W, dev(psf))
+    assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
+    # a handful of pixels gives no averaging: chi^2 inherits 2 eps_pixel M / rho of a
+    # single fp32 pixel, so degenerate cutouts get 1e-4
+    assert_chi2(chi2, oc, rtol=1e-5 if H * W >= 64 else 1e-4)
+    assert_grad(grad, og)
+
+
+def test_psf_orientation_not_flipped_or_transposed():
+    # a delta PSF off centre must shift the model the way the oracle does
+    model = models.single_sersic()
+    H = W = 24
+    par = np.array([[12.3, 11.6, 1.0, 3.0, 1.5, 0.6, 0.8]], dtype=np.float32)
+    psf = np.zeros((5, 5), dtype=np.float32); psf[1, 4] = 1.0
+    img = gm.gm_render(model, dev(par), H, W, dev(psf)).cpu().numpy()
+    assert_pixels(img, oracle.render(model, par, H, W, psf))
+
+
+def test_shared_and_per_galaxy_psf_agree_bitwise():
+    model = models.single_sersic()
+    b = configs.make_batch(0, range(4), oracle_render)
+    rep = np.ascontiguousarray(np.broadcast_to(b["psf"], (4, 15, 15)))
+    a = gm.gm_render(model, dev(b["start"]), 64, 64, dev(b["psf"]))
+    c = gm.gm_render(model, dev(b["start"]), 64, 64, dev(rep))
+    assert torch.equal(a, c)
+
+
+# ---- mask / sigma properties on the GPU (reading X1) -------------------------------
+def test_mask_properties():
+    model = models.single_sersic()
+    par, data, sigma, mask, psf = synth(model, 2, 32, 32, 9, seed=3)
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    z, gz = run_loss_grad(model, par, data, sigma, np.zeros_like(mask), psf)
+    assert not z.any() and not gz.any()
+    bad = data.copy(); bs = sigma.copy()
+    i, j = np.argwhere(mask[0] == 0)[0]
+    bad[0, i, j] = np.nan; bs[0, i, j] = 0.0
+    cn, gn = run_loss_grad(model, par, bad, bs, mask, psf)
+    assert np.array_equal(cn, chi2) and np.array_equal(gn, grad)
+    c_none, _ = run_loss_grad(model, par, data, sigma, None, psf)
+    c_ones, _ = run_loss_grad(model, par, data, sigma, np.ones_like(mask), psf)
+    assert np.array_equal(c_none, c_ones)
+    oc, _ = oracle.loss_grad(model, par, data, sigma, None, psf)
+    assert_chi2(c_none, oc)
+
+
+def test_centre_on_pixel_centre_S4():
+    model = models.single_sersic()
+    H = W = 16
+    psf = asymmetric_psf(5).astype(np.float32)
+    par = np.array([[8.5, 7.5, 1.0, 3.0, 4.0, 0.7, 0.3], [8.5, 7.5, 1.0, 3.0, 1.2, 1.0, 0.0]], dtype=np.float32)
+    M = oracle.render(model, par, H, W, psf)
+    img = gm.gm_render(model, dev(par), H, W, dev(psf)).cpu().numpy()
+    assert np.isfinite(img).all()
+    assert_pixels(img, M)
+    sigma = np.full((2, H, W), 0.1, dtype=np.float32)
+    data = (M * 1.1).astype(np.float32)
+    chi2, grad = run_loss_grad(model, par, data, sigma, None, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, None, psf)
+    assert np.isfinite(grad).all()
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+
+
+def test_results_are_deterministic():
+    b = configs.make_batch(0, range(8), oracle_render)
+    a1 = run_loss_grad(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"])
+    a2 = run_loss_grad(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"])
+    assert np.array_equal(a1[0], a2[0]) and np.array_equal(a1[1], a2[1])
+
+
+# ---- host-buffer entry points agree with the device ones ------------------------------
+def test_host_entry_points():
+    b = configs.make_batch(0, range(5), oracle_render)
+    model = b["model"]
+    img_h = gm.gm_render_host(model, b["start"], 64, 64, b["psf"])
+    img_d = gm.gm_render(model, dev(b["start"]), 64, 64, dev(b["psf"])).cpu().numpy()
+    assert np.array_equal(img_h, img_d)
+    c_h, g_h = gm.gm_loss_grad_host(model, b["start"], b["data"], b["sigma"], None, b["psf"])
+    c_d, g_d = run_loss_grad(model, b["start"], b["data"], b["sigma"], None, b["psf"])
+    assert np.array_equal(c_h, c_d) and np.array_equal(g_h, g_d)
