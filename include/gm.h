@@ -180,6 +180,17 @@ const char* gm_last_cuda_error_string(void);
  * caller (bench.py "gpu_launches") count launches without a profiler */
 int64_t     gm_last_launch_count(void);
 
+
+/* ---- measurement hooks (used by bench.py for the roofline line) ---------------- */
+/* While enabled, every launch of the two tile kernels (forward: render + PSF
+ * convolution + residual; backward: adjoint convolution + gradient sums) is
+ * bracketed by CUDA events recorded on the launching stream (at most 8192 launches
+ * are kept).  gm_profile_read waits for them, returns the summed durations in
+ * milliseconds (ms[0] forward, ms[1] backward) and the launch counts, and clears
+ * the list.  Off by default; enabling or disabling also clears it. */
+int gm_profile_enable(int on);
+int gm_profile_read(double* ms /* host [2] */, int64_t* count /* host [2] */);
+
 #ifdef __cplusplus
 }
 #endif

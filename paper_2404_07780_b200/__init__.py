@@ -11,6 +11,8 @@ from .binding import (  # noqa: F401
     gm_last_launch_count,
     gm_loss_grad,
     gm_loss_grad_host,
+    gm_profile_enable,
+    gm_profile_read,
     gm_render,
     gm_render_host,
     gm_strerror,

@@ -84,6 +84,9 @@ def _lib():
         L.gm_last_cuda_error.restype = i; L.gm_last_cuda_error.argtypes = []
         L.gm_last_cuda_error_string.restype = C.c_char_p; L.gm_last_cuda_error_string.argtypes = []
         L.gm_last_launch_count.restype = C.c_int64; L.gm_last_launch_count.argtypes = []
+        L.gm_profile_enable.restype = i; L.gm_profile_enable.argtypes = [i]
+        L.gm_profile_read.restype = i
+        L.gm_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         _handle = L
     return _handle
 
@@ -179,6 +182,17 @@ def gm_strerror(status: int) -> str:
 
 def gm_last_launch_count() -> int:
     return int(_lib().gm_last_launch_count())
+
+
+def gm_profile_enable(on: bool) -> None:
+    _check(_lib().gm_profile_enable(1 if on else 0), "gm_profile_enable")
+
+
+def gm_profile_read():
+    """-> {"forward": (ms, launches), "backward": (ms, launches)} since the last read."""
+    ms = (C.c_double * 2)(); n = (C.c_int64 * 2)()
+    _check(_lib().gm_profile_read(ms, n), "gm_profile_read")
+    return {"forward": (ms[0], int(n[0])), "backward": (ms[1], int(n[1]))}
 
 
 def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) -> int:

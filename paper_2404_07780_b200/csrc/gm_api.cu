@@ -24,6 +24,38 @@ static thread_local int64_t t_launches = 0;
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// optional per-launch timing of the two tile kernels with CUDA events recorded on
+// the launching stream (gm_profile_enable / gm_profile_read); off by default
+struct Profiler {
+  static constexpr int kCap = 8192;
+  bool on = false;
+  int n = 0;
+  cudaEvent_t ev[kCap][2] = {};
+  uint8_t kind[kCap] = {};
+  int created = 0;
+  std::mutex mu;
+};
+static Profiler g_prof;
+
+static int prof_begin(int kind, cudaStream_t st) {
+  if (!g_prof.on) return -1;
+  std::lock_guard<std::mutex> lk(g_prof.mu);
+  if (g_prof.n >= Profiler::kCap) return -1;
+  const int i = g_prof.n;
+  if (i >= g_prof.created) {
+    if (cudaEventCreate(&g_prof.ev[i][0]) != cudaSuccess || cudaEventCreate(&g_prof.ev[i][1]) != cudaSuccess)
+      return -1;
+    g_prof.created = i + 1;
+  }
+  g_prof.kind[i] = (uint8_t)kind;
+  g_prof.n = i + 1;
+  cudaEventRecord(g_prof.ev[i][0], st);
+  return i;
+}
+static void prof_end(int i, cudaStream_t st) {
+  if (i >= 0) cudaEventRecord(g_prof.ev[i][1], st);
+}
+
 // ---------------------------------------------------------------------------
 // small kernels: PSF padding, prologue, gradient assembly, fit state
 // ---------------------------------------------------------------------------
@@ -322,6 +354,7 @@ GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33
 static int dispatch_forward(int KP, const FwdArgs& a, bool render, int B, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
+  const int pi = prof_begin(0, st);
   switch (KP) {
     case 5: rc = launch_forward_5(a, render, B, st, &err); break;
     case 9: rc = launch_forward_9(a, render, B, st, &err); break;
@@ -332,6 +365,7 @@ static int dispatch_forward(int KP, const FwdArgs& a, bool render, int B, cudaSt
     case 41: rc = launch_forward_41(a, render, B, st, &err); break;
     default: return GM_ENOTSUP;
   }
+  prof_end(pi, st);
   if (rc == GM_OK) ++t_launches;
   if (rc == GM_ECUDA) t_last_err = err;
   return rc;
@@ -340,6 +374,7 @@ static int dispatch_forward(int KP, const FwdArgs& a, bool render, int B, cudaSt
 static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
+  const int pi = prof_begin(1, st);
   switch (KP) {
     case 5: rc = launch_backward_5(a, B, st, &err); break;
     case 9: rc = launch_backward_9(a, B, st, &err); break;
@@ -350,6 +385,7 @@ static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
     case 41: rc = launch_backward_41(a, B, st, &err); break;
     default: return GM_ENOTSUP;
   }
+  prof_end(pi, st);
   if (rc == GM_OK) ++t_launches;
   if (rc == GM_ECUDA) t_last_err = err;
   return rc;
@@ -647,6 +683,29 @@ const char* gm_strerror(int status) {
     case GM_EWORKSPACE: return "workspace missing, misaligned or too small";
     default: return "unknown status";
   }
+}
+
+int gm_profile_enable(int on) {
+  std::lock_guard<std::mutex> lk(g_prof.mu);
+  g_prof.on = on != 0;
+  g_prof.n = 0;
+  return GM_OK;
+}
+
+int gm_profile_read(double* ms, int64_t* count) {
+  if (!ms || !count) return GM_EINVAL;
+  std::lock_guard<std::mutex> lk(g_prof.mu);
+  ms[0] = ms[1] = 0.0;
+  count[0] = count[1] = 0;
+  for (int i = 0; i < g_prof.n; ++i) {
+    GM_CUDA(cudaEventSynchronize(g_prof.ev[i][1]));
+    float t = 0.0f;
+    GM_CUDA(cudaEventElapsedTime(&t, g_prof.ev[i][0], g_prof.ev[i][1]));
+    ms[g_prof.kind[i]] += t;
+    count[g_prof.kind[i]] += 1;
+  }
+  g_prof.n = 0;
+  return GM_OK;
 }
 
 int gm_version(void) { return GM_VERSION; }
