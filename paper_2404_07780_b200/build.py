@@ -20,8 +20,9 @@ LIB = PKG / "libgm.so"
 INCLUDE = PKG.parent / "include"
 
 KS = (5, 9, 15, 21, 25, 33, 41)          # keep in sync with kCompiledK in gm_api.cu
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC"]
+EXTRA = os.environ.get("GM_NVCC_EXTRA", "").split()
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++20",
+              "-Xcompiler", "-fPIC", *EXTRA]
 
 
 def _nvcc() -> str:
@@ -35,6 +36,7 @@ def _stamp() -> str:
     h = hashlib.sha256()
     for p in sorted(list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + [INCLUDE / "gm.h", Path(__file__)]):
         h.update(p.name.encode()); h.update(p.read_bytes())
+    h.update(" ".join(EXTRA).encode())
     return h.hexdigest()
 
 

@@ -8,8 +8,10 @@
 #include <cstring>
 #include <limits>
 #include <mutex>
+#include <vector>
 
 #include "gm_kernels.cuh"
+#include "gm_prologue.cuh"
 
 namespace gm {
 
@@ -57,6 +59,36 @@ static void prof_end(int i, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------------------
+// nu_n table (gm_device.cuh): built once per process on the host with the exact
+// fp64 solver, uploaded once per device into the g_nu_table symbol.
+// ---------------------------------------------------------------------------
+static int ensure_nu_table(cudaStream_t st) {
+  static std::mutex mu;
+  static std::vector<double2> host_table;
+  static bool uploaded[64] = {};
+  int dev = 0;
+  GM_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GM_ENOTSUP;
+  std::lock_guard<std::mutex> lk(mu);
+  if (uploaded[dev]) return GM_OK;
+  if (host_table.empty()) {
+    host_table.resize(kNuTableN + 1);
+    const double h = (kNuTableS1 - kNuTableS0) / kNuTableN;
+    for (int i = 0; i <= kNuTableN; ++i) {
+      const double n = std::exp(kNuTableS0 + h * i);
+      double nu, dnu;
+      sersic_nu_exact(n, &nu, &dnu);
+      host_table[i] = make_double2(nu, dnu * n);         // (nu, d nu / d ln n)
+    }
+  }
+  // synchronous copy: later launches on any stream see the table
+  (void)st;
+  GM_CUDA(cudaMemcpyToSymbol(g_nu_table, host_table.data(), sizeof(double2) * (kNuTableN + 1)));
+  uploaded[dev] = true;
+  return GM_OK;
+}
+
+// ---------------------------------------------------------------------------
 // small kernels: PSF padding, prologue, gradient assembly, fit state
 // ---------------------------------------------------------------------------
 __global__ void k_pad_psf(const float* __restrict__ psf, long long stride, int n_psf, int K, int KP,
@@ -71,6 +103,22 @@ __global__ void k_pad_psf(const float* __restrict__ psf, long long stride, int n
   float v = 0.0f;
   if (aa >= 0 && aa < K && bb >= 0 && bb < K) v = psf[(long long)p * stride + aa * K + bb];
   out[idx] = v;
+}
+
+// paired taps for both convolutions of every PSF: out[p][0] = flipped (forward),
+// out[p][1] = as given (adjoint); each (KP+1) x (KP+1) float2 (see gm_kernels.cuh)
+__global__ void k_make_taps(const float* __restrict__ psf, long long stride, int n_psf, int KP,
+                            float2* __restrict__ out) {
+  const int TP = KP + 1;
+  const int per = (KP + 1) * TP;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_psf * 2 * per) return;
+  const int p = idx / (2 * per);
+  const int r = idx - p * 2 * per;
+  const int which = r / per, e = r - which * per;
+  const int row = e / TP, t = e - row * TP;
+  const float* src = psf + (long long)p * stride;
+  out[idx] = which == 0 ? tap_pair<true>(src, KP, row, t) : tap_pair<false>(src, KP, row, t);
 }
 
 __global__ void k_prologue(const ModelDesc md, int B, const float* __restrict__ params,
@@ -304,6 +352,7 @@ static TileGeom make_geom(int H, int W, int KP) {
   const int win = ((kTC + KP - 1) + 3) / 4 * 4;            // floats read per thread window row
   tg.pitch = (tg.TW - kTC + win + 3) / 4 * 4;
   tg.rows = tg.TH + KP - 1;
+  tg.vec = 0;
   return tg;
 }
 
@@ -313,6 +362,7 @@ struct Workspace {
   float* chi2_part;
   float* grad_part;
   float* psf_pad;
+  float2* taps;
   float *u, *m, *s, *p_prev, *chi2_prev;
   int *calm, *frozen;
   size_t total;
@@ -333,6 +383,7 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   w.grad_part = (float*)take(B * tiles * md.n_comp * kNSum * 4);
   const size_t n_psf = bt->psf_stride == 0 ? 1 : B;
   w.psf_pad = (float*)take(KP != bt->K ? n_psf * KP * KP * 4 : 0);
+  w.taps = (float2*)take(n_psf * 2 * (size_t)(KP + 1) * (KP + 1) * sizeof(float2));
   w.u = (float*)take(B * P * 4);
   w.m = (float*)take(B * P * 4);
   w.s = (float*)take(B * P * 4);
@@ -398,6 +449,7 @@ struct Plan {
   Workspace ws;
   int KP;
   const float* psf; long long psf_stride;
+  const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int tiles;
 };
 
@@ -423,11 +475,24 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
     pl->psf = pl->ws.psf_pad;
     pl->psf_stride = bt->psf_stride == 0 ? 0 : (long long)pl->KP * pl->KP;
   }
+  {
+    const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
+    const int per = (pl->KP + 1) * (pl->KP + 1);
+    const long long n = (long long)n_psf * 2 * per;
+    k_make_taps<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pl->psf, pl->psf_stride, n_psf, pl->KP, pl->ws.taps);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+    pl->taps_fwd = pl->ws.taps;
+    pl->taps_adj = pl->ws.taps + per;
+    pl->taps_stride = bt->psf_stride == 0 ? 0 : 2ll * per;
+  }
   return GM_OK;
 }
 
 static int run_prologue(const Plan& pl, int B, const float* params, const int* frozen, cudaStream_t st) {
   const int n = B * pl.md.n_comp;
+  int rc = ensure_nu_table(st);
+  if (rc != GM_OK) return rc;
   k_prologue<<<(n + 127) / 128, 128, 0, st>>>(pl.md, B, params, pl.ws.cc, frozen);
   ++t_launches;
   GM_CUDA(cudaGetLastError());
@@ -437,7 +502,9 @@ static int run_prologue(const Plan& pl, int B, const float* params, const int* f
 static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const int* frozen) {
   FwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
-  a.psf = pl.psf; a.psf_stride = pl.psf_stride;
+  const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
+  a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
+  a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part; a.frozen = frozen;
   return a;
@@ -446,7 +513,7 @@ static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const in
 static BwdArgs bwd_args(const Plan& pl, const int* frozen) {
   BwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
-  a.psf = pl.psf; a.psf_stride = pl.psf_stride;
+  a.taps = pl.taps_adj; a.taps_stride = pl.taps_stride;
   a.G = pl.ws.G; a.grad_part = pl.ws.grad_part; a.frozen = frozen;
   return a;
 }

@@ -25,6 +25,11 @@ namespace gm {
 
 constexpr int kTR = 8, kTC = 8;            // thread tile (rows x cols)
 constexpr int kNSum = 8;                   // partial sums per component
+#ifdef GM_FAST_FORWARD
+constexpr bool kFastForward = true;        // experiment: SFU approximations in the forward render
+#else
+constexpr bool kFastForward = false;
+#endif
 
 struct TileGeom {
   int H, W;                // cutout
@@ -33,13 +38,14 @@ struct TileGeom {
   int ntx, nty;            // thread tiles per CTA tile
   int pitch;               // shared row pitch (floats), multiple of 4
   int rows;                // TH + K - 1
+  int vec;                 // 1: W % 4 == 0 and data/sigma/mask/out aligned for 128-bit access
 };
 
 struct FwdArgs {
   ModelDesc md;
   TileGeom tg;
   const CompConst* cc;     // [B, n_comp]
-  const float* psf; long long psf_stride;
+  const float2* taps; long long taps_stride;   // paired flipped taps, float2 per galaxy (0 = shared)
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                // [B,H,W] workspace (or model_out when RENDER)
   float* chi2_part;        // [B, tiles]
@@ -50,7 +56,7 @@ struct BwdArgs {
   ModelDesc md;
   TileGeom tg;
   const CompConst* cc;
-  const float* psf; long long psf_stride;
+  const float2* taps; long long taps_stride;   // paired unflipped taps
   const float* G;          // [B,H,W]
   float* grad_part;        // [B, tiles, n_comp, 8]
   const int* frozen;
@@ -63,22 +69,18 @@ template <int K> struct ConvCfg {
   static constexpr int kInRows = kTR + K - 1;
 };
 
-// paired taps: T2[a][t] = (P[a][t], P[a-1][t]), a = 0..K, P[-1] = P[K] = 0.
-// FLIP selects the flipped PSF (true convolution) or the PSF itself (adjoint).
-template <int K, bool FLIP>
-__device__ __forceinline__ void load_tap_pairs(float2* taps, const float* __restrict__ psf, int tid,
-                                               int nthreads) {
-  constexpr int TP = ConvCfg<K>::kTapPitch;
-  for (int idx = tid; idx < (K + 1) * TP; idx += nthreads) {
-    const int a = idx / TP, t = idx - a * TP;
-    float lo = 0.0f, hi = 0.0f;
-    if (t < K) {
-      const int tt = FLIP ? (K - 1 - t) : t;
-      if (a < K) lo = psf[(FLIP ? (K - 1 - a) : a) * K + tt];
-      if (a >= 1) hi = psf[(FLIP ? (K - a) : (a - 1)) * K + tt];
-    }
-    taps[idx] = make_float2(lo, hi);
+// paired taps: T2[a][t] = (P[a][t], P[a-1][t]), a = 0..K, t = 0..K (column K is a zero
+// pad), P[-1] = P[K] = 0.  FLIP selects the flipped PSF (true convolution, R:C1) or the
+// PSF itself (adjoint, R:C2).  Built once per call by k_make_taps (gm_api.cu).
+template <bool FLIP>
+__device__ __forceinline__ float2 tap_pair(const float* __restrict__ psf, int K, int a, int t) {
+  float lo = 0.0f, hi = 0.0f;
+  if (t < K) {
+    const int tt = FLIP ? (K - 1 - t) : t;
+    if (a < K) lo = psf[(FLIP ? (K - 1 - a) : a) * K + tt];
+    if (a >= 1) hi = psf[(FLIP ? (K - a) : (a - 1)) * K + tt];
   }
+  return make_float2(lo, hi);
 }
 
 // 8x8 outputs per thread.  win points at the thread's window origin in the shared
@@ -120,6 +122,29 @@ __device__ __forceinline__ void conv8x8(const float* __restrict__ win, int pitch
       }
     }
   }
+}
+
+// cp.async with zero fill: copies `bytes` (4 or 16) when valid, writes zeros otherwise
+__device__ __forceinline__ void cp_async_zfill4(float* dst, const float* src, bool valid) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(dst);
+  const int n = valid ? 4 : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(sa), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_zfill16(float* dst, const float* src, bool valid) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(dst);
+  const int n = valid ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+// (K+1) x (K+1) float2 of paired taps, global -> shared, 16 bytes per cp.async
+template <int K>
+__device__ __forceinline__ void copy_taps(float2* dst, const float2* __restrict__ src, int tid, int nthr) {
+  constexpr int n16 = (K + 1) * ConvCfg<K>::kTapPitch / 2;
+  for (int i = tid; i < n16; i += nthr)
+    cp_async_zfill16(reinterpret_cast<float*>(dst) + 4 * i, reinterpret_cast<const float*>(src) + 4 * i, true);
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -169,32 +194,38 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
   float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
 
-  load_tap_pairs<K, true>(taps, a.psf + (long long)b * a.psf_stride, tid, nthr);
+  copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 
-  // a1: S on the tile plus its halo; zero outside the cutout (R:C1) and in the pad
+  // a1: S on the tile plus its halo; zero outside the cutout (R:C1) and in the pad.
+  // One pass per convolved component, its radial law selected outside the pixel loops.
   const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
   const int cols = tg.TW + K - 1;
-  for (int yy = wid; yy < tg.rows; yy += nwarps) {
-    const int i = i0 - h + yy;
-    float* rowp = tilebuf + (size_t)yy * tg.pitch;
-    const bool row_in = (i >= 0 && i < tg.H);
-    const float y = (float)tg.H - 0.5f - (float)i;       // R:G1
-    for (int xx = lane; xx < tg.pitch; xx += 32) {
-      const int j = j0 - h + xx;
-      float s = 0.0f;
-      if (row_in && xx < cols && j >= 0 && j < tg.W) {
-        const float x = (float)j + 0.5f;
-        for (int c = 0; c < a.md.n_comp; ++c) {
-          if (a.md.conv[c]) {
-            const CompConst cc = ccb[c];
-            const Geo g = geometry(cc, x, y);
-            s = fmaf(cc.amp, profile_value(a.md.kind[c], cc, g.r), s);
-          }
+  bool first = true;
+  for (int c = 0; c <= a.md.n_comp; ++c) {
+    const bool zero_pass = (c == a.md.n_comp);
+    if (zero_pass && !first) break;                    // at least one component wrote the tile
+    if (!zero_pass && !a.md.conv[c]) continue;
+    const CompConst cc = ccb[zero_pass ? 0 : c];
+    dispatch_kind(zero_pass ? (int)GM_SKY : a.md.kind[c], [&]<int KIND>() {
+      for (int yy = wid; yy < tg.rows; yy += nwarps) {
+        const int i = i0 - h + yy;
+        float* rowp = tilebuf + (size_t)yy * tg.pitch;
+        const bool row_in = (i >= 0 && i < tg.H);
+        const float y = (float)tg.H - 0.5f - (float)i;   // R:G1
+        for (int xx = lane; xx < tg.pitch; xx += 32) {
+          const int j = j0 - h + xx;
+          const bool in = row_in && xx < cols && j >= 0 && j < tg.W;
+          float s = 0.0f;
+          if (KIND != GM_SKY && in)
+            s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry(cc, (float)j + 0.5f, y).r);
+          if (first) rowp[xx] = s;
+          else if (in) rowp[xx] += s;
         }
       }
-      rowp[xx] = s;
-    }
+    });
+    first = false;
   }
+  cp_async_wait_all();
   __syncthreads();
 
   // a2: M = PSF (*) S on this thread's 8x8 block
@@ -216,36 +247,91 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
   // a3: unconvolved components, residual, chi2, back-seed G
   float chi2 = 0.0f;
   const size_t img = (size_t)b * tg.H * tg.W;
-  for (int yy = wid; yy < tg.TH; yy += nwarps) {
-    const int i = i0 + yy;
-    if (i >= tg.H) break;
-    const float y = (float)tg.H - 0.5f - (float)i;
-    for (int xx = lane; xx < tg.TW; xx += 32) {
-      const int j = j0 + xx;
-      if (j >= tg.W) break;
-      float m = tilebuf[(size_t)yy * tg.pitch + xx];
-      const float x = (float)j + 0.5f;
-      for (int c = 0; c < a.md.n_comp; ++c) {
-        if (a.md.conv[c]) continue;
-        const CompConst cc = ccb[c];
-        const int kind = a.md.kind[c];
-        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
-        m = fmaf(cc.amp, U, m);
-      }
-      const size_t off = img + (size_t)i * tg.W + j;
-      if (RENDER) {
-        a.G[off] = m;
-      } else {
-        const bool used = a.mask ? (a.mask[off] != 0) : true;
-        float g = 0.0f;
-        if (used) {                                      // select, never multiply by 0 (R:X1)
-          const float sg = a.sigma[off];
-          const float w = __frcp_rn(sg * sg);
-          const float rho = a.data[off] - m;
-          chi2 = fmaf(w * rho, rho, chi2);
-          g = -2.0f * w * rho;
+  bool any_unconv = false;
+  for (int c = 0; c < a.md.n_comp; ++c) any_unconv |= (a.md.conv[c] == 0);
+  auto add_unconv = [&](float m, float x, float y) {
+    for (int c = 0; c < a.md.n_comp; ++c) {
+      if (a.md.conv[c]) continue;
+      const CompConst cc = ccb[c];
+      const int kind = a.md.kind[c];
+      const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
+      m = fmaf(cc.amp, U, m);
+    }
+    return m;
+  };
+  auto residual = [&](float m, float d, float sg, bool used, float& g) {
+    g = 0.0f;
+    if (used) {                                        // select, never multiply by 0 (R:X1)
+      const float w = __fdividef(1.0f, sg * sg);
+      const float rho = d - m;
+      chi2 = fmaf(w * rho, rho, chi2);
+      g = -2.0f * w * rho;
+    }
+  };
+  if (tg.vec) {
+    // 128-bit path: one lane = 4 consecutive pixels, two rows per warp in flight
+    for (int yy = wid; yy < tg.TH; yy += 2 * nwarps) {
+      float4 m4[2], d4[2], s4[2];
+      uchar4 k4[2];
+      bool ok[2];
+      size_t off[2];
+      const int xx = lane * 4;
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int yr = yy + u * nwarps;
+        const int i = i0 + yr, j = j0 + xx;
+        ok[u] = (yr < tg.TH) && (i < tg.H) && (xx < tg.TW) && (j < tg.W);
+        off[u] = img + (size_t)i * tg.W + j;
+        if (ok[u]) {
+          m4[u] = *reinterpret_cast<const float4*>(tilebuf + (size_t)yr * tg.pitch + xx);
+          if (!RENDER) {
+            d4[u] = *reinterpret_cast<const float4*>(a.data + off[u]);
+            s4[u] = *reinterpret_cast<const float4*>(a.sigma + off[u]);
+            k4[u] = a.mask ? *reinterpret_cast<const uchar4*>(a.mask + off[u]) : make_uchar4(1, 1, 1, 1);
+          }
         }
-        a.G[off] = g;
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        if (!ok[u]) continue;
+        if (any_unconv) {
+          const float y = (float)tg.H - 0.5f - (float)(i0 + yy + u * nwarps);
+          const float x = (float)(j0 + xx) + 0.5f;
+          m4[u].x = add_unconv(m4[u].x, x, y);
+          m4[u].y = add_unconv(m4[u].y, x + 1.0f, y);
+          m4[u].z = add_unconv(m4[u].z, x + 2.0f, y);
+          m4[u].w = add_unconv(m4[u].w, x + 3.0f, y);
+        }
+        if (RENDER) {
+          *reinterpret_cast<float4*>(a.G + off[u]) = m4[u];
+        } else {
+          float4 g;
+          residual(m4[u].x, d4[u].x, s4[u].x, k4[u].x != 0, g.x);
+          residual(m4[u].y, d4[u].y, s4[u].y, k4[u].y != 0, g.y);
+          residual(m4[u].z, d4[u].z, s4[u].z, k4[u].z != 0, g.z);
+          residual(m4[u].w, d4[u].w, s4[u].w, k4[u].w != 0, g.w);
+          *reinterpret_cast<float4*>(a.G + off[u]) = g;
+        }
+      }
+    }
+  } else {
+    for (int yy = wid; yy < tg.TH; yy += nwarps) {
+      const int i = i0 + yy;
+      if (i >= tg.H) break;
+      const float y = (float)tg.H - 0.5f - (float)i;
+      for (int xx = lane; xx < tg.TW; xx += 32) {
+        const int j = j0 + xx;
+        if (j >= tg.W) break;
+        float m = tilebuf[(size_t)yy * tg.pitch + xx];
+        if (any_unconv) m = add_unconv(m, (float)j + 0.5f, y);
+        const size_t o = img + (size_t)i * tg.W + j;
+        if (RENDER) {
+          a.G[o] = m;
+        } else {
+          float g;
+          residual(m, a.data[o], a.sigma[o], a.mask ? (a.mask[o] != 0) : true, g);
+          a.G[o] = g;
+        }
       }
     }
   }
@@ -284,22 +370,39 @@ __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
   float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
 
-  load_tap_pairs<K, false>(taps, a.psf + (long long)b * a.psf_stride, tid, nthr);
+  copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 
-  // G tile + halo, zero outside the cutout
+  // G tile + halo through cp.async (no register staging, all copies in flight at
+  // once); zero outside the cutout (R:C2) and in the pad columns
   const float* Gb = a.G + (size_t)b * tg.H * tg.W;
-  const int cols = tg.TW + K - 1;
-  for (int yy = wid; yy < tg.rows; yy += nwarps) {
-    const int i = i0 - h + yy;
-    float* rowp = tilebuf + (size_t)yy * tg.pitch;
-    const bool row_in = (i >= 0 && i < tg.H);
-    for (int xx = lane; xx < tg.pitch; xx += 32) {
-      const int j = j0 - h + xx;
-      float s = 0.0f;
-      if (row_in && xx < cols && j >= 0 && j < tg.W) s = Gb[(size_t)i * tg.W + j];
-      rowp[xx] = s;
+  const bool vec16 = ((tg.W & 3) == 0) && ((h & 3) == 0);
+  if (vec16) {
+    const int chunks = tg.pitch >> 2;
+    for (int yy = wid; yy < tg.rows; yy += nwarps) {
+      const int i = i0 - h + yy;
+      float* rowp = tilebuf + (size_t)yy * tg.pitch;
+      const bool row_in = (i >= 0 && i < tg.H);
+      const float* src_row = Gb + (size_t)(row_in ? i : 0) * tg.W;
+      for (int ch = lane; ch < chunks; ch += 32) {
+        const int j = j0 - h + 4 * ch;
+        const bool ok = row_in && j >= 0 && j < tg.W;
+        cp_async_zfill16(rowp + 4 * ch, src_row + (ok ? j : 0), ok);
+      }
+    }
+  } else {
+    for (int yy = wid; yy < tg.rows; yy += nwarps) {
+      const int i = i0 - h + yy;
+      float* rowp = tilebuf + (size_t)yy * tg.pitch;
+      const bool row_in = (i >= 0 && i < tg.H);
+      const float* src_row = Gb + (size_t)(row_in ? i : 0) * tg.W;
+      for (int xx = lane; xx < tg.pitch; xx += 32) {
+        const int j = j0 - h + xx;
+        const bool ok = row_in && j >= 0 && j < tg.W;
+        cp_async_zfill4(rowp + xx, src_row + (ok ? j : 0), ok);
+      }
     }
   }
+  cp_async_wait_all();
   __syncthreads();
 
   const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
@@ -325,36 +428,36 @@ __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
 #pragma unroll
     for (int k = 0; k < kNSum; ++k) s[k] = 0.0f;
     const CompConst cc = ccb[c];
-    const int kind = a.md.kind[c];
     const bool conv = a.md.conv[c] != 0;
-    for (int yy = wid; yy < tg.TH; yy += nwarps) {
-      const int i = i0 + yy;
-      if (i >= tg.H) break;
-      const float y = (float)tg.H - 0.5f - (float)i;
-      for (int xx = lane; xx < tg.TW; xx += 32) {
-        const int j = j0 + xx;
-        if (j >= tg.W) break;
-        const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
-        if (kind == GM_SKY) { s[4] += seed; continue; }
-        const float x = (float)j + 0.5f;
-        const Geo g = geometry(cc, x, y);
-        const float rg = fmaxf(g.r, kRGuard);
-        float U, dUdr, d0, d1, d2;
-        profile_grad(kind, cc, rg, U, dUdr, d0, d1, d2);
-        // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
-        const float Uv = (g.r < kRGuard) ? profile_value(kind, cc, g.r) : U;
-        const float sa = seed * cc.amp;
-        const float cgeo = __fdividef(sa * dUdr, rg);
-        s[0] = fmaf(cgeo, g.u, s[0]);
-        s[1] = fmaf(cgeo, g.vq, s[1]);
-        s[2] = fmaf(cgeo * g.u, g.vq, s[2]);
-        s[3] = fmaf(cgeo * g.vq, g.vq, s[3]);
-        s[4] = fmaf(seed, Uv, s[4]);
-        s[5] = fmaf(sa, d0, s[5]);
-        s[6] = fmaf(sa, d1, s[6]);
-        s[7] = fmaf(sa, d2, s[7]);
+    dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+      for (int yy = wid; yy < tg.TH; yy += nwarps) {
+        const int i = i0 + yy;
+        if (i >= tg.H) break;
+        const float y = (float)tg.H - 0.5f - (float)i;
+        for (int xx = lane; xx < tg.TW; xx += 32) {
+          const int j = j0 + xx;
+          if (j >= tg.W) break;
+          const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
+          if (KIND == GM_SKY) { s[4] += seed; continue; }
+          const Geo g = geometry(cc, (float)j + 0.5f, y);
+          const float rg = fmaxf(g.r, kRGuard);
+          float U, dUdr, d0, d1, d2;
+          profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
+          // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
+          const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+          const float sa = seed * cc.amp;
+          const float cgeo = __fdividef(sa * dUdr, rg);
+          s[0] = fmaf(cgeo, g.u, s[0]);
+          s[1] = fmaf(cgeo, g.vq, s[1]);
+          s[2] = fmaf(cgeo * g.u, g.vq, s[2]);
+          s[3] = fmaf(cgeo * g.vq, g.vq, s[3]);
+          s[4] = fmaf(seed, Uv, s[4]);
+          s[5] = fmaf(sa, d0, s[5]);
+          s[6] = fmaf(sa, d1, s[6]);
+          s[7] = fmaf(sa, d2, s[7]);
+        }
       }
-    }
+    });
 #pragma unroll
     for (int k = 0; k < kNSum; ++k) {
       const float v = warp_sum(s[k]);
