@@ -287,11 +287,20 @@ def run_ours(args):
     flops_per_launch = 2.0 * B * H * W * K * K                     # one K^2-tap convolution of the batch
     kern = {}
     for name, (ms, n) in prof.items():
-        if n:
-            avg = ms / n
-            kern[name] = {"launches": n, "avg_ms": avg, "tflops": flops_per_launch / (avg * 1e-3) / 1e12,
-                          "share_of_step": ms / t_ms if world == 1 else None}
-    dom = max(kern, key=lambda k: kern[k]["avg_ms"]) if kern else None
+        if not n:
+            continue
+        avg = ms / n
+        if name == "fused":
+            # per step: n_iter launches with both convolutions + the closing chi^2-only launch
+            flops = args.steps * (2 * n_iter + 1) * flops_per_launch
+            convs = (2 * n_iter + 1) / (n_iter + 1)
+        else:
+            flops = n * flops_per_launch
+            convs = 1
+        kern[name] = {"launches": n, "avg_ms": avg, "convolutions_per_launch": convs,
+                      "tflops": flops / (ms * 1e-3) / 1e12,
+                      "share_of_step": ms / t_ms if world == 1 else None}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     traffic = None
     tf = ROOT / "profiles" / "traffic.json"
     if tf.exists():
@@ -304,7 +313,7 @@ def run_ours(args):
                     "peak_source": f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 flop x {f_mhz:.0f} MHz "
                                    f"(sm_max_mhz of {pk_src} MEASURED_PEAKS.json; an FFMA2 loop measured "
                                    "36.8 TFMA/s = 73.7 TFLOP/s on this pool, DESIGN.md)",
-                    "algorithmic_flops_per_launch": flops_per_launch,
+                    "algorithmic_flops_per_launch": flops_per_launch * kern[dom]["convolutions_per_launch"],
                     "hbm_gbs_algorithmic": (B * H * W * (9 if b['mask'] is not None else 8)) /
                                            (kern[dom]["avg_ms"] * 1e-3) / 1e9,
                     "hbm_peak_gbs": pk.get("hbm_gbs"), "kernels": kern}

@@ -182,14 +182,16 @@ int64_t     gm_last_launch_count(void);
 
 
 /* ---- measurement hooks (used by bench.py for the roofline line) ---------------- */
-/* While enabled, every launch of the two tile kernels (forward: render + PSF
- * convolution + residual; backward: adjoint convolution + gradient sums) is
- * bracketed by CUDA events recorded on the launching stream (at most 8192 launches
- * are kept).  gm_profile_read waits for them, returns the summed durations in
- * milliseconds (ms[0] forward, ms[1] backward) and the launch counts, and clears
- * the list.  Off by default; enabling or disabling also clears it. */
+/* While enabled, every launch of the heavy kernels is bracketed by CUDA events
+ * recorded on the launching stream (at most 8192 launches are kept):
+ *   [0] forward tile kernel  (render + PSF convolution + residual)
+ *   [1] backward tile kernel (adjoint convolution + gradient sums)
+ *   [2] fused kernel         (all of the above for cutouts that fit one CTA)
+ * gm_profile_read waits for them, returns the summed durations in milliseconds and
+ * the launch counts per kind, and clears the list.  Off by default; enabling or
+ * disabling also clears it. */
 int gm_profile_enable(int on);
-int gm_profile_read(double* ms /* host [2] */, int64_t* count /* host [2] */);
+int gm_profile_read(double* ms /* host [3] */, int64_t* count /* host [3] */);
 
 #ifdef __cplusplus
 }

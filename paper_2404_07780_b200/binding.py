@@ -189,10 +189,10 @@ def gm_profile_enable(on: bool) -> None:
 
 
 def gm_profile_read():
-    """-> {"forward": (ms, launches), "backward": (ms, launches)} since the last read."""
-    ms = (C.c_double * 2)(); n = (C.c_int64 * 2)()
+    """-> {"forward"|"backward"|"fused": (ms, launches)} since the last read."""
+    ms = (C.c_double * 3)(); n = (C.c_int64 * 3)()
     _check(_lib().gm_profile_read(ms, n), "gm_profile_read")
-    return {"forward": (ms[0], int(n[0])), "backward": (ms[1], int(n[1]))}
+    return {"forward": (ms[0], int(n[0])), "backward": (ms[1], int(n[1])), "fused": (ms[2], int(n[2]))}
 
 
 def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) -> int:

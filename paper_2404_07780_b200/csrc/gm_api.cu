@@ -5,12 +5,13 @@
 // device and returns GM_ECUDA without one.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <mutex>
 #include <vector>
 
-#include "gm_kernels.cuh"
+#include "gm_fused.cuh"
 #include "gm_prologue.cuh"
 
 namespace gm {
@@ -398,7 +399,8 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
 // per-K launchers live in gm_tiles.cu, compiled once per PSF side (-DGM_K=..)
 #define GM_DECL_K(K)                                                                          \
   int launch_forward_##K(const FwdArgs& a, bool render, int B, cudaStream_t st, cudaError_t* err); \
-  int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);
+  int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
+  int launch_fused_##K(const FusedArgs& a, int n_sm, size_t smem_limit, cudaStream_t st, cudaError_t* err);
 GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
 #undef GM_DECL_K
 
@@ -442,6 +444,46 @@ static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
   return rc;
 }
 
+static int dispatch_fused(int KP, const FusedArgs& a, int n_sm, size_t lim, cudaStream_t st) {
+  int rc;
+  cudaError_t err = cudaSuccess;
+  const int pi = prof_begin(2, st);
+  switch (KP) {
+    case 5: rc = launch_fused_5(a, n_sm, lim, st, &err); break;
+    case 9: rc = launch_fused_9(a, n_sm, lim, st, &err); break;
+    case 15: rc = launch_fused_15(a, n_sm, lim, st, &err); break;
+    case 21: rc = launch_fused_21(a, n_sm, lim, st, &err); break;
+    case 25: rc = launch_fused_25(a, n_sm, lim, st, &err); break;
+    case 33: rc = launch_fused_33(a, n_sm, lim, st, &err); break;
+    case 41: rc = launch_fused_41(a, n_sm, lim, st, &err); break;
+    default: return GM_ENOTSUP;
+  }
+  prof_end(pi, st);
+  if (rc == GM_OK) ++t_launches;
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+
+struct DevCaps { int n_sm; size_t smem_optin; };
+static int device_caps(DevCaps* out) {
+  static std::mutex mu;
+  static DevCaps caps[64];
+  static bool have[64] = {};
+  int dev = 0;
+  GM_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GM_ENOTSUP;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!have[dev]) {
+    int n = 0, s = 0;
+    GM_CUDA(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
+    GM_CUDA(cudaDeviceGetAttribute(&s, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    caps[dev] = {n, (size_t)s};
+    have[dev] = true;
+  }
+  *out = caps[dev];
+  return GM_OK;
+}
+
 // everything a call needs after validation
 struct Plan {
   ModelDesc md;
@@ -451,7 +493,14 @@ struct Plan {
   const float* psf; long long psf_stride;
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int tiles;
+  bool fused;                // whole cutout per CTA and two buffers fit: k_fused path
+  DevCaps caps;
 };
+
+static size_t fused_smem_for(int KP, const TileGeom& tg) {
+  return 2 * (size_t)tg.rows * tg.pitch * 4 + 4 * (size_t)(KP + 1) * (KP + 1) * 8 +
+         (size_t)kHelpWarps * kNSum * 4 + 64;
+}
 
 static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, void* workspace,
                      size_t workspace_bytes, cudaStream_t st, Plan* pl) {
@@ -464,6 +513,9 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   if ((size_t)bt->B * pl->tiles > 0x7fffffffull) return GM_EINVAL;
   pl->ws = carve(workspace, pl->md, bt, pl->KP, pl->tg);
   if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < pl->ws.total) return GM_EWORKSPACE;
+  if ((rc = device_caps(&pl->caps)) != GM_OK) return rc;
+  pl->fused = pl->tiles == 1 && pl->tg.ntx * pl->tg.nty <= 32 * kConvWarps &&
+              fused_smem_for(pl->KP, pl->tg) <= pl->caps.smem_optin && !getenv("GM_NO_FUSED");
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
   if (pl->KP != bt->K) {
@@ -518,6 +570,30 @@ static BwdArgs bwd_args(const Plan& pl, const int* frozen) {
   return a;
 }
 
+static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float* out, const int* frozen) {
+  FusedArgs a;
+  a.md = pl.md; a.tg = pl.tg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
+  a.any_unconv = 0;
+  for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
+  a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride;
+  a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
+  a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part; a.frozen = frozen;
+  const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
+  a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
+  return a;
+}
+
+// one evaluation of every (non-frozen) galaxy: chi^2 partials and, if wanted, gradient partials
+static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const int* frozen, cudaStream_t st) {
+  int rc;
+  if (pl.fused)
+    return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, frozen), pl.caps.n_sm,
+                          pl.caps.smem_optin, st);
+  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, frozen), false, bt->B, st)) != GM_OK) return rc;
+  if (with_grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, frozen), bt->B, st)) != GM_OK) return rc;
+  return GM_OK;
+}
+
 static FinArgs fin_args(const Plan& pl, int B, bool with_grad, float* chi2, float* grad) {
   FinArgs a;
   a.md = pl.md; a.B = B; a.tiles = pl.tiles; a.cc = pl.ws.cc;
@@ -555,6 +631,8 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
   if (rc != GM_OK) return rc;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
+  if (pl.fused)
+    return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, nullptr), pl.caps.n_sm, pl.caps.smem_optin, st);
   return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, nullptr), true, bt->B, st);
 }
 
@@ -569,8 +647,7 @@ int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params,
   if (rc != GM_OK) return rc;
   if (jtj || jtr) return GM_ENOTSUP;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
-  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, nullptr), false, bt->B, st)) != GM_OK) return rc;
-  if (grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, nullptr), bt->B, st)) != GM_OK) return rc;
+  if ((rc = run_eval(pl, bt, grad != nullptr, nullptr, st)) != GM_OK) return rc;
   k_finalize<<<(bt->B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(
       fin_args(pl, bt->B, grad != nullptr, chi2, grad));
   ++t_launches;
@@ -609,14 +686,11 @@ int gm_fit(const gm_model* model, const gm_batch* bt, float* params, const gm_fi
   ++t_launches;
   GM_CUDA(cudaGetLastError());
 
-  const FwdArgs fa = fwd_args(pl, bt, pl.ws.G, fs.frozen);
-  const BwdArgs ba = bwd_args(pl, fs.frozen);
   const int fin_grid = (B + kFinWarps - 1) / kFinWarps;
   for (int t = 1; t <= opts->n_iter + 1; ++t) {
     const int last = (t == opts->n_iter + 1);
     if ((rc = run_prologue(pl, B, params, fs.frozen, st)) != GM_OK) return rc;
-    if ((rc = dispatch_forward(pl.KP, fa, false, B, st)) != GM_OK) return rc;
-    if (!last && (rc = dispatch_backward(pl.KP, ba, B, st)) != GM_OK) return rc;
+    if ((rc = run_eval(pl, bt, !last, fs.frozen, st)) != GM_OK) return rc;
     const float c1 = (float)(1.0 - std::pow((double)opts->beta1, (double)t));
     const float c2 = (float)(1.0 - std::pow((double)opts->beta2, (double)t));
     const float dec = (float)std::pow((double)opts->lr_decay, (double)(t - 1));
@@ -762,8 +836,8 @@ int gm_profile_enable(int on) {
 int gm_profile_read(double* ms, int64_t* count) {
   if (!ms || !count) return GM_EINVAL;
   std::lock_guard<std::mutex> lk(g_prof.mu);
-  ms[0] = ms[1] = 0.0;
-  count[0] = count[1] = 0;
+  ms[0] = ms[1] = ms[2] = 0.0;
+  count[0] = count[1] = count[2] = 0;
   for (int i = 0; i < g_prof.n; ++i) {
     GM_CUDA(cudaEventSynchronize(g_prof.ev[i][1]));
     float t = 0.0f;
