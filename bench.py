@@ -115,8 +115,9 @@ def run_reference(args):
     cores = oracle.num_threads()
     n_gal, n_iter = cores, 3
     side = cfg.sides[len(cfg.sides) // 2]
-    b = configs.make_batch(cfg.cid, range(n_gal), lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf),
-                           side=side)
+    cand = list(range(40 * cores))
+    gal = [g for g, s in zip(cand, configs.sides_for(cfg, cand)) if s == side][:n_gal]
+    b = configs.make_batch(cfg.cid, gal, lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf), side=side)
     n_gal = len(b["galaxies"])
     opts = configs.fit_options(b["model"], b["H"], b["W"], n_iter)
 
@@ -149,8 +150,9 @@ def cpu_baseline(cfg, side):
     from gen import configs
     cores = oracle.num_threads()
     n_gal = 2 * cores
-    b = configs.make_batch(cfg.cid, range(n_gal), lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf),
-                           side=side)
+    cand = list(range(40 * cores))
+    gal = [g for g, s in zip(cand, configs.sides_for(cfg, cand)) if s == side][:n_gal]
+    b = configs.make_batch(cfg.cid, gal, lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf), side=side)
     n_gal = len(b["galaxies"])
     # size the iteration count from one timed evaluation so the sample takes ~15 s
     t0 = time.perf_counter()
@@ -185,36 +187,51 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cfg = configs.CONFIGS[args.config]
-    side = args.side or cfg.sides[len(cfg.sides) // 2]
-    B = args.batch or min(cfg.B, 4096)
+    Btot = args.batch or min(cfg.B, 8289)
     n_iter = args.iters or cfg.n_iter or 200
-    gal = range(rank * B, rank * B + B)            # weak scaling: every rank its own galaxies
+    gal = range(rank * Btot, rank * Btot + Btot)   # weak scaling: every rank its own galaxies
 
     def render(model, p, H, W, psf):               # truth images from the CUDA path itself
         out = gm.gm_render(model, torch.from_numpy(p).cuda(), H, W, torch.from_numpy(psf).cuda())
         torch.cuda.synchronize()
         return out.cpu().numpy()
 
-    b = configs.make_batch(cfg.cid, gal, render, side=side)
-    B = len(b["galaxies"])
-    model, H, W, K = b["model"], b["H"], b["W"], b["K"]
-    opts = dict(b["opts"]); opts["n_iter"] = n_iter
-    opts["lr_decay"] = 0.01 ** (1.0 / max(n_iter - 1, 1))
-    if args.no_early_stop:
-        opts["tol"] = 0.0
-
+    # one bucket per cutout side (C2: five; every other config: one), each its own gm_batch
     pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
-    h_data, h_sigma, h_mask, h_psf, h_start = map(pin, (b["data"], b["sigma"], b["mask"], b["psf"], b["start"]))
     d = lambda t: None if t is None else t.cuda(non_blocking=True)
-    data, sigma, mask, psf, start = map(d, (h_data, h_sigma, h_mask, h_psf, h_start))
-    params = start.clone()
-    ws = torch.empty(gm.gm_workspace_bytes(model, B, H, W, K) + 256, dtype=torch.uint8, device="cuda")
+    sides = [args.side] if args.side else list(cfg.sides)
+    buckets = []
+    for side in sides:
+        b = configs.make_batch(cfg.cid, gal, render, side=side)
+        if not b["galaxies"]:
+            continue
+        opts = dict(b["opts"]); opts["n_iter"] = n_iter
+        opts["lr_decay"] = 0.01 ** (1.0 / max(n_iter - 1, 1))
+        if args.no_early_stop:
+            opts["tol"] = 0.0
+        host = tuple(map(pin, (b["data"], b["sigma"], b["mask"], b["psf"], b["start"])))
+        devt = tuple(map(d, host))
+        B, H, W, K = len(b["galaxies"]), b["H"], b["W"], b["K"]
+        buckets.append({"b": b, "B": B, "H": H, "W": W, "K": K, "opts": opts, "host": host, "dev": devt,
+                        "params": devt[4].clone(),
+                        "ws": torch.empty(gm.gm_workspace_bytes(b["model"], B, H, W, K) + 256,
+                                          dtype=torch.uint8, device="cuda")})
+    model = buckets[0]["b"]["model"]
+    K = buckets[0]["K"]
+    B = sum(k["B"] for k in buckets)
+    early = any(k["opts"]["tol"] > 0.0 for k in buckets)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     def step():
-        params.copy_(start)
-        return gm.gm_fit(model, params, data, sigma, mask, psf, opts, workspace=ws, stream=stream)
+        outs, n = [], 0
+        for k in buckets:
+            data, sigma, mask, psf, start = k["dev"]
+            k["params"].copy_(start)
+            outs.append(gm.gm_fit(model, k["params"], data, sigma, mask, psf, k["opts"], workspace=k["ws"],
+                                  stream=stream))
+            n += gm.gm_last_launch_count()
+        return outs, n
 
     def barrier():
         if dist is not None:
@@ -223,7 +240,7 @@ def run_ours(args):
 
     for _ in range(max(args.warmup, 3)):
         flush.zero_()
-        out = step()
+        outs, _ = step()
     barrier()
 
     # ---- timed region: K steps, device time by CUDA events on the launching stream
@@ -235,9 +252,9 @@ def run_ours(args):
         for s in range(args.steps):
             flush.zero_()                           # L2 flushed between steps (not timed)
             ev[s][0].record(stream)
-            out = step()
+            outs, n = step()
             ev[s][1].record(stream)
-            launches += gm.gm_last_launch_count()
+            launches += n
         barrier()
     prof = gm.gm_profile_read()
     gm.gm_profile_enable(False)
@@ -247,30 +264,47 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     t_ms = float(t.item())
     ms_per_step = t_ms / args.steps
-    evals = B * H * W * n_iter
-    value = world * evals / (ms_per_step * 1e-3)
 
-    status = out["status"].cpu().numpy(); iters = out["iters_used"].cpu().numpy()
-    chi2 = out["chi2"].cpu().numpy()
-    npix = H * W if b["mask"] is None else b["mask"].reshape(B, -1).sum(1)
+    # chi^2+gradient evaluations actually made: iters_used per galaxy (= n_iter without early stop)
+    status = np.concatenate([o["status"].cpu().numpy() for o in outs])
+    iters = np.concatenate([o["iters_used"].cpu().numpy() for o in outs])
+    red = np.concatenate([o["chi2"].cpu().numpy() /
+                          np.maximum(k["H"] * k["W"] if k["b"]["mask"] is None
+                                     else k["b"]["mask"].reshape(k["B"], -1).sum(1), 1)
+                          for o, k in zip(outs, buckets)])
+    evals = float(sum(o["iters_used"].sum().item() * k["H"] * k["W"] for o, k in zip(outs, buckets)))
+    # algorithmic convolution flops of one step: 2 convolutions per evaluation + the closing forward
+    # (status 0: n_iter evaluations + closing forward; stopped early or non-finite: the evaluation
+    # that triggered the stop ran both convolutions but applied no update)
+    def n_convs(o):
+        it = o["iters_used"].cpu().numpy().astype(np.float64); st = o["status"].cpu().numpy()
+        return float(np.where(st == 0, 2.0 * it + 1.0, 2.0 * (it + 1.0)).sum())
+    conv_flops = float(sum(n_convs(o) * 2.0 * k["H"] * k["W"] * k["K"] ** 2 for o, k in zip(outs, buckets)))
+    value = world * evals / (ms_per_step * 1e-3)
 
     # ---- e2e: the same step through the host-buffer C-ABI call (copies inside)
     e2e = None
     if rank == 0 or world > 1:
-        hp = h_start.numpy().copy()
-        hargs = (h_data.numpy(), h_sigma.numpy(), None if h_mask is None else h_mask.numpy(), h_psf.numpy())
-        gm.gm_fit_host(model, hp, *hargs, opts)                       # warm-up
+        hps = [k["host"][4].numpy().copy() for k in buckets]
+        hargs = [tuple(None if t is None else t.numpy() for t in k["host"][:4]) for k in buckets]
+
+        def host_step():
+            for k, hp, ha in zip(buckets, hps, hargs):
+                hp[...] = k["b"]["start"]
+                gm.gm_fit_host(model, hp, *ha, k["opts"])
+
+        host_step()                                                   # warm-up
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            hp[...] = b["start"]
-            gm.gm_fit_host(model, hp, *hargs, opts)
+            host_step()
         te = torch.tensor([(time.perf_counter() - t0) / args.steps], dtype=torch.float64, device="cuda")
         if dist is not None:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        h2d = sum(a.nbytes for a in hargs if a is not None) + hp.nbytes
-        d2h = hp.nbytes + 3 * B * 4
+        h2d = sum(a.nbytes for ha in hargs for a in ha if a is not None) + sum(hp.nbytes for hp in hps)
+        d2h = sum(hp.nbytes for hp in hps) + 3 * B * 4
         e2e = {"value": world * evals / float(te.item()), "unit": UNIT, "ms_per_step": float(te.item()) * 1e3,
+               "galaxies_fitted_per_s": world * B / float(te.item()),
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "api": "gm_fit_host (host buffers; cudaMalloc + H2D + fit + D2H inside the call)"}
 
@@ -279,61 +313,60 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernels (both run the same K^2-tap FFMA2 loop)
+    # ---- roofline of the heavy kernels (all run the same K^2-tap FFMA2 loop)
     pk, pk_src = peaks()
     clocks = clk.summary()
     f_mhz = pk.get("sm_max_mhz", 1965.0)
     peak_tflops = SM_COUNT * FP32_LANES * 2 * f_mhz * 1e6 / 1e12
-    flops_per_launch = 2.0 * B * H * W * K * K                     # one K^2-tap convolution of the batch
-    kern = {}
-    for name, (ms, n) in prof.items():
-        if not n:
-            continue
-        avg = ms / n
-        if name == "fused":
-            # per step: n_iter launches with both convolutions + the closing chi^2-only launch
-            flops = args.steps * (2 * n_iter + 1) * flops_per_launch
-            convs = (2 * n_iter + 1) / (n_iter + 1)
-        else:
-            flops = n * flops_per_launch
-            convs = 1
-        kern[name] = {"launches": n, "avg_ms": avg, "convolutions_per_launch": convs,
-                      "tflops": flops / (ms * 1e-3) / 1e12,
-                      "share_of_step": ms / t_ms if world == 1 else None}
+    kern = {name: {"launches": n, "avg_ms": ms / n, "share_of_step": ms / t_ms if world == 1 else None}
+            for name, (ms, n) in prof.items() if n}
+    heavy_ms = sum(ms for ms, n in prof.values() if n)
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
-    traffic = None
-    tf = ROOT / "profiles" / "traffic.json"
-    if tf.exists():
-        traffic = json.loads(tf.read_text()).get(f"{dom}_K{K}_{H}x{W}_B{B}")
     roofline = None
     if dom:
-        roofline = {"bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": kern[dom]["tflops"],
-                    "peak": peak_tflops, "unit": "TFLOP/s", "frac": kern[dom]["tflops"] / peak_tflops,
+        achieved = args.steps * conv_flops / (heavy_ms * 1e-3) / 1e12
+        n_dom = kern[dom]["launches"]
+        big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
+        traffic = None
+        tf = ROOT / "profiles" / "traffic.json"
+        if tf.exists() and len(buckets) == 1:
+            traffic = json.loads(tf.read_text()).get(f"{dom}_K{K}_{big['H']}x{big['W']}_B{big['B']}")
+        px_bytes = 9 if big["b"]["mask"] is not None else 8
+        roofline = {"bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved,
+                    "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                     "traffic": traffic,
                     "peak_source": f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 flop x {f_mhz:.0f} MHz "
                                    f"(sm_max_mhz of {pk_src} MEASURED_PEAKS.json; an FFMA2 loop measured "
                                    "36.8 TFMA/s = 73.7 TFLOP/s on this pool, DESIGN.md)",
-                    "algorithmic_flops_per_launch": flops_per_launch * kern[dom]["convolutions_per_launch"],
-                    "hbm_gbs_algorithmic": (B * H * W * (9 if b['mask'] is not None else 8)) /
-                                           (kern[dom]["avg_ms"] * 1e-3) / 1e9,
+                    "algorithmic_flops_per_launch": args.steps * conv_flops / max(n_dom, 1)
+                    if len(kern) == 1 else None,
+                    "how": "2*K^2 flops per pixel per convolution x convolutions actually run "
+                           "(2 per chi^2+gradient evaluation + the closing forward) / summed CUDA-event time of the "
+                           "heavy kernels (forward, backward, fused) inside the timed region",
+                    "hbm_gbs_algorithmic": (evals * args.steps * px_bytes) / (heavy_ms * 1e-3) / 1e9,
                     "hbm_peak_gbs": pk.get("hbm_gbs"), "kernels": kern}
-        # whole-step view: both convolutions of every evaluation against the same peak
-        roofline["step_frac"] = (2.0 * flops_per_launch * n_iter / (ms_per_step * 1e-3) / 1e12) / peak_tflops
+        # whole-step view: the same flops against the step time (small kernels and gaps included)
+        roofline["step_frac"] = (conv_flops / (ms_per_step * 1e-3) / 1e12) / peak_tflops
 
+    wl = (workload_name(cfg, B, buckets[0]["H"], buckets[0]["W"], K, n_iter) if len(buckets) == 1 else
+          f"{cfg.name}: {B} galaxies, {cfg.model_name}, sides " +
+          ", ".join(f"{k['H']}px x{k['B']}" for k in buckets) +
+          f", {K}x{K} Moffat PSF, {'10% masked, ' if cfg.mask_frac else ''}gm_fit capped at {n_iter} iterations"
+          + (" with early stop" if early else ""))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(cfg, B, H, W, K, n_iter), "global_batch": B * world,
+            "config": {"workload": wl, "global_batch": B * world,
                        "parallelism": f"dp{world} (independent galaxies, no collective)",
                        "l2": "flushed between steps (256 MiB write)",
                        "inputs": "seeded synthetic SDSS-like (gen/configs.py), resident in HBM"},
             "galaxies_fitted_per_s": world * B / (ms_per_step * 1e-3),
             "fit_summary": {"status_counts": {str(k): int((status == k).sum()) for k in np.unique(status)},
                             "mean_iters": float(iters.mean()),
-                            "median_reduced_chi2": float(np.median(chi2 / np.maximum(npix, 1)))},
+                            "median_reduced_chi2": float(np.median(red))},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if world == 1 and not args.no_cpu:
-        line["cpu_baseline"] = cpu_baseline(cfg, side)
+        line["cpu_baseline"] = cpu_baseline(cfg, buckets[len(buckets) // 2]["H"])
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -141,8 +141,10 @@ int gm_render(const gm_model* model, const gm_batch* batch, const float* params,
 
 /* chi^2 (Eq. 18) and its gradient with respect to the PHYSICAL parameters.
  * chi2: dev [B].  grad: dev [B,P] (NULL = not wanted).
- * jtj: dev [B,P,P], jtr: dev [B,P] = J^T W J and J^T W (D-M), or NULL;
- * requesting them returns GM_ENOTSUP until the covariance row is built. */
+ * jtj: dev [B,P,P], jtr: dev [B,P] = J^T W J and J^T W (D-M) with J = dM/dp and
+ * W = Omega / sigma^2, or NULL.  jtr costs nothing extra (it is -grad/2);
+ * jtj runs P more forward convolutions (one Jacobian column each) and needs a
+ * workspace of gm_uncertainty_workspace_bytes(), else GM_EWORKSPACE. */
 int gm_loss_grad(const gm_model* model, const gm_batch* batch, const float* params,
                  float* chi2, float* grad, float* jtj, float* jtr,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -156,6 +158,19 @@ int gm_fit(const gm_model* model, const gm_batch* batch, float* params,
            const gm_fit_opts* opts, float* chi2_out, int32_t* iters_used,
            int32_t* status, void* workspace, size_t workspace_bytes,
            void* cuda_stream);
+
+/* Covariance-matrix uncertainties (Sec. 5.2):
+ *   sigma_p = sqrt(diag[(J^T W J)^-1]),  J = dM/dp at `params`,  W = Omega / sigma^2,
+ * over the FREE parameters (free_mask: host [P], 0 = held fixed and left out of the
+ * matrix; NULL = all free); fixed parameters get sigma_p = 0.  J^T W J is accumulated and
+ * inverted in fp64 (Jacobi scaling + Cholesky).  sigma_p: dev [B,P].  jtj: dev [B,P,P]
+ * full matrix as float, or NULL.  status: dev [B], 0 ok, 1 matrix not positive definite
+ * or not finite (that galaxy's sigma_p is NaN), or NULL.  batch->data is not read.
+ * Workspace: gm_uncertainty_workspace_bytes(model, batch). */
+size_t gm_uncertainty_workspace_bytes(const gm_model* model, const gm_batch* batch);
+int gm_uncertainty(const gm_model* model, const gm_batch* batch, const float* params,
+                   const uint8_t* free_mask, float* sigma_p, float* jtj, int32_t* status,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---- host-buffer entry points (synchronous, end to end) -------------------- */
 /* Same operations with every pointer of `batch` and every array argument in HOST

@@ -68,6 +68,7 @@ def lib():
         L.gmo_render.argtypes = [i, ip, i, i, i, i, i, dp, C.c_int64, dp, dp]
         L.gmo_loss_grad.restype = i
         L.gmo_loss_grad.argtypes = [i, ip, i, i, i, i, i, dp, C.c_int64, dp, dp, bp, dp, dp, dp, dp, dp]
+        L.gmo_covariance_sigma.restype = i; L.gmo_covariance_sigma.argtypes = [i, dp, bp, dp]
         L.gmo_adam_step.restype = None
         L.gmo_adam_step.argtypes = [i, dp, dp, dp, dp, i, dp, d, d, d, d, dp, dp, bp]
         L.gmo_fit.restype = i
@@ -209,6 +210,30 @@ def loss_grad(model, params, data, sigma, mask, psf, want_jtj=False):
     if want_jtj:
         return chi2, grad, jtj, jtr
     return chi2, grad
+
+
+def covariance_sigma(jtj, free_mask=None):
+    """sigma_p = sqrt(diag[(J^T W J)^-1]) over the free parameters.
+    jtj [P,P] -> (sigma_p [P], status)."""
+    jtj = _f64(jtj)
+    P = jtj.shape[0]
+    out = np.empty(P)
+    fm = _u8(free_mask)
+    rc = lib().gmo_covariance_sigma(P, _dp(jtj), _bp(fm), _dp(out))
+    return out, rc
+
+
+def uncertainty(model, params, sigma, mask, psf, free_mask=None):
+    """Covariance-matrix uncertainties of every galaxy (Sec. 5.2).
+    -> {"sigma_p" [B,P], "status" [B], "jtj" [B,P,P]}"""
+    params = _f64(params)
+    B, P = params.shape
+    zeros = np.zeros_like(_f64(sigma))                    # J = dM/dp does not depend on the data
+    _, _, jtj, _ = loss_grad(model, params, zeros, sigma, mask, psf, want_jtj=True)
+    sp = np.empty((B, P)); st = np.zeros(B, dtype=np.int32)
+    for g in range(B):
+        sp[g], st[g] = covariance_sigma(jtj[g], free_mask)
+    return {"sigma_p": sp, "status": st, "jtj": jtj}
 
 
 def adam_step(u, g_u, m, s, t, lr, lr_decay, beta1, beta2, eps, ulo, uhi, free_mask=None):

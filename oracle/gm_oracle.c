@@ -32,7 +32,9 @@
  *
  * Pins (tests/test_oracle_*.py): closed-form total fluxes (Eq. 5, 8, 10, 15),
  * scipy.special.gammaincinv, scipy.signal.convolve2d, central finite
- * differences, brute-force chi^2, torch.optim.Adam, identities n=0.5/n=1.
+ * differences, brute-force chi^2, torch.optim.Adam, identities n=0.5/n=1;
+ * covariance sigma_p: numpy.linalg.inv, the closed form of a linear model, and the
+ * scatter of refits over noise realisations.
  */
 #include <math.h>
 #include <stdint.h>
@@ -573,6 +575,52 @@ int gmo_loss_grad(int n_comp, const int32_t *desc, int n_par, int B, int H, int 
                                 jtr ? jtr + (int64_t)g * n_par : NULL);
     }
     return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* covariance-matrix uncertainties (Sec. 5.2):                          */
+/*   sigma_p = sqrt(diag[(J^T W J)^-1]) over the free parameters.              */
+/* The inverse is the textbook Gauss-Jordan elimination with partial pivoting  */
+/* on [A | I]; fixed parameters are left out of A and get sigma_p = 0.         */
+/* returns 0, or 1 when A is singular / not finite / has a non-positive        */
+/* diagonal in its inverse (sigma_p then NaN).                                 */
+/* ------------------------------------------------------------------------- */
+int gmo_covariance_sigma(int P, const double *jtj /*[P*P]*/, const uint8_t *free_mask, double *sigma_p /*[P]*/)
+{
+    int idx[64], nf = 0;
+    for (int k = 0; k < P; ++k) { sigma_p[k] = 0.0; if (!free_mask || free_mask[k]) idx[nf++] = k; }
+    if (nf == 0) return 0;
+    long double *M = (long double *)malloc(sizeof(long double) * (size_t)nf * 2 * nf);
+    const int Wd = 2 * nf;
+    for (int i = 0; i < nf; ++i)
+        for (int j = 0; j < nf; ++j) {
+            M[i * Wd + j] = jtj[idx[i] * P + idx[j]];
+            M[i * Wd + nf + j] = (i == j) ? 1.0L : 0.0L;
+        }
+    int bad = 0;
+    for (int c = 0; c < nf && !bad; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < nf; ++r)
+            if (fabsl(M[r * Wd + c]) > fabsl(M[piv * Wd + c])) piv = r;
+        if (!(fabsl(M[piv * Wd + c]) > 0.0L) || !isfinite((double)M[piv * Wd + c])) { bad = 1; break; }
+        if (piv != c)
+            for (int j = 0; j < Wd; ++j) { long double t = M[c * Wd + j]; M[c * Wd + j] = M[piv * Wd + j]; M[piv * Wd + j] = t; }
+        const long double d = M[c * Wd + c];
+        for (int j = 0; j < Wd; ++j) M[c * Wd + j] /= d;
+        for (int r = 0; r < nf; ++r) {
+            if (r == c) continue;
+            const long double f = M[r * Wd + c];
+            if (f == 0.0L) continue;
+            for (int j = 0; j < Wd; ++j) M[r * Wd + j] -= f * M[c * Wd + j];
+        }
+    }
+    for (int i = 0; i < nf; ++i) {
+        const long double v = bad ? -1.0L : M[i * Wd + nf + i];
+        if (!(v > 0.0L)) bad = 1;
+    }
+    for (int i = 0; i < nf; ++i) sigma_p[idx[i]] = bad ? NAN : (double)sqrtl(M[i * Wd + nf + i]);
+    free(M);
+    return bad;
 }
 
 /* ------------------------------------------------------------------------- */

@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     gm_render,
     gm_render_host,
     gm_strerror,
+    gm_uncertainty,
+    gm_uncertainty_workspace_bytes,
     gm_version,
     gm_workspace_bytes,
     library_path,

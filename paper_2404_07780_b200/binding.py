@@ -76,6 +76,8 @@ def _lib():
         L.gm_render.restype = i; L.gm_render.argtypes = [mp, bp, vp, vp, vp, sz, vp]
         L.gm_loss_grad.restype = i; L.gm_loss_grad.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gm_fit.restype = i; L.gm_fit.argtypes = [mp, bp, vp, op, vp, vp, vp, vp, sz, vp]
+        L.gm_uncertainty_workspace_bytes.restype = sz; L.gm_uncertainty_workspace_bytes.argtypes = [mp, bp]
+        L.gm_uncertainty.restype = i; L.gm_uncertainty.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gm_render_host.restype = i; L.gm_render_host.argtypes = [mp, bp, vp, vp]
         L.gm_loss_grad_host.restype = i; L.gm_loss_grad_host.argtypes = [mp, bp, vp, vp, vp]
         L.gm_fit_host.restype = i; L.gm_fit_host.argtypes = [mp, bp, vp, op, vp, vp, vp]
@@ -139,8 +141,9 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
-def _workspace(m, b, workspace):
-    need = _lib().gm_workspace_bytes(C.byref(m), C.byref(b))
+def _workspace(m, b, workspace, uncertainty=False):
+    fn = _lib().gm_uncertainty_workspace_bytes if uncertainty else _lib().gm_workspace_bytes
+    need = fn(C.byref(m), C.byref(b))
     if need == 0:
         raise GmError(-1, "gm_workspace_bytes")
     if workspace is None:
@@ -217,8 +220,9 @@ def gm_render(model, params, H, W, psf, out=None, workspace=None, stream=None):
 
 
 def gm_loss_grad(model, params, data, sigma, mask, psf, want_grad=True, chi2=None, grad=None,
-                 workspace=None, stream=None):
-    """chi^2[B] (Eq. 18) and d chi^2 / d p [B,P].  Asynchronous on the stream."""
+                 workspace=None, stream=None, want_jtj=False):
+    """chi^2[B] (Eq. 18) and d chi^2 / d p [B,P].  Asynchronous on the stream.
+    want_jtj: also J^T W J [B,P,P] and J^T W (D-M) [B,P]; returns 4 tensors."""
     B, P = params.shape
     _, H, W = data.shape
     m = _model_struct(model)
@@ -227,14 +231,52 @@ def gm_loss_grad(model, params, data, sigma, mask, psf, want_grad=True, chi2=Non
         chi2 = torch.empty(B, dtype=torch.float32, device=params.device)
     if want_grad and grad is None:
         grad = torch.empty((B, P), dtype=torch.float32, device=params.device)
-    ws, wp, wn = _workspace(m, b, workspace)
+    jtj = torch.empty((B, P, P), dtype=torch.float32, device=params.device) if want_jtj else None
+    jtr = torch.empty((B, P), dtype=torch.float32, device=params.device) if want_jtj else None
+    ws, wp, wn = _workspace(m, b, workspace, uncertainty=want_jtj)
     rc = _lib().gm_loss_grad(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"),
                              _dev(chi2, torch.float32, "chi2"),
                              _dev(grad, torch.float32, "grad") if want_grad else None,
-                             None, None, wp, wn, _stream_ptr(stream))
+                             _dev(jtj, torch.float32, "jtj"), _dev(jtr, torch.float32, "jtr"),
+                             wp, wn, _stream_ptr(stream))
     _check(rc, "gm_loss_grad")
     chi2._gm_ws = ws
+    if want_jtj:
+        return chi2, grad, jtj, jtr
     return (chi2, grad) if want_grad else chi2
+
+
+def gm_uncertainty_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) -> int:
+    m = _model_struct(model)
+    b = _Batch(B, H, W, K, None, None, None, None, 0)
+    return int(_lib().gm_uncertainty_workspace_bytes(C.byref(m), C.byref(b)))
+
+
+def gm_uncertainty(model, params, sigma, mask, psf, free_mask=None, want_jtj=False, workspace=None,
+                   stream=None):
+    """sigma_p[B,P] = sqrt(diag[(J^T W J)^-1]) at params (Sec. 5.2).  Asynchronous.
+    -> {"sigma_p", "status", ["jtj"]}"""
+    B, P = params.shape
+    _, H, W = sigma.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, None, sigma, mask)
+    fm = None
+    if free_mask is not None:
+        fm = np.ascontiguousarray(free_mask, dtype=np.uint8)
+        if fm.shape != (P,):
+            raise ValueError("free_mask must have n_par entries")
+    sp = torch.empty((B, P), dtype=torch.float32, device=params.device)
+    status = torch.empty(B, dtype=torch.int32, device=params.device)
+    jtj = torch.empty((B, P, P), dtype=torch.float32, device=params.device) if want_jtj else None
+    ws, wp, wn = _workspace(m, b, workspace, uncertainty=True)
+    rc = _lib().gm_uncertainty(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"),
+                               None if fm is None else fm.ctypes.data, sp.data_ptr(),
+                               _dev(jtj, torch.float32, "jtj"), status.data_ptr(), wp, wn, _stream_ptr(stream))
+    _check(rc, "gm_uncertainty")
+    out = {"sigma_p": sp, "status": status, "_ws": ws}
+    if want_jtj:
+        out["jtj"] = jtj
+    return out
 
 
 def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=None):

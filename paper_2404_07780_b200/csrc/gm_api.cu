@@ -151,6 +151,7 @@ struct FinArgs {
   const float* grad_part;
   float* chi2;      // [B] out (loss_grad) / chi2_out (fit)
   float* grad;      // [B,P] out or nullptr
+  float* jtr;       // [B,P] out or nullptr: J^T W (D - M) = -grad / 2
 };
 
 // chi2 and d chi2 / d p of galaxy b from the per-tile partials; one warp per galaxy.
@@ -209,6 +210,7 @@ __global__ void __launch_bounds__(kFinWarps * 32) k_finalize(const FinArgs a) {
   const float c2 = assemble(a, b, lane, sh[wid], &g);
   if (lane == 0) a.chi2[b] = c2;
   if (a.grad && lane < a.md.n_par) a.grad[(size_t)b * a.md.n_par + lane] = g;
+  if (a.jtr && lane < a.md.n_par) a.jtr[(size_t)b * a.md.n_par + lane] = -0.5f * g;
 }
 
 __global__ void k_fit_init(int B, int P, const float* __restrict__ params, FitOptsDev o, FitState st,
@@ -292,6 +294,157 @@ k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* __restrict__
       params[pk] = o.lg[lane] ? exp10f(u) : u;
     }
   }
+}
+
+// ---------------------------------------------------------------------------
+// covariance row: J^T W J from the P Jacobian columns that
+// k_forward<FWD_DERIV> wrote, then sigma_p = sqrt(diag[(J^T W J)^-1]).
+// ---------------------------------------------------------------------------
+constexpr int kGramPx = 64;                   // pixels staged per step
+constexpr int kGramThreads = 256;
+constexpr int kMaxPairs = GM_MAX_PAR * (GM_MAX_PAR + 1) / 2;
+
+struct GramArgs {
+  int b0, Bc, N, P;          // first galaxy and number of galaxies of the chunk, pixels, parameters
+  const float* J;            // [P][Bc][N] Jacobian columns of the chunk
+  const float* sigma; const uint8_t* mask;      // [B,N]
+  double* jtj;               // [B,P,P] (both triangles written)
+};
+
+// one CTA per galaxy.  Work item = (pair k<=l, pixel slice); each accumulates fp32
+// products over 64 staged pixels and adds them into its own fp64 sum; slices are then
+// added in order, so the result is deterministic.
+__global__ void __launch_bounds__(kGramThreads) k_gram(const GramArgs a) {
+  __shared__ float Js[kGramPx][GM_MAX_PAR + 1];
+  __shared__ float wsh[kGramPx];
+  __shared__ uint8_t pk[kMaxPairs], pl[kMaxPairs];
+  __shared__ double red[kMaxPairs > kGramThreads ? kMaxPairs : kGramThreads];
+  const int tid = threadIdx.x;
+  const int bl = blockIdx.x, b = a.b0 + bl;
+  const int P = a.P, N = a.N;
+  const int npairs = P * (P + 1) / 2;
+  const int nsl = npairs >= kGramThreads ? 1 : kGramThreads / npairs;
+  const int items = npairs * nsl;
+  for (int k = 0, idx = 0; k < P; ++k)
+    for (int l = k; l < P; ++l, ++idx)
+      if (idx % kGramThreads == tid) { pk[idx] = (uint8_t)k; pl[idx] = (uint8_t)l; }
+  double acc[3] = {0.0, 0.0, 0.0};
+  const float* sg = a.sigma + (size_t)b * N;
+  const uint8_t* mk = a.mask ? a.mask + (size_t)b * N : nullptr;
+  for (int p0 = 0; p0 < N; p0 += kGramPx) {
+    __syncthreads();
+    for (int idx = tid; idx < P * kGramPx; idx += kGramThreads) {
+      const int k = idx / kGramPx, px = idx - k * kGramPx;
+      Js[px][k] = (p0 + px < N) ? a.J[((size_t)k * a.Bc + bl) * N + p0 + px] : 0.0f;
+    }
+    if (tid < kGramPx) {
+      const int px = p0 + tid;
+      float w = 0.0f;
+      if (px < N && (mk ? mk[px] != 0 : true)) {       // select (R:X1)
+        const float s1 = sg[px];
+        w = 1.0f / (s1 * s1);
+      }
+      wsh[tid] = w;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < 3; ++it) {
+      const int item = tid + it * kGramThreads;
+      if (item < items) {
+        const int pair = item % npairs, sl = item / npairs;
+        const int k = pk[pair], l = pl[pair];
+        float sum = 0.0f;
+        for (int px = sl; px < kGramPx; px += nsl) sum = fmaf(wsh[px] * Js[px][k], Js[px][l], sum);
+        acc[it] += (double)sum;
+      }
+    }
+  }
+  // slices of one pair, added in slice order
+  for (int it = 0; it < 3; ++it) {
+    __syncthreads();
+    const int lo = it * kGramThreads;
+    if (tid + lo < items) red[tid] = acc[it];
+    __syncthreads();
+    // items lo .. lo+255 hold (pair = item % npairs, sl = item / npairs)
+    if (nsl == 1) {
+      const int pair = tid + lo;
+      if (pair < npairs) {
+        const int k = pk[pair], l = pl[pair];
+        a.jtj[((size_t)b * P + k) * P + l] = red[tid];
+        a.jtj[((size_t)b * P + l) * P + k] = red[tid];
+      }
+    } else if (it == 0 && tid < npairs) {
+      double t = 0.0;
+      for (int sl = 0; sl < nsl; ++sl) t += red[sl * npairs + tid];
+      const int k = pk[tid], l = pl[tid];
+      a.jtj[((size_t)b * P + k) * P + l] = t;
+      a.jtj[((size_t)b * P + l) * P + k] = t;
+    }
+  }
+}
+
+struct FreeSet { int nf; uint8_t idx[GM_MAX_PAR]; };
+
+__global__ void k_jtj_to_float(long long n, const double* __restrict__ in, float* __restrict__ out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (float)in[i];
+}
+
+// sigma_p = sqrt(diag[(J^T W J)^-1]) over the free parameters; one warp per galaxy,
+// fp64: Jacobi scaling, Cholesky, columns of L^-1 by forward substitution.
+// status: 0 ok, 1 matrix not positive definite / not finite (sigma_p = NaN).
+__global__ void __launch_bounds__(kFinWarps * 32)
+k_covar(int B, int P, const FreeSet fs, const double* __restrict__ jtj, float* __restrict__ sigma_p,
+        int* __restrict__ status) {
+  __shared__ double Ash[kFinWarps][GM_MAX_PAR][GM_MAX_PAR + 1];
+  __shared__ double scl[kFinWarps][GM_MAX_PAR];
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int b = blockIdx.x * kFinWarps + wid;
+  if (b >= B) return;
+  double (*A)[GM_MAX_PAR + 1] = Ash[wid];
+  const int nf = fs.nf;
+  const double* src = jtj + (size_t)b * P * P;
+  bool ok = true;
+  if (lane < nf) {
+    const double d = src[fs.idx[lane] * P + fs.idx[lane]];
+    ok = (d > 0.0) && isfinite(d);
+    scl[wid][lane] = ok ? rsqrt(d) : 0.0;
+  }
+  ok = __all_sync(0xffffffffu, ok);
+  __syncwarp();
+  for (int i = 0; i < nf; ++i)
+    if (lane < nf) A[i][lane] = src[fs.idx[i] * P + fs.idx[lane]] * scl[wid][i] * scl[wid][lane];
+  __syncwarp();
+  for (int j = 0; j < nf && ok; ++j) {                      // Cholesky, lower triangle in place
+    double sum = 0.0;
+    if (lane >= j && lane < nf) {
+      sum = A[lane][j];
+      for (int k = 0; k < j; ++k) sum -= A[lane][k] * A[j][k];
+    }
+    const double djj = __shfl_sync(0xffffffffu, sum, j);
+    if (!(djj > 0.0) || !isfinite(djj)) { ok = false; break; }
+    const double ljj = sqrt(djj);
+    if (lane >= j && lane < nf) A[lane][j] = (lane == j) ? ljj : sum / ljj;
+    __syncwarp();
+  }
+  float out = 0.0f;
+  if (ok && lane < nf) {                                    // column `lane` of L^-1
+    const int c = lane;
+    const double xc = 1.0 / A[c][c];
+    double ss = xc * xc;
+    for (int i = c + 1; i < nf; ++i) {
+      double t = A[i][c] * xc;
+      for (int k = c + 1; k < i; ++k) t += A[i][k] * A[c][k];      // x_k parked in the upper triangle
+      const double xi = -t / A[i][i];
+      A[c][i] = xi;
+      ss += xi * xi;
+    }
+    out = (float)(sqrt(ss) * scl[wid][c]);
+  }
+  for (int k = lane; k < P; k += 32) sigma_p[(size_t)b * P + k] = ok ? 0.0f : NAN;
+  __syncwarp();
+  if (lane < nf) sigma_p[(size_t)b * P + fs.idx[lane]] = ok ? out : NAN;
+  if (status && lane == 0) status[b] = ok ? 0 : 1;
 }
 
 // ---------------------------------------------------------------------------
@@ -398,24 +551,24 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
 
 // per-K launchers live in gm_tiles.cu, compiled once per PSF side (-DGM_K=..)
 #define GM_DECL_K(K)                                                                          \
-  int launch_forward_##K(const FwdArgs& a, bool render, int B, cudaStream_t st, cudaError_t* err); \
+  int launch_forward_##K(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err); \
   int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
   int launch_fused_##K(const FusedArgs& a, int n_sm, size_t smem_limit, cudaStream_t st, cudaError_t* err);
 GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
 #undef GM_DECL_K
 
-static int dispatch_forward(int KP, const FwdArgs& a, bool render, int B, cudaStream_t st) {
+static int dispatch_forward(int KP, const FwdArgs& a, int mode, int B, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
   const int pi = prof_begin(0, st);
   switch (KP) {
-    case 5: rc = launch_forward_5(a, render, B, st, &err); break;
-    case 9: rc = launch_forward_9(a, render, B, st, &err); break;
-    case 15: rc = launch_forward_15(a, render, B, st, &err); break;
-    case 21: rc = launch_forward_21(a, render, B, st, &err); break;
-    case 25: rc = launch_forward_25(a, render, B, st, &err); break;
-    case 33: rc = launch_forward_33(a, render, B, st, &err); break;
-    case 41: rc = launch_forward_41(a, render, B, st, &err); break;
+    case 5: rc = launch_forward_5(a, mode, B, st, &err); break;
+    case 9: rc = launch_forward_9(a, mode, B, st, &err); break;
+    case 15: rc = launch_forward_15(a, mode, B, st, &err); break;
+    case 21: rc = launch_forward_21(a, mode, B, st, &err); break;
+    case 25: rc = launch_forward_25(a, mode, B, st, &err); break;
+    case 33: rc = launch_forward_33(a, mode, B, st, &err); break;
+    case 41: rc = launch_forward_41(a, mode, B, st, &err); break;
     default: return GM_ENOTSUP;
   }
   prof_end(pi, st);
@@ -559,6 +712,7 @@ static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const in
   a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part; a.frozen = frozen;
+  a.b0 = 0; a.dpar = -1;
   return a;
 }
 
@@ -589,7 +743,7 @@ static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const in
   if (pl.fused)
     return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, frozen), pl.caps.n_sm,
                           pl.caps.smem_optin, st);
-  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, frozen), false, bt->B, st)) != GM_OK) return rc;
+  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, frozen), FWD_LOSS, bt->B, st)) != GM_OK) return rc;
   if (with_grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, frozen), bt->B, st)) != GM_OK) return rc;
   return GM_OK;
 }
@@ -599,8 +753,66 @@ static FinArgs fin_args(const Plan& pl, int B, bool with_grad, float* chi2, floa
   a.md = pl.md; a.B = B; a.tiles = pl.tiles; a.cc = pl.ws.cc;
   a.chi2_part = pl.ws.chi2_part;
   a.grad_part = with_grad ? pl.ws.grad_part : nullptr;
-  a.chi2 = chi2; a.grad = grad;
+  a.chi2 = chi2; a.grad = grad; a.jtr = nullptr;
   return a;
+}
+
+// ---- covariance row: workspace tail and launch sequence ------------------------
+struct UncWorkspace {
+  double* jtj;               // [B,P,P]
+  float* J;                  // [P][Bc][N]
+  int Bc;                    // galaxies per chunk
+  size_t total;              // bytes including the base workspace
+};
+
+static UncWorkspace carve_unc(void* base, size_t base_total, const ModelDesc& md, const gm_batch* bt) {
+  UncWorkspace u;
+  const size_t B = bt->B, P = md.n_par, N = (size_t)bt->H * bt->W;
+  size_t off = align_up(base_total, 256);
+  auto take = [&](size_t bytes) {
+    void* p = base ? (void*)((char*)base + off) : nullptr;
+    off += align_up(bytes, 256);
+    return p;
+  };
+  u.jtj = (double*)take(B * P * P * sizeof(double));
+  const size_t per_gal = P * N * 4;
+  size_t bc = (256ull << 20) / per_gal;                   // ~256 MiB of Jacobian columns in flight
+  if (bc < 1) bc = 1;
+  if (bc > B) bc = B;
+  u.Bc = (int)bc;
+  u.J = (float*)take(bc * per_gal);
+  u.total = off;
+  return u;
+}
+
+// J^T W J of every galaxy into uw.jtj (fp64).  The prologue must have run.
+static int run_jtj(const Plan& pl, const gm_batch* bt, const UncWorkspace& uw, cudaStream_t st) {
+  const int B = bt->B, P = pl.md.n_par;
+  const size_t N = (size_t)bt->H * bt->W;
+  for (int b0 = 0; b0 < B; b0 += uw.Bc) {
+    const int bc = (B - b0 < uw.Bc) ? B - b0 : uw.Bc;
+    for (int k = 0; k < P; ++k) {
+      FwdArgs a = fwd_args(pl, bt, uw.J + (size_t)k * bc * N, nullptr);
+      a.b0 = b0; a.dpar = k;
+      a.tg.vec = a.tg.vec && ((((uintptr_t)a.G) & 15) == 0);
+      int rc = dispatch_forward(pl.KP, a, FWD_DERIV, bc, st);
+      if (rc != GM_OK) return rc;
+    }
+    GramArgs g;
+    g.b0 = b0; g.Bc = bc; g.N = (int)N; g.P = P;
+    g.J = uw.J; g.sigma = bt->sigma; g.mask = bt->mask; g.jtj = uw.jtj;
+    k_gram<<<bc, kGramThreads, 0, st>>>(g);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+  }
+  return GM_OK;
+}
+
+static int jtj_to_float(const UncWorkspace& uw, size_t n, float* out, cudaStream_t st) {
+  k_jtj_to_float<<<(unsigned)((n + 255) / 256), 256, 0, st>>>((long long)n, uw.jtj, out);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  return GM_OK;
 }
 
 }  // namespace gm
@@ -622,6 +834,17 @@ size_t gm_workspace_bytes(const gm_model* model, const gm_batch* bt) {
   return carve(nullptr, md, bt, KP, tg).total;
 }
 
+size_t gm_uncertainty_workspace_bytes(const gm_model* model, const gm_batch* bt) {
+  const size_t base = gm_workspace_bytes(model, bt);
+  if (base == 0) return 0;
+  ModelDesc md;
+  gm_batch tmp = *bt;
+  static const float dummy = 0.0f;
+  if (!tmp.psf) tmp.psf = &dummy;
+  if (validate(model, &tmp, false, &md) != GM_OK) return 0;
+  return carve_unc(nullptr, base, md, bt).total;
+}
+
 int gm_render(const gm_model* model, const gm_batch* bt, const float* params, float* model_out,
               void* workspace, size_t workspace_bytes, void* cuda_stream) {
   t_launches = 0;
@@ -633,7 +856,7 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
   if (pl.fused)
     return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, nullptr), pl.caps.n_sm, pl.caps.smem_optin, st);
-  return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, nullptr), true, bt->B, st);
+  return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, nullptr), FWD_RENDER, bt->B, st);
 }
 
 int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params, float* chi2,
@@ -645,11 +868,47 @@ int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params,
   Plan pl;
   int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl);
   if (rc != GM_OK) return rc;
-  if (jtj || jtr) return GM_ENOTSUP;
+  UncWorkspace uw{};
+  if (jtj) {
+    uw = carve_unc(workspace, pl.ws.total, pl.md, bt);
+    if (workspace_bytes < uw.total) return GM_EWORKSPACE;
+  }
+  const bool with_grad = grad != nullptr || jtr != nullptr;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
-  if ((rc = run_eval(pl, bt, grad != nullptr, nullptr, st)) != GM_OK) return rc;
-  k_finalize<<<(bt->B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(
-      fin_args(pl, bt->B, grad != nullptr, chi2, grad));
+  if ((rc = run_eval(pl, bt, with_grad, nullptr, st)) != GM_OK) return rc;
+  FinArgs fa = fin_args(pl, bt->B, with_grad, chi2, grad);
+  fa.jtr = jtr;
+  k_finalize<<<(bt->B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(fa);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  if (jtj) {
+    if ((rc = run_jtj(pl, bt, uw, st)) != GM_OK) return rc;
+    if ((rc = jtj_to_float(uw, (size_t)bt->B * pl.md.n_par * pl.md.n_par, jtj, st)) != GM_OK) return rc;
+  }
+  return GM_OK;
+}
+
+int gm_uncertainty(const gm_model* model, const gm_batch* bt, const float* params,
+                   const uint8_t* free_mask, float* sigma_p, float* jtj, int32_t* status,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  if (!params || !sigma_p || !bt || !bt->sigma) return GM_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Plan pl;
+  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
+  if (rc != GM_OK) return rc;
+  const UncWorkspace uw = carve_unc(workspace, pl.ws.total, pl.md, bt);
+  if (workspace_bytes < uw.total) return GM_EWORKSPACE;
+  const int B = bt->B, P = pl.md.n_par;
+  FreeSet fs;
+  fs.nf = 0;
+  for (int k = 0; k < P; ++k)
+    if (!free_mask || free_mask[k]) fs.idx[fs.nf++] = (uint8_t)k;
+  if (fs.nf == 0) return GM_EINVAL;
+  if ((rc = run_prologue(pl, B, params, nullptr, st)) != GM_OK) return rc;
+  if ((rc = run_jtj(pl, bt, uw, st)) != GM_OK) return rc;
+  if (jtj && (rc = jtj_to_float(uw, (size_t)B * P * P, jtj, st)) != GM_OK) return rc;
+  k_covar<<<(B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(B, P, fs, uw.jtj, sigma_p, status);
   ++t_launches;
   GM_CUDA(cudaGetLastError());
   return GM_OK;

@@ -169,4 +169,34 @@ __device__ __forceinline__ void profile_grad_t(const CompConst& cc, float rg, fl
   }
 }
 
+// d I / d (slot k) of one component at pixel centre (x, y): the forward-mode column of
+// the Jacobian J = dM/dp used by the covariance row.  Same guards as the
+// gradient pass (R:S4): derivative factors at rg = max(r, 1e-6), d/d amp at r itself.
+template <int KIND>
+__device__ __forceinline__ float component_deriv_t(const CompConst& cc, int k, float x, float y) {
+  if (KIND == GM_SKY) return k == GM_SLOT_AMP ? 1.0f : 0.0f;
+  const Geo g = geometry(cc, x, y);
+  const float rg = fmaxf(g.r, kRGuard);
+  float U, dUdr, d0, d1, d2;
+  profile_grad_t<KIND, false>(cc, rg, U, dUdr, d0, d1, d2);
+  const float cgeo = cc.amp * dUdr / rg;
+  switch (k) {
+    case GM_SLOT_XC: return cgeo * (-cc.ct * g.u + cc.st * cc.iq * g.vq);
+    case GM_SLOT_YC: return cgeo * (-cc.st * g.u - cc.ct * cc.iq * g.vq);
+    case GM_SLOT_THETA: return cgeo * (cc.q - cc.iq) * g.u * g.vq;
+    case GM_SLOT_Q: return -cc.iq * cgeo * g.vq * g.vq;
+    case GM_SLOT_AMP: return (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+    case GM_SLOT_S0: return cc.amp * d0;
+    case GM_SLOT_S1: return cc.amp * d1;
+    case GM_SLOT_S2: return cc.amp * d2;
+    default: return 0.0f;
+  }
+}
+
+__device__ __forceinline__ float component_deriv(int kind, const CompConst& cc, int k, float x, float y) {
+  float v = 0.0f;
+  dispatch_kind(kind, [&]<int KIND>() { v = component_deriv_t<KIND>(cc, k, x, y); });
+  return v;
+}
+
 }  // namespace gm

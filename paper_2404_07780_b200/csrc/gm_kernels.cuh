@@ -50,7 +50,13 @@ struct FwdArgs {
   float* G;                // [B,H,W] workspace (or model_out when RENDER)
   float* chi2_part;        // [B, tiles]
   const int* frozen;       // [B] or nullptr: skip galaxies that stopped
+  int b0;                  // first galaxy of this launch (FWD_DERIV chunks; 0 otherwise)
+  int dpar;                // FWD_DERIV: index of the parameter to differentiate with respect to
 };
+
+// what k_forward produces: G = -2 w rho and chi^2 partials (a3), the model image M
+// (gm_render), or one column of the Jacobian dM/dp_dpar (covariance row)
+enum { FWD_LOSS = 0, FWD_RENDER = 1, FWD_DERIV = 2 };
 
 struct BwdArgs {
   ModelDesc md;
@@ -176,13 +182,14 @@ __host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int
 // ---------------------------------------------------------------------------
 // forward: render + convolve + residual
 // ---------------------------------------------------------------------------
-template <int K, bool RENDER>
+template <int K, int MODE>
 __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
+  constexpr bool RENDER = (MODE != FWD_LOSS);            // an image is written, no residual
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
   const int tiles = tg.tiles_x * tg.tiles_y;
-  const int b = blockIdx.x / tiles;
-  const int tile = blockIdx.x - b * tiles;
+  const int b = a.b0 + blockIdx.x / tiles;
+  const int tile = blockIdx.x % tiles;
   if (a.frozen && a.frozen[b]) return;
   const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
   const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;     // tile origin in the cutout
@@ -198,15 +205,13 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
 
   // a1: S on the tile plus its halo; zero outside the cutout (R:C1) and in the pad.
   // One pass per convolved component, its radial law selected outside the pixel loops.
+  // FWD_DERIV: one pass per (component, slot) that names parameter dpar, filling
+  // dS/dp_dpar instead (tied parameters add).
   const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
   const int cols = tg.TW + K - 1;
   bool first = true;
-  for (int c = 0; c <= a.md.n_comp; ++c) {
-    const bool zero_pass = (c == a.md.n_comp);
-    if (zero_pass && !first) break;                    // at least one component wrote the tile
-    if (!zero_pass && !a.md.conv[c]) continue;
-    const CompConst cc = ccb[zero_pass ? 0 : c];
-    dispatch_kind(zero_pass ? (int)GM_SKY : a.md.kind[c], [&]<int KIND>() {
+  auto fill = [&](int kind, const CompConst cc, int slot) {
+    dispatch_kind(kind, [&]<int KIND>() {
       for (int yy = wid; yy < tg.rows; yy += nwarps) {
         const int i = i0 - h + yy;
         float* rowp = tilebuf + (size_t)yy * tg.pitch;
@@ -216,15 +221,27 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
           const int j = j0 - h + xx;
           const bool in = row_in && xx < cols && j >= 0 && j < tg.W;
           float s = 0.0f;
-          if (KIND != GM_SKY && in)
-            s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry(cc, (float)j + 0.5f, y).r);
+          if (KIND != GM_SKY && in) {
+            if (MODE == FWD_DERIV) s = component_deriv_t<KIND>(cc, slot, (float)j + 0.5f, y);
+            else s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry(cc, (float)j + 0.5f, y).r);
+          }
           if (first) rowp[xx] = s;
           else if (in) rowp[xx] += s;
         }
       }
     });
     first = false;
+  };
+  for (int c = 0; c < a.md.n_comp; ++c) {
+    if (!a.md.conv[c]) continue;
+    if (MODE == FWD_DERIV) {
+      for (int k = 0; k < GM_SLOT_BOX; ++k)
+        if (a.md.slot[c][k] == a.dpar) fill(a.md.kind[c], ccb[c], k);
+    } else {
+      fill(a.md.kind[c], ccb[c], -1);
+    }
   }
+  if (first) fill((int)GM_SKY, ccb[0], -1);            // nothing convolved: a zero tile
   cp_async_wait_all();
   __syncthreads();
 
@@ -246,7 +263,7 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
 
   // a3: unconvolved components, residual, chi2, back-seed G
   float chi2 = 0.0f;
-  const size_t img = (size_t)b * tg.H * tg.W;
+  const size_t img = (size_t)(MODE == FWD_DERIV ? b - a.b0 : b) * tg.H * tg.W;
   bool any_unconv = false;
   for (int c = 0; c < a.md.n_comp; ++c) any_unconv |= (a.md.conv[c] == 0);
   auto add_unconv = [&](float m, float x, float y) {
@@ -254,8 +271,13 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
       if (a.md.conv[c]) continue;
       const CompConst cc = ccb[c];
       const int kind = a.md.kind[c];
-      const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
-      m = fmaf(cc.amp, U, m);
+      if (MODE == FWD_DERIV) {
+        for (int k = 0; k < GM_SLOT_BOX; ++k)
+          if (a.md.slot[c][k] == a.dpar) m += component_deriv(kind, cc, k, x, y);
+      } else {
+        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
+        m = fmaf(cc.amp, U, m);
+      }
     }
     return m;
   };

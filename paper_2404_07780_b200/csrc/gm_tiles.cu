@@ -21,18 +21,21 @@ static cudaError_t set_smem(Kern kern, size_t bytes) {
   return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, bool render, int B, cudaStream_t st, cudaError_t* err) {
+int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err) {
   constexpr int K = GM_K;
   const int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
   if (nthr > 256) return GM_ENOTSUP;
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
-  if (render) {
-    GM_TRY(set_smem(k_forward<K, true>, sm));
-    k_forward<K, true><<<grid, nthr, sm, st>>>(a);
+  if (mode == FWD_RENDER) {
+    GM_TRY(set_smem(k_forward<K, FWD_RENDER>, sm));
+    k_forward<K, FWD_RENDER><<<grid, nthr, sm, st>>>(a);
+  } else if (mode == FWD_DERIV) {
+    GM_TRY(set_smem(k_forward<K, FWD_DERIV>, sm));
+    k_forward<K, FWD_DERIV><<<grid, nthr, sm, st>>>(a);
   } else {
-    GM_TRY(set_smem(k_forward<K, false>, sm));
-    k_forward<K, false><<<grid, nthr, sm, st>>>(a);
+    GM_TRY(set_smem(k_forward<K, FWD_LOSS>, sm));
+    k_forward<K, FWD_LOSS><<<grid, nthr, sm, st>>>(a);
   }
   GM_TRY(cudaGetLastError());
   return GM_OK;
