@@ -2,8 +2,10 @@
 
 A model is ``{"n_par": P, "names": [...], "roles": [...], "components": [...]}``.
 Each component is ``{"kind": str, "convolve": 0|1, "slots": {slot: index}}``
-with slot names ``xc yc theta q amp s0 s1 s2 box`` (paper: P:35 p = {p_G, p_L};
-P:61 summed components; P:322-327 shared parameters; P:598 psf flag).
+with slot names ``xc yc theta q amp s0 s1 s2 box m0`` (paper: P:35 p = {p_G, p_L};
+P:61 summed components; P:322-327 shared parameters; P:598 psf flag).  ``box`` is the
+boxiness B of Eq. 2.  A used ``m0`` slot (the zero point) means the
+``amp`` slot holds a magnitude m and the intensity follows Eq. 5 / 8 / 10 / 15.
 
     Sersic   amp=Ie  s0=re    s1=n           (Eq. 1)
     ExpDisk  amp=I0  s0=rs                   (Eq. 7)
@@ -15,7 +17,7 @@ P:61 summed components; P:322-327 shared parameters; P:598 psf flag).
 
 ``roles`` drive the default fit options (step size, bounds, log10 space) of
 ``gen.configs.fit_options``: one of
-``cx cy amp radius index q theta shape sky``.
+``cx cy amp radius index q theta shape sky box mag zeropoint``.
 """
 from __future__ import annotations
 
@@ -102,8 +104,9 @@ def all_profiles():
     return _model(names, roles, comps)
 
 
-def one_component(kind: str, convolve: int = 1):
-    """Single component of the given kind with its own full geometry."""
+def one_component(kind: str, convolve: int = 1, box: bool = False, mag: bool = False):
+    """Single component of the given kind with its own full geometry; ``box`` adds the
+    boxiness B (Eq. 2), ``mag`` the magnitude parameterisation (amp slot = m, plus m0)."""
     shape = {"sersic": (["Ie", "re", "n"], ["amp", "radius", "index"]),
              "expdisk": (["I0", "rs"], ["amp", "radius"]),
              "ferrer": (["I0", "rout", "a", "b"], ["amp", "radius", "shape", "shape"]),
@@ -115,4 +118,24 @@ def one_component(kind: str, convolve: int = 1):
     slots = {"xc": 0, "yc": 1, "theta": 2, "q": 3, "amp": 4}
     for k in range(len(shape[0]) - 1):
         slots[f"s{k}"] = 5 + k
+    if mag:
+        names[4] = "mag"; roles[4] = "mag"
+    if box:
+        slots["box"] = len(names); names.append("box"); roles.append("box")
+    if mag:
+        slots["m0"] = len(names); names.append("m0"); roles.append("zeropoint")
     return _model(names, roles, [{"kind": kind, "convolve": convolve, "slots": slots}])
+
+
+def boxy_bulge_disk_mag():
+    """Parity model for SURVEY 8(f)-2: boxy Sersic bulge + disky exponential disk, both
+    in magnitudes with one shared zero point, shared centre, P = 14."""
+    return _model(
+        ["xc", "yc", "b_mag", "b_re", "b_n", "b_q", "b_theta", "b_box",
+         "d_mag", "d_rs", "d_q", "d_theta", "d_box", "m0"],
+        ["cx", "cy", "mag", "radius", "index", "q", "theta", "box",
+         "mag", "radius", "q", "theta", "box", "zeropoint"],
+        [{"kind": "sersic", "convolve": 1,
+          "slots": {"xc": 0, "yc": 1, "amp": 2, "s0": 3, "s1": 4, "q": 5, "theta": 6, "box": 7, "m0": 13}},
+         {"kind": "expdisk", "convolve": 1,
+          "slots": {"xc": 0, "yc": 1, "amp": 8, "s0": 9, "q": 10, "theta": 11, "box": 12, "m0": 13}}])

@@ -7,8 +7,9 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only ``tests/``,
 
 Models are described by plain data (see ``gen.models``): a dict
 ``{"n_par": P, "components": [{"kind": str, "convolve": 0|1, "slots": {...}}]}``
-where ``slots`` maps the names ``xc yc theta q amp s0 s1 s2 box`` to indices in
-the per-galaxy parameter vector (missing = unused).  Cites: P:35 (inputs),
+where ``slots`` maps the names ``xc yc theta q amp s0 s1 s2 box m0`` to indices in
+the per-galaxy parameter vector (missing = unused; a used ``m0`` slot means the
+``amp`` slot holds a magnitude, Eq. 5/8/10/15).  Cites: P:35 (inputs),
 P:61/P:322-327 (summed components, shared parameters), P:598 (psf flag).
 """
 from __future__ import annotations
@@ -25,7 +26,7 @@ _SRC = _HERE / "gm_oracle.c"
 _LIB = _HERE / "libgm_oracle.so"
 
 KINDS = {"sersic": 0, "expdisk": 1, "ferrer": 2, "king": 3, "gaussian": 4, "moffat": 5, "sky": 6}
-SLOT_NAMES = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box")
+SLOT_NAMES = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box", "m0")
 
 _lib = None
 
@@ -61,7 +62,8 @@ def lib():
         L.gmo_moffat_rd.restype = d; L.gmo_moffat_rd.argtypes = [d, d]
         L.gmo_moffat_I0_from_flux.restype = d; L.gmo_moffat_I0_from_flux.argtypes = [d] * 5
         L.gmo_loglike.restype = d; L.gmo_loglike.argtypes = [d, d]
-        L.gmo_component_at.restype = None; L.gmo_component_at.argtypes = [i, dp, d, d, dp, dp]
+        L.gmo_component_at.restype = None; L.gmo_component_at.argtypes = [i, i, dp, d, d, dp, dp]
+        L.gmo_amplitude_from_mag.restype = i; L.gmo_amplitude_from_mag.argtypes = [i, dp, dp, dp]
         L.gmo_conv2d_same.restype = None; L.gmo_conv2d_same.argtypes = [dp, i, i, dp, i, dp]
         L.gmo_corr2d_same.restype = None; L.gmo_corr2d_same.argtypes = [dp, i, i, dp, i, dp]
         L.gmo_render.restype = i
@@ -98,7 +100,7 @@ def _u8(a):
 
 def descriptor(model: dict) -> np.ndarray:
     comps = model["components"]
-    d = np.full((len(comps), 11), -1, dtype=np.int32)
+    d = np.full((len(comps), 2 + len(SLOT_NAMES)), -1, dtype=np.int32)
     for c, comp in enumerate(comps):
         d[c, 0] = KINDS[comp["kind"]]
         d[c, 1] = int(comp.get("convolve", 1))
@@ -156,14 +158,29 @@ def loglike(chi2, k):
     return lib().gmo_loglike(float(chi2), float(k))
 
 
-def component_at(kind: str, p9, x, y):
-    """Value and d/d(xc,yc,theta,q,amp,s0,s1,s2,box) of one component at (x,y)."""
-    p = _f64(p9)
-    assert p.shape == (9,)
+def component_at(kind: str, p, x, y, mag=False):
+    """Value and d/d(xc,yc,theta,q,amp,s0,s1,s2,box[,m0]) of one component at (x,y).
+    p has 9 entries (intensity amplitude) or 10 (mag=True: amp slot = magnitude m,
+    last entry = zero point m0); the derivative vector has as many."""
+    p = _f64(p)
+    n = p.shape[0]
+    assert n in (9, 10) and (n == 10 or not mag)
+    p10 = np.zeros(10); p10[:n] = p
     I = C.c_double(0.0)
-    dI = np.zeros(9)
-    lib().gmo_component_at(KINDS[kind], _dp(p), float(x), float(y), C.byref(I), _dp(dI))
-    return I.value, dI
+    dI = np.zeros(10)
+    lib().gmo_component_at(KINDS[kind], int(bool(mag)), _dp(p10), float(x), float(y), C.byref(I), _dp(dI))
+    return I.value, dI[:n]
+
+
+def amplitude_from_mag(kind: str, p10):
+    """Eq. 5 / 8 / 10 / 15: (amplitude, d ln amp / d slot [10]) for slot values p10."""
+    p = _f64(p10)
+    assert p.shape == (10,)
+    amp = C.c_double(0.0)
+    dla = np.zeros(10)
+    rc = lib().gmo_amplitude_from_mag(KINDS[kind], _dp(p), C.byref(amp), _dp(dla))
+    assert rc == 0, rc
+    return amp.value, dla
 
 
 def conv2d_same(S, psf):

@@ -49,15 +49,19 @@
 #define GMO_MOFFAT   5
 #define GMO_SKY      6
 
-/* component descriptor: 11 int32 per component
- *   [0] kind  [1] convolve flag  [2..10] parameter-vector index ("slot") for
- *   xc, yc, theta[rad], q, amplitude, s0, s1, s2, boxiness B ; -1 = unused.
+/* component descriptor: 12 int32 per component
+ *   [0] kind  [1] convolve flag  [2..11] parameter-vector index ("slot") for
+ *   xc, yc, theta[rad], q, amplitude, s0, s1, s2, boxiness B, zero point m0 ;
+ *   -1 = unused.  When the m0 slot is used the amplitude slot holds a MAGNITUDE m
+ *   and the intensity follows from Eq. 5 / 8 / 10 / 15 (P:84-93, P:115, P:129,
+ *   P:178) with the zero point m0 = par[slot m0] (the paper's gm.p(m, M0=...),
+ *   P:279-281; m0 is normally held fixed by the caller's free_mask).
  *   Sersic: amp=Ie s0=re s1=n | Exp: amp=I0 s0=rs | Ferrer: amp=I0 s0=r_out
  *   s1=a s2=b | King: amp=I0 s0=rc s1=rt s2=alpha | Gaussian: amp=I0 s0=FWHM |
  *   Moffat: amp=I0 s0=FWHM s1=n | Sky: amp=I_sky.
  *   Two components naming the same index share ("tie") that parameter. */
-#define GMO_DESC 11
-enum { S_XC = 0, S_YC, S_TH, S_Q, S_AMP, S_S0, S_S1, S_S2, S_BOX, N_SLOT };
+#define GMO_DESC 12
+enum { S_XC = 0, S_YC, S_TH, S_Q, S_AMP, S_S0, S_S1, S_S2, S_BOX, S_M0, N_SLOT };
 
 #define GMO_RGUARD 1e-6 /* reading S4 */
 
@@ -196,6 +200,59 @@ double gmo_loglike(double chi2, double k)
     return -0.5 * k * log(2.0) - lgamma(0.5 * k) + (0.5 * k - 1.0) * log(chi2) - 0.5 * chi2;
 }
 
+/* Amplitude (I_e or I_0) from the magnitude parameterisation, and the derivatives
+ * of its logarithm with respect to every slot it depends on:
+ *   flux = 10^{-0.4 (m - m0)};  amp = Eq. 5 (Sersic), 8 (ExpDisk), 10 (Ferrer),
+ *   15 (Moffat) exactly as printed (the helpers above).
+ * dla[k] = d ln(amp) / d slot_k.  With c = 2 + B, from Eq. 6:
+ *   ln r_box = ln(pi c / 2) - 2 lnGamma(1/c) + lnGamma(2/c)
+ *   d ln r_box / dB = 1/c + 2 [psi(1/c) - psi(2/c)] / c^2.
+ * Returns 0, or -1 for a kind the paper gives no magnitude relation for.        */
+static int amplitude_from_mag(int kind, const double p[/*N_SLOT*/], double nu, double dnu,
+                              double *amp, double dla[/*N_SLOT*/])
+{
+    const double ln10 = log(10.0);
+    const double m = p[S_AMP], m0 = p[S_M0], q = p[S_Q], B = p[S_BOX];
+    const double s0 = p[S_S0], s1 = p[S_S1], s2 = p[S_S2];
+    const double flux = pow(10.0, -0.4 * (m - m0));
+    const double c = 2.0 + B;
+    for (int k = 0; k < N_SLOT; ++k) dla[k] = 0.0;
+    dla[S_AMP] = -0.4 * ln10;                 /* d/dm  */
+    dla[S_M0] = +0.4 * ln10;                 /* d/dm0 */
+    dla[S_Q] = -1.0 / q;                    /* every relation carries 1/q */
+    dla[S_BOX] = 1.0 / c + 2.0 * (digamma_pos(1.0 / c) - digamma_pos(2.0 / c)) / (c * c);
+    switch (kind) {
+    case GMO_SERSIC: {  /* Eq. 5: r_box nu^{2n} F / (2 pi q re^2 n Gamma(2n) e^{nu}) */
+        const double re = s0, n = s1;
+        *amp = gmo_sersic_Ie_from_flux(flux, re, n, q, B);
+        dla[S_S0] = -2.0 / re;
+        dla[S_S1] = 2.0 * log(nu) + 2.0 * n * dnu / nu - 1.0 / n - 2.0 * digamma_pos(2.0 * n) - dnu;
+        return 0; }
+    case GMO_EXPDISK:   /* Eq. 8: r_box F / (2 pi q rs^2) */
+        *amp = gmo_expdisk_I0_from_flux(flux, s0, q, B);
+        dla[S_S0] = -2.0 / s0;
+        return 0;
+    case GMO_FERRER: {  /* Eq. 10: r_box F / (pi q rout^2 a beta(a, 1 + 2/(2-b))) */
+        const double rout = s0, a = s1, b = s2;
+        const double z = 1.0 + 2.0 / (2.0 - b);
+        *amp = gmo_ferrer_I0_from_flux(flux, rout, a, b, q, B);
+        dla[S_S0] = -2.0 / rout;
+        dla[S_S1] = -1.0 / a - (digamma_pos(a) - digamma_pos(a + z));
+        dla[S_S2] = -(digamma_pos(z) - digamma_pos(a + z)) * 2.0 / ((2.0 - b) * (2.0 - b));
+        return 0; }
+    case GMO_MOFFAT: {  /* Eq. 15 with rd of Eq. 14: r_box (n-1) F / (pi q rd^2) */
+        const double fwhm = s0, n = s1;
+        const double p2 = pow(2.0, 1.0 / n);
+        *amp = gmo_moffat_I0_from_flux(flux, fwhm, n, q, B);
+        dla[S_S0] = -2.0 / fwhm;
+        dla[S_S1] = 1.0 / (n - 1.0) - p2 * log(2.0) / (n * n * (p2 - 1.0));
+        return 0; }
+    default:
+        *amp = NAN;
+        return -1;
+    }
+}
+
 /* ------------------------------------------------------------------------- */
 /* radial profiles, Eq. 1, 7, 9, 11, 12, 13, 16, with their derivatives.      */
 /* value at r; derivative factors at rg = max(r, GMO_RGUARD) (reading S4).    */
@@ -296,8 +353,10 @@ static void profile_unit(int kind, double r, const double s[3], const gmo_aux *a
     }
 }
 
-/* one component at pixel centre (x,y): value I and dI/d(slot) for the 9 slots */
-static void component_eval(int kind, const double p[N_SLOT], const gmo_aux *aux,
+/* one component at pixel centre (x,y): value I and dI/d(slot) for the 10 slots.
+ * mag != 0: the amplitude slot holds a magnitude (amplitude_from_mag above); then
+ * dI/d(slot) gains I * d ln(amp)/d(slot) for every slot the amplitude depends on. */
+static void component_eval(int kind, int mag, const double p[N_SLOT], const gmo_aux *aux,
                            double x, double y, double *I, double dI[N_SLOT], int want_grad)
 {
     for (int k = 0; k < N_SLOT; ++k) dI[k] = 0.0;
@@ -306,8 +365,10 @@ static void component_eval(int kind, const double p[N_SLOT], const gmo_aux *aux,
         dI[S_AMP] = 1.0;
         return;
     }
-    const double xc = p[S_XC], yc = p[S_YC], th = p[S_TH], q = p[S_Q], amp = p[S_AMP];
+    const double xc = p[S_XC], yc = p[S_YC], th = p[S_TH], q = p[S_Q];
     const double B = p[S_BOX];
+    double amp = p[S_AMP], dla[N_SLOT];
+    if (mag) amplitude_from_mag(kind, p, aux->nu, aux->dnu, &amp, dla);
     const double c = B + 2.0;
     const double ct = cos(th), st = sin(th);
     const double dx = x - xc, dy = y - yc;
@@ -345,6 +406,10 @@ static void component_eval(int kind, const double p[N_SLOT], const gmo_aux *aux,
     dI[S_TH] = A * (dr_du * v + dr_dv * (-u));
     dI[S_Q]  = A * dr_dq;
     dI[S_BOX] = A * dr_dB;
+    if (mag) {
+        dI[S_AMP] = 0.0;
+        for (int k = 0; k < N_SLOT; ++k) dI[k] += (*I) * dla[k];
+    }
 }
 
 static void gather_params(const int32_t *d, const double *par, double p[N_SLOT])
@@ -372,10 +437,31 @@ static double pix_x(int j) { return j + 0.5; }
 static double pix_y(int i, int H) { return H - 0.5 - i; }
 
 /* exported for unit pins: one component, amplitude and all, at one point */
-void gmo_component_at(int kind, const double p[N_SLOT], double x, double y, double *I, double *dI /*[9]*/)
+void gmo_component_at(int kind, int mag, const double p[N_SLOT], double x, double y, double *I, double *dI /*[10]*/)
 {
     gmo_aux aux; make_aux(kind, p, &aux);
-    component_eval(kind, p, &aux, x, y, I, dI, 1);
+    component_eval(kind, mag, p, &aux, x, y, I, dI, 1);
+}
+
+/* exported for unit pins: amplitude of the magnitude parameterisation and d ln(amp)/d slot */
+int gmo_amplitude_from_mag(int kind, const double p[N_SLOT], double *amp, double *dla /*[10]*/)
+{
+    gmo_aux aux; make_aux(kind, p, &aux);
+    return amplitude_from_mag(kind, p, aux.nu, aux.dnu, amp, dla);
+}
+
+static int uses_mag(const int32_t *d) { return d[2 + S_M0] >= 0; }
+
+/* descriptor check shared by the batched entry points: the paper gives a magnitude
+ * relation for Sersic, ExpDisk, Ferrer and Moffat only */
+static int desc_ok(int n_comp, const int32_t *desc)
+{
+    for (int c = 0; c < n_comp; ++c) {
+        const int32_t *d = desc + c * GMO_DESC;
+        if (uses_mag(d) && !(d[0] == GMO_SERSIC || d[0] == GMO_EXPDISK || d[0] == GMO_FERRER || d[0] == GMO_MOFFAT))
+            return 0;
+    }
+    return 1;
 }
 
 /* ------------------------------------------------------------------------- */
@@ -439,7 +525,7 @@ static void model_one(int n_comp, const int32_t *desc, int H, int W, int K, cons
         double *dst = is_convolved(d) ? S : U;
         for (int i = 0; i < H; ++i)
             for (int j = 0; j < W; ++j) {
-                component_eval(d[0], p, &aux, pix_x(j), pix_y(i, H), &I, dI, 0);
+                component_eval(d[0], uses_mag(d), p, &aux, pix_x(j), pix_y(i, H), &I, dI, 0);
                 dst[i * W + j] += I;
             }
     }
@@ -451,6 +537,7 @@ int gmo_render(int n_comp, const int32_t *desc, int n_par, int B, int H, int W, 
                const double *psf, int64_t psf_stride, const double *params, double *model)
 {
     if (K < 1 || (K & 1) == 0) return -1;
+    if (!desc_ok(n_comp, desc)) return -3;
     const int64_t N = (int64_t)H * W;
     int err = 0;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -503,7 +590,7 @@ static double loss_grad_one(int n_comp, const int32_t *desc, int n_par, int H, i
             double acc[N_SLOT] = { 0 };
             for (int i = 0; i < H; ++i)
                 for (int j = 0; j < W; ++j) {
-                    component_eval(d[0], p, &aux, pix_x(j), pix_y(i, H), &I, dI, 1);
+                    component_eval(d[0], uses_mag(d), p, &aux, pix_x(j), pix_y(i, H), &I, dI, 1);
                     const double sd = seed[i * W + j];
                     for (int k = 0; k < N_SLOT; ++k) acc[k] += sd * dI[k];
                 }
@@ -527,7 +614,7 @@ static double loss_grad_one(int n_comp, const int32_t *desc, int n_par, int H, i
                 if (slot < 0) continue;
                 for (int i = 0; i < H; ++i)
                     for (int j = 0; j < W; ++j) {
-                        component_eval(d[0], p, &aux, pix_x(j), pix_y(i, H), &I, dI, 1);
+                        component_eval(d[0], uses_mag(d), p, &aux, pix_x(j), pix_y(i, H), &I, dI, 1);
                         dS[i * W + j] = dI[k];
                     }
                 if (is_convolved(d)) gmo_conv2d_same(dS, H, W, psf, K, dM);
@@ -564,6 +651,7 @@ int gmo_loss_grad(int n_comp, const int32_t *desc, int n_par, int B, int H, int 
                   double *jtj, double *jtr)
 {
     if (K < 1 || (K & 1) == 0) return -1;
+    if (!desc_ok(n_comp, desc)) return -3;
     const int64_t N = (int64_t)H * W;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int g = 0; g < B; ++g) {
@@ -718,6 +806,7 @@ int gmo_fit(int n_comp, const int32_t *desc, int n_par, int B, int H, int W, int
             double *chi2_out, int32_t *iters_used, int32_t *status, double *trace /*[B,n_iter] or NULL*/)
 {
     if (K < 1 || (K & 1) == 0) return -1;
+    if (!desc_ok(n_comp, desc)) return -3;
     const int64_t N = (int64_t)H * W;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int g = 0; g < B; ++g) {
