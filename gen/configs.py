@@ -113,6 +113,10 @@ _ROLE = {  # role: (lr, log10_space, lo, hi)   lo/hi None = set from the cutout 
     "index": (0.01, 1, 0.3, 8.0), "q": (0.01, 0, 0.05, 1.0),
     "theta": (0.02, 0, -np.inf, np.inf), "shape": (0.01, 0, 0.05, 10.0),
     "sky": (0.01, 0, -np.inf, np.inf),
+    # boxiness B of Eq. 2 (c = B + 2 stays well above 0), magnitude m with
+    # its zero point m0 (Eq. 5; 0.025 mag = 0.01 dex in flux, the step of an "amp")
+    "box": (0.01, 0, -1.0, 2.0), "mag": (0.025, 0, -np.inf, np.inf),
+    "zeropoint": (0.0, 0, -np.inf, np.inf),
 }
 
 
@@ -142,7 +146,9 @@ def fit_options(model: dict, H: int, W: int, n_iter: int, tol: float = 0.0, pati
     decay = 0.01 ** (1.0 / max(n_iter - 1, 1))      # last step ~1 % of the first (O2)
     return {"n_iter": int(n_iter), "beta1": 0.9, "beta2": 0.999, "eps": 1e-8, "lr_decay": decay,
             "lr": lr.astype(np.float32), "lo": lo.astype(np.float32), "hi": hi.astype(np.float32),
-            "log10_space": lg, "free_mask": np.ones(P, dtype=np.uint8), "tol": float(tol),
+            "log10_space": lg,
+            "free_mask": np.array([r != "zeropoint" for r in model["roles"]], dtype=np.uint8),   # m0 is given
+            "tol": float(tol),
             "patience": int(patience)}
 
 

@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   100     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   101     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
@@ -64,7 +64,7 @@ typedef enum {
 
 /* index of each quantity inside gm_component.slot[] */
 enum { GM_SLOT_XC = 0, GM_SLOT_YC, GM_SLOT_THETA, GM_SLOT_Q, GM_SLOT_AMP,
-       GM_SLOT_S0, GM_SLOT_S1, GM_SLOT_S2, GM_SLOT_BOX, GM_NSLOT };
+       GM_SLOT_S0, GM_SLOT_S1, GM_SLOT_S2, GM_SLOT_BOX, GM_SLOT_M0, GM_NSLOT };
 
 /* One summed component (host memory, POD).  slot[k] is the index, inside the
  * galaxy's parameter vector, of the k-th quantity, or -1 when unused:
@@ -78,8 +78,19 @@ enum { GM_SLOT_XC = 0, GM_SLOT_YC, GM_SLOT_THETA, GM_SLOT_Q, GM_SLOT_AMP,
  * Unused q means 1 (circular), unused theta means 0, unused box means B = 0.
  * Two components naming the same index are TIED: their gradients add.
  * convolve = 1: the component goes through the PSF; 0: added after it.
- * A boxiness slot (Eq. 2 with B != 0) is accepted by the ABI; kernels for it
- * are not built yet and the call returns GM_ENOTSUP. */
+ * box: the boxiness B of the generalised ellipse, Eq. 2:
+ *   r = (|u|^(B+2) + |v/q|^(B+2))^(1/(B+2)), B > -2; its gradient entry is d chi2 / dB.
+ * m0: when this slot is used the amplitude slot holds a MAGNITUDE m and the slot itself
+ *   the zero point m0 (the paper's gm.p(m, M0=...)); the intensity is
+ *     Sersic  Ie = r_box nu^(2n) F / (2 pi q re^2 n Gamma(2n) e^nu)          Eq. 5
+ *     ExpDisk I0 = r_box F / (2 pi q rs^2)                                     Eq. 8
+ *     Ferrer  I0 = r_box F / (pi q r_out^2 a beta(a, 1 + 2/(2-b)))             Eq. 10
+ *     Moffat  I0 = r_box (n-1) F / (pi q rd^2), rd of Eq. 14                   Eq. 15
+ *   with F = 10^(-0.4 (m - m0)) and r_box = pi (2+B) / (2 beta(1/(2+B), 1/(2+B))) (Eq. 6),
+ *   evaluated in fp64 per galaxy; the gradient is then with respect to m (and m0, q, the
+ *   shape slots and B gain the terms through the amplitude).  m0 is normally held fixed
+ *   through gm_fit_opts.free_mask.  King, Gaussian and Sky have no magnitude relation in
+ *   the paper: a used m0 slot there is GM_EINVAL. */
 typedef struct {
   int32_t kind;
   int32_t convolve;

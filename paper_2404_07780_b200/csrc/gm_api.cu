@@ -175,6 +175,9 @@ __device__ __forceinline__ float assemble(const FinArgs& a, int b, int lane, flo
     for (int c = 0; c < a.md.n_comp; ++c) {
       const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
       const float* s = sh + c * kNSum;
+      // magnitude mode (Eq. 5, 8, 10, 15): d chi2 / d ln(amp) = amp * sum seed U, spread over
+      // every slot the amplitude depends on
+      const float dlamp = a.md.mag[c] ? cc.amp * s[4] : 0.0f;
 #pragma unroll
       for (int k = 0; k < GM_NSLOT; ++k) {
         if (a.md.slot[c][k] != lane) continue;
@@ -182,12 +185,14 @@ __device__ __forceinline__ float assemble(const FinArgs& a, int b, int lane, flo
         switch (k) {
           case GM_SLOT_XC: v = -cc.ct * s[0] + cc.st * cc.iq * s[1]; break;
           case GM_SLOT_YC: v = -cc.st * s[0] - cc.ct * cc.iq * s[1]; break;
-          case GM_SLOT_THETA: v = (cc.q - cc.iq) * s[2]; break;
-          case GM_SLOT_Q: v = -cc.iq * s[3]; break;
-          case GM_SLOT_AMP: v = s[4]; break;
-          case GM_SLOT_S0: v = s[5]; break;
-          case GM_SLOT_S1: v = s[6]; break;
-          case GM_SLOT_S2: v = s[7]; break;
+          case GM_SLOT_THETA: v = cc.q * s[2] - cc.iq * s[8]; break;
+          case GM_SLOT_Q: v = -cc.iq * s[3] + dlamp * cc.dl_q; break;
+          case GM_SLOT_AMP: v = a.md.mag[c] ? dlamp * cc.dl_m : s[4]; break;
+          case GM_SLOT_S0: v = s[5] + dlamp * cc.dl_s0; break;
+          case GM_SLOT_S1: v = s[6] + dlamp * cc.dl_s1; break;
+          case GM_SLOT_S2: v = s[7] + dlamp * cc.dl_s2; break;
+          case GM_SLOT_BOX: v = s[9] + dlamp * cc.dl_box; break;
+          case GM_SLOT_M0: v = -dlamp * cc.dl_m; break;
           default: break;
         }
         g += v;
@@ -469,7 +474,7 @@ static int validate(const gm_model* m, const gm_batch* bt, bool need_data, Model
   md->n_comp = m->n_comp;
   md->n_par = m->n_par;
   for (int c = 0; c < GM_MAX_COMP; ++c) {
-    md->kind[c] = GM_SKY; md->conv[c] = 0;
+    md->kind[c] = GM_SKY; md->conv[c] = 0; md->box[c] = 0; md->mag[c] = 0;
     for (int k = 0; k < GM_NSLOT; ++k) md->slot[c][k] = -1;
   }
   for (int c = 0; c < m->n_comp; ++c) {
@@ -484,7 +489,12 @@ static int validate(const gm_model* m, const gm_batch* bt, bool need_data, Model
     }
     if (gc.slot[GM_SLOT_AMP] < 0) return GM_EINVAL;
     if (gc.kind != GM_SKY && gc.slot[GM_SLOT_S0] < 0) return GM_EINVAL;
-    if (gc.slot[GM_SLOT_BOX] >= 0) return GM_ENOTSUP;     // Eq. 2 with B != 0: not built yet
+    md->box[c] = (gc.kind != GM_SKY && gc.slot[GM_SLOT_BOX] >= 0) ? 1 : 0;
+    md->mag[c] = gc.slot[GM_SLOT_M0] >= 0 ? 1 : 0;
+    // the paper gives a magnitude relation for Eq. 1, 7, 9 and 13 only (Eq. 5, 8, 10, 15)
+    if (md->mag[c] && !(gc.kind == GM_SERSIC || gc.kind == GM_EXPDISK || gc.kind == GM_FERRER ||
+                        gc.kind == GM_MOFFAT))
+      return GM_EINVAL;
   }
   return GM_OK;
 }

@@ -21,29 +21,26 @@ struct ModelDesc {
   int32_t kind[GM_MAX_COMP];
   int32_t conv[GM_MAX_COMP];                   // 1: through the PSF
   int8_t slot[GM_MAX_COMP][GM_NSLOT];          // -1 unused
+  int8_t box[GM_MAX_COMP];                     // 1: boxiness slot used (Eq. 2 with B != 0)
+  int8_t mag[GM_MAX_COMP];                     // 1: amplitude slot holds a magnitude (Eq. 5/8/10/15)
 };
 
-// per (galaxy, component) constants produced by the prologue (step a0), 64 bytes
+// per (galaxy, component) constants produced by the prologue (step a0), 96 bytes
 struct __align__(16) CompConst {
   float xc, yc, ct, st;      // centre, cos/sin(theta)
-  float iq, q, amp, a0;      // 1/q, q, amplitude, kind specific ...
+  float iq, q, amp, a0;      // 1/q, q, amplitude (intensity), kind specific ...
   float a1, a2, a3, a4;
   float a5, a6, a7, a8;
+  float c, ic, cm1, dl_box;  // Eq. 2 exponent c = B + 2, 1/c, c - 1; d ln(amp) / dB
+  float dl_m, dl_q, dl_s0, dl_s1;   // magnitude mode: d ln(amp) / d (m, q, s0, s1, s2);
+  float dl_s2, pad0, pad1, pad2;    //   d/d m0 = -dl_m
 };
 
 // ---------------------------------------------------------------------------
-// step a1: elliptical radius, Eq. 2-4 with B = 0 (R:G2): rotate, then scale v by 1/q
+// step a1: elliptical radius, Eq. 2-4 (R:G2): rotate, then scale v by 1/q;
+// r = sqrt(u^2 + (v/q)^2) for B = 0, else r = (|u|^c + |v/q|^c)^(1/c), c = B + 2
 // ---------------------------------------------------------------------------
 struct Geo { float u, vq, r; };
-
-__device__ __forceinline__ Geo geometry(const CompConst& cc, float x, float y) {
-  const float dx = x - cc.xc, dy = y - cc.yc;
-  Geo g;
-  g.u = fmaf(cc.ct, dx, cc.st * dy);
-  g.vq = fmaf(cc.ct, dy, -cc.st * dx) * cc.iq;
-  g.r = sqrtf(fmaf(g.u, g.u, g.vq * g.vq));
-  return g;
-}
 
 // SFU forms.  FAST = MUFU.LG2 / MUFU.EX2 approximations (~2^-22 error): used by the
 // gradient pass (tolerance 1e-3 of the gradient norm).  !FAST = log2f / exp2f of the
@@ -55,6 +52,45 @@ template <bool FAST> __device__ __forceinline__ float lg2(float x) {
 template <bool FAST> __device__ __forceinline__ float ex2(float x) {
   if (FAST) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   return exp2f(x);
+}
+
+template <bool FAST>
+__device__ __forceinline__ Geo geometry(const CompConst& cc, bool box, float x, float y) {
+  const float dx = x - cc.xc, dy = y - cc.yc;
+  Geo g;
+  g.u = fmaf(cc.ct, dx, cc.st * dy);
+  g.vq = fmaf(cc.ct, dy, -cc.st * dx) * cc.iq;
+  if (box) {                                   // warp-uniform: a property of the component
+    const float uc = ex2<FAST>(cc.c * lg2<FAST>(fabsf(g.u)));      // 0 at u = 0 (c > 0)
+    const float vc = ex2<FAST>(cc.c * lg2<FAST>(fabsf(g.vq)));
+    g.r = ex2<FAST>(cc.ic * lg2<FAST>(uc + vc));
+  } else {
+    g.r = sqrtf(fmaf(g.u, g.u, g.vq * g.vq));
+  }
+  return g;
+}
+
+// d r / d u, d r / d (v/q) and d r / d B at rg = max(r, 1e-6) (R:S4), Eq. 2:
+//   dr/du = sgn(u) |u|^(c-1) / rg^(c-1)                      (u / rg when B = 0)
+//   dr/dB = (rg / c) [(|u|^c ln|u| + |v/q|^c ln|v/q|) / (|u|^c + |v/q|^c) - ln rg]
+struct GeoGrad { float gu, gv, db; };
+template <bool FAST>
+__device__ __forceinline__ GeoGrad geometry_grad(const CompConst& cc, bool box, const Geo& g, float rg) {
+  GeoGrad d;
+  if (box) {
+    const float au = fabsf(g.u), av = fabsf(g.vq);
+    const float lu = lg2<FAST>(au), lv = lg2<FAST>(av), lr = lg2<FAST>(rg);
+    const float uc = ex2<FAST>(cc.c * lu), vc = ex2<FAST>(cc.c * lv);
+    d.gu = au > 0.0f ? copysignf(ex2<FAST>(cc.cm1 * (lu - lr)), g.u) : 0.0f;
+    d.gv = av > 0.0f ? copysignf(ex2<FAST>(cc.cm1 * (lv - lr)), g.vq) : 0.0f;
+    const float tu = au > 0.0f ? uc * lu : 0.0f, tv = av > 0.0f ? vc * lv : 0.0f;
+    const float sum = uc + vc;
+    d.db = sum > 0.0f ? rg * cc.ic * kLn2 * (__fdividef(tu + tv, sum) - lr) : 0.0f;
+  } else {
+    const float ir = __fdividef(1.0f, rg);
+    d.gu = g.u * ir; d.gv = g.vq * ir; d.db = 0.0f;
+  }
+  return d;
 }
 
 // radial law with unit amplitude at radius r (value only); KIND is a gm_kind
@@ -172,31 +208,86 @@ __device__ __forceinline__ void profile_grad_t(const CompConst& cc, float rg, fl
 // d I / d (slot k) of one component at pixel centre (x, y): the forward-mode column of
 // the Jacobian J = dM/dp used by the covariance row.  Same guards as the
 // gradient pass (R:S4): derivative factors at rg = max(r, 1e-6), d/d amp at r itself.
+// mag: the amplitude slot is a magnitude; every slot the amplitude depends on gains
+// I * d ln(amp) / d slot (Eq. 5, 8, 10, 15).
 template <int KIND>
-__device__ __forceinline__ float component_deriv_t(const CompConst& cc, int k, float x, float y) {
+__device__ __forceinline__ float component_deriv_t(const CompConst& cc, bool box, bool mag, int k, float x, float y) {
   if (KIND == GM_SKY) return k == GM_SLOT_AMP ? 1.0f : 0.0f;
-  const Geo g = geometry(cc, x, y);
+  const Geo g = geometry<false>(cc, box, x, y);
   const float rg = fmaxf(g.r, kRGuard);
   float U, dUdr, d0, d1, d2;
   profile_grad_t<KIND, false>(cc, rg, U, dUdr, d0, d1, d2);
-  const float cgeo = cc.amp * dUdr / rg;
+  const GeoGrad d = geometry_grad<false>(cc, box, g, rg);
+  const float A = cc.amp * dUdr;
+  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+  const float I = cc.amp * Uv;
   switch (k) {
-    case GM_SLOT_XC: return cgeo * (-cc.ct * g.u + cc.st * cc.iq * g.vq);
-    case GM_SLOT_YC: return cgeo * (-cc.st * g.u - cc.ct * cc.iq * g.vq);
-    case GM_SLOT_THETA: return cgeo * (cc.q - cc.iq) * g.u * g.vq;
-    case GM_SLOT_Q: return -cc.iq * cgeo * g.vq * g.vq;
-    case GM_SLOT_AMP: return (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
-    case GM_SLOT_S0: return cc.amp * d0;
-    case GM_SLOT_S1: return cc.amp * d1;
-    case GM_SLOT_S2: return cc.amp * d2;
+    case GM_SLOT_XC: return A * (-cc.ct * d.gu + cc.st * cc.iq * d.gv);
+    case GM_SLOT_YC: return A * (-cc.st * d.gu - cc.ct * cc.iq * d.gv);
+    case GM_SLOT_THETA:                        // B = 0: u (v/q) (q - 1/q) / r, exactly 0 at q = 1
+      return box ? A * (cc.q * d.gu * g.vq - cc.iq * d.gv * g.u) : A * d.gu * g.vq * (cc.q - cc.iq);
+    case GM_SLOT_Q: return -cc.iq * A * d.gv * g.vq + (mag ? I * cc.dl_q : 0.0f);
+    case GM_SLOT_AMP: return mag ? I * cc.dl_m : Uv;
+    case GM_SLOT_S0: return cc.amp * d0 + (mag ? I * cc.dl_s0 : 0.0f);
+    case GM_SLOT_S1: return cc.amp * d1 + (mag ? I * cc.dl_s1 : 0.0f);
+    case GM_SLOT_S2: return cc.amp * d2 + (mag ? I * cc.dl_s2 : 0.0f);
+    case GM_SLOT_BOX: return A * d.db + (mag ? I * cc.dl_box : 0.0f);
+    case GM_SLOT_M0: return mag ? -I * cc.dl_m : 0.0f;
     default: return 0.0f;
   }
 }
 
-__device__ __forceinline__ float component_deriv(int kind, const CompConst& cc, int k, float x, float y) {
+__device__ __forceinline__ float component_deriv(int kind, const CompConst& cc, bool box, bool mag, int k,
+                                                 float x, float y) {
   float v = 0.0f;
-  dispatch_kind(kind, [&]<int KIND>() { v = component_deriv_t<KIND>(cc, k, x, y); });
+  dispatch_kind(kind, [&]<int KIND>() { v = component_deriv_t<KIND>(cc, box, mag, k, x, y); });
   return v;
+}
+
+// ---------------------------------------------------------------------------
+// step a5: one pixel's contribution to the partial sums of a component.  With
+// seed = A (convolved) or G (unconvolved), X = seed * amp * dU/dr:
+//   s0 = sum X dr/du        s1 = sum X dr/d(v/q)     s2 = sum X dr/du (v/q)
+//   s3 = sum X dr/d(v/q) (v/q)                       s4 = sum seed U
+//   s5..s7 = sum seed amp dU/d(s0, s1, s2)
+//   s8 = sum X dr/d(v/q) u  (= s2 when B = 0)        s9 = sum X dr/dB
+// from which (assemble, gm_api.cu)
+//   d/dxc = -ct s0 + st s1 / q      d/dyc = -st s0 - ct s1 / q
+//   d/dtheta = q s2 - s8 / q        d/dq = -s3 / q        d/dB = s9
+// ---------------------------------------------------------------------------
+constexpr int kNSum = 10;
+
+template <int KIND>
+__device__ __forceinline__ void grad_accumulate(const CompConst& cc, bool box, float seed, float x, float y,
+                                                float (&s)[kNSum]) {
+  if (KIND == GM_SKY) { s[4] += seed; return; }
+  const Geo g = geometry<true>(cc, box, x, y);
+  const float rg = fmaxf(g.r, kRGuard);
+  float U, dUdr, d0, d1, d2;
+  profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
+  // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
+  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+  const float sa = seed * cc.amp;
+  if (box) {
+    const GeoGrad d = geometry_grad<true>(cc, true, g, rg);
+    const float X = sa * dUdr;
+    s[0] = fmaf(X, d.gu, s[0]);
+    s[1] = fmaf(X, d.gv, s[1]);
+    s[2] = fmaf(X * d.gu, g.vq, s[2]);
+    s[3] = fmaf(X * d.gv, g.vq, s[3]);
+    s[8] = fmaf(X * d.gv, g.u, s[8]);
+    s[9] = fmaf(X, d.db, s[9]);
+  } else {
+    const float cgeo = __fdividef(sa * dUdr, rg);
+    s[0] = fmaf(cgeo, g.u, s[0]);
+    s[1] = fmaf(cgeo, g.vq, s[1]);
+    s[2] = fmaf(cgeo * g.u, g.vq, s[2]);
+    s[3] = fmaf(cgeo * g.vq, g.vq, s[3]);
+  }
+  s[4] = fmaf(seed, Uv, s[4]);
+  s[5] = fmaf(sa, d0, s[5]);
+  s[6] = fmaf(sa, d1, s[6]);
+  s[7] = fmaf(sa, d2, s[7]);
 }
 
 }  // namespace gm

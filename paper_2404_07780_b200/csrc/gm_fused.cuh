@@ -1,6 +1,6 @@
 // gm_fused.cuh -- the fused loss + gradient kernel for cutouts that fit one CTA tile
 // (H, W <= 128): steps a1..a5 of SURVEY.md section 8(a) in ONE launch, with nothing but
-// chi^2 and the 8 partial sums per component leaving the SM.
+// chi^2 and the kNSum partial sums per component leaving the SM.
 //
 // One persistent CTA per SM, 512 threads, two roles that run concurrently:
 //
@@ -38,7 +38,7 @@ struct FusedArgs {
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                  // [B,H,W]: model_out (mode 0) or back-seed spill (any_unconv)
   float* chi2_part;          // [B]      (tiles = 1)
-  float* grad_part;          // [B, n_comp, 8]
+  float* grad_part;          // [B, n_comp, kNSum]
   const int* frozen;
 };
 
@@ -148,6 +148,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
       if (zero_pass && !first) break;
       if (!zero_pass && !a.md.conv[c]) continue;
       const CompConst cc = ccb[zero_pass ? 0 : c];
+      const bool box = !zero_pass && a.md.box[c] != 0;
       dispatch_kind(zero_pass ? (int)GM_SKY : a.md.kind[c], [&]<int KIND>() {
         for (int yy = hw; yy < tg.rows; yy += kHelpWarps) {
           const int i = yy - h;
@@ -159,7 +160,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
             const bool in = row_in && xx < cols && j >= 0 && j < tg.W;
             float sv = 0.0f;
             if (KIND != GM_SKY && in)
-              sv = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry(cc, (float)j + 0.5f, y).r);
+              sv = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry<kFastForward>(cc, box, (float)j + 0.5f, y).r);
             if (first) rowp[xx] = sv;
             else if (in) rowp[xx] += sv;
           }
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
         if (a.md.conv[c]) continue;
         const CompConst cc = ccb[c];
         const int kind = a.md.kind[c];
-        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
+        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry<false>(cc, a.md.box[c] != 0, x, y).r);
         m = fmaf(cc.amp, U, m);
       }
       return m;
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
     }
   };
 
-  // a5: the 8 partial sums of every component from A (buffer interior)
+  // a5: the partial sums of every component from A (buffer interior)
   auto gradient = [&](int g, int s) {
     const float* buf = buf0 + s * buf_elems;
     const CompConst* ccb = a.cc + (size_t)g * a.md.n_comp;
@@ -286,31 +287,17 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
 #pragma unroll
       for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
       const CompConst cc = ccb[c];
-      const bool conv = a.md.conv[c] != 0;
+      const bool conv = a.md.conv[c] != 0, box = a.md.box[c] != 0;
       dispatch_kind(a.md.kind[c], [&]<int KIND>() {
         for (int i = hw; i < tg.H; i += kHelpWarps) {
           const float y = (float)tg.H - 0.5f - (float)i;
           for (int j = lane; j < tg.W; j += 32) {
             const float seed = conv ? buf[(size_t)(i + h) * tg.pitch + j + h] : Gb[(size_t)i * tg.W + j];
-            if (KIND == GM_SKY) { sm[4] += seed; continue; }
-            const Geo ge = geometry(cc, (float)j + 0.5f, y);
-            const float rg = fmaxf(ge.r, kRGuard);
-            float U, dUdr, d0, d1, d2;
-            profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
-            const float Uv = (ge.r < kRGuard) ? profile_value_t<KIND, false>(cc, ge.r) : U;
-            const float sa = seed * cc.amp;
-            const float cgeo = __fdividef(sa * dUdr, rg);
-            sm[0] = fmaf(cgeo, ge.u, sm[0]);
-            sm[1] = fmaf(cgeo, ge.vq, sm[1]);
-            sm[2] = fmaf(cgeo * ge.u, ge.vq, sm[2]);
-            sm[3] = fmaf(cgeo * ge.vq, ge.vq, sm[3]);
-            sm[4] = fmaf(seed, Uv, sm[4]);
-            sm[5] = fmaf(sa, d0, sm[5]);
-            sm[6] = fmaf(sa, d1, sm[6]);
-            sm[7] = fmaf(sa, d2, sm[7]);
+            grad_accumulate<KIND>(cc, box, seed, (float)j + 0.5f, y, sm);
           }
         }
       });
+      if (!box) sm[8] = sm[2];
 #pragma unroll
       for (int k = 0; k < kNSum; ++k) {
         const float v = warp_sum(sm[k]);

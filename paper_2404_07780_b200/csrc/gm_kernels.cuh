@@ -24,7 +24,6 @@
 namespace gm {
 
 constexpr int kTR = 8, kTC = 8;            // thread tile (rows x cols)
-constexpr int kNSum = 8;                   // partial sums per component
 #ifdef GM_FAST_FORWARD
 constexpr bool kFastForward = true;        // experiment: SFU approximations in the forward render
 #else
@@ -64,7 +63,7 @@ struct BwdArgs {
   const CompConst* cc;
   const float2* taps; long long taps_stride;   // paired unflipped taps
   const float* G;          // [B,H,W]
-  float* grad_part;        // [B, tiles, n_comp, 8]
+  float* grad_part;        // [B, tiles, n_comp, kNSum]
   const int* frozen;
 };
 
@@ -210,7 +209,7 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
   const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
   const int cols = tg.TW + K - 1;
   bool first = true;
-  auto fill = [&](int kind, const CompConst cc, int slot) {
+  auto fill = [&](int kind, const CompConst cc, bool box, bool mag, int slot) {
     dispatch_kind(kind, [&]<int KIND>() {
       for (int yy = wid; yy < tg.rows; yy += nwarps) {
         const int i = i0 - h + yy;
@@ -222,8 +221,8 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
           const bool in = row_in && xx < cols && j >= 0 && j < tg.W;
           float s = 0.0f;
           if (KIND != GM_SKY && in) {
-            if (MODE == FWD_DERIV) s = component_deriv_t<KIND>(cc, slot, (float)j + 0.5f, y);
-            else s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry(cc, (float)j + 0.5f, y).r);
+            if (MODE == FWD_DERIV) s = component_deriv_t<KIND>(cc, box, mag, slot, (float)j + 0.5f, y);
+            else s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry<kFastForward>(cc, box, (float)j + 0.5f, y).r);
           }
           if (first) rowp[xx] = s;
           else if (in) rowp[xx] += s;
@@ -234,14 +233,15 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
   };
   for (int c = 0; c < a.md.n_comp; ++c) {
     if (!a.md.conv[c]) continue;
+    const bool box = a.md.box[c] != 0, mag = a.md.mag[c] != 0;
     if (MODE == FWD_DERIV) {
-      for (int k = 0; k < GM_SLOT_BOX; ++k)
-        if (a.md.slot[c][k] == a.dpar) fill(a.md.kind[c], ccb[c], k);
+      for (int k = 0; k < GM_NSLOT; ++k)
+        if (a.md.slot[c][k] == a.dpar) fill(a.md.kind[c], ccb[c], box, mag, k);
     } else {
-      fill(a.md.kind[c], ccb[c], -1);
+      fill(a.md.kind[c], ccb[c], box, mag, -1);
     }
   }
-  if (first) fill((int)GM_SKY, ccb[0], -1);            // nothing convolved: a zero tile
+  if (first) fill((int)GM_SKY, ccb[0], false, false, -1);   // nothing convolved: a zero tile
   cp_async_wait_all();
   __syncthreads();
 
@@ -271,11 +271,12 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
       if (a.md.conv[c]) continue;
       const CompConst cc = ccb[c];
       const int kind = a.md.kind[c];
+      const bool box = a.md.box[c] != 0;
       if (MODE == FWD_DERIV) {
-        for (int k = 0; k < GM_SLOT_BOX; ++k)
-          if (a.md.slot[c][k] == a.dpar) m += component_deriv(kind, cc, k, x, y);
+        for (int k = 0; k < GM_NSLOT; ++k)
+          if (a.md.slot[c][k] == a.dpar) m += component_deriv(kind, cc, box, a.md.mag[c] != 0, k, x, y);
       } else {
-        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry(cc, x, y).r);
+        const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry<false>(cc, box, x, y).r);
         m = fmaf(cc.amp, U, m);
       }
     }
@@ -371,8 +372,7 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
 
 // ---------------------------------------------------------------------------
 // backward: adjoint convolution + parameter-gradient partial sums
-// per component: s0 = sum c u, s1 = sum c v/q, s2 = sum c u v/q, s3 = sum c (v/q)^2
-//   with c = seed amp dU/dr / rg ; s4 = sum seed U ; s5..s7 = sum seed amp dU/ds
+// (10 per component, see grad_accumulate in gm_device.cuh)
 // ---------------------------------------------------------------------------
 template <int K>
 __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
@@ -450,7 +450,7 @@ __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
 #pragma unroll
     for (int k = 0; k < kNSum; ++k) s[k] = 0.0f;
     const CompConst cc = ccb[c];
-    const bool conv = a.md.conv[c] != 0;
+    const bool conv = a.md.conv[c] != 0, box = a.md.box[c] != 0;
     dispatch_kind(a.md.kind[c], [&]<int KIND>() {
       for (int yy = wid; yy < tg.TH; yy += nwarps) {
         const int i = i0 + yy;
@@ -460,26 +460,11 @@ __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
           const int j = j0 + xx;
           if (j >= tg.W) break;
           const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
-          if (KIND == GM_SKY) { s[4] += seed; continue; }
-          const Geo g = geometry(cc, (float)j + 0.5f, y);
-          const float rg = fmaxf(g.r, kRGuard);
-          float U, dUdr, d0, d1, d2;
-          profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
-          // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
-          const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
-          const float sa = seed * cc.amp;
-          const float cgeo = __fdividef(sa * dUdr, rg);
-          s[0] = fmaf(cgeo, g.u, s[0]);
-          s[1] = fmaf(cgeo, g.vq, s[1]);
-          s[2] = fmaf(cgeo * g.u, g.vq, s[2]);
-          s[3] = fmaf(cgeo * g.vq, g.vq, s[3]);
-          s[4] = fmaf(seed, Uv, s[4]);
-          s[5] = fmaf(sa, d0, s[5]);
-          s[6] = fmaf(sa, d1, s[6]);
-          s[7] = fmaf(sa, d2, s[7]);
+          grad_accumulate<KIND>(cc, box, seed, (float)j + 0.5f, y, s);
         }
       }
     });
+    if (!box) s[8] = s[2];
 #pragma unroll
     for (int k = 0; k < kNSum; ++k) {
       const float v = warp_sum(s[k]);

@@ -161,6 +161,50 @@ __device__ inline void make_comp_const(const ModelDesc& md, int c, const float* 
     }
     default: break;                         // sky: amplitude only
   }
+  // Eq. 2 exponent and, in magnitude mode, the amplitude of Eq. 5 / 8 / 10 / 15 with the
+  // logarithmic derivatives the gradient needs (all fp64, once per galaxy and component)
+  const double Bx = get(GM_SLOT_BOX, 0.0), cexp = 2.0 + Bx;
+  cc.c = (float)cexp; cc.ic = (float)(1.0 / cexp); cc.cm1 = (float)(cexp - 1.0);
+  cc.dl_box = 0.0f; cc.dl_m = 0.0f; cc.dl_q = 0.0f; cc.dl_s0 = 0.0f; cc.dl_s1 = 0.0f; cc.dl_s2 = 0.0f;
+  cc.pad0 = cc.pad1 = cc.pad2 = 0.0f;
+  if (md.mag[c]) {
+    const double ln10 = 2.302585092994045684, pi = 3.14159265358979323846;
+    const double m = get(GM_SLOT_AMP, 0.0), m0 = get(GM_SLOT_M0, 0.0);
+    // Eq. 6: ln r_box = ln(pi c / 2) - 2 lnGamma(1/c) + lnGamma(2/c)
+    double lamp = log(pi * cexp / 2.0) - 2.0 * lgamma(1.0 / cexp) + lgamma(2.0 / cexp)
+                  - 0.4 * ln10 * (m - m0) - log(q);
+    cc.dl_box = (float)(1.0 / cexp + 2.0 * (digamma_pos(1.0 / cexp) - digamma_pos(2.0 / cexp)) / (cexp * cexp));
+    cc.dl_m = (float)(-0.4 * ln10);
+    cc.dl_q = (float)(-1.0 / q);
+    cc.dl_s0 = (float)(-2.0 / s0);
+    switch (md.kind[c]) {
+      case GM_SERSIC: {                     // Eq. 5
+        const double nu = a[3], dnu = a[4], n = s1;
+        lamp += 2.0 * n * log(nu) - log(2.0 * pi * s0 * s0 * n) - lgamma(2.0 * n) - nu;
+        cc.dl_s1 = (float)(2.0 * log(nu) + 2.0 * n * dnu / nu - 1.0 / n - 2.0 * digamma_pos(2.0 * n) - dnu);
+        break;
+      }
+      case GM_EXPDISK:                      // Eq. 8
+        lamp -= log(2.0 * pi * s0 * s0);
+        break;
+      case GM_FERRER: {                     // Eq. 10
+        const double fa = s1, z = 1.0 + 2.0 / (2.0 - s2);
+        lamp -= log(pi * s0 * s0 * fa) + lgamma(fa) + lgamma(z) - lgamma(fa + z);
+        cc.dl_s1 = (float)(-1.0 / fa - digamma_pos(fa) + digamma_pos(fa + z));
+        cc.dl_s2 = (float)((digamma_pos(fa + z) - digamma_pos(z)) * 2.0 / ((2.0 - s2) * (2.0 - s2)));
+        break;
+      }
+      case GM_MOFFAT: {                     // Eq. 15 with rd of Eq. 14
+        const double p2 = pow(2.0, 1.0 / s1);
+        const double rd = s0 / (2.0 * sqrt(p2 - 1.0));
+        lamp += log(s1 - 1.0) - log(pi * rd * rd);
+        cc.dl_s1 = (float)(1.0 / (s1 - 1.0) - p2 * log(2.0) / (s1 * s1 * (p2 - 1.0)));
+        break;
+      }
+      default: lamp = NAN; break;           // rejected by validate()
+    }
+    cc.amp = (float)exp(lamp);
+  }
   cc.a0 = (float)a[0]; cc.a1 = (float)a[1]; cc.a2 = (float)a[2]; cc.a3 = (float)a[3];
   cc.a4 = (float)a[4]; cc.a5 = (float)a[5]; cc.a6 = (float)a[6]; cc.a7 = (float)a[7];
   cc.a8 = (float)a[8];

@@ -25,6 +25,9 @@ def sample_params(model, H, W, rng):
         elif role == "theta": p[k] = rng.uniform(0.1, 3.0)
         elif role == "shape": p[k] = rng.uniform(1.2, 2.5)
         elif role == "sky": p[k] = rng.uniform(-0.1, 0.1)
+        elif role == "box": p[k] = rng.uniform(-0.5, 0.8)
+        elif role == "mag": p[k] = rng.uniform(16.5, 18.0)
+        elif role == "zeropoint": p[k] = 22.5
         if name.endswith("_b") or name == "b": p[k] = rng.uniform(0.2, 1.2)
         if name.endswith("rt"): p[k] = rng.uniform(9.0, 14.0)
         if name.endswith("rout"): p[k] = rng.uniform(7.0, 11.0)
