@@ -223,11 +223,29 @@ def run_ours(args):
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    multi = len(buckets) > 1 and not args.serial_buckets
+    side_streams = [torch.cuda.Stream() for _ in buckets] if multi else None
+
     def step():
         outs, n = [], 0
         for k in buckets:
+            k["params"].copy_(k["dev"][4])
+        if multi:
+            # every size bucket on its own stream, iterations interleaved (gm_fit_multi): the SMs a
+            # bucket leaves idle once most of its galaxies stopped early take another bucket's work
+            ev0 = torch.cuda.Event(); ev0.record(stream)
+            for s in side_streams:
+                s.wait_event(ev0)
+            outs = gm.gm_fit_multi(model, [{"params": k["params"], "data": k["dev"][0], "sigma": k["dev"][1],
+                                            "mask": k["dev"][2], "psf": k["dev"][3], "opts": k["opts"],
+                                            "workspace": k["ws"]} for k in buckets], streams=side_streams)
+            n = gm.gm_last_launch_count()
+            for s in side_streams:
+                e = torch.cuda.Event(); e.record(s)
+                stream.wait_event(e)
+            return outs, n
+        for k in buckets:
             data, sigma, mask, psf, start = k["dev"]
-            k["params"].copy_(start)
             outs.append(gm.gm_fit(model, k["params"], data, sigma, mask, psf, k["opts"], workspace=k["ws"],
                                   stream=stream))
             n += gm.gm_last_launch_count()
@@ -289,8 +307,14 @@ def run_ours(args):
         hargs = [tuple(None if t is None else t.numpy() for t in k["host"][:4]) for k in buckets]
 
         def host_step():
-            for k, hp, ha in zip(buckets, hps, hargs):
+            for k, hp in zip(buckets, hps):
                 hp[...] = k["b"]["start"]
+            if multi:
+                gm.gm_fit_multi_host(model, [{"params": hp, "data": ha[0], "sigma": ha[1], "mask": ha[2],
+                                              "psf": ha[3], "opts": k["opts"]}
+                                             for k, hp, ha in zip(buckets, hps, hargs)])
+                return
+            for k, hp, ha in zip(buckets, hps, hargs):
                 gm.gm_fit_host(model, hp, *ha, k["opts"])
 
         host_step()                                                   # warm-up
@@ -306,7 +330,8 @@ def run_ours(args):
         e2e = {"value": world * evals / float(te.item()), "unit": UNIT, "ms_per_step": float(te.item()) * 1e3,
                "galaxies_fitted_per_s": world * B / float(te.item()),
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-               "api": "gm_fit_host (host buffers; cudaMalloc + H2D + fit + D2H inside the call)"}
+               "api": ("gm_fit_multi_host" if multi else "gm_fit_host") +
+                      " (host buffers; cudaMalloc + H2D + fit + D2H inside the call)"}
 
     if rank != 0:
         if dist is not None:
@@ -324,7 +349,10 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
     roofline = None
     if dom:
-        achieved = args.steps * conv_flops / (heavy_ms * 1e-3) / 1e12
+        # buckets on concurrent streams: per-launch event times overlap one another, so the
+        # kernels' time is the step's own device time, not the sum over launches
+        achieved = (conv_flops / (ms_per_step * 1e-3) if multi else
+                    args.steps * conv_flops / (heavy_ms * 1e-3)) / 1e12
         n_dom = kern[dom]["launches"]
         big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
         traffic = None
@@ -342,7 +370,10 @@ def run_ours(args):
                     if len(kern) == 1 else None,
                     "how": "2*K^2 flops per pixel per convolution x convolutions actually run "
                            "(2 per chi^2+gradient evaluation + the closing forward) / summed CUDA-event time of the "
-                           "heavy kernels (forward, backward, fused) inside the timed region",
+                           "heavy kernels (forward, backward, fused) inside the timed region" +
+                           ("; size buckets run concurrently on one stream each, so the divisor is the step's "
+                            "device time and the per-kernel averages include time shared between streams"
+                            if multi else ""),
                     "hbm_gbs_algorithmic": (evals * args.steps * px_bytes) / (heavy_ms * 1e-3) / 1e9,
                     "hbm_peak_gbs": pk.get("hbm_gbs"), "kernels": kern}
         # whole-step view: the same flops against the step time (small kernels and gaps included)
@@ -357,6 +388,8 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl, "global_batch": B * world,
+                       "buckets": ("gm_fit_multi, one stream per cutout side" if multi else
+                                   "gm_fit per cutout side, one after the other") if len(buckets) > 1 else None,
                        "parallelism": f"dp{world} (independent galaxies, no collective)",
                        "l2": "flushed between steps (256 MiB write)",
                        "inputs": "seeded synthetic SDSS-like (gen/configs.py), resident in HBM"},
@@ -384,6 +417,8 @@ def main():
     ap.add_argument("--side", type=int, default=0, help="cutout side for the mixed-size config C2")
     ap.add_argument("--iters", type=int, default=0, help="override the iteration count")
     ap.add_argument("--no-early-stop", action="store_true")
+    ap.add_argument("--serial-buckets", action="store_true",
+                    help="C2: one gm_fit per size bucket, one after the other, instead of gm_fit_multi")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -42,10 +42,11 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   101     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   102     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
+#define GM_MAX_BATCHES 64    /* size buckets per gm_fit_multi call                  */
 
 typedef enum {
   GM_OK = 0,
@@ -170,6 +171,25 @@ int gm_fit(const gm_model* model, const gm_batch* batch, float* params,
            int32_t* status, void* workspace, size_t workspace_bytes,
            void* cuda_stream);
 
+/* The same fit for several batches of different cutout size at once (the paper's sample
+ * mixes sizes; BASELINE config 2 has five).  Entry i of every array argument
+ * belongs to batches[i]: params[i] dev [B_i,P] in/out, opts[i], chi2_out[i] dev [B_i],
+ * iters_used[i] / status[i] dev [B_i] (the array or single entries may be NULL),
+ * workspaces[i] of workspace_bytes[i] >= gm_workspace_bytes(model, &batches[i]), and
+ * cuda_streams[i], the stream batch i is enqueued on.  All arrays are HOST arrays of
+ * n_batches (1..GM_MAX_BATCHES).  Iteration t of every batch is enqueued before
+ * iteration t+1 of any; with distinct streams the batches run concurrently, so the
+ * SMs one batch leaves idle once most of its galaxies stopped early (R:O5) take
+ * another batch's galaxies.  Results are identical to calling gm_fit per batch: no
+ * batch reads another's data.  Ordering against the caller's other work is the
+ * caller's (events on the given streams); nothing is launched if any entry fails
+ * validation. */
+int gm_fit_multi(const gm_model* model, int32_t n_batches, const gm_batch* batches,
+                 float* const* params, const gm_fit_opts* opts, float* const* chi2_out,
+                 int32_t* const* iters_used, int32_t* const* status,
+                 void* const* workspaces, const size_t* workspace_bytes,
+                 void* const* cuda_streams);
+
 /* Covariance-matrix uncertainties (Sec. 5.2):
  *   sigma_p = sqrt(diag[(J^T W J)^-1]),  J = dM/dp at `params`,  W = Omega / sigma^2,
  * over the FREE parameters (free_mask: host [P], 0 = held fixed and left out of the
@@ -195,6 +215,12 @@ int gm_loss_grad_host(const gm_model* model, const gm_batch* host_batch,
 int gm_fit_host(const gm_model* model, const gm_batch* host_batch, float* params,
                 const gm_fit_opts* opts, float* chi2_out, int32_t* iters_used,
                 int32_t* status);
+
+/* gm_fit_multi with host buffers: every batch is staged on its own stream, fitted
+ * concurrently and copied back; returns after all of them are idle. */
+int gm_fit_multi_host(const gm_model* model, int32_t n_batches, const gm_batch* host_batches,
+                      float* const* params, const gm_fit_opts* opts, float* const* chi2_out,
+                      int32_t* const* iters_used, int32_t* const* status);
 
 /* ---- misc ------------------------------------------------------------------ */
 const char* gm_strerror(int status);

@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     GmError,
     gm_fit,
     gm_fit_host,
+    gm_fit_multi,
+    gm_fit_multi_host,
     gm_last_launch_count,
     gm_loss_grad,
     gm_loss_grad_host,

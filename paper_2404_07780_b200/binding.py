@@ -76,6 +76,11 @@ def _lib():
         L.gm_render.restype = i; L.gm_render.argtypes = [mp, bp, vp, vp, vp, sz, vp]
         L.gm_loss_grad.restype = i; L.gm_loss_grad.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gm_fit.restype = i; L.gm_fit.argtypes = [mp, bp, vp, op, vp, vp, vp, vp, sz, vp]
+        pp = C.POINTER(C.c_void_p)
+        L.gm_fit_multi.restype = i
+        L.gm_fit_multi.argtypes = [mp, C.c_int32, bp, pp, op, pp, pp, pp, pp, C.POINTER(sz), pp]
+        L.gm_fit_multi_host.restype = i
+        L.gm_fit_multi_host.argtypes = [mp, C.c_int32, bp, pp, op, pp, pp, pp]
         L.gm_uncertainty_workspace_bytes.restype = sz; L.gm_uncertainty_workspace_bytes.argtypes = [mp, bp]
         L.gm_uncertainty.restype = i; L.gm_uncertainty.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gm_render_host.restype = i; L.gm_render_host.argtypes = [mp, bp, vp, vp]
@@ -296,6 +301,56 @@ def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=N
     return {"params": params, "chi2": chi2, "iters_used": iters, "status": status, "_ws": ws}
 
 
+def gm_fit_multi(model, batches, streams=None):
+    """gm_fit of several size buckets at once, batch i on streams[i] (mixed cutout
+    sizes).  batches: list of dicts {"params", "data", "sigma", "mask", "psf", "opts",
+    ["workspace"]}; params are updated IN PLACE.  streams: list of torch.cuda.Stream
+    (default: one new stream per batch, each made to wait for the current stream; the
+    current stream then waits for all of them, so the call orders like gm_fit).
+    Asynchronous.  -> list of result dicts like gm_fit's."""
+    n = len(batches)
+    m = _model_struct(model)
+    own = streams is None
+    cur = torch.cuda.current_stream()
+    if own:
+        streams = [torch.cuda.Stream() for _ in range(n)]
+        ev = torch.cuda.Event(); ev.record(cur)
+        for s in streams:
+            s.wait_event(ev)
+    if len(streams) != n:
+        raise ValueError("one stream per batch")
+    barr = (_Batch * n)(); oarr = (_FitOpts * n)()
+    vpa = lambda: (C.c_void_p * n)()
+    par, chi, its, sts, wsp, stp = vpa(), vpa(), vpa(), vpa(), vpa(), vpa()
+    wsn = (C.c_size_t * n)()
+    keep, outs = [], []
+    for k, bt in enumerate(batches):
+        params = bt["params"]
+        B, P = params.shape
+        _, H, W = bt["data"].shape
+        barr[k] = _batch_struct(B, H, W, bt["psf"], bt["data"], bt["sigma"], bt.get("mask"))
+        o = _opts_struct(bt["opts"], P)
+        oarr[k] = o
+        chi2 = torch.empty(B, dtype=torch.float32, device=params.device)
+        iters = torch.empty(B, dtype=torch.int32, device=params.device)
+        status = torch.empty(B, dtype=torch.int32, device=params.device)
+        ws, wp, wn = _workspace(m, barr[k], bt.get("workspace"))
+        par[k] = _dev(params, torch.float32, "params"); chi[k] = chi2.data_ptr()
+        its[k] = iters.data_ptr(); sts[k] = status.data_ptr(); wsp[k] = wp; wsn[k] = wn
+        stp[k] = streams[k].cuda_stream
+        keep.append(o)
+        outs.append({"params": params, "chi2": chi2, "iters_used": iters, "status": status, "_ws": ws})
+    rc = _lib().gm_fit_multi(C.byref(m), n, barr, par, oarr, chi, its, sts, wsp, wsn, stp)
+    _check(rc, "gm_fit_multi")
+    if own:
+        for s, o in zip(streams, outs):
+            e = torch.cuda.Event(); e.record(s)
+            cur.wait_event(e)
+            for t in (o["params"], o["chi2"], o["iters_used"], o["status"], o["_ws"]):
+                t.record_stream(s)
+    return outs
+
+
 # ---- host-buffer entry points (numpy in, numpy out; copies inside the call) ------
 def _np(a, dtype, name):
     if a is None:
@@ -344,3 +399,32 @@ def gm_fit_host(model, params, data, sigma, mask, psf, opts):
     _check(_lib().gm_fit_host(C.byref(m), C.byref(b), params.ctypes.data, C.byref(o), chi2.ctypes.data,
                               iters.ctypes.data, status.ctypes.data), "gm_fit_host")
     return {"params": params, "chi2": chi2, "iters_used": iters, "status": status}
+
+
+def gm_fit_multi_host(model, batches):
+    """gm_fit_multi with numpy buffers (copies inside the call, every bucket on its own
+    stream).  batches: list of dicts {"params", "data", "sigma", "mask", "psf", "opts"};
+    params updated in place.  -> list of dicts of numpy arrays."""
+    n = len(batches)
+    m = _model_struct(model)
+    barr = (_Batch * n)(); oarr = (_FitOpts * n)()
+    vpa = lambda: (C.c_void_p * n)()
+    par, chi, its, sts = vpa(), vpa(), vpa(), vpa()
+    keep, outs = [], []
+    for k, bt in enumerate(batches):
+        params = _np(bt["params"], np.float32, "params"); psf = _np(bt["psf"], np.float32, "psf")
+        data = _np(bt["data"], np.float32, "data"); sigma = _np(bt["sigma"], np.float32, "sigma")
+        mask = _np(bt.get("mask"), np.uint8, "mask")
+        B, P = params.shape
+        _, H, W = data.shape
+        barr[k] = _batch_struct(B, H, W, psf, data, sigma, mask, host=True)
+        o = _opts_struct(bt["opts"], P)
+        oarr[k] = o
+        chi2 = np.empty(B, dtype=np.float32)
+        iters = np.empty(B, dtype=np.int32); status = np.empty(B, dtype=np.int32)
+        par[k] = params.ctypes.data; chi[k] = chi2.ctypes.data
+        its[k] = iters.ctypes.data; sts[k] = status.ctypes.data
+        keep.append(o)
+        outs.append({"params": params, "chi2": chi2, "iters_used": iters, "status": status})
+    _check(_lib().gm_fit_multi_host(C.byref(m), n, barr, par, oarr, chi, its, sts), "gm_fit_multi_host")
+    return outs

@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <memory>
 #include <mutex>
 #include <vector>
 
@@ -141,6 +142,7 @@ struct FitOptsDev {
 struct FitState {
   float *u, *m, *s, *p_prev, *chi2_prev;
   int *calm, *frozen;
+  int *live, *n_live;      // ascending list of the galaxies still iterating, and its length
 };
 
 struct FinArgs {
@@ -231,6 +233,8 @@ __global__ void k_fit_init(int B, int P, const float* __restrict__ params, FitOp
   if (k == 0) {
     const int b = idx / P;
     st.calm[b] = 0; st.frozen[b] = 0; st.chi2_prev[b] = 0.0f;
+    st.live[b] = b;
+    if (b == 0) *st.n_live = B;
     if (iters) iters[b] = 0;
     if (status) status[b] = GM_FIT_OK;
   }
@@ -299,6 +303,45 @@ k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* __restrict__
       params[pk] = o.lg[lane] ? exp10f(u) : u;
     }
   }
+}
+
+// Rebuild the ascending list of galaxies that still iterate (early stop, R:O5, or a
+// non-finite chi^2, R:X3).  One CTA; thread i owns a contiguous slice of the batch, so
+// the list order does not depend on timing.  The heavy kernels walk this list, which
+// keeps the per-SM work balanced once galaxies have stopped and lets CTAs without
+// work exit at once (their SMs then take another stream's CTAs, gm_fit_multi).
+constexpr int kCompactThreads = 1024;
+__global__ void __launch_bounds__(kCompactThreads) k_compact(int B, FitState st) {
+  __shared__ int wsum[kCompactThreads / 32];
+  __shared__ int total;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int per = (B + kCompactThreads - 1) / kCompactThreads;
+  const int lo = min(tid * per, B), hi = min(lo + per, B);
+  int n = 0;
+  for (int b = lo; b < hi; ++b) n += st.frozen[b] == 0;
+  int incl = n;                                           // inclusive scan inside the warp
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int v = wsum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += t;
+    }
+    wsum[lane] = v;                                       // inclusive over warps
+    if (lane == 31) total = v;
+  }
+  __syncthreads();
+  int off = incl - n + (wid ? wsum[wid - 1] : 0);
+  for (int b = lo; b < hi; ++b)
+    if (st.frozen[b] == 0) st.live[off++] = b;
+  if (tid == 0) *st.n_live = total;
 }
 
 // ---------------------------------------------------------------------------
@@ -528,7 +571,7 @@ struct Workspace {
   float* psf_pad;
   float2* taps;
   float *u, *m, *s, *p_prev, *chi2_prev;
-  int *calm, *frozen;
+  int *calm, *frozen, *live, *n_live;
   size_t total;
 };
 
@@ -555,6 +598,8 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   w.chi2_prev = (float*)take(B * 4);
   w.calm = (int*)take(B * 4);
   w.frozen = (int*)take(B * 4);
+  w.live = (int*)take(B * 4);
+  w.n_live = (int*)take(4);
   w.total = off;
   return w;
 }
@@ -714,47 +759,57 @@ static int run_prologue(const Plan& pl, int B, const float* params, const int* f
   return GM_OK;
 }
 
-static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const int* frozen) {
+// which galaxies an evaluation covers: all (gm_render, gm_loss_grad) or the fit's live list
+struct LiveSet {
+  const int* frozen = nullptr;
+  const int* live = nullptr;
+  const int* n_live = nullptr;
+};
+
+static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const LiveSet& ls) {
   FwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
   a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
   a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
-  a.G = out; a.chi2_part = pl.ws.chi2_part; a.frozen = frozen;
+  a.G = out; a.chi2_part = pl.ws.chi2_part;
+  a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   a.b0 = 0; a.dpar = -1;
   return a;
 }
 
-static BwdArgs bwd_args(const Plan& pl, const int* frozen) {
+static BwdArgs bwd_args(const Plan& pl, const LiveSet& ls) {
   BwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   a.taps = pl.taps_adj; a.taps_stride = pl.taps_stride;
-  a.G = pl.ws.G; a.grad_part = pl.ws.grad_part; a.frozen = frozen;
+  a.G = pl.ws.G; a.grad_part = pl.ws.grad_part;
+  a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   return a;
 }
 
-static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float* out, const int* frozen) {
+static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float* out, const LiveSet& ls) {
   FusedArgs a;
   a.md = pl.md; a.tg = pl.tg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
   a.any_unconv = 0;
   for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
   a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
-  a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part; a.frozen = frozen;
+  a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+  a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
   a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
   return a;
 }
 
 // one evaluation of every (non-frozen) galaxy: chi^2 partials and, if wanted, gradient partials
-static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const int* frozen, cudaStream_t st) {
+static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const LiveSet& ls, cudaStream_t st) {
   int rc;
   if (pl.fused)
-    return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, frozen), pl.caps.n_sm,
+    return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, ls), pl.caps.n_sm,
                           pl.caps.smem_optin, st);
-  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, frozen), FWD_LOSS, bt->B, st)) != GM_OK) return rc;
-  if (with_grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, frozen), bt->B, st)) != GM_OK) return rc;
+  if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, ls), FWD_LOSS, bt->B, st)) != GM_OK) return rc;
+  if (with_grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, ls), bt->B, st)) != GM_OK) return rc;
   return GM_OK;
 }
 
@@ -802,7 +857,7 @@ static int run_jtj(const Plan& pl, const gm_batch* bt, const UncWorkspace& uw, c
   for (int b0 = 0; b0 < B; b0 += uw.Bc) {
     const int bc = (B - b0 < uw.Bc) ? B - b0 : uw.Bc;
     for (int k = 0; k < P; ++k) {
-      FwdArgs a = fwd_args(pl, bt, uw.J + (size_t)k * bc * N, nullptr);
+      FwdArgs a = fwd_args(pl, bt, uw.J + (size_t)k * bc * N, LiveSet{});
       a.b0 = b0; a.dpar = k;
       a.tg.vec = a.tg.vec && ((((uintptr_t)a.G) & 15) == 0);
       int rc = dispatch_forward(pl.KP, a, FWD_DERIV, bc, st);
@@ -865,8 +920,8 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   if (rc != GM_OK) return rc;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
   if (pl.fused)
-    return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, nullptr), pl.caps.n_sm, pl.caps.smem_optin, st);
-  return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, nullptr), FWD_RENDER, bt->B, st);
+    return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, LiveSet{}), pl.caps.n_sm, pl.caps.smem_optin, st);
+  return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, LiveSet{}), FWD_RENDER, bt->B, st);
 }
 
 int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params, float* chi2,
@@ -885,7 +940,7 @@ int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params,
   }
   const bool with_grad = grad != nullptr || jtr != nullptr;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
-  if ((rc = run_eval(pl, bt, with_grad, nullptr, st)) != GM_OK) return rc;
+  if ((rc = run_eval(pl, bt, with_grad, LiveSet{}, st)) != GM_OK) return rc;
   FinArgs fa = fin_args(pl, bt->B, with_grad, chi2, grad);
   fa.jtr = jtr;
   k_finalize<<<(bt->B + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(fa);
@@ -924,19 +979,32 @@ int gm_uncertainty(const gm_model* model, const gm_batch* bt, const float* param
   return GM_OK;
 }
 
-int gm_fit(const gm_model* model, const gm_batch* bt, float* params, const gm_fit_opts* opts,
-           float* chi2_out, int32_t* iters_used, int32_t* status, void* workspace,
-           size_t workspace_bytes, void* cuda_stream) {
-  t_launches = 0;
+}  // extern "C"
+
+namespace gm {
+
+// one gm_fit in flight: everything the iteration loop needs, so that several fits
+// (gm_fit_multi) can be enqueued iteration by iteration on their own streams
+struct FitRun {
+  Plan pl;
+  const gm_batch* bt;
+  const gm_fit_opts* opts;
+  FitOptsDev o;
+  FitState fs;
+  float* params; float* chi2_out; int32_t* iters_used; int32_t* status;
+  cudaStream_t st;
+};
+
+static int fit_begin(FitRun* r, const gm_model* model, const gm_batch* bt, float* params, const gm_fit_opts* opts,
+                     float* chi2_out, int32_t* iters_used, int32_t* status, void* workspace,
+                     size_t workspace_bytes, cudaStream_t st) {
   if (!params || !chi2_out || !opts || !opts->lr || !opts->lo || !opts->hi) return GM_EINVAL;
   if (opts->n_iter < 0 || opts->patience < 0) return GM_EINVAL;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  Plan pl;
-  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl);
+  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &r->pl);
   if (rc != GM_OK) return rc;
+  const Plan& pl = r->pl;
   const int B = bt->B, P = pl.md.n_par;
-
-  FitOptsDev o;
+  FitOptsDev& o = r->o;
   memset(&o, 0, sizeof(o));
   for (int k = 0; k < P; ++k) {
     const bool lg = opts->log10_space && opts->log10_space[k];
@@ -949,25 +1017,101 @@ int gm_fit(const gm_model* model, const gm_batch* bt, float* params, const gm_fi
   }
   o.beta1 = opts->beta1; o.beta2 = opts->beta2; o.eps = opts->eps; o.tol = opts->tol;
   o.patience = opts->patience;
-  FitState fs{pl.ws.u, pl.ws.m, pl.ws.s, pl.ws.p_prev, pl.ws.chi2_prev, pl.ws.calm, pl.ws.frozen};
-
-  k_fit_init<<<(B * P + 127) / 128, 128, 0, st>>>(B, P, params, o, fs, iters_used, status);
+  r->fs = FitState{pl.ws.u, pl.ws.m, pl.ws.s, pl.ws.p_prev, pl.ws.chi2_prev, pl.ws.calm, pl.ws.frozen,
+                   pl.ws.live, pl.ws.n_live};
+  r->bt = bt; r->opts = opts; r->params = params; r->chi2_out = chi2_out;
+  r->iters_used = iters_used; r->status = status; r->st = st;
+  k_fit_init<<<(B * P + 127) / 128, 128, 0, st>>>(B, P, params, o, r->fs, iters_used, status);
   ++t_launches;
   GM_CUDA(cudaGetLastError());
+  return GM_OK;
+}
 
+// iteration t = 1..n_iter (update) or n_iter + 1 (closing evaluation)
+static int fit_iter(FitRun* r, int t) {
+  const Plan& pl = r->pl;
+  const gm_fit_opts* opts = r->opts;
+  const int B = r->bt->B;
+  cudaStream_t st = r->st;
+  int rc;
+  const int last = (t == opts->n_iter + 1);
+  // the compacted list only exists where galaxies can stop (early stop on); a non-finite
+  // chi^2 without it is skipped through frozen[]
+  const bool compact = opts->tol > 0.0f;
+  LiveSet ls;
+  ls.frozen = r->fs.frozen;
+  if (compact) { ls.live = r->fs.live; ls.n_live = r->fs.n_live; }
+  if ((rc = run_prologue(pl, B, r->params, r->fs.frozen, st)) != GM_OK) return rc;
+  if ((rc = run_eval(pl, r->bt, !last, ls, st)) != GM_OK) return rc;
+  const float c1 = (float)(1.0 - std::pow((double)opts->beta1, (double)t));
+  const float c2 = (float)(1.0 - std::pow((double)opts->beta2, (double)t));
+  const float dec = (float)std::pow((double)opts->lr_decay, (double)(t - 1));
   const int fin_grid = (B + kFinWarps - 1) / kFinWarps;
-  for (int t = 1; t <= opts->n_iter + 1; ++t) {
-    const int last = (t == opts->n_iter + 1);
-    if ((rc = run_prologue(pl, B, params, fs.frozen, st)) != GM_OK) return rc;
-    if ((rc = run_eval(pl, bt, !last, fs.frozen, st)) != GM_OK) return rc;
-    const float c1 = (float)(1.0 - std::pow((double)opts->beta1, (double)t));
-    const float c2 = (float)(1.0 - std::pow((double)opts->beta2, (double)t));
-    const float dec = (float)std::pow((double)opts->lr_decay, (double)(t - 1));
-    k_fit_step<<<fin_grid, kFinWarps * 32, 0, st>>>(fin_args(pl, B, !last, chi2_out, nullptr), o, fs, params,
-                                                   t, last, c1, c2, dec, iters_used, status);
+  k_fit_step<<<fin_grid, kFinWarps * 32, 0, st>>>(fin_args(pl, B, !last, r->chi2_out, nullptr), r->o, r->fs,
+                                                 r->params, t, last, c1, c2, dec, r->iters_used, r->status);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  if (compact && !last) {
+    k_compact<<<1, kCompactThreads, 0, st>>>(B, r->fs);
     ++t_launches;
     GM_CUDA(cudaGetLastError());
   }
+  return GM_OK;
+}
+
+}  // namespace gm
+
+extern "C" {
+
+int gm_fit(const gm_model* model, const gm_batch* bt, float* params, const gm_fit_opts* opts,
+           float* chi2_out, int32_t* iters_used, int32_t* status, void* workspace,
+           size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  FitRun r;
+  int rc = fit_begin(&r, model, bt, params, opts, chi2_out, iters_used, status, workspace, workspace_bytes,
+                     (cudaStream_t)cuda_stream);
+  if (rc != GM_OK) return rc;
+  for (int t = 1; t <= opts->n_iter + 1; ++t)
+    if ((rc = fit_iter(&r, t)) != GM_OK) return rc;
+  return GM_OK;
+}
+
+int gm_fit_multi(const gm_model* model, int32_t n_batches, const gm_batch* batches, float* const* params,
+                 const gm_fit_opts* opts, float* const* chi2_out, int32_t* const* iters_used,
+                 int32_t* const* status, void* const* workspaces, const size_t* workspace_bytes,
+                 void* const* cuda_streams) {
+  t_launches = 0;
+  if (n_batches < 1 || n_batches > GM_MAX_BATCHES) return GM_EINVAL;
+  if (!batches || !params || !opts || !chi2_out || !workspaces || !workspace_bytes || !cuda_streams) return GM_EINVAL;
+  // validate everything before the first launch
+  for (int i = 0; i < n_batches; ++i) {
+    ModelDesc md;
+    int rc = validate(model, &batches[i], true, &md);
+    if (rc != GM_OK) return rc;
+    if (!params[i] || !chi2_out[i] || !opts[i].lr || !opts[i].lo || !opts[i].hi) return GM_EINVAL;
+    if (opts[i].n_iter < 0 || opts[i].patience < 0) return GM_EINVAL;
+    if (padded_K(batches[i].K) < 0) return GM_ENOTSUP;
+    if (!workspaces[i] || ((uintptr_t)workspaces[i] & 255) ||
+        workspace_bytes[i] < gm_workspace_bytes(model, &batches[i]))
+      return GM_EWORKSPACE;
+  }
+  std::unique_ptr<FitRun[]> runs(new FitRun[n_batches]);
+  int t_max = 0;
+  for (int i = 0; i < n_batches; ++i) {
+    int rc = fit_begin(&runs[i], model, &batches[i], params[i], &opts[i], chi2_out[i],
+                       iters_used ? iters_used[i] : nullptr, status ? status[i] : nullptr, workspaces[i],
+                       workspace_bytes[i], (cudaStream_t)cuda_streams[i]);
+    if (rc != GM_OK) return rc;
+    if (opts[i].n_iter + 1 > t_max) t_max = opts[i].n_iter + 1;
+  }
+  // iteration t of every batch is enqueued before iteration t + 1 of any, so that the
+  // streams advance together and one batch's stragglers share the GPU with the others
+  for (int t = 1; t <= t_max; ++t)
+    for (int i = 0; i < n_batches; ++i)
+      if (t <= opts[i].n_iter + 1) {
+        int rc = fit_iter(&runs[i], t);
+        if (rc != GM_OK) return rc;
+      }
   return GM_OK;
 }
 
@@ -989,6 +1133,8 @@ struct HostCall {
   gm_batch dev;
   size_t ws_bytes = 0;
 };
+
+struct FitOutBufs { DevBuf chi2, it, st; };
 
 int stage_in(const gm_model* model, const gm_batch* hb, const float* params, bool need_data, HostCall* hc) {
   if (!model || !hb || !params || !hb->psf) return GM_EINVAL;
@@ -1081,6 +1227,48 @@ int gm_fit_host(const gm_model* model, const gm_batch* hb, float* params, const 
   if (iters_used) GM_CUDA(cudaMemcpyAsync(iters_used, dit.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
   if (status) GM_CUDA(cudaMemcpyAsync(status, dst.p, B * 4, cudaMemcpyDeviceToHost, hc.sg.s));
   GM_CUDA(cudaStreamSynchronize(hc.sg.s));
+  return GM_OK;
+}
+
+int gm_fit_multi_host(const gm_model* model, int32_t n_batches, const gm_batch* hbs, float* const* params,
+                      const gm_fit_opts* opts, float* const* chi2_out, int32_t* const* iters_used,
+                      int32_t* const* status) {
+  if (n_batches < 1 || n_batches > GM_MAX_BATCHES || !model || !hbs || !params || !opts || !chi2_out)
+    return GM_EINVAL;
+  std::unique_ptr<HostCall[]> hc(new HostCall[n_batches]);
+  std::unique_ptr<FitOutBufs[]> out(new FitOutBufs[n_batches]);
+  gm_batch dev[GM_MAX_BATCHES];
+  std::vector<float*> dpar((size_t)n_batches), dchi2((size_t)n_batches);
+  std::vector<int32_t*> dit((size_t)n_batches), dst((size_t)n_batches);
+  std::vector<void*> ws((size_t)n_batches), streams((size_t)n_batches);
+  std::vector<size_t> wsb((size_t)n_batches);
+  for (int i = 0; i < n_batches; ++i) {
+    if (!params[i] || !chi2_out[i]) return GM_EINVAL;
+    int rc = stage_in(model, &hbs[i], params[i], true, &hc[i]);
+    if (rc != GM_OK) return rc;
+    const size_t B = hbs[i].B;
+    GM_CUDA(out[i].chi2.alloc(B * 4));
+    GM_CUDA(out[i].it.alloc(B * 4));
+    GM_CUDA(out[i].st.alloc(B * 4));
+    dev[i] = hc[i].dev;
+    dpar[i] = (float*)hc[i].params.p; dchi2[i] = (float*)out[i].chi2.p;
+    dit[i] = (int32_t*)out[i].it.p; dst[i] = (int32_t*)out[i].st.p;
+    ws[i] = hc[i].ws.p; wsb[i] = hc[i].ws_bytes; streams[i] = (void*)hc[i].sg.s;
+  }
+  int rc = gm_fit_multi(model, n_batches, dev, dpar.data(), opts, dchi2.data(), dit.data(), dst.data(),
+                        ws.data(), wsb.data(), streams.data());
+  if (rc != GM_OK) return rc;
+  const int64_t n = t_launches;
+  for (int i = 0; i < n_batches; ++i) {
+    const size_t B = hbs[i].B, P = model->n_par;
+    cudaStream_t st = hc[i].sg.s;
+    GM_CUDA(cudaMemcpyAsync(params[i], dpar[i], B * P * 4, cudaMemcpyDeviceToHost, st));
+    GM_CUDA(cudaMemcpyAsync(chi2_out[i], dchi2[i], B * 4, cudaMemcpyDeviceToHost, st));
+    if (iters_used && iters_used[i]) GM_CUDA(cudaMemcpyAsync(iters_used[i], dit[i], B * 4, cudaMemcpyDeviceToHost, st));
+    if (status && status[i]) GM_CUDA(cudaMemcpyAsync(status[i], dst[i], B * 4, cudaMemcpyDeviceToHost, st));
+  }
+  for (int i = 0; i < n_batches; ++i) GM_CUDA(cudaStreamSynchronize(hc[i].sg.s));
+  t_launches = n;
   return GM_OK;
 }
 

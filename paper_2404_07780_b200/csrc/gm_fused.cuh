@@ -40,6 +40,7 @@ struct FusedArgs {
   float* chi2_part;          // [B]      (tiles = 1)
   float* grad_part;          // [B, n_comp, kNSum]
   const int* frozen;
+  const int* live; const int* n_live;   // compacted list of galaxies still iterating (gm_fit) or nullptr
 };
 
 enum { BAR_FULL0 = 1, BAR_FULL1 = 2, BAR_DONE0 = 3, BAR_DONE1 = 4, BAR_CONV = 5, BAR_HELP = 6 };
@@ -95,8 +96,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
   const int tid = threadIdx.x;
   const int wid = tid >> 5, lane = tid & 31;
   const bool with_grad = a.mode == 2;
-  const int n_k = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // galaxies of this CTA
-  auto galaxy = [&](int k) { return (int)blockIdx.x + k * (int)gridDim.x; };
+  const int n_gal = a.live ? *a.n_live : a.B;
+  const int n_k = (n_gal - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // galaxies of this CTA
+  auto galaxy = [&](int k) {
+    const int i = (int)blockIdx.x + k * (int)gridDim.x;
+    return a.live ? a.live[i] : i;
+  };
   auto live = [&](int k) { return k < n_k && !(a.frozen && a.frozen[galaxy(k)]); };
 
   if (wid < kConvWarps) {

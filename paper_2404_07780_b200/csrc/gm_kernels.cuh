@@ -49,6 +49,7 @@ struct FwdArgs {
   float* G;                // [B,H,W] workspace (or model_out when RENDER)
   float* chi2_part;        // [B, tiles]
   const int* frozen;       // [B] or nullptr: skip galaxies that stopped
+  const int* live; const int* n_live;   // compacted list of galaxies still iterating, or nullptr
   int b0;                  // first galaxy of this launch (FWD_DERIV chunks; 0 otherwise)
   int dpar;                // FWD_DERIV: index of the parameter to differentiate with respect to
 };
@@ -65,6 +66,7 @@ struct BwdArgs {
   const float* G;          // [B,H,W]
   float* grad_part;        // [B, tiles, n_comp, kNSum]
   const int* frozen;
+  const int* live; const int* n_live;
 };
 
 template <int K> struct ConvCfg {
@@ -187,8 +189,12 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
   const int tiles = tg.tiles_x * tg.tiles_y;
-  const int b = a.b0 + blockIdx.x / tiles;
+  int b = a.b0 + blockIdx.x / tiles;
   const int tile = blockIdx.x % tiles;
+  if (a.live) {
+    if (b >= *a.n_live) return;
+    b = a.live[b];
+  }
   if (a.frozen && a.frozen[b]) return;
   const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
   const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;     // tile origin in the cutout
@@ -379,8 +385,12 @@ __global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
   const int tiles = tg.tiles_x * tg.tiles_y;
-  const int b = blockIdx.x / tiles;
+  int b = blockIdx.x / tiles;
   const int tile = blockIdx.x - b * tiles;
+  if (a.live) {
+    if (b >= *a.n_live) return;
+    b = a.live[b];
+  }
   if (a.frozen && a.frozen[b]) return;
   const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
   const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;

@@ -119,3 +119,50 @@ def test_fit_host_matches_device():
     p = b["start"].copy()
     h = gm.gm_fit_host(b["model"], p, b["data"], b["sigma"], None, b["psf"], opts)
     assert np.array_equal(h["params"], g["params"]) and np.array_equal(h["chi2"], g["chi2"])
+
+
+def _bucket(cid, gal, side, n_iter, tol):
+    b = configs.make_batch(cid, gal, oracle_render, side=side)
+    opts = configs.fit_options(b["model"], b["H"], b["W"], n_iter, tol=tol, patience=5)
+    return b, opts
+
+
+def test_fit_multi_equals_fit_per_batch_bitwise():
+    # three size buckets with early stop: gm_fit_multi (one stream per bucket, iterations
+    # interleaved) must give exactly what gm_fit gives bucket by bucket
+    buckets = [_bucket(2, range(40), side, 120, 1e-5) for side in (64, 96, 192)]
+    buckets = [(b, o) for b, o in buckets if len(b["galaxies"])]
+    assert len(buckets) >= 2
+    single = [gpu_fit(b, o) for b, o in buckets]
+    batches = [{"params": dev(b["start"]).clone(), "data": dev(b["data"]), "sigma": dev(b["sigma"]),
+                "mask": dev(b["mask"]), "psf": dev(b["psf"]), "opts": o} for b, o in buckets]
+    outs = gm.gm_fit_multi(buckets[0][0]["model"], batches)
+    torch.cuda.synchronize()
+    for s, m in zip(single, outs):
+        for key in ("params", "chi2", "iters_used", "status"):
+            assert np.array_equal(s[key], m[key].cpu().numpy(), equal_nan=True), key
+    assert any((s["status"] == 1).any() for s in single), "early stop never triggered: test is vacuous"
+    # and the host-buffer variant
+    hb = [{"params": b["start"].copy(), "data": b["data"], "sigma": b["sigma"], "mask": b["mask"],
+           "psf": b["psf"], "opts": o} for b, o in buckets]
+    houts = gm.gm_fit_multi_host(buckets[0][0]["model"], hb)
+    for s, m in zip(single, houts):
+        for key in ("params", "chi2", "iters_used", "status"):
+            assert np.array_equal(s[key], m[key], equal_nan=True), key
+
+
+def test_live_list_after_early_stop_matches_oracle():
+    # many more galaxies than stop at the same time: the compacted live list changes every few
+    # iterations; per-galaxy results must not depend on it (compare with the oracle, which has none)
+    b, opts = _bucket(0, range(48), None, 200, 1e-5)
+    g = gpu_fit(b, opts)
+    o = oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
+    assert np.array_equal(g["status"], o["status"])
+    assert (g["status"] == 1).sum() >= 10
+    assert len(np.unique(g["iters_used"])) >= 5
+    assert np.all(np.abs(g["iters_used"] - o["iters_used"]) <= 15)
+    assert_chi2(g["chi2"], o["chi2"], rtol=1e-4)
+    # a second run is bitwise identical (list order is deterministic)
+    g2 = gpu_fit(b, opts)
+    for key in ("params", "chi2", "iters_used", "status"):
+        assert np.array_equal(g[key], g2[key])
