@@ -12,7 +12,7 @@
 #include <mutex>
 #include <vector>
 
-#include "gm_fused.cuh"
+#include "gm_fusedg.cuh"
 #include "gm_prologue.cuh"
 
 namespace gm {
@@ -608,7 +608,8 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
 #define GM_DECL_K(K)                                                                          \
   int launch_forward_##K(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err); \
   int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
-  int launch_fused_##K(const FusedArgs& a, int n_sm, size_t smem_limit, cudaStream_t st, cudaError_t* err);
+  int launch_fused_##K(const FusedArgs& a, int variant, int n_sm, size_t smem_limit, cudaStream_t st,         \
+                       cudaError_t* err);
 GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
 #undef GM_DECL_K
 
@@ -652,18 +653,18 @@ static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
   return rc;
 }
 
-static int dispatch_fused(int KP, const FusedArgs& a, int n_sm, size_t lim, cudaStream_t st) {
+static int dispatch_fused(int KP, const FusedArgs& a, int v, int n_sm, size_t lim, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
   const int pi = prof_begin(2, st);
   switch (KP) {
-    case 5: rc = launch_fused_5(a, n_sm, lim, st, &err); break;
-    case 9: rc = launch_fused_9(a, n_sm, lim, st, &err); break;
-    case 15: rc = launch_fused_15(a, n_sm, lim, st, &err); break;
-    case 21: rc = launch_fused_21(a, n_sm, lim, st, &err); break;
-    case 25: rc = launch_fused_25(a, n_sm, lim, st, &err); break;
-    case 33: rc = launch_fused_33(a, n_sm, lim, st, &err); break;
-    case 41: rc = launch_fused_41(a, n_sm, lim, st, &err); break;
+    case 5: rc = launch_fused_5(a, v, n_sm, lim, st, &err); break;
+    case 9: rc = launch_fused_9(a, v, n_sm, lim, st, &err); break;
+    case 15: rc = launch_fused_15(a, v, n_sm, lim, st, &err); break;
+    case 21: rc = launch_fused_21(a, v, n_sm, lim, st, &err); break;
+    case 25: rc = launch_fused_25(a, v, n_sm, lim, st, &err); break;
+    case 33: rc = launch_fused_33(a, v, n_sm, lim, st, &err); break;
+    case 41: rc = launch_fused_41(a, v, n_sm, lim, st, &err); break;
     default: return GM_ENOTSUP;
   }
   prof_end(pi, st);
@@ -701,13 +702,38 @@ struct Plan {
   const float* psf; long long psf_stride;
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int tiles;
-  bool fused;                // whole cutout per CTA and two buffers fit: k_fused path
+  bool fused;                // whole cutouts per CTA and two slots fit: k_fused path
+  FusedGeom fg; int fused_variant;
   DevCaps caps;
 };
 
-static size_t fused_smem_for(int KP, const TileGeom& tg) {
-  return 2 * (size_t)tg.rows * tg.pitch * 4 + 4 * (size_t)(KP + 1) * (KP + 1) * 8 +
-         (size_t)kHelpWarps * kNSum * 4 + 64;
+// Geometry of the fused kernel for an H x W cutout: thread-tile variant (0: 8x8, 1: 6x12) and
+// cutouts per slot G, chosen to keep the most of the 256 conv threads busy within the
+// shared-memory limit.  false: the cutout does not fit the fused kernel.
+static bool make_fused_geom(int H, int W, int KP, bool shared_taps, size_t smem_limit, FusedGeom* out, int* variant) {
+  static const int kRP[2] = {4, 3}, kTCs[2] = {8, 12};
+  double best = 0.0;
+  for (int v = 0; v < 2; ++v) {
+    FusedGeom fg;
+    fg.H = H; fg.W = W;
+    fg.ntx = (W + kTCs[v] - 1) / kTCs[v];
+    fg.nty = (H + 2 * kRP[v] - 1) / (2 * kRP[v]);
+    fg.tpg = fg.ntx * fg.nty;
+    if (fg.tpg > kConvThreads) continue;
+    const int nw4 = ((kTCs[v] + KP - 1) + 3) / 4 * 4;       // floats one thread reads per input row
+    fg.pitch = (fg.ntx - 1) * kTCs[v] + nw4;
+    fg.gal_elems = (H + 1) * fg.pitch;
+    fg.vec = 0;
+    fg.shared_taps = shared_taps ? 1 : 0;
+    for (int G = 8; G >= 1; G >>= 1) {
+      fg.G = G;
+      if (G * fg.tpg > kConvThreads || fused_smem_bytes(KP, fg) > smem_limit) continue;
+      const double eff = (double)G * H * W / ((double)kConvThreads * 2 * kRP[v] * kTCs[v]);
+      if (eff > best * 1.02) { best = eff; *out = fg; *variant = v; }
+      break;
+    }
+  }
+  return best > 0.0;
 }
 
 static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, void* workspace,
@@ -722,8 +748,9 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   pl->ws = carve(workspace, pl->md, bt, pl->KP, pl->tg);
   if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < pl->ws.total) return GM_EWORKSPACE;
   if ((rc = device_caps(&pl->caps)) != GM_OK) return rc;
-  pl->fused = pl->tiles == 1 && pl->tg.ntx * pl->tg.nty <= 32 * kConvWarps &&
-              fused_smem_for(pl->KP, pl->tg) <= pl->caps.smem_optin && !getenv("GM_NO_FUSED");
+  pl->fused = bt->H <= 128 && bt->W <= 128 && !getenv("GM_NO_FUSED") &&
+              make_fused_geom(bt->H, bt->W, pl->KP, bt->psf_stride == 0, pl->caps.smem_optin, &pl->fg,
+                              &pl->fused_variant);
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
   if (pl->KP != bt->K) {
@@ -790,7 +817,7 @@ static BwdArgs bwd_args(const Plan& pl, const LiveSet& ls) {
 
 static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float* out, const LiveSet& ls) {
   FusedArgs a;
-  a.md = pl.md; a.tg = pl.tg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
+  a.md = pl.md; a.fg = pl.fg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
   a.any_unconv = 0;
   for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
   a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride;
@@ -798,7 +825,7 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
   a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
-  a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
+  a.fg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
   return a;
 }
 
@@ -806,8 +833,8 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
 static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const LiveSet& ls, cudaStream_t st) {
   int rc;
   if (pl.fused)
-    return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, ls), pl.caps.n_sm,
-                          pl.caps.smem_optin, st);
+    return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, ls), pl.fused_variant,
+                          pl.caps.n_sm, pl.caps.smem_optin, st);
   if ((rc = dispatch_forward(pl.KP, fwd_args(pl, bt, pl.ws.G, ls), FWD_LOSS, bt->B, st)) != GM_OK) return rc;
   if (with_grad && (rc = dispatch_backward(pl.KP, bwd_args(pl, ls), bt->B, st)) != GM_OK) return rc;
   return GM_OK;
@@ -920,7 +947,8 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   if (rc != GM_OK) return rc;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
   if (pl.fused)
-    return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, LiveSet{}), pl.caps.n_sm, pl.caps.smem_optin, st);
+    return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, LiveSet{}), pl.fused_variant, pl.caps.n_sm,
+                          pl.caps.smem_optin, st);
   return dispatch_forward(pl.KP, fwd_args(pl, bt, model_out, LiveSet{}), FWD_RENDER, bt->B, st);
 }
 

@@ -1,6 +1,6 @@
 // gm_tiles.cu -- instantiates the tile kernels for one PSF side, -DGM_K=<odd>.
 // Compiled once per supported K (see build.py) so the builds run in parallel.
-#include "gm_fused.cuh"
+#include "gm_fusedg.cuh"
 
 #ifndef GM_K
 #error "compile with -DGM_K=<PSF side>"
@@ -53,15 +53,21 @@ int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cud
   return GM_OK;
 }
 
-// fused loss + gradient (whole cutout per CTA); GM_ENOTSUP when the two buffers do not fit
-int GM_CAT(launch_fused_, GM_K)(const FusedArgs& a, int n_sm, size_t smem_limit, cudaStream_t st, cudaError_t* err) {
+// fused loss + gradient (whole cutouts per CTA); variant 0: 8x8 thread tiles, 1: 6x12
+int GM_CAT(launch_fused_, GM_K)(const FusedArgs& a, int variant, int n_sm, size_t smem_limit, cudaStream_t st,
+                                cudaError_t* err) {
   constexpr int K = GM_K;
-  if (a.tg.tiles_x != 1 || a.tg.tiles_y != 1 || a.tg.ntx * a.tg.nty > 32 * kConvWarps) return GM_ENOTSUP;
-  const size_t sm = fused_smem_bytes<K>(a.tg);
+  if (a.fg.tpg * a.fg.G > kConvThreads) return GM_ENOTSUP;
+  const size_t sm = fused_smem_bytes(K, a.fg);
   if (sm > smem_limit) return GM_ENOTSUP;
-  GM_TRY(set_smem(k_fused<K>, sm));
   const unsigned grid = (unsigned)(a.B < n_sm ? a.B : n_sm);
-  k_fused<K><<<grid, kFusedThreads, sm, st>>>(a);
+  if (variant == 0) {
+    GM_TRY(set_smem(k_fused<K, 4, 8>, sm));
+    k_fused<K, 4, 8><<<grid, kFusedThreads, sm, st>>>(a);
+  } else {
+    GM_TRY(set_smem(k_fused<K, 3, 12>, sm));
+    k_fused<K, 3, 12><<<grid, kFusedThreads, sm, st>>>(a);
+  }
   GM_TRY(cudaGetLastError());
   return GM_OK;
 }
