@@ -12,7 +12,7 @@
 #include <mutex>
 #include <vector>
 
-#include "gm_fusedg.cuh"
+#include "gm_fused.cuh"
 #include "gm_prologue.cuh"
 
 namespace gm {

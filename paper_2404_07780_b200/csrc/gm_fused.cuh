@@ -1,4 +1,4 @@
-// gm_fusedg.cuh -- the fused loss + gradient kernel for cutouts that fit one CTA
+// gm_fused.cuh -- the fused loss + gradient kernel for cutouts that fit one CTA
 // (H, W <= 128): steps a1..a5 of SURVEY.md section 8(a) in ONE launch, with nothing but
 // chi^2 and the kNSum partial sums per component leaving the SM.
 //

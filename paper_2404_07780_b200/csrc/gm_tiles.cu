@@ -1,6 +1,6 @@
 // gm_tiles.cu -- instantiates the tile kernels for one PSF side, -DGM_K=<odd>.
 // Compiled once per supported K (see build.py) so the builds run in parallel.
-#include "gm_fusedg.cuh"
+#include "gm_fused.cuh"
 
 #ifndef GM_K
 #error "compile with -DGM_K=<PSF side>"
