@@ -53,6 +53,9 @@ CONFIGS = {
               500, mask_frac=0.10, tol=1e-6, patience=10),
     3: Config(3, "C3", 4096, (128,), 25, "moffat3.5", "bulge_disk", "ccd", "c1", 300),
     4: Config(4, "C4", 65536, (256,), 41, "moffat3.5", "sersic_bar_nucleus", "ccd", "c1", 200),
+    # not a BASELINE.json entry: the SHAPES of the paper's own SDSS run (8,289 cutouts of 128x128
+    # with 41x41 PSFs), single Sersic, otherwise as C1
+    5: Config(5, "P1", 8289, (128,), 41, "moffat3.5", "single_sersic", "ccd", "c1", 200),
 }
 
 

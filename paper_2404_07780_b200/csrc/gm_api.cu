@@ -542,18 +542,19 @@ static int validate(const gm_model* m, const gm_batch* bt, bool need_data, Model
   return GM_OK;
 }
 
-static void tile_for(int D, int* T, int* n) {
-  const int nt = (D + 127) / 128;
+static void tile_for(int D, int max_t, int* T, int* n) {
+  const int nt = (D + max_t - 1) / max_t;
   const int per = (D + nt - 1) / nt;
   *T = (per + 7) / 8 * 8;
   *n = (D + *T - 1) / *T;
 }
 
+// Tiles of the per-tile kernels (k_forward / k_backward): at most 128 x 128.
 static TileGeom make_geom(int H, int W, int KP) {
   TileGeom tg;
   tg.H = H; tg.W = W;
-  tile_for(H, &tg.TH, &tg.tiles_y);
-  tile_for(W, &tg.TW, &tg.tiles_x);
+  tile_for(H, 128, &tg.TH, &tg.tiles_y);
+  tile_for(W, 128, &tg.TW, &tg.tiles_x);
   tg.ntx = tg.TW / kTC;
   tg.nty = tg.TH / kTR;
   const int win = ((kTC + KP - 1) + 3) / 4 * 4;            // floats read per thread window row

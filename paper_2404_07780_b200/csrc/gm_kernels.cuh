@@ -184,7 +184,7 @@ __host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int
 // forward: render + convolve + residual
 // ---------------------------------------------------------------------------
 template <int K, int MODE>
-__global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
+__global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   constexpr bool RENDER = (MODE != FWD_LOSS);            // an image is written, no residual
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
@@ -381,7 +381,7 @@ __global__ void __launch_bounds__(256) k_forward(const FwdArgs a) {
 // (10 per component, see grad_accumulate in gm_device.cuh)
 // ---------------------------------------------------------------------------
 template <int K>
-__global__ void __launch_bounds__(256) k_backward(const BwdArgs a) {
+__global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
   const int tiles = tg.tiles_x * tg.tiles_y;

@@ -21,10 +21,21 @@ static cudaError_t set_smem(Kern kern, size_t bytes) {
   return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// Threads of a tile CTA.  When the tile is so large that only one CTA fits an SM (K = 41 with
+// 128 x 128 tiles) the CTA gets 512 threads: the upper 256 own no output pixels and only
+// help with the render, the tile load and the epilogue, which run with the
+// convolution warps idle and need the extra warps to hide the SFU / memory latency.
+template <int K>
+static int tile_threads(const TileGeom& tg, int nthr) {
+  const size_t one = smem_bytes<K>(tg, 16, kNSum) + 1024;
+  return (2 * one > 233472) ? 512 : nthr;
+}
+
 int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err) {
   constexpr int K = GM_K;
-  const int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
+  int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
   if (nthr > 256) return GM_ENOTSUP;
+  nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
   if (mode == FWD_RENDER) {
@@ -43,8 +54,9 @@ int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_
 
 int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err) {
   constexpr int K = GM_K;
-  const int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
+  int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
   if (nthr > 256) return GM_ENOTSUP;
+  nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
   GM_TRY(set_smem(k_backward<K>, sm));
