@@ -76,6 +76,9 @@ def lib():
         L.gmo_fit.restype = i
         L.gmo_fit.argtypes = [i, ip, i, i, i, i, i, dp, C.c_int64, dp, dp, bp, dp, i, d, d, d, d,
                               dp, dp, dp, bp, bp, d, i, dp, ip, ip, dp]
+        L.gmo_mix64.restype = C.c_uint64; L.gmo_mix64.argtypes = [C.c_uint64]
+        L.gmo_bootstrap_counts.restype = C.c_int64
+        L.gmo_bootstrap_counts.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, bp, C.c_int64, ip]
         L.gmo_num_threads.restype = i; L.gmo_num_threads.argtypes = []
         L.gmo_set_num_threads.restype = None; L.gmo_set_num_threads.argtypes = [i]
         _lib = L
@@ -289,6 +292,41 @@ def fit(model, params, data, sigma, mask, psf, opts: dict, want_trace=False):
     if want_trace:
         out["trace"] = trace
     return out
+
+
+def mix64(z: int) -> int:
+    return int(lib().gmo_mix64(C.c_uint64(z & 0xFFFFFFFFFFFFFFFF)))
+
+
+def bootstrap_counts(seed: int, gid: int, r: int, mask, shape):
+    """Multiplicities c[H,W] of resample r of galaxy gid (reading B1)."""
+    N = int(np.prod(shape))
+    m = None if mask is None else _u8(mask).reshape(-1)
+    counts = np.zeros(N, dtype=np.int32)
+    n_used = lib().gmo_bootstrap_counts(C.c_uint64(seed), C.c_uint64(gid), C.c_uint64(r), _bp(m), N,
+                                        counts.ctypes.data_as(C.POINTER(C.c_int32)))
+    return counts.reshape(shape), int(n_used)
+
+
+def bootstrap(model, params, data, sigma, mask, psf, opts: dict, n_resample: int, seed: int, id_offset: int = 0):
+    """Bootstrap uncertainties (Sec. 5.2): n_resample refits from `params`, each on
+    pixels resampled with replacement (weights c / sigma^2, pixels with c = 0 ignored);
+    sigma_boot^2 = (1/M) sum (m_i - mean)^2.
+    -> {"sigma_boot" [B,P], "mean" [B,P], "samples" [M,B,P], "counts" [B,H,W] of the last resample}"""
+    params = _f64(params); data = _f64(data); sigma = _f64(sigma)
+    B, P = params.shape
+    _, H, W = data.shape
+    samples = np.empty((n_resample, B, P))
+    counts = np.zeros((B, H, W), dtype=np.int32)
+    for r in range(n_resample):
+        for g in range(B):
+            counts[g], _ = bootstrap_counts(seed, id_offset + g, r, None if mask is None else mask[g], (H, W))
+        used = counts > 0
+        sig_r = np.where(used, sigma / np.sqrt(np.maximum(counts, 1)), sigma)     # w = c / sigma^2
+        samples[r] = fit(model, params, data, sig_r, used.astype(np.uint8), psf, opts)["params"]
+    mean = samples.mean(axis=0)
+    return {"sigma_boot": np.sqrt(((samples - mean) ** 2).sum(axis=0) / n_resample), "mean": mean,
+            "samples": samples, "counts": counts}
 
 
 def num_threads() -> int:

@@ -34,7 +34,9 @@
  * scipy.special.gammaincinv, scipy.signal.convolve2d, central finite
  * differences, brute-force chi^2, torch.optim.Adam, identities n=0.5/n=1;
  * covariance sigma_p: numpy.linalg.inv, the closed form of a linear model, and the
- * scatter of refits over noise realisations.
+ * scatter of refits over noise realisations; bootstrap: splitmix64 test vectors, count
+ * invariants, chi^2 over the explicit list of drawn pixels, numpy.std, the closed form
+ * sigma/sqrt(N) of a resampled mean.
  */
 #include <math.h>
 #include <stdint.h>
@@ -817,6 +819,53 @@ int gmo_fit(int n_comp, const int32_t *desc, int n_par, int B, int H, int W, int
                 trace ? trace + (int64_t)g * n_iter : NULL);
     }
     return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * Bootstrap resampling (Sec. 5.2): "resampling with replacement each galaxy
+ * image multiple times (typically 100 iterations) and refitting", then
+ * sigma^2 = (1/M) sum_i (m_i - mean)^2.
+ *
+ * Reading B1: one resample draws n_used pixel positions, independently
+ * and uniformly WITH replacement, from the n_used pixels of the galaxy that have
+ * mask = 1 (row-major order); c_ij = how often pixel (i,j) was drawn, so
+ * sum c = n_used and the resampled loss is chi2 = sum c_ij (D-M)^2 / sigma^2
+ * (a pixel drawn twice counts twice, a pixel never drawn is ignored).
+ *
+ * The draws come from a counter-based generator that each side implements itself
+ * from this definition (nothing is shared with the CUDA path):
+ *   mix(z): z = (z ^ z>>30) * 0xBF58476D1CE4E5B9; z = (z ^ z>>27) * 0x94D049BB133111EB;
+ *           return z ^ z>>31                        (the splitmix64 finaliser)
+ *   z(d)  = mix(mix(mix(seed ^ (id * 0x9E3779B97F4A7C15)) + r) + d),  64-bit wrap-around
+ *   k(d)  = ((z >> 32) * n_used) >> 32             (k-th used pixel), d = 0 .. n_used-1
+ * with id the galaxy's identifier and r the resample index.  Pins: the published
+ * splitmix64 test vectors, sum c = n_used, zero on masked pixels, P(c = 0) ~ 1/e.
+ * ------------------------------------------------------------------------- */
+uint64_t gmo_mix64(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+/* counts [N] of one galaxy and one resample; returns n_used */
+int64_t gmo_bootstrap_counts(uint64_t seed, uint64_t id, uint64_t r, const uint8_t *mask /*[N] or NULL*/,
+                             int64_t N, int32_t *counts /*[N]*/)
+{
+    int64_t n_used = 0;
+    int64_t *used = (int64_t *)malloc(sizeof(int64_t) * (size_t)(N > 0 ? N : 1));
+    for (int64_t i = 0; i < N; ++i) {
+        counts[i] = 0;
+        if (!mask || mask[i]) used[n_used++] = i;
+    }
+    const uint64_t base = gmo_mix64(gmo_mix64(seed ^ (id * 0x9E3779B97F4A7C15ull)) + r);
+    for (int64_t d = 0; d < n_used; ++d) {
+        const uint64_t z = gmo_mix64(base + (uint64_t)d);
+        const uint64_t k = ((z >> 32) * (uint64_t)n_used) >> 32;
+        counts[used[k]] += 1;
+    }
+    free(used);
+    return n_used;
 }
 
 /* number of OpenMP threads the parallel loops above use */
