@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   102     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   103     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
@@ -202,6 +202,43 @@ size_t gm_uncertainty_workspace_bytes(const gm_model* model, const gm_batch* bat
 int gm_uncertainty(const gm_model* model, const gm_batch* batch, const float* params,
                    const uint8_t* free_mask, float* sigma_p, float* jtj, int32_t* status,
                    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Bootstrap uncertainties (Sec. 5.2): "resampling with replacement each galaxy
+ * image multiple times (typically 100 iterations) and refitting"; the uncertainty is
+ * sigma^2 = (1/M) sum_i (m_i - mean)^2 over the M refits (population variance).
+ * Reading B1: one resample draws n_used pixel positions uniformly with replacement from
+ * the n_used pixels of the galaxy with mask != 0 (row-major order); c_ij = number of
+ * times pixel (i,j) was drawn, and the refit minimises sum c_ij (D-M)^2 / sigma^2.
+ * Draws are counter based, so a result does not depend on batching or timing:
+ *   mix(z): z = (z ^ z>>30) * 0xBF58476D1CE4E5B9; z = (z ^ z>>27) * 0x94D049BB133111EB;
+ *           z ^ z>>31                                    (splitmix64 finaliser, 64-bit wrap)
+ *   z(d) = mix(mix(mix(seed ^ (id * 0x9E3779B97F4A7C15)) + r) + d),  d = 0 .. n_used-1
+ *   k(d) = ((z >> 32) * n_used) >> 32  = index of the drawn pixel among the used ones
+ * with id = id_offset + index of the galaxy in the batch and r the resample index. */
+typedef struct {
+  int32_t  n_resample;         /* M, 1..GM_MAX_RESAMPLE                              */
+  uint64_t seed;
+  uint64_t id_offset;          /* identifier of the batch's first galaxy             */
+} gm_boot_opts;
+#define GM_MAX_RESAMPLE 4096
+
+/* Multiplicities of resample r of every galaxy: counts dev [B,H,W] int32 (0 on masked
+ * pixels; sums to n_used per galaxy).  Only B, H, W and mask of `batch` are read.
+ * workspace: dev, 256-byte aligned, at least 4*B*(H*W + 1) + 512 bytes. */
+int gm_bootstrap_counts(const gm_batch* batch, const gm_boot_opts* boot, int32_t r,
+                        int32_t* counts, void* workspace, size_t workspace_bytes,
+                        void* cuda_stream);
+
+/* M refits, every one started from `params` (dev [B,P], not modified) with `opts`.
+ * sigma_boot: dev [B,P].  mean: dev [B,P] or NULL.  samples: dev [M,B,P] fitted
+ * parameters of every refit, or NULL.  Fixed parameters get sigma_boot = 0.
+ * The mean and variance are accumulated in fp64 in resample order.
+ * Workspace: gm_bootstrap_workspace_bytes(model, batch, M). */
+size_t gm_bootstrap_workspace_bytes(const gm_model* model, const gm_batch* batch, int32_t n_resample);
+int gm_bootstrap(const gm_model* model, const gm_batch* batch, const float* params,
+                 const gm_fit_opts* opts, const gm_boot_opts* boot, float* sigma_boot,
+                 float* mean, float* samples, void* workspace, size_t workspace_bytes,
+                 void* cuda_stream);
 
 /* ---- host-buffer entry points (synchronous, end to end) -------------------- */
 /* Same operations with every pointer of `batch` and every array argument in HOST

@@ -6,6 +6,8 @@ under ``csrc/``.  PyTorch supplies device memory and streams.
 """
 from .binding import (  # noqa: F401
     GmError,
+    gm_bootstrap,
+    gm_bootstrap_counts,
     gm_fit,
     gm_fit_host,
     gm_fit_multi,

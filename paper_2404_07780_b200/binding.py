@@ -47,6 +47,10 @@ class _Batch(C.Structure):
                 ("psf", C.c_void_p), ("psf_stride", C.c_int64)]
 
 
+class _BootOpts(C.Structure):
+    _fields_ = [("n_resample", C.c_int32), ("seed", C.c_uint64), ("id_offset", C.c_uint64)]
+
+
 class _FitOpts(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
                 ("lr_decay", C.c_float), ("lr", C.c_void_p), ("lo", C.c_void_p), ("hi", C.c_void_p),
@@ -81,6 +85,10 @@ def _lib():
         L.gm_fit_multi.argtypes = [mp, C.c_int32, bp, pp, op, pp, pp, pp, pp, C.POINTER(sz), pp]
         L.gm_fit_multi_host.restype = i
         L.gm_fit_multi_host.argtypes = [mp, C.c_int32, bp, pp, op, pp, pp, pp]
+        bo = C.POINTER(_BootOpts)
+        L.gm_bootstrap_workspace_bytes.restype = sz; L.gm_bootstrap_workspace_bytes.argtypes = [mp, bp, C.c_int32]
+        L.gm_bootstrap_counts.restype = i; L.gm_bootstrap_counts.argtypes = [bp, bo, C.c_int32, vp, vp, sz, vp]
+        L.gm_bootstrap.restype = i; L.gm_bootstrap.argtypes = [mp, bp, vp, op, bo, vp, vp, vp, vp, sz, vp]
         L.gm_uncertainty_workspace_bytes.restype = sz; L.gm_uncertainty_workspace_bytes.argtypes = [mp, bp]
         L.gm_uncertainty.restype = i; L.gm_uncertainty.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gm_render_host.restype = i; L.gm_render_host.argtypes = [mp, bp, vp, vp]
@@ -299,6 +307,50 @@ def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=N
                        chi2.data_ptr(), iters.data_ptr(), status.data_ptr(), wp, wn, _stream_ptr(stream))
     _check(rc, "gm_fit")
     return {"params": params, "chi2": chi2, "iters_used": iters, "status": status, "_ws": ws}
+
+
+def gm_bootstrap_counts(B, H, W, mask, seed, r, id_offset=0, stream=None):
+    """int32 multiplicities [B,H,W] of bootstrap resample r (reading B1).  Asynchronous."""
+    dev = mask.device if mask is not None else torch.device("cuda")
+    b = _Batch(B, H, W, 1, None, None, _dev(mask, torch.uint8, "mask"), None, 0)
+    o = _BootOpts(1, int(seed), int(id_offset))
+    counts = torch.empty((B, H, W), dtype=torch.int32, device=dev)
+    ws = torch.empty(4 * B * (H * W + 1) + 1024, dtype=torch.uint8, device=dev)
+    off = (-ws.data_ptr()) % 256
+    rc = _lib().gm_bootstrap_counts(C.byref(b), C.byref(o), int(r), counts.data_ptr(), ws.data_ptr() + off,
+                                    ws.numel() - off, _stream_ptr(stream))
+    _check(rc, "gm_bootstrap_counts")
+    counts._gm_ws = ws
+    return counts
+
+
+def gm_bootstrap(model, params, data, sigma, mask, psf, opts, n_resample, seed, id_offset=0,
+                 want_samples=False, workspace=None, stream=None):
+    """Bootstrap uncertainties (Sec. 5.2): n_resample refits from params[B,P] (not
+    modified).  Asynchronous.  -> {"sigma_boot" [B,P], "mean" [B,P], ["samples" [M,B,P]]}"""
+    B, P = params.shape
+    _, H, W = data.shape
+    m = _model_struct(model)
+    b = _batch_struct(B, H, W, psf, data, sigma, mask)
+    o = _opts_struct(opts, P)
+    bo = _BootOpts(int(n_resample), int(seed), int(id_offset))
+    need = _lib().gm_bootstrap_workspace_bytes(C.byref(m), C.byref(b), int(n_resample))
+    if need == 0:
+        raise GmError(-1, "gm_bootstrap_workspace_bytes")
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=params.device)
+    off = (-workspace.data_ptr()) % 256
+    sb = torch.empty((B, P), dtype=torch.float32, device=params.device)
+    mean = torch.empty((B, P), dtype=torch.float32, device=params.device)
+    smp = torch.empty((n_resample, B, P), dtype=torch.float32, device=params.device) if want_samples else None
+    rc = _lib().gm_bootstrap(C.byref(m), C.byref(b), _dev(params, torch.float32, "params"), C.byref(o),
+                             C.byref(bo), sb.data_ptr(), mean.data_ptr(), None if smp is None else smp.data_ptr(),
+                             workspace.data_ptr() + off, workspace.numel() - off, _stream_ptr(stream))
+    _check(rc, "gm_bootstrap")
+    out = {"sigma_boot": sb, "mean": mean, "_ws": workspace}
+    if want_samples:
+        out["samples"] = smp
+    return out
 
 
 def gm_fit_multi(model, batches, streams=None):

@@ -14,6 +14,7 @@
 
 #include "gm_fused.cuh"
 #include "gm_prologue.cuh"
+#include "gm_boot.cuh"
 
 namespace gm {
 
@@ -1143,6 +1144,128 @@ int gm_fit_multi(const gm_model* model, int32_t n_batches, const gm_batch* batch
       }
   return GM_OK;
 }
+
+}  // extern "C"
+
+// ---- bootstrap row (reading B1) ------------------------------------------
+namespace gm {
+struct BootWorkspace {
+  int* used; int* n_used; int* counts;
+  float* sigma_r; uint8_t* mask_r; float* samples; float* chi2;
+  size_t total;
+};
+
+static BootWorkspace carve_boot(void* base, size_t base_total, const gm_batch* bt, int P, int M) {
+  BootWorkspace w;
+  const size_t B = bt->B, N = (size_t)bt->H * bt->W;
+  size_t off = align_up(base_total, 256);
+  auto take = [&](size_t bytes) {
+    void* p = base ? (void*)((char*)base + off) : nullptr;
+    off += align_up(bytes, 256);
+    return p;
+  };
+  w.used = (int*)take(B * N * 4);
+  w.n_used = (int*)take(B * 4);
+  w.counts = (int*)take(B * N * 4);
+  w.sigma_r = (float*)take(B * N * 4);
+  w.mask_r = (uint8_t*)take(B * N);
+  w.samples = (float*)take((size_t)M * B * P * 4);
+  w.chi2 = (float*)take(B * 4);
+  w.total = off;
+  return w;
+}
+
+// counts of resample r of every galaxy (used / n_used must have been built)
+static int boot_counts(const gm_batch* bt, const gm_boot_opts* bo, int r, const int* used, const int* n_used,
+                       int* counts, cudaStream_t st) {
+  const int N = bt->H * bt->W;
+  GM_CUDA(cudaMemsetAsync(counts, 0, (size_t)bt->B * N * 4, st));
+  for (int b0 = 0; b0 < bt->B; b0 += 65535) {               // gridDim.y limit
+    const int nb = bt->B - b0 < 65535 ? bt->B - b0 : 65535;
+    dim3 grid((N + 255) / 256, nb);
+    k_boot_draw<<<grid, 256, 0, st>>>(N, bo->seed, bo->id_offset + (unsigned long long)b0, (unsigned long long)r,
+                                      used + (size_t)b0 * N, n_used + b0, bt->mask != nullptr,
+                                      counts + (size_t)b0 * N);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+  }
+  return GM_OK;
+}
+
+static int boot_used(const gm_batch* bt, int* used, int* n_used, cudaStream_t st) {
+  k_used_list<<<bt->B, kUsedThreads, 0, st>>>(bt->H * bt->W, bt->mask, used, n_used);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  return GM_OK;
+}
+}  // namespace gm
+
+extern "C" {
+
+size_t gm_bootstrap_workspace_bytes(const gm_model* model, const gm_batch* bt, int32_t n_resample) {
+  const size_t base = gm_workspace_bytes(model, bt);
+  if (base == 0 || n_resample < 1 || n_resample > GM_MAX_RESAMPLE) return 0;
+  return carve_boot(nullptr, base, bt, model->n_par, n_resample).total;
+}
+
+int gm_bootstrap_counts(const gm_batch* bt, const gm_boot_opts* bo, int32_t r, int32_t* counts, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  if (!bt || !bo || !counts || r < 0) return GM_EINVAL;
+  if (bt->B < 1 || bt->H < 1 || bt->W < 1) return GM_EINVAL;
+  const size_t B = bt->B, N = (size_t)bt->H * bt->W;
+  if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < 4 * B * (N + 1) + 512) return GM_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int* used = (int*)workspace;
+  int* n_used = (int*)((char*)workspace + align_up(B * N * 4, 256));
+  int rc = boot_used(bt, used, n_used, st);
+  if (rc != GM_OK) return rc;
+  return boot_counts(bt, bo, r, used, n_used, counts, st);
+}
+
+int gm_bootstrap(const gm_model* model, const gm_batch* bt, const float* params, const gm_fit_opts* opts,
+                 const gm_boot_opts* bo, float* sigma_boot, float* mean, float* samples, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  if (!params || !opts || !bo || !sigma_boot) return GM_EINVAL;
+  if (bo->n_resample < 1 || bo->n_resample > GM_MAX_RESAMPLE) return GM_EINVAL;
+  ModelDesc md;
+  int rc = validate(model, bt, true, &md);
+  if (rc != GM_OK) return rc;
+  const size_t base = gm_workspace_bytes(model, bt);
+  if (base == 0) return GM_EINVAL;
+  const int M = bo->n_resample, B = bt->B, P = md.n_par;
+  const BootWorkspace bw = carve_boot(workspace, base, bt, P, M);
+  if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < bw.total) return GM_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  float* smp = samples ? samples : bw.samples;
+  const long long npx = (long long)B * bt->H * bt->W;
+  if ((rc = boot_used(bt, bw.used, bw.n_used, st)) != GM_OK) return rc;
+  gm_batch rb = *bt;                                        // the resampled batch: same data, new weights
+  rb.sigma = bw.sigma_r;
+  rb.mask = bw.mask_r;
+  for (int r = 0; r < M; ++r) {
+    if ((rc = boot_counts(bt, bo, r, bw.used, bw.n_used, bw.counts, st)) != GM_OK) return rc;
+    k_boot_fold<<<(unsigned)((npx + 255) / 256), 256, 0, st>>>(npx, bw.counts, bt->sigma, bw.sigma_r, bw.mask_r);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+    float* pr = smp + (size_t)r * B * P;
+    GM_CUDA(cudaMemcpyAsync(pr, params, (size_t)B * P * 4, cudaMemcpyDeviceToDevice, st));
+    FitRun run;
+    if ((rc = fit_begin(&run, model, &rb, pr, opts, bw.chi2, nullptr, nullptr, workspace, base, st)) != GM_OK)
+      return rc;
+    for (int t = 1; t <= opts->n_iter + 1; ++t)
+      if ((rc = fit_iter(&run, t)) != GM_OK) return rc;
+  }
+  k_boot_stats<<<(B * P + 127) / 128, 128, 0, st>>>(B * P, M, smp, sigma_boot, mean);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  return GM_OK;
+}
+
+}  // extern "C"
+
+extern "C" {
 
 // ---- host-buffer variants ----------------------------------------------------
 namespace {
