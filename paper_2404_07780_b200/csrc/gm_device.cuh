@@ -65,7 +65,9 @@ __device__ __forceinline__ Geo geometry(const CompConst& cc, bool box, float x, 
     const float vc = ex2<FAST>(cc.c * lg2<FAST>(fabsf(g.vq)));
     g.r = ex2<FAST>(cc.ic * lg2<FAST>(uc + vc));
   } else {
-    g.r = sqrtf(fmaf(g.u, g.u, g.vq * g.vq));
+    const float r2 = fmaf(g.u, g.u, g.vq * g.vq);
+    if (FAST) asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(g.r) : "f"(r2));   // MUFU.SQRT, <= 1 ulp
+    else g.r = sqrtf(r2);
   }
   return g;
 }
@@ -219,7 +221,7 @@ __device__ __forceinline__ float component_deriv_t(const CompConst& cc, bool box
   profile_grad_t<KIND, false>(cc, rg, U, dUdr, d0, d1, d2);
   const GeoGrad d = geometry_grad<false>(cc, box, g, rg);
   const float A = cc.amp * dUdr;
-  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, true>(cc, g.r) : U;
   const float I = cc.amp * Uv;
   switch (k) {
     case GM_SLOT_XC: return A * (-cc.ct * d.gu + cc.st * cc.iq * d.gv);
@@ -266,7 +268,7 @@ __device__ __forceinline__ void grad_accumulate(const CompConst& cc, bool box, f
   float U, dUdr, d0, d1, d2;
   profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
   // d/d amp uses the value at r itself (differs from rg only below 1e-6 px)
-  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, false>(cc, g.r) : U;
+  const float Uv = (g.r < kRGuard) ? profile_value_t<KIND, true>(cc, g.r) : U;
   const float sa = seed * cc.amp;
   if (box) {
     const GeoGrad d = geometry_grad<true>(cc, true, g, rg);
