@@ -33,7 +33,8 @@ struct __align__(16) CompConst {
   float a5, a6, a7, a8;
   float c, ic, cm1, dl_box;  // Eq. 2 exponent c = B + 2, 1/c, c - 1; d ln(amp) / dB
   float dl_m, dl_q, dl_s0, dl_s1;   // magnitude mode: d ln(amp) / d (m, q, s0, s1, s2);
-  float dl_s2, pad0, pad1, pad2;    //   d/d m0 = -dl_m
+  float dl_s2, b0, b1, b2;          //   d/d m0 = -dl_m; b0, b1: Sersic 1/re^2 and 1/(2n) for the
+                                    //   sqrt-free forms of value_uv / GradAcc
 };
 
 // ---------------------------------------------------------------------------
@@ -290,6 +291,204 @@ __device__ __forceinline__ void grad_accumulate(const CompConst& cc, bool box, f
   s[5] = fmaf(sa, d0, s[5]);
   s[6] = fmaf(sa, d1, s[6]);
   s[7] = fmaf(sa, d2, s[7]);
+}
+
+
+// ---------------------------------------------------------------------------
+// Row forms of a1 and a5 (B = 0).  Every instruction of the helper warps costs an issue
+// cycle that the FFMA2 convolution loop wants (FFMA2 holds the issue port for both of
+// its cycles: DESIGN.md section 5), so the per-pixel arithmetic is kept minimal:
+//   * u and v/q are linear in the column: four consecutive pixels of a row share one
+//     evaluation of the rotation (row4),
+//   * laws that are functions of r^2 skip the square root (Sersic: (r/re)^(1/n) =
+//     2^(lg2(r^2/re^2) / 2n)),
+//   * the gradient sums of the Sersic and exponential laws accumulate seed-weighted
+//     monomials and apply the per-galaxy constant factors once per thread (GradAcc).
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_fast(float x) {
+  float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y;
+}
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y;
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+  float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y;
+}
+
+// rotated coordinates (u, v/q) of the pixels (x0 + k, y), k = 0..3 (x0, y: pixel centres)
+__device__ __forceinline__ void row4(const CompConst& cc, float x0, float y, float (&u)[4], float (&vq)[4]) {
+  const float dx = x0 - cc.xc, dy = y - cc.yc;
+  const float u0 = fmaf(cc.ct, dx, cc.st * dy);
+  const float v0 = fmaf(cc.ct, dy, -cc.st * dx) * cc.iq;
+  const float dv = -cc.st * cc.iq;
+  u[0] = u0; vq[0] = v0;
+#pragma unroll
+  for (int k = 1; k < 4; ++k) { u[k] = fmaf((float)k, cc.ct, u0); vq[k] = fmaf((float)k, dv, v0); }
+}
+
+// radial law with unit amplitude from (u, v/q), B = 0
+template <int KIND, bool FAST>
+__device__ __forceinline__ float value_uv(const CompConst& cc, float u, float vq) {
+  const float r2 = fmaf(u, u, vq * vq);
+  if (KIND == GM_SERSIC) {
+    const float t = ex2<FAST>(lg2<FAST>(r2 * cc.b0) * cc.b1);      // (r/re)^(1/n); 0 at r = 0
+    return ex2<FAST>(fmaf(-cc.a2, t, cc.a2));
+  } else if (KIND == GM_GAUSSIAN) {
+    return ex2<FAST>(-r2 * cc.a0);
+  } else if (KIND == GM_MOFFAT) {
+    return ex2<FAST>(-cc.a1 * lg2<FAST>(fmaf(r2, cc.a0, 1.0f)));
+  } else if (KIND == GM_SKY) {
+    return 1.0f;
+  }
+  return profile_value_t<KIND, FAST>(cc, FAST ? sqrt_fast(r2) : sqrtf(r2));
+}
+
+// amp * U at the four pixels (x0 + k, y); box: Eq. 2 with B != 0 (per-pixel geometry)
+template <int KIND, bool FAST>
+__device__ __forceinline__ void value4(const CompConst& cc, bool box, float x0, float y, float (&v)[4]) {
+  if (box) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = cc.amp * profile_value_t<KIND, FAST>(cc, geometry<FAST>(cc, true, x0 + (float)k, y).r);
+  } else {
+    float u[4], vq[4];
+    row4(cc, x0, y, u, vq);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = cc.amp * value_uv<KIND, FAST>(cc, u[k], vq[k]);
+  }
+}
+
+// a5 accumulators of one component, B = 0.  add() takes one pixel (seed, u, v/q);
+// finish() returns the kNSum sums defined above grad_accumulate.
+template <int KIND> struct GradAcc {                       // generic: the sums themselves
+  float s[kNSum];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int k = 0; k < kNSum; ++k) s[k] = 0.0f;
+  }
+  __device__ __forceinline__ void add(const CompConst& cc, float seed, float u, float vq) {
+    if (KIND == GM_SKY) { s[4] += seed; return; }
+    const float r = sqrt_fast(fmaf(u, u, vq * vq));
+    const float rg = fmaxf(r, kRGuard);
+    float U, dUdr, d0, d1, d2;
+    profile_grad_t<KIND, true>(cc, rg, U, dUdr, d0, d1, d2);
+    const float Uv = (r < kRGuard) ? profile_value_t<KIND, true>(cc, r) : U;
+    const float sa = seed * cc.amp;
+    const float cgeo = sa * dUdr * rcp_fast(rg);
+    s[0] = fmaf(cgeo, u, s[0]);
+    s[1] = fmaf(cgeo, vq, s[1]);
+    s[2] = fmaf(cgeo * u, vq, s[2]);
+    s[3] = fmaf(cgeo * vq, vq, s[3]);
+    s[4] = fmaf(seed, Uv, s[4]);
+    s[5] = fmaf(sa, d0, s[5]);
+    s[6] = fmaf(sa, d1, s[6]);
+    s[7] = fmaf(sa, d2, s[7]);
+  }
+  __device__ __forceinline__ void fix(const CompConst&, float, float) {}   // add() already did
+  __device__ __forceinline__ void finish(const CompConst&, float (&out)[kNSum]) const {
+#pragma unroll
+    for (int k = 0; k < kNSum; ++k) out[k] = s[k];
+    out[8] = s[2];
+  }
+};
+
+constexpr float kRGuard2 = 1e-12f;                         // kRGuard^2
+
+// Sersic (Eq. 1): with L2 = lg2(rg^2 / re^2), t = 2^(L2 / 2n), U = 2^(nu lg2e (1 - t)):
+//   dU/dr = -U nu t / (n rg)         dU/dre = U nu t / (n re)
+//   dU/dn = -nu' U (t - 1) + (nu ln2 / 2 n^2) U t L2
+// so with sU = seed U and W = sU t the sums are multiples of
+//   q0..q3 = sum (W / rg^2) (u, v/q, u v/q, (v/q)^2),  q4 = sum sU,  q5 = sum W,
+//   q6 = sum sU (t - 1),  q7 = sum W L2
+template <> struct GradAcc<GM_SERSIC> {
+  float q[8];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) q[k] = 0.0f;
+  }
+  __device__ __forceinline__ void add(const CompConst& cc, float seed, float u, float vq) {
+    const float r2 = fmaf(u, u, vq * vq);
+    const float r2g = fmaxf(r2, kRGuard2);
+    const float L2 = lg2<true>(r2g * cc.b0);
+    const float t = ex2<true>(L2 * cc.b1);
+    const float U = ex2<true>(fmaf(-cc.a2, t, cc.a2));
+    const float sU = seed * U, W = sU * t;
+    const float cg = W * rcp_fast(r2g);
+    q[0] = fmaf(cg, u, q[0]);
+    q[1] = fmaf(cg, vq, q[1]);
+    q[2] = fmaf(cg * u, vq, q[2]);
+    q[3] = fmaf(cg * vq, vq, q[3]);
+    q[4] += sU;
+    q[5] += W;
+    q[6] = fmaf(sU, t - 1.0f, q[6]);
+    q[7] = fmaf(W, L2, q[7]);
+  }
+  // R:S4: d/d amp takes the value at r itself; called only for a pixel with r^2 < kRGuard2
+  __device__ __forceinline__ void fix(const CompConst& cc, float seed, float r2) {
+    const float Ug = ex2<true>(fmaf(-cc.a2, ex2<true>(lg2<true>(kRGuard2 * cc.b0) * cc.b1), cc.a2));
+    q[4] += seed * (profile_value_t<GM_SERSIC, true>(cc, sqrt_fast(r2)) - Ug);
+  }
+  __device__ __forceinline__ void finish(const CompConst& cc, float (&out)[kNSum]) const {
+    const float kf = cc.amp * cc.a3 * cc.a1;               // amp nu / n
+    out[0] = -kf * q[0]; out[1] = -kf * q[1]; out[2] = -kf * q[2]; out[3] = -kf * q[3];
+    out[4] = q[4];
+    out[5] = kf * cc.a0 * q[5];
+    out[6] = cc.amp * (-cc.a4 * q[6] + cc.a3 * cc.a1 * cc.a1 * (0.5f * kLn2) * q[7]);
+    out[7] = 0.0f; out[8] = out[2]; out[9] = 0.0f;
+  }
+};
+
+// exponential disk (Eq. 7): U = exp(-rg / rs), dU/dr = -U / rs, dU/drs = U rg / rs^2
+template <> struct GradAcc<GM_EXPDISK> {
+  float q[6];
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int k = 0; k < 6; ++k) q[k] = 0.0f;
+  }
+  __device__ __forceinline__ void add(const CompConst& cc, float seed, float u, float vq) {
+    const float r2 = fmaf(u, u, vq * vq);
+    const float r2g = fmaxf(r2, kRGuard2);
+    const float ir = rsqrt_fast(r2g), rg = r2g * ir;
+    const float U = ex2<true>(-rg * cc.a0);
+    const float sU = seed * U, cg = sU * ir;
+    q[0] = fmaf(cg, u, q[0]);
+    q[1] = fmaf(cg, vq, q[1]);
+    q[2] = fmaf(cg * u, vq, q[2]);
+    q[3] = fmaf(cg * vq, vq, q[3]);
+    q[4] += sU;
+    q[5] = fmaf(sU, rg, q[5]);
+  }
+  __device__ __forceinline__ void fix(const CompConst& cc, float seed, float r2) {
+    const float Ug = ex2<true>(-(kRGuard2 * rsqrt_fast(kRGuard2)) * cc.a0);
+    q[4] += seed * (ex2<true>(-sqrt_fast(r2) * cc.a0) - Ug);
+  }
+  __device__ __forceinline__ void finish(const CompConst& cc, float (&out)[kNSum]) const {
+    const float kf = cc.amp * cc.a1;
+    out[0] = -kf * q[0]; out[1] = -kf * q[1]; out[2] = -kf * q[2]; out[3] = -kf * q[3];
+    out[4] = q[4];
+    out[5] = kf * cc.a1 * q[5];
+    out[6] = 0.0f; out[7] = 0.0f; out[8] = out[2]; out[9] = 0.0f;
+  }
+};
+
+// the sums of four consecutive pixels of a row: seed[k] at (x0 + k, y)
+template <int KIND>
+__device__ __forceinline__ void grad_add4(GradAcc<KIND>& acc, const CompConst& cc, const float (&seed)[4], float x0, float y) {
+  if (KIND == GM_SKY) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc.add(cc, seed[k], 0.0f, 0.0f);
+    return;
+  }
+  float u[4], vq[4], r2[4];
+  row4(cc, x0, y, u, vq);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { acc.add(cc, seed[k], u[k], vq[k]); r2[k] = fmaf(u[k], u[k], vq[k] * vq[k]); }
+  if (KIND == GM_SERSIC || KIND == GM_EXPDISK) {           // one test per group for the rare r < 1e-6 pixel
+    if (fminf(fminf(r2[0], r2[1]), fminf(r2[2], r2[3])) < kRGuard2) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (r2[k] < kRGuard2) acc.fix(cc, seed[k], r2[k]);
+    }
+  }
 }
 
 }  // namespace gm

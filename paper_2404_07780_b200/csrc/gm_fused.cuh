@@ -223,10 +223,13 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
   const int hpg = kHelpWarps / G;                  // helper warps per cutout of a slot
   const int hg = hw / hpg, lw = hw - hg * hpg;     // this warp's cutout and its rank there
 
-  // the zero row of every cutout place, and the taps of a shared PSF: once per CTA
-  for (int i = htid; i < 2 * G * fg.pitch; i += HN) {
-    const int place = i / fg.pitch;
-    buf0[(size_t)place * fg.gal_elems + (size_t)fg.H * fg.pitch + (i - place * fg.pitch)] = 0.0f;
+  // Every slot is zeroed once per CTA: the zero row and the left / right margins of the
+  // rows stay zero from then on (render, convolution output and residual only ever write
+  // the H x W interior).  The taps of a shared PSF are loaded once per CTA as well.
+  {
+    float4* z = reinterpret_cast<float4*>(buf0);
+    const int n4 = (int)((2 * slot_elems) >> 2);            // gal_elems is a multiple of 4
+    for (int i = htid; i < n4; i += HN) z[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   if (fg.shared_taps) {
     for (int i = htid; i < TAPN / 2; i += HN) {
@@ -237,7 +240,16 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
     cp_async_wait_all();
   }
 
-  // a1: S of this group's cutout (zero left/right margins), and its taps when per galaxy
+  // The helper loops walk a cutout in groups of four consecutive pixels of a row, one group
+  // per lane: group idx -> (row, first column).  The warps of a cutout interleave by 32 groups.
+  const int W4 = (fg.W + 3) >> 2;
+  const int ngrp = fg.H * W4;
+  const float inv_w4 = 1.0f / (float)W4;
+  const int gstart = lw * 32 + lane, gstep = hpg * 32;
+  auto group_row = [&](int idx) -> int { return (int)(((float)idx + 0.5f) * inv_w4); };   // exact: idx < 2^16
+  constexpr bool kAligned = (h & 3) == 0;                  // slot interior is 16-byte aligned
+
+  // a1: S of this group's cutout, and its taps when they are per galaxy
   auto produce = [&](int item, int s) {
     const int b = galaxy(item, hg);
     if (b < 0) return;
@@ -254,23 +266,28 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
     const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
     bool first = true;
     for (int c = 0; c <= a.md.n_comp; ++c) {
-      const bool zero_pass = (c == a.md.n_comp);
+      const bool zero_pass = (c == a.md.n_comp);           // nothing convolved: S = 0
       if (zero_pass && !first) break;
-      if (!zero_pass && !a.md.conv[c]) continue;
+      if (!zero_pass && (!a.md.conv[c] || a.md.kind[c] == GM_SKY)) continue;
       const CompConst cc = ccb[zero_pass ? 0 : c];
       const bool box = !zero_pass && a.md.box[c] != 0;
       dispatch_kind(zero_pass ? (int)GM_SKY : a.md.kind[c], [&]<int KIND>() {
-        for (int i = lw; i < fg.H; i += hpg) {
-          float* rowp = gal + (size_t)i * fg.pitch;
-          const float y = (float)fg.H - 0.5f - (float)i;        // R:G1
-          for (int xx = lane; xx < fg.pitch; xx += 32) {
-            const int j = xx - h;
-            const bool in = j >= 0 && j < fg.W;
-            float sv = 0.0f;
-            if (KIND != GM_SKY && in)
-              sv = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry<kFastForward>(cc, box, (float)j + 0.5f, y).r);
-            if (first) rowp[xx] = sv;
-            else if (in) rowp[xx] += sv;
+        for (int idx = gstart; idx < ngrp; idx += gstep) {
+          const int i = group_row(idx), x = (idx - i * W4) << 2;
+          float v[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+          if (KIND != GM_SKY) value4<KIND, kFastForward>(cc, box, (float)x + 0.5f, (float)fg.H - 0.5f - (float)i, v);   // R:G1
+          float* p = gal + (size_t)i * fg.pitch + h + x;
+          if (kAligned && x + 4 <= fg.W) {
+            float4 o = make_float4(v[0], v[1], v[2], v[3]);
+            if (!first) {
+              const float4 q = *reinterpret_cast<const float4*>(p);
+              o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
+            }
+            *reinterpret_cast<float4*>(p) = o;
+          } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              if (x + k < fg.W) p[k] = first ? v[k] : p[k] + v[k];
           }
         }
       });
@@ -297,37 +314,79 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
         }
         return m;
       };
+      // branch free; the weight and the residual are SELECTED for unused pixels, never
+      // multiplied by 0, so NaN / sigma = 0 under the mask cannot propagate (R:X1)
       auto one = [&](float m, float d, float sg, bool used, float& gv) {
-        gv = 0.0f;
-        if (used) {                                       // select, never multiply by 0 (R:X1)
-          const float w = __fdividef(1.0f, sg * sg);
-          const float rho = d - m;
-          chi2 = fmaf(w * rho, rho, chi2);
-          gv = -2.0f * w * rho;
-        }
+        float w = rcp_fast(sg * sg), rho = d - m;
+        w = used ? w : 0.0f;
+        rho = used ? rho : 0.0f;
+        const float t = w * rho;
+        chi2 = fmaf(t, rho, chi2);
+        gv = -2.0f * t;
       };
-      if (fg.vec && (h & 3) == 0) {
-        // 128-bit path: one lane = 4 pixels, two rows per warp in flight
-        for (int yy = lw; yy < fg.H; yy += 2 * hpg) {
-          float4 m4[2], d4[2], s4[2];
-          uchar4 k4[2];
-          bool ok[2];
-          size_t off[2];
-          float* mp[2];
+      if (fg.vec && kAligned && a.mode != 0 && !a.any_unconv) {
+        // the hot form: chi^2 (+ gradient) of a model without unconvolved components.
+        // 128-bit accesses, one lane = 4 pixels, two groups per lane in flight, 32-bit offsets
+        const float* dptr = a.data + img;
+        const float* sptr = a.sigma + img;
+        auto hot = [&]<bool MASKED>() {
+          const uint8_t* kptr = MASKED ? a.mask + img : nullptr;
 #pragma unroll 1
-          for (int xx = lane * 4; xx < fg.W; xx += 128) {
+          for (int idx = gstart; idx < ngrp; idx += 2 * gstep) {
+            const int id1 = idx + gstep;
+            const bool ok1 = id1 < ngrp;
+            const int r0 = group_row(idx), r1 = group_row(ok1 ? id1 : idx);
+            const int c0 = (idx - r0 * W4) << 2, c1 = ((ok1 ? id1 : idx) - r1 * W4) << 2;
+            const int o0 = r0 * fg.W + c0, o1 = r1 * fg.W + c1;
+            float* mp0 = gal + r0 * fg.pitch + c0 + h;
+            float* mp1 = gal + r1 * fg.pitch + c1 + h;
+            const float4 d0 = *reinterpret_cast<const float4*>(dptr + o0), d1 = *reinterpret_cast<const float4*>(dptr + o1);
+            const float4 s0 = *reinterpret_cast<const float4*>(sptr + o0), s1 = *reinterpret_cast<const float4*>(sptr + o1);
+            uchar4 k0 = make_uchar4(1, 1, 1, 1), k1 = k0;
+            if (MASKED) { k0 = *reinterpret_cast<const uchar4*>(kptr + o0); k1 = *reinterpret_cast<const uchar4*>(kptr + o1); }
+            const float4 m0 = *reinterpret_cast<const float4*>(mp0), m1 = *reinterpret_cast<const float4*>(mp1);
+            float4 g0, g1;
+            one(m0.x, d0.x, s0.x, !MASKED || k0.x != 0, g0.x);
+            one(m0.y, d0.y, s0.y, !MASKED || k0.y != 0, g0.y);
+            one(m0.z, d0.z, s0.z, !MASKED || k0.z != 0, g0.z);
+            one(m0.w, d0.w, s0.w, !MASKED || k0.w != 0, g0.w);
+            *reinterpret_cast<float4*>(mp0) = g0;
+            if (ok1) {                                     // the pair of a last, odd group is the group itself
+              one(m1.x, d1.x, s1.x, !MASKED || k1.x != 0, g1.x);
+              one(m1.y, d1.y, s1.y, !MASKED || k1.y != 0, g1.y);
+              one(m1.z, d1.z, s1.z, !MASKED || k1.z != 0, g1.z);
+              one(m1.w, d1.w, s1.w, !MASKED || k1.w != 0, g1.w);
+              *reinterpret_cast<float4*>(mp1) = g1;
+            }
+          }
+        };
+        if (a.mask) hot.template operator()<true>();
+        else hot.template operator()<false>();
+      } else if (fg.vec && kAligned) {
+        // general 128-bit path (render output, unconvolved components)
+        auto pass = [&]<bool MASKED>() {
+#pragma unroll 1
+          for (int idx = gstart; idx < ngrp; idx += 2 * gstep) {
+            float4 m4[2], d4[2], s4[2];
+            uchar4 k4[2];
+            bool ok[2];
+            size_t off[2];
+            float* mp[2];
+            int row[2], col[2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-              const int i = yy + u * hpg;
-              ok[u] = i < fg.H;
-              off[u] = img + (size_t)i * fg.W + xx;
-              mp[u] = gal + (size_t)i * fg.pitch + xx + h;
+              const int id = idx + u * gstep;
+              ok[u] = id < ngrp;
+              row[u] = group_row(id); col[u] = (id - row[u] * W4) << 2;
+              off[u] = img + (size_t)row[u] * fg.W + col[u];
+              mp[u] = gal + (size_t)row[u] * fg.pitch + col[u] + h;
+              k4[u] = make_uchar4(1, 1, 1, 1);
               if (ok[u]) {
                 m4[u] = *reinterpret_cast<const float4*>(mp[u]);
                 if (a.mode != 0) {
                   d4[u] = *reinterpret_cast<const float4*>(a.data + off[u]);
                   s4[u] = *reinterpret_cast<const float4*>(a.sigma + off[u]);
-                  k4[u] = a.mask ? *reinterpret_cast<const uchar4*>(a.mask + off[u]) : make_uchar4(1, 1, 1, 1);
+                  if (MASKED) k4[u] = *reinterpret_cast<const uchar4*>(a.mask + off[u]);
                 }
               }
             }
@@ -335,8 +394,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
             for (int u = 0; u < 2; ++u) {
               if (!ok[u]) continue;
               if (a.any_unconv) {
-                const float y = (float)fg.H - 0.5f - (float)(yy + u * hpg);
-                const float x = (float)xx + 0.5f;
+                const float y = (float)fg.H - 0.5f - (float)row[u];
+                const float x = (float)col[u] + 0.5f;
                 m4[u].x = add_unconv(m4[u].x, x, y);
                 m4[u].y = add_unconv(m4[u].y, x + 1.0f, y);
                 m4[u].z = add_unconv(m4[u].z, x + 2.0f, y);
@@ -346,16 +405,18 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
                 *reinterpret_cast<float4*>(a.G + off[u]) = m4[u];
               } else {
                 float4 gv;
-                one(m4[u].x, d4[u].x, s4[u].x, k4[u].x != 0, gv.x);
-                one(m4[u].y, d4[u].y, s4[u].y, k4[u].y != 0, gv.y);
-                one(m4[u].z, d4[u].z, s4[u].z, k4[u].z != 0, gv.z);
-                one(m4[u].w, d4[u].w, s4[u].w, k4[u].w != 0, gv.w);
+                one(m4[u].x, d4[u].x, s4[u].x, !MASKED || k4[u].x != 0, gv.x);
+                one(m4[u].y, d4[u].y, s4[u].y, !MASKED || k4[u].y != 0, gv.y);
+                one(m4[u].z, d4[u].z, s4[u].z, !MASKED || k4[u].z != 0, gv.z);
+                one(m4[u].w, d4[u].w, s4[u].w, !MASKED || k4[u].w != 0, gv.w);
                 *reinterpret_cast<float4*>(mp[u]) = gv;
                 if (a.any_unconv && with_grad) *reinterpret_cast<float4*>(a.G + off[u]) = gv;
               }
             }
           }
-        }
+        };
+        if (a.mask) pass.template operator()<true>();
+        else pass.template operator()<false>();
       } else {
         for (int i = lw; i < fg.H; i += hpg) {
           const float y = (float)fg.H - 0.5f - (float)i;
@@ -405,12 +466,31 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
         const float* Gb = a.G + (size_t)b * fg.H * fg.W;
         const bool conv = a.md.conv[c] != 0, box = a.md.box[c] != 0;
         dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-          for (int i = lw; i < fg.H; i += hpg) {
-            const float y = (float)fg.H - 0.5f - (float)i;
-            for (int j = lane; j < fg.W; j += 32) {
-              const float seed = conv ? gal[(size_t)i * fg.pitch + j + h] : Gb[(size_t)i * fg.W + j];
-              grad_accumulate<KIND>(cc, box, seed, (float)j + 0.5f, y, sm);
+          if (box) {                                       // Eq. 2 with B != 0: per-pixel geometry
+            for (int i = lw; i < fg.H; i += hpg) {
+              const float y = (float)fg.H - 0.5f - (float)i;
+              for (int j = lane; j < fg.W; j += 32) {
+                const float seed = conv ? gal[(size_t)i * fg.pitch + j + h] : Gb[(size_t)i * fg.W + j];
+                grad_accumulate<KIND>(cc, true, seed, (float)j + 0.5f, y, sm);
+              }
             }
+          } else {
+            GradAcc<KIND> acc;
+            acc.init();
+            for (int idx = gstart; idx < ngrp; idx += gstep) {
+              const int i = group_row(idx), x = (idx - i * W4) << 2;
+              float seed[4];
+              if (conv && kAligned && x + 4 <= fg.W) {
+                const float4 q = *reinterpret_cast<const float4*>(gal + (size_t)i * fg.pitch + h + x);
+                seed[0] = q.x; seed[1] = q.y; seed[2] = q.z; seed[3] = q.w;
+              } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                  seed[k] = (x + k < fg.W) ? (conv ? gal[(size_t)i * fg.pitch + h + x + k] : Gb[(size_t)i * fg.W + x + k]) : 0.0f;
+              }
+              grad_add4<KIND>(acc, cc, seed, (float)x + 0.5f, (float)fg.H - 0.5f - (float)i);
+            }
+            acc.finish(cc, sm);
           }
         });
         if (!box) sm[8] = sm[2];

@@ -219,24 +219,38 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
   const int cols = tg.TW + K - 1;
   bool first = true;
+  // groups of four consecutive columns, one group per lane (row4 / value4, gm_device.cuh)
+  const int P4 = tg.pitch >> 2;
+  const int ngrp = tg.rows * P4;
+  const float inv_p4 = 1.0f / (float)P4;
   auto fill = [&](int kind, const CompConst cc, bool box, bool mag, int slot) {
     dispatch_kind(kind, [&]<int KIND>() {
-      for (int yy = wid; yy < tg.rows; yy += nwarps) {
-        const int i = i0 - h + yy;
-        float* rowp = tilebuf + (size_t)yy * tg.pitch;
-        const bool row_in = (i >= 0 && i < tg.H);
-        const float y = (float)tg.H - 0.5f - (float)i;   // R:G1
-        for (int xx = lane; xx < tg.pitch; xx += 32) {
-          const int j = j0 - h + xx;
-          const bool in = row_in && xx < cols && j >= 0 && j < tg.W;
-          float s = 0.0f;
-          if (KIND != GM_SKY && in) {
-            if (MODE == FWD_DERIV) s = component_deriv_t<KIND>(cc, box, mag, slot, (float)j + 0.5f, y);
-            else s = cc.amp * profile_value_t<KIND, kFastForward>(cc, geometry<kFastForward>(cc, box, (float)j + 0.5f, y).r);
-          }
-          if (first) rowp[xx] = s;
-          else if (in) rowp[xx] += s;
+      for (int idx = tid; idx < ngrp; idx += nthr) {
+        const int yy = (int)(((float)idx + 0.5f) * inv_p4), xx = (idx - yy * P4) << 2;
+        const int i = i0 - h + yy, j = j0 - h + xx;
+        float4* dst = reinterpret_cast<float4*>(tilebuf + (size_t)yy * tg.pitch + xx);
+        const bool any = KIND != GM_SKY && i >= 0 && i < tg.H && xx < cols && j + 3 >= 0 && j < tg.W;
+        if (!any) {
+          if (first) *dst = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          continue;
         }
+        const float y = (float)tg.H - 0.5f - (float)i;   // R:G1
+        float v[4];
+        if (MODE == FWD_DERIV) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) v[k] = component_deriv_t<KIND>(cc, box, mag, slot, (float)(j + k) + 0.5f, y);
+        } else {
+          value4<KIND, kFastForward>(cc, box, (float)j + 0.5f, y, v);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (!(xx + k < cols && j + k >= 0 && j + k < tg.W)) v[k] = 0.0f;
+        float4 o = make_float4(v[0], v[1], v[2], v[3]);
+        if (!first) {
+          const float4 q = *dst;
+          o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
+        }
+        *dst = o;
       }
     });
     first = false;
@@ -466,16 +480,41 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
     const CompConst cc = ccb[c];
     const bool conv = a.md.conv[c] != 0, box = a.md.box[c] != 0;
     dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-      for (int yy = wid; yy < tg.TH; yy += nwarps) {
-        const int i = i0 + yy;
-        if (i >= tg.H) break;
-        const float y = (float)tg.H - 0.5f - (float)i;
-        for (int xx = lane; xx < tg.TW; xx += 32) {
-          const int j = j0 + xx;
-          if (j >= tg.W) break;
-          const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
-          grad_accumulate<KIND>(cc, box, seed, (float)j + 0.5f, y, s);
+      if (box) {                                           // Eq. 2 with B != 0: per-pixel geometry
+        for (int yy = wid; yy < tg.TH; yy += nwarps) {
+          const int i = i0 + yy;
+          if (i >= tg.H) break;
+          const float y = (float)tg.H - 0.5f - (float)i;
+          for (int xx = lane; xx < tg.TW; xx += 32) {
+            const int j = j0 + xx;
+            if (j >= tg.W) break;
+            const float seed = conv ? tilebuf[(size_t)yy * tg.pitch + xx] : Gb[(size_t)i * tg.W + j];
+            grad_accumulate<KIND>(cc, true, seed, (float)j + 0.5f, y, s);
+          }
         }
+      } else {                                             // groups of four pixels of a row per lane
+        GradAcc<KIND> acc;
+        acc.init();
+        const int T4 = (tg.TW + 3) >> 2, ng = tg.TH * T4;
+        const float inv_t4 = 1.0f / (float)T4;
+        for (int idx = tid; idx < ng; idx += nthr) {
+          const int yy = (int)(((float)idx + 0.5f) * inv_t4), xx = (idx - yy * T4) << 2;
+          const int i = i0 + yy, j = j0 + xx;
+          if (i >= tg.H || j >= tg.W) continue;
+          float seed[4];
+          if (conv) {
+            const float4 q = *reinterpret_cast<const float4*>(tilebuf + (size_t)yy * tg.pitch + xx);
+            seed[0] = q.x; seed[1] = q.y; seed[2] = q.z; seed[3] = q.w;
+          }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const bool in = xx + k < tg.TW && j + k < tg.W;
+            if (!conv) seed[k] = in ? Gb[(size_t)i * tg.W + j + k] : 0.0f;
+            else if (!in) seed[k] = 0.0f;
+          }
+          grad_add4<KIND>(acc, cc, seed, (float)j + 0.5f, (float)tg.H - 0.5f - (float)i);
+        }
+        acc.finish(cc, s);
       }
     });
     if (!box) s[8] = s[2];

@@ -102,6 +102,7 @@ __device__ inline void make_comp_const(const ModelDesc& md, int c, const float* 
   cc.iq = (float)(1.0 / q);
   cc.q = (float)q;
   cc.amp = (float)get(GM_SLOT_AMP, 0.0);
+  cc.b0 = cc.b1 = cc.b2 = 0.0f;
   double a[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
   const double s0 = get(GM_SLOT_S0, 1.0), s1 = get(GM_SLOT_S1, 1.0), s2 = get(GM_SLOT_S2, 1.0);
   const double log2e = 1.4426950408889634074;
@@ -114,6 +115,8 @@ __device__ inline void make_comp_const(const ModelDesc& md, int c, const float* 
       a[2] = nu * log2e;
       a[3] = nu;
       a[4] = dnu;
+      cc.b0 = (float)(1.0 / (s0 * s0));     // value_uv, GradAcc: lg2(r^2 / re^2) / (2n)
+      cc.b1 = (float)(0.5 / s1);
       break;
     }
     case GM_EXPDISK:                        // Eq. 7
@@ -166,7 +169,6 @@ __device__ inline void make_comp_const(const ModelDesc& md, int c, const float* 
   const double Bx = get(GM_SLOT_BOX, 0.0), cexp = 2.0 + Bx;
   cc.c = (float)cexp; cc.ic = (float)(1.0 / cexp); cc.cm1 = (float)(cexp - 1.0);
   cc.dl_box = 0.0f; cc.dl_m = 0.0f; cc.dl_q = 0.0f; cc.dl_s0 = 0.0f; cc.dl_s1 = 0.0f; cc.dl_s2 = 0.0f;
-  cc.pad0 = cc.pad1 = cc.pad2 = 0.0f;
   if (md.mag[c]) {
     const double ln10 = 2.302585092994045684, pi = 3.14159265358979323846;
     const double m = get(GM_SLOT_AMP, 0.0), m0 = get(GM_SLOT_M0, 0.0);
