@@ -243,7 +243,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
   // The helper loops walk a cutout in groups of four consecutive pixels of a row, one group
   // per lane: group idx -> (row, first column).  The warps of a cutout interleave by 32 groups.
   const int W4 = (fg.W + 3) >> 2;
+#ifdef GM_EXP_NOHELP
+  const int ngrp = 0;
+#else
   const int ngrp = fg.H * W4;
+#endif
   const float inv_w4 = 1.0f / (float)W4;
   const int gstart = lw * 32 + lane, gstep = hpg * 32;
   auto group_row = [&](int idx) -> int { return (int)(((float)idx + 0.5f) * inv_w4); };   // exact: idx < 2^16

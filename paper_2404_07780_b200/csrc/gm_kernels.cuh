@@ -39,6 +39,7 @@ struct TileGeom {
   int TH, TW;              // CTA tile (multiples of 8)
   int tiles_x, tiles_y;    // tiles per cutout
   int ntx, nty;            // thread tiles per CTA tile
+  int variant;             // thread tile: 0 = 8 x 8 (RP 4, TC 8), 1 = 6 x 12 (RP 3, TC 12)
   int pitch;               // shared row pitch (floats), multiple of 4
   int rows;                // TH + K - 1
   int vec;                 // 1: W % 4 == 0 and data/sigma/mask/out aligned for 128-bit access
@@ -94,16 +95,18 @@ __device__ __forceinline__ float2 tap_pair(const float* __restrict__ psf, int K,
   return make_float2(lo, hi);
 }
 
-// 8x8 outputs per thread.  win points at the thread's window origin in the shared
-// tile (row 0 of its 8 + K - 1 input rows, first of its 8 + K - 1 input columns).
-// acc[rp][c] = (out[2rp][c], out[2rp+1][c]).
-template <int K>
-__device__ __forceinline__ void conv8x8(const float* __restrict__ win, int pitch,
-                                        const float2* __restrict__ taps, float2 (&acc)[4][kTC]) {
-  constexpr int NW = ConvCfg<K>::kWin;
+// (2 RP) x TC outputs per thread (8 x 8 or 6 x 12).  win points at the thread's window
+// origin in the shared tile (row 0 of its 2 RP + K - 1 input rows, first of its TC + K - 1
+// input columns).  acc[rp][c] = (out[2rp][c], out[2rp+1][c]).  With TC = 12 the windows
+// of the 8 lanes of a shared-memory wavefront start 12 words apart and touch all 32
+// banks once; with TC = 8 they collide two by two.
+template <int K, int RP, int TC>
+__device__ __forceinline__ void conv_tile(const float* __restrict__ win, int pitch,
+                                          const float2* __restrict__ taps, float2 (&acc)[RP][TC]) {
+  constexpr int NW = ((TC + K - 1) + 3) / 4;
   constexpr int TP = ConvCfg<K>::kTapPitch;
 #pragma unroll 1
-  for (int y = 0; y < ConvCfg<K>::kInRows; ++y) {
+  for (int y = 0; y < 2 * RP + K - 1; ++y) {
     float in[NW * 4];
     const float4* row = reinterpret_cast<const float4*>(win + y * pitch);
 #pragma unroll
@@ -112,7 +115,7 @@ __device__ __forceinline__ void conv8x8(const float* __restrict__ win, int pitch
       in[4 * j + 0] = v.x; in[4 * j + 1] = v.y; in[4 * j + 2] = v.z; in[4 * j + 3] = v.w;
     }
 #pragma unroll
-    for (int rp = 0; rp < 4; ++rp) {
+    for (int rp = 0; rp < RP; ++rp) {
       const int a = y - 2 * rp;
       if (a >= 0 && a <= K) {
         const float4* tp = reinterpret_cast<const float4*>(taps + a * TP);
@@ -120,12 +123,12 @@ __device__ __forceinline__ void conv8x8(const float* __restrict__ win, int pitch
         for (int t2 = 0; t2 < (K + 1) / 2; ++t2) {
           const float4 w = tp[t2];                      // two tap pairs
 #pragma unroll
-          for (int c = 0; c < kTC; ++c)
+          for (int c = 0; c < TC; ++c)
             acc[rp][c] = __ffma2_rn(make_float2(in[c + 2 * t2], in[c + 2 * t2]),
                                     make_float2(w.x, w.y), acc[rp][c]);
           if (2 * t2 + 1 < K) {
 #pragma unroll
-            for (int c = 0; c < kTC; ++c)
+            for (int c = 0; c < TC; ++c)
               acc[rp][c] = __ffma2_rn(make_float2(in[c + 2 * t2 + 1], in[c + 2 * t2 + 1]),
                                       make_float2(w.z, w.w), acc[rp][c]);
           }
@@ -164,16 +167,18 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-// acc -> 8x8 block of the shared tile (rows 2rp, 2rp+1), two float4 per row
-__device__ __forceinline__ void store_acc(float* dst, int pitch, const float2 (&acc)[4][kTC]) {
+// acc -> the thread's block of the shared tile (rows 2rp, 2rp+1), TC / 4 float4 per row
+template <int RP, int TC>
+__device__ __forceinline__ void store_acc(float* dst, int pitch, const float2 (&acc)[RP][TC]) {
 #pragma unroll
-  for (int rp = 0; rp < 4; ++rp) {
+  for (int rp = 0; rp < RP; ++rp) {
     float4* r0 = reinterpret_cast<float4*>(dst + (size_t)(2 * rp) * pitch);
     float4* r1 = reinterpret_cast<float4*>(dst + (size_t)(2 * rp + 1) * pitch);
-    r0[0] = make_float4(acc[rp][0].x, acc[rp][1].x, acc[rp][2].x, acc[rp][3].x);
-    r0[1] = make_float4(acc[rp][4].x, acc[rp][5].x, acc[rp][6].x, acc[rp][7].x);
-    r1[0] = make_float4(acc[rp][0].y, acc[rp][1].y, acc[rp][2].y, acc[rp][3].y);
-    r1[1] = make_float4(acc[rp][4].y, acc[rp][5].y, acc[rp][6].y, acc[rp][7].y);
+#pragma unroll
+    for (int c = 0; c < TC; c += 4) {
+      r0[c >> 2] = make_float4(acc[rp][c].x, acc[rp][c + 1].x, acc[rp][c + 2].x, acc[rp][c + 3].x);
+      r1[c >> 2] = make_float4(acc[rp][c].y, acc[rp][c + 1].y, acc[rp][c + 2].y, acc[rp][c + 3].y);
+    }
   }
 }
 
@@ -187,7 +192,7 @@ __host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int
 // ---------------------------------------------------------------------------
 // forward: render + convolve + residual
 // ---------------------------------------------------------------------------
-template <int K, int MODE>
+template <int K, int MODE, int RP, int TC>
 __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   constexpr bool RENDER = (MODE != FWD_LOSS);            // an image is written, no residual
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -272,17 +277,17 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   // a2: M = PSF (*) S on this thread's 8x8 block
   const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
   const bool active = ty < tg.nty;
-  float2 acc[4][kTC];
+  float2 acc[RP][TC];
 #pragma unroll
-  for (int rp = 0; rp < 4; ++rp)
+  for (int rp = 0; rp < RP; ++rp)
 #pragma unroll
-    for (int c = 0; c < kTC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
-  if (active) conv8x8<K>(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, taps, acc);
+    for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
+  if (active) conv_tile<K, RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, taps, acc);
 
   // park M in the (now dead) tile buffer so that the epilogue can walk the tile
   // row-major with coalesced global accesses
   __syncthreads();
-  if (active) store_acc(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, acc);
+  if (active) store_acc<RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, acc);
   __syncthreads();
 
   // a3: unconvolved components, residual, chi2, back-seed G
@@ -306,35 +311,40 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
     }
     return m;
   };
+  // branch free; weight and residual are SELECTED for unused pixels, never multiplied by 0 (R:X1)
   auto residual = [&](float m, float d, float sg, bool used, float& g) {
-    g = 0.0f;
-    if (used) {                                        // select, never multiply by 0 (R:X1)
-      const float w = __fdividef(1.0f, sg * sg);
-      const float rho = d - m;
-      chi2 = fmaf(w * rho, rho, chi2);
-      g = -2.0f * w * rho;
-    }
+    float w = rcp_fast(sg * sg), rho = d - m;
+    w = used ? w : 0.0f;
+    rho = used ? rho : 0.0f;
+    const float t = w * rho;
+    chi2 = fmaf(t, rho, chi2);
+    g = -2.0f * t;
   };
   if (tg.vec) {
-    // 128-bit path: one lane = 4 consecutive pixels, two rows per warp in flight
-    for (int yy = wid; yy < tg.TH; yy += 2 * nwarps) {
+    // 128-bit path: one lane = 4 consecutive pixels, two groups per thread in flight
+    const int T4 = tg.TW >> 2, ng = tg.TH * T4;
+    const float inv_t4 = 1.0f / (float)T4;
+#pragma unroll 1
+    for (int idx = tid; idx < ng; idx += 2 * nthr) {
       float4 m4[2], d4[2], s4[2];
       uchar4 k4[2];
       bool ok[2];
       size_t off[2];
-      const int xx = lane * 4;
+      int yr[2], xc[2];
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
-        const int yr = yy + u * nwarps;
-        const int i = i0 + yr, j = j0 + xx;
-        ok[u] = (yr < tg.TH) && (i < tg.H) && (xx < tg.TW) && (j < tg.W);
+        const int id = idx + u * nthr;
+        yr[u] = (int)(((float)id + 0.5f) * inv_t4); xc[u] = (id - yr[u] * T4) << 2;
+        const int i = i0 + yr[u], j = j0 + xc[u];
+        ok[u] = (id < ng) && (i < tg.H) && (j < tg.W);
         off[u] = img + (size_t)i * tg.W + j;
+        k4[u] = make_uchar4(1, 1, 1, 1);
         if (ok[u]) {
-          m4[u] = *reinterpret_cast<const float4*>(tilebuf + (size_t)yr * tg.pitch + xx);
+          m4[u] = *reinterpret_cast<const float4*>(tilebuf + (size_t)yr[u] * tg.pitch + xc[u]);
           if (!RENDER) {
             d4[u] = *reinterpret_cast<const float4*>(a.data + off[u]);
             s4[u] = *reinterpret_cast<const float4*>(a.sigma + off[u]);
-            k4[u] = a.mask ? *reinterpret_cast<const uchar4*>(a.mask + off[u]) : make_uchar4(1, 1, 1, 1);
+            if (a.mask) k4[u] = *reinterpret_cast<const uchar4*>(a.mask + off[u]);
           }
         }
       }
@@ -342,8 +352,8 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
       for (int u = 0; u < 2; ++u) {
         if (!ok[u]) continue;
         if (any_unconv) {
-          const float y = (float)tg.H - 0.5f - (float)(i0 + yy + u * nwarps);
-          const float x = (float)(j0 + xx) + 0.5f;
+          const float y = (float)tg.H - 0.5f - (float)(i0 + yr[u]);
+          const float x = (float)(j0 + xc[u]) + 0.5f;
           m4[u].x = add_unconv(m4[u].x, x, y);
           m4[u].y = add_unconv(m4[u].y, x + 1.0f, y);
           m4[u].z = add_unconv(m4[u].z, x + 2.0f, y);
@@ -398,7 +408,7 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
 // backward: adjoint convolution + parameter-gradient partial sums
 // (10 per component, see grad_accumulate in gm_device.cuh)
 // ---------------------------------------------------------------------------
-template <int K>
+template <int K, int RP, int TC>
 __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
@@ -457,17 +467,17 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
 
   const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
   const bool active = ty < tg.nty;
-  float2 acc[4][kTC];
+  float2 acc[RP][TC];
 #pragma unroll
-  for (int rp = 0; rp < 4; ++rp)
+  for (int rp = 0; rp < RP; ++rp)
 #pragma unroll
-    for (int c = 0; c < kTC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
-  if (active) conv8x8<K>(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, taps, acc);
+    for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
+  if (active) conv_tile<K, RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, taps, acc);
 
   // park A in the tile buffer (G itself stays in global memory for the
   // unconvolved components), then walk the tile row-major
   __syncthreads();
-  if (active) store_acc(tilebuf + (size_t)(ty * kTR) * tg.pitch + tx * kTC, tg.pitch, acc);
+  if (active) store_acc<RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, acc);
   __syncthreads();
 
   // a5: partial sums per component

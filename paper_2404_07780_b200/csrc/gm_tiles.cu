@@ -31,6 +31,22 @@ static int tile_threads(const TileGeom& tg, int nthr) {
   return (2 * one > 233472) ? 512 : nthr;
 }
 
+template <int K, int RP, int TC>
+static int launch_forward_v(const FwdArgs& a, int mode, int nthr, size_t sm, unsigned grid, cudaStream_t st, cudaError_t* err) {
+  if (mode == FWD_RENDER) {
+    GM_TRY(set_smem(k_forward<K, FWD_RENDER, RP, TC>, sm));
+    k_forward<K, FWD_RENDER, RP, TC><<<grid, nthr, sm, st>>>(a);
+  } else if (mode == FWD_DERIV) {
+    GM_TRY(set_smem(k_forward<K, FWD_DERIV, RP, TC>, sm));
+    k_forward<K, FWD_DERIV, RP, TC><<<grid, nthr, sm, st>>>(a);
+  } else {
+    GM_TRY(set_smem(k_forward<K, FWD_LOSS, RP, TC>, sm));
+    k_forward<K, FWD_LOSS, RP, TC><<<grid, nthr, sm, st>>>(a);
+  }
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
 int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err) {
   constexpr int K = GM_K;
   int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
@@ -38,18 +54,8 @@ int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_
   nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
-  if (mode == FWD_RENDER) {
-    GM_TRY(set_smem(k_forward<K, FWD_RENDER>, sm));
-    k_forward<K, FWD_RENDER><<<grid, nthr, sm, st>>>(a);
-  } else if (mode == FWD_DERIV) {
-    GM_TRY(set_smem(k_forward<K, FWD_DERIV>, sm));
-    k_forward<K, FWD_DERIV><<<grid, nthr, sm, st>>>(a);
-  } else {
-    GM_TRY(set_smem(k_forward<K, FWD_LOSS>, sm));
-    k_forward<K, FWD_LOSS><<<grid, nthr, sm, st>>>(a);
-  }
-  GM_TRY(cudaGetLastError());
-  return GM_OK;
+  return a.tg.variant == 1 ? launch_forward_v<K, 3, 12>(a, mode, nthr, sm, grid, st, err)
+                           : launch_forward_v<K, 4, 8>(a, mode, nthr, sm, grid, st, err);
 }
 
 int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err) {
@@ -59,8 +65,13 @@ int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cud
   nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
-  GM_TRY(set_smem(k_backward<K>, sm));
-  k_backward<K><<<grid, nthr, sm, st>>>(a);
+  if (a.tg.variant == 1) {
+    GM_TRY(set_smem(k_backward<K, 3, 12>, sm));
+    k_backward<K, 3, 12><<<grid, nthr, sm, st>>>(a);
+  } else {
+    GM_TRY(set_smem(k_backward<K, 4, 8>, sm));
+    k_backward<K, 4, 8><<<grid, nthr, sm, st>>>(a);
+  }
   GM_TRY(cudaGetLastError());
   return GM_OK;
 }

@@ -82,7 +82,9 @@ def test_each_profile_alone(kind, convolve):
 # ---- several tiles per cutout, ragged tails, every compiled PSF side ------------------
 @pytest.mark.parametrize("H,W,K", [(150, 140, 25), (131, 70, 15), (64, 200, 21), (96, 96, 25),
                                    (50, 50, 41), (40, 40, 33), (9, 300, 5), (5, 7, 3), (1, 1, 1),
-                                   (130, 129, 11)])
+                                   (130, 129, 11),
+                                   # 6 x 12 thread tiles (96 x 192 / 192 x 96 CTA tiles), full and ragged
+                                   (192, 192, 25), (180, 96, 9), (96, 190, 15), (200, 380, 5)])
 def test_multi_tile_and_ragged(H, W, K):
     model = models.bulge_disk()
     par, data, sigma, mask, psf = synth(model, 2, H, W, K, seed=H + W + K)
