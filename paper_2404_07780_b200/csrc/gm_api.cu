@@ -758,8 +758,10 @@ static bool make_fused_geom(int H, int W, int KP, bool shared_taps, size_t smem_
   return best > 0.0;
 }
 
+// early_stop: the call is a fit whose galaxies stop one by one (tol > 0), so the number of live
+// galaxies shrinks during the call.
 static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, void* workspace,
-                     size_t workspace_bytes, cudaStream_t st, Plan* pl) {
+                     size_t workspace_bytes, cudaStream_t st, Plan* pl, bool early_stop = false) {
   int rc = validate(model, bt, need_data, &pl->md);
   if (rc != GM_OK) return rc;
   pl->KP = padded_K(bt->K);
@@ -773,6 +775,18 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   pl->fused = bt->H <= 128 && bt->W <= 128 && !getenv("GM_NO_FUSED") &&
               make_fused_geom(bt->H, bt->W, pl->KP, bt->psf_stride == 0, pl->caps.smem_optin, &pl->fg,
                               &pl->fused_variant);
+  // One cutout per slot (sides above 96): k_fused and the tile kernels run the same loop at the
+  // same rate (0.70 against 0.71 of the FP32 peak at 128 x 128, K = 25), but k_fused hands whole
+  // galaxies to 148 CTAs while the tile kernels schedule B x tiles CTAs two per SM.  Take the
+  // tiles when the galaxy count does not fill the last round of k_fused, or shrinks during
+  // the call, provided two tile CTAs fit an SM (K <= 33; at K = 41 only k_fused overlaps).
+  if (pl->fused && pl->fg.G == 1) {
+    const size_t tile_smem = (size_t)pl->tg.rows * pl->tg.pitch * 4 + (size_t)(pl->KP + 1) * (pl->KP + 1) * 8 + 2048;
+    const bool two_fit = 2 * tile_smem <= pl->caps.smem_optin;
+    const int rounds = (bt->B + pl->caps.n_sm - 1) / pl->caps.n_sm;
+    const double fill = (double)bt->B / ((double)rounds * pl->caps.n_sm);
+    if (two_fit && (early_stop || fill < 0.97)) pl->fused = false;
+  }
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
   if (pl->KP != bt->K) {
@@ -1050,7 +1064,7 @@ static int fit_begin(FitRun* r, const gm_model* model, const gm_batch* bt, float
                      size_t workspace_bytes, cudaStream_t st) {
   if (!params || !chi2_out || !opts || !opts->lr || !opts->lo || !opts->hi) return GM_EINVAL;
   if (opts->n_iter < 0 || opts->patience < 0) return GM_EINVAL;
-  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &r->pl);
+  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &r->pl, opts->tol > 0.0f);
   if (rc != GM_OK) return rc;
   const Plan& pl = r->pl;
   const int B = bt->B, P = pl.md.n_par;
