@@ -631,7 +631,9 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   int launch_forward_##K(const FwdArgs& a, int mode, int B, cudaStream_t st, cudaError_t* err); \
   int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
   int launch_fused_##K(const FusedArgs& a, int variant, int n_sm, size_t smem_limit, cudaStream_t st,         \
-                       cudaError_t* err);
+                       cudaError_t* err);                                                     \
+  int tap_pool_acquire_##K(const float2* taps_dev, int n, cudaStream_t st, int* off, cudaError_t* err); \
+  void tap_pool_release_##K(int off, cudaStream_t st);
 GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
 #undef GM_DECL_K
 
@@ -695,6 +697,36 @@ static int dispatch_fused(int KP, const FusedArgs& a, int v, int n_sm, size_t li
   return rc;
 }
 
+// region of the constant-bank tap pool of side KP (gm_kernels.cuh); *off = -1 when none is free
+static int tap_pool_acquire(int KP, const float2* taps_dev, int n, cudaStream_t st, int* off) {
+  int rc;
+  cudaError_t err = cudaSuccess;
+  switch (KP) {
+    case 5: rc = tap_pool_acquire_5(taps_dev, n, st, off, &err); break;
+    case 9: rc = tap_pool_acquire_9(taps_dev, n, st, off, &err); break;
+    case 15: rc = tap_pool_acquire_15(taps_dev, n, st, off, &err); break;
+    case 21: rc = tap_pool_acquire_21(taps_dev, n, st, off, &err); break;
+    case 25: rc = tap_pool_acquire_25(taps_dev, n, st, off, &err); break;
+    case 33: rc = tap_pool_acquire_33(taps_dev, n, st, off, &err); break;
+    case 41: rc = tap_pool_acquire_41(taps_dev, n, st, off, &err); break;
+    default: *off = -1; return GM_OK;
+  }
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+static void tap_pool_release(int KP, int off, cudaStream_t st) {
+  switch (KP) {
+    case 5: tap_pool_release_5(off, st); break;
+    case 9: tap_pool_release_9(off, st); break;
+    case 15: tap_pool_release_15(off, st); break;
+    case 21: tap_pool_release_21(off, st); break;
+    case 25: tap_pool_release_25(off, st); break;
+    case 33: tap_pool_release_33(off, st); break;
+    case 41: tap_pool_release_41(off, st); break;
+    default: break;
+  }
+}
+
 struct DevCaps { int n_sm; size_t smem_optin; };
 static int device_caps(DevCaps* out) {
   static std::mutex mu;
@@ -727,6 +759,13 @@ struct Plan {
   bool fused;                // whole cutouts per CTA and two slots fit: k_fused path
   FusedGeom fg; int fused_variant;
   DevCaps caps;
+  // lease of a region of the constant-bank tap pool (shared PSF only); handed back, by an event
+  // on the call's stream, when the plan goes out of scope at the end of the API call
+  int ct_off = -1; cudaStream_t ct_stream = nullptr;
+  Plan() = default;
+  Plan(const Plan&) = delete;
+  Plan& operator=(const Plan&) = delete;
+  ~Plan() { if (ct_off >= 0) tap_pool_release(KP, ct_off, ct_stream); }
 };
 
 // Geometry of the fused kernel for an H x W cutout: thread-tile variant (0: 8x8, 1: 6x12) and
@@ -808,6 +847,10 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
     pl->taps_fwd = pl->ws.taps;
     pl->taps_adj = pl->ws.taps + per;
     pl->taps_stride = bt->psf_stride == 0 ? 0 : 2ll * per;
+    if (bt->psf_stride == 0 && !getenv("GM_NO_CONST_TAPS")) {
+      if ((rc = tap_pool_acquire(pl->KP, pl->ws.taps, 2 * per, st, &pl->ct_off)) != GM_OK) return rc;
+      pl->ct_stream = st;
+    }
   }
   return GM_OK;
 }
@@ -834,7 +877,7 @@ static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const Li
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
   a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
-  a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride;
+  a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
@@ -846,6 +889,7 @@ static BwdArgs bwd_args(const Plan& pl, const LiveSet& ls) {
   BwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   a.taps = pl.taps_adj; a.taps_stride = pl.taps_stride;
+  a.ct_off = pl.ct_off >= 0 ? pl.ct_off + (pl.KP + 1) * (pl.KP + 1) : -1;
   a.G = pl.ws.G; a.grad_part = pl.ws.grad_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   return a;
@@ -856,7 +900,7 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
   a.md = pl.md; a.fg = pl.fg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
   a.any_unconv = 0;
   for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
-  a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride;
+  a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;

@@ -55,6 +55,7 @@ struct FusedArgs {
   int any_unconv;            // model has unconvolved components (G also goes to global)
   const CompConst* cc;
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
+  int ct_off;                // >= 0: both tap sets of the shared PSF at c_tap_pool[ct_off ..] (forward, then adjoint)
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                  // [B,H,W]: model_out (mode 0) or back-seed spill (any_unconv)
   float* chi2_part;          // [B]
@@ -124,6 +125,38 @@ __device__ __forceinline__ void conv_rows(const float* __restrict__ gal, int pit
   }
 }
 
+// the same with the taps in the constant bank (conv_tile_ct, gm_kernels.cuh): tap row a
+// outermost, the input row (or the zero row) reloaded for every row pair
+template <int K, int RP, int TC>
+__device__ __forceinline__ void conv_rows_ct(const float* __restrict__ gal, int pitch, int H, int i0, int c0,
+                                             int ct_off, float2 (&acc)[RP][TC]) {
+  constexpr int NW = ((TC + K - 1) + 3) / 4;
+  constexpr int TP = ConvCfg<K>::kTapPitch;
+#pragma unroll 2
+  for (int a = 0; a <= K; ++a) {
+    const float2* tp = c_tap_pool + ct_off + a * TP;
+#pragma unroll
+    for (int rp = 0; rp < RP; ++rp) {
+      const int i = i0 + a + 2 * rp;
+      const int r = ((unsigned)i < (unsigned)H) ? i : H;          // outside the cutout: the zero row
+      float in[NW * 4];
+      const float4* row = reinterpret_cast<const float4*>(gal + r * pitch + c0);
+#pragma unroll
+      for (int j = 0; j < NW; ++j) {
+        const float4 v = row[j];
+        in[4 * j + 0] = v.x; in[4 * j + 1] = v.y; in[4 * j + 2] = v.z; in[4 * j + 3] = v.w;
+      }
+#pragma unroll
+      for (int t = 0; t < K; ++t) {
+        const float2 w = tp[t];
+#pragma unroll
+        for (int c = 0; c < TC; ++c)
+          acc[rp][c] = __ffma2_rn(make_float2(in[c + t], in[c + t]), w, acc[rp][c]);
+      }
+    }
+  }
+}
+
 // acc -> interior of the cutout's slot (row r, column c + h); 128-bit stores when aligned.
 // Outputs that fall outside the H x W cutout (ragged thread tile) are not stored: the slot
 // is the input of the adjoint convolution next, whose zero fill starts at the cutout edge.
@@ -156,7 +189,7 @@ __device__ __forceinline__ void store_acc_slot(float* gal, int pitch, int r0, in
   }
 }
 
-template <int K, int RP, int TC>
+template <int K, int RP, int TC, bool CT>
 __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const FusedGeom& fg = a.fg;
@@ -205,8 +238,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
           for (int rp = 0; rp < RP; ++rp)
 #pragma unroll
             for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
-          if (active)
-            conv_rows<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, taps_of(s, g, phase), acc);
+          if (active) {
+            if (CT) conv_rows_ct<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, a.ct_off + phase * TAPN, acc);
+            else conv_rows<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, taps_of(s, g, phase), acc);
+          }
           bar_sync(BAR_CONV, kConvThreads);                     // every conv thread is done reading
           if (active) store_acc_slot<K, RP, TC>(gal, fg.pitch, ty * 2 * RP, tx * TC, fg.H, fg.W, acc);
           bar_arrive(BAR_DONE0 + s, kFusedThreads);             // M (or A) is parked in the slot
@@ -231,7 +266,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
     const int n4 = (int)((2 * slot_elems) >> 2);            // gal_elems is a multiple of 4
     for (int i = htid; i < n4; i += HN) z[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
-  if (fg.shared_taps) {
+  if (!CT && fg.shared_taps) {
     for (int i = htid; i < TAPN / 2; i += HN) {
       cp_async_zfill16(reinterpret_cast<float*>(taps0) + 4 * i, reinterpret_cast<const float*>(a.taps_fwd) + 4 * i, true);
       cp_async_zfill16(reinterpret_cast<float*>(taps0 + TAPN) + 4 * i,

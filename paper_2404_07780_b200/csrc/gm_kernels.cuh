@@ -50,6 +50,7 @@ struct FwdArgs {
   TileGeom tg;
   const CompConst* cc;     // [B, n_comp]
   const float2* taps; long long taps_stride;   // paired flipped taps, float2 per galaxy (0 = shared)
+  int ct_off;              // >= 0: the taps of the shared PSF sit at c_tap_pool[ct_off ..] (constant bank)
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                // [B,H,W] workspace (or model_out when RENDER)
   float* chi2_part;        // [B, tiles]
@@ -68,6 +69,7 @@ struct BwdArgs {
   TileGeom tg;
   const CompConst* cc;
   const float2* taps; long long taps_stride;   // paired unflipped taps
+  int ct_off;              // >= 0: taps at c_tap_pool[ct_off ..]
   const float* G;          // [B,H,W]
   float* grad_part;        // [B, tiles, n_comp, kNSum]
   const int* frozen;
@@ -138,6 +140,50 @@ __device__ __forceinline__ void conv_tile(const float* __restrict__ win, int pit
   }
 }
 
+// ---------------------------------------------------------------------------
+// Taps in the constant bank.  FFMA2 takes its tap pair straight from a UNIFORM register
+// (FFMA2 R, R.F32, UR.F32x2, R) that LDCU fills from constant memory: no shared-memory
+// load, no vector register and no register-bank conflict per tap.  That needs a tap
+// address that is uniform over the warp and a constant-bank home for the taps, so the
+// paired taps of a batch-wide PSF are copied (device to device, on the call's stream)
+// into a region of this pool for the duration of the call; the region is handed out by
+// the host-side allocator in gm_tiles.cu, and when none is free, or the PSF is per
+// galaxy, the shared-memory form above runs instead.  The loop runs tap row a outermost
+// (so the row's taps are loop constants) and reloads the input row for each row pair;
+// every accumulator still sees its K^2 products in the same (a, t) order as conv_tile.
+// Stand-alone (148 CTAs, 128 x 128, K = 25): 0.935 of the FP32 peak against 0.823.
+// ---------------------------------------------------------------------------
+constexpr int kTapPoolN = 7424;                           // float2: 59,392 bytes of the 64 KB bank
+__constant__ float2 c_tap_pool[kTapPoolN];
+
+template <int K, int RP, int TC>
+__device__ __forceinline__ void conv_tile_ct(const float* __restrict__ win, int pitch, int ct_off,
+                                             float2 (&acc)[RP][TC]) {
+  constexpr int NW = ((TC + K - 1) + 3) / 4;
+  constexpr int TP = ConvCfg<K>::kTapPitch;
+#pragma unroll 2
+  for (int a = 0; a <= K; ++a) {
+    const float2* tp = c_tap_pool + ct_off + a * TP;
+#pragma unroll
+    for (int rp = 0; rp < RP; ++rp) {
+      float in[NW * 4];
+      const float4* row = reinterpret_cast<const float4*>(win + (a + 2 * rp) * pitch);
+#pragma unroll
+      for (int j = 0; j < NW; ++j) {
+        const float4 v = row[j];
+        in[4 * j + 0] = v.x; in[4 * j + 1] = v.y; in[4 * j + 2] = v.z; in[4 * j + 3] = v.w;
+      }
+#pragma unroll
+      for (int t = 0; t < K; ++t) {
+        const float2 w = tp[t];
+#pragma unroll
+        for (int c = 0; c < TC; ++c)
+          acc[rp][c] = __ffma2_rn(make_float2(in[c + t], in[c + t]), w, acc[rp][c]);
+      }
+    }
+  }
+}
+
 // cp.async with zero fill: copies `bytes` (4 or 16) when valid, writes zeros otherwise
 __device__ __forceinline__ void cp_async_zfill4(float* dst, const float* src, bool valid) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(dst);
@@ -192,7 +238,7 @@ __host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int
 // ---------------------------------------------------------------------------
 // forward: render + convolve + residual
 // ---------------------------------------------------------------------------
-template <int K, int MODE, int RP, int TC>
+template <int K, int MODE, int RP, int TC, bool CT>
 __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   constexpr bool RENDER = (MODE != FWD_LOSS);            // an image is written, no residual
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -215,7 +261,7 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
   float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
 
-  copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
+  if (!CT) copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 
   // a1: S on the tile plus its halo; zero outside the cutout (R:C1) and in the pad.
   // One pass per convolved component, its radial law selected outside the pixel loops.
@@ -282,7 +328,11 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
   for (int rp = 0; rp < RP; ++rp)
 #pragma unroll
     for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
-  if (active) conv_tile<K, RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, taps, acc);
+  if (active) {
+    const float* win = tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC;
+    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, acc);
+    else conv_tile<K, RP, TC>(win, tg.pitch, taps, acc);
+  }
 
   // park M in the (now dead) tile buffer so that the epilogue can walk the tile
   // row-major with coalesced global accesses
@@ -408,7 +458,7 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
 // backward: adjoint convolution + parameter-gradient partial sums
 // (10 per component, see grad_accumulate in gm_device.cuh)
 // ---------------------------------------------------------------------------
-template <int K, int RP, int TC>
+template <int K, int RP, int TC, bool CT>
 __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const TileGeom& tg = a.tg;
@@ -430,7 +480,7 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
   float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
 
-  copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
+  if (!CT) copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 
   // G tile + halo through cp.async (no register staging, all copies in flight at
   // once); zero outside the cutout (R:C2) and in the pad columns
@@ -472,7 +522,11 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   for (int rp = 0; rp < RP; ++rp)
 #pragma unroll
     for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
-  if (active) conv_tile<K, RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, taps, acc);
+  if (active) {
+    const float* win = tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC;
+    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, acc);
+    else conv_tile<K, RP, TC>(win, tg.pitch, taps, acc);
+  }
 
   // park A in the tile buffer (G itself stays in global memory for the
   // unconvolved components), then walk the tile row-major

@@ -2,6 +2,9 @@
 // Compiled once per supported K (see build.py) so the builds run in parallel.
 #include "gm_fused.cuh"
 
+#include <mutex>
+#include <vector>
+
 #ifndef GM_K
 #error "compile with -DGM_K=<PSF side>"
 #endif
@@ -31,17 +34,79 @@ static int tile_threads(const TileGeom& tg, int nthr) {
   return (2 * one > 233472) ? 512 : nthr;
 }
 
-template <int K, int RP, int TC>
+// ---------------------------------------------------------------------------
+// Host-side allocator of c_tap_pool (one pool per PSF side: each gm_tiles object is its own
+// module with its own constant bank).  A region holds the forward + adjoint tap sets of one
+// call; it is filled on the call's stream and handed back by an event recorded on that
+// stream after the call's last launch, so concurrent calls (gm_fit_multi runs one stream per
+// size bucket) never share a region that is still being read.  No region free: the caller
+// runs the shared-memory taps instead.  Nothing here blocks or synchronises.
+// ---------------------------------------------------------------------------
+namespace {
+struct TapRegion { int dev, off, n; cudaEvent_t ev; bool recorded; };
+std::mutex g_pool_mu;
+std::vector<TapRegion> g_pool_used;
+}  // namespace
+
+int GM_CAT(tap_pool_acquire_, GM_K)(const float2* taps_dev, int n, cudaStream_t st, int* off, cudaError_t* err) {
+  *off = -1;
+  if (n <= 0 || n > kTapPoolN || (n & 1)) return GM_OK;
+  int dev = 0;
+  GM_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lk(g_pool_mu);
+  for (size_t i = 0; i < g_pool_used.size();) {           // hand back the regions whose call has finished
+    TapRegion& r = g_pool_used[i];
+    if (r.recorded && cudaEventQuery(r.ev) == cudaSuccess) {
+      cudaEventDestroy(r.ev);
+      g_pool_used.erase(g_pool_used.begin() + i);
+    } else {
+      ++i;
+    }
+  }
+  (void)cudaGetLastError();                                // cudaErrorNotReady of the queries above
+  int start = 0;
+  bool moved = true;
+  while (moved) {                                          // first fit among this device's regions
+    moved = false;
+    for (const TapRegion& r : g_pool_used)
+      if (r.dev == dev && start < r.off + r.n && r.off < start + n) { start = r.off + r.n; moved = true; }
+  }
+  if (start + n > kTapPoolN) return GM_OK;
+  GM_TRY(cudaMemcpyToSymbolAsync(c_tap_pool, taps_dev, (size_t)n * sizeof(float2), (size_t)start * sizeof(float2),
+                                 cudaMemcpyDeviceToDevice, st));
+  g_pool_used.push_back({dev, start, n, nullptr, false});
+  *off = start;
+  return GM_OK;
+}
+
+void GM_CAT(tap_pool_release_, GM_K)(int off, cudaStream_t st) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return;
+  std::lock_guard<std::mutex> lk(g_pool_mu);
+  for (size_t i = 0; i < g_pool_used.size(); ++i) {
+    TapRegion& r = g_pool_used[i];
+    if (r.dev != dev || r.off != off || r.recorded) continue;
+    if (cudaEventCreateWithFlags(&r.ev, cudaEventDisableTiming) == cudaSuccess && cudaEventRecord(r.ev, st) == cudaSuccess) {
+      r.recorded = true;
+    } else {                                               // cannot track it: wait once, then free
+      cudaStreamSynchronize(st);
+      g_pool_used.erase(g_pool_used.begin() + i);
+    }
+    return;
+  }
+}
+
+template <int K, int RP, int TC, bool CT>
 static int launch_forward_v(const FwdArgs& a, int mode, int nthr, size_t sm, unsigned grid, cudaStream_t st, cudaError_t* err) {
   if (mode == FWD_RENDER) {
-    GM_TRY(set_smem(k_forward<K, FWD_RENDER, RP, TC>, sm));
-    k_forward<K, FWD_RENDER, RP, TC><<<grid, nthr, sm, st>>>(a);
+    GM_TRY(set_smem(k_forward<K, FWD_RENDER, RP, TC, CT>, sm));
+    k_forward<K, FWD_RENDER, RP, TC, CT><<<grid, nthr, sm, st>>>(a);
   } else if (mode == FWD_DERIV) {
-    GM_TRY(set_smem(k_forward<K, FWD_DERIV, RP, TC>, sm));
-    k_forward<K, FWD_DERIV, RP, TC><<<grid, nthr, sm, st>>>(a);
+    GM_TRY(set_smem(k_forward<K, FWD_DERIV, RP, TC, CT>, sm));
+    k_forward<K, FWD_DERIV, RP, TC, CT><<<grid, nthr, sm, st>>>(a);
   } else {
-    GM_TRY(set_smem(k_forward<K, FWD_LOSS, RP, TC>, sm));
-    k_forward<K, FWD_LOSS, RP, TC><<<grid, nthr, sm, st>>>(a);
+    GM_TRY(set_smem(k_forward<K, FWD_LOSS, RP, TC, CT>, sm));
+    k_forward<K, FWD_LOSS, RP, TC, CT><<<grid, nthr, sm, st>>>(a);
   }
   GM_TRY(cudaGetLastError());
   return GM_OK;
@@ -54,8 +119,11 @@ int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_
   nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
-  return a.tg.variant == 1 ? launch_forward_v<K, 3, 12>(a, mode, nthr, sm, grid, st, err)
-                           : launch_forward_v<K, 4, 8>(a, mode, nthr, sm, grid, st, err);
+  if (a.ct_off >= 0)
+    return a.tg.variant == 1 ? launch_forward_v<K, 3, 12, true>(a, mode, nthr, sm, grid, st, err)
+                             : launch_forward_v<K, 4, 8, true>(a, mode, nthr, sm, grid, st, err);
+  return a.tg.variant == 1 ? launch_forward_v<K, 3, 12, false>(a, mode, nthr, sm, grid, st, err)
+                           : launch_forward_v<K, 4, 8, false>(a, mode, nthr, sm, grid, st, err);
 }
 
 int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err) {
@@ -65,12 +133,19 @@ int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cud
   nthr = tile_threads<K>(a.tg, nthr);
   const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
-  if (a.tg.variant == 1) {
-    GM_TRY(set_smem(k_backward<K, 3, 12>, sm));
-    k_backward<K, 3, 12><<<grid, nthr, sm, st>>>(a);
+  const bool ct = a.ct_off >= 0;
+  if (a.tg.variant == 1 && ct) {
+    GM_TRY(set_smem(k_backward<K, 3, 12, true>, sm));
+    k_backward<K, 3, 12, true><<<grid, nthr, sm, st>>>(a);
+  } else if (a.tg.variant == 1) {
+    GM_TRY(set_smem(k_backward<K, 3, 12, false>, sm));
+    k_backward<K, 3, 12, false><<<grid, nthr, sm, st>>>(a);
+  } else if (ct) {
+    GM_TRY(set_smem(k_backward<K, 4, 8, true>, sm));
+    k_backward<K, 4, 8, true><<<grid, nthr, sm, st>>>(a);
   } else {
-    GM_TRY(set_smem(k_backward<K, 4, 8>, sm));
-    k_backward<K, 4, 8><<<grid, nthr, sm, st>>>(a);
+    GM_TRY(set_smem(k_backward<K, 4, 8, false>, sm));
+    k_backward<K, 4, 8, false><<<grid, nthr, sm, st>>>(a);
   }
   GM_TRY(cudaGetLastError());
   return GM_OK;
@@ -84,12 +159,19 @@ int GM_CAT(launch_fused_, GM_K)(const FusedArgs& a, int variant, int n_sm, size_
   const size_t sm = fused_smem_bytes(K, a.fg);
   if (sm > smem_limit) return GM_ENOTSUP;
   const unsigned grid = (unsigned)(a.B < n_sm ? a.B : n_sm);
-  if (variant == 0) {
-    GM_TRY(set_smem(k_fused<K, 4, 8>, sm));
-    k_fused<K, 4, 8><<<grid, kFusedThreads, sm, st>>>(a);
+  const bool ct = a.ct_off >= 0;
+  if (variant == 0 && ct) {
+    GM_TRY(set_smem(k_fused<K, 4, 8, true>, sm));
+    k_fused<K, 4, 8, true><<<grid, kFusedThreads, sm, st>>>(a);
+  } else if (variant == 0) {
+    GM_TRY(set_smem(k_fused<K, 4, 8, false>, sm));
+    k_fused<K, 4, 8, false><<<grid, kFusedThreads, sm, st>>>(a);
+  } else if (ct) {
+    GM_TRY(set_smem(k_fused<K, 3, 12, true>, sm));
+    k_fused<K, 3, 12, true><<<grid, kFusedThreads, sm, st>>>(a);
   } else {
-    GM_TRY(set_smem(k_fused<K, 3, 12>, sm));
-    k_fused<K, 3, 12><<<grid, kFusedThreads, sm, st>>>(a);
+    GM_TRY(set_smem(k_fused<K, 3, 12, false>, sm));
+    k_fused<K, 3, 12, false><<<grid, kFusedThreads, sm, st>>>(a);
   }
   GM_TRY(cudaGetLastError());
   return GM_OK;
