@@ -814,18 +814,6 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   pl->fused = bt->H <= 128 && bt->W <= 128 && !getenv("GM_NO_FUSED") &&
               make_fused_geom(bt->H, bt->W, pl->KP, bt->psf_stride == 0, pl->caps.smem_optin, &pl->fg,
                               &pl->fused_variant);
-  // One cutout per slot (sides above 96): k_fused and the tile kernels run the same loop at the
-  // same rate (0.70 against 0.71 of the FP32 peak at 128 x 128, K = 25), but k_fused hands whole
-  // galaxies to 148 CTAs while the tile kernels schedule B x tiles CTAs two per SM.  Take the
-  // tiles when the galaxy count does not fill the last round of k_fused, or shrinks during
-  // the call, provided two tile CTAs fit an SM (K <= 33; at K = 41 only k_fused overlaps).
-  if (pl->fused && pl->fg.G == 1) {
-    const size_t tile_smem = (size_t)pl->tg.rows * pl->tg.pitch * 4 + (size_t)(pl->KP + 1) * (pl->KP + 1) * 8 + 2048;
-    const bool two_fit = 2 * tile_smem <= pl->caps.smem_optin;
-    const int rounds = (bt->B + pl->caps.n_sm - 1) / pl->caps.n_sm;
-    const double fill = (double)bt->B / ((double)rounds * pl->caps.n_sm);
-    if (two_fit && (early_stop || fill < 0.97)) pl->fused = false;
-  }
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
   if (pl->KP != bt->K) {
@@ -852,6 +840,20 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
       pl->ct_stream = st;
     }
   }
+  // One cutout per slot (sides above 96) with the taps in shared memory (per-galaxy PSFs, or no
+  // free region of the constant pool): k_fused and the tile kernels run the same loop at the
+  // same rate (0.70 against 0.71 of the FP32 peak at 128 x 128, K = 25), but k_fused hands whole
+  // galaxies to 148 CTAs while the tile kernels schedule B x tiles CTAs two per SM.  Take the
+  // tiles when the galaxy count does not fill the last round of k_fused, or shrinks during
+  // the call, provided two tile CTAs fit an SM (K <= 33; at K = 41 only k_fused overlaps).  With
+  // the taps in the constant bank k_fused is the faster one (0.80 against 0.74) and stays.
+  if (pl->fused && pl->fg.G == 1 && pl->ct_off < 0) {
+    const size_t tile_smem = (size_t)pl->tg.rows * pl->tg.pitch * 4 + (size_t)(pl->KP + 1) * (pl->KP + 1) * 8 + 2048;
+    const bool two_fit = 2 * tile_smem <= pl->caps.smem_optin;
+    const int rounds = (bt->B + pl->caps.n_sm - 1) / pl->caps.n_sm;
+    const double fill = (double)bt->B / ((double)rounds * pl->caps.n_sm);
+    if (two_fit && (early_stop || fill < 0.97)) pl->fused = false;
+  }
   return GM_OK;
 }
 
@@ -877,7 +879,7 @@ static FwdArgs fwd_args(const Plan& pl, const gm_batch* bt, float* out, const Li
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma | (uintptr_t)out;
   a.tg.vec = ((bt->W & 3) == 0) && ((bits & 15) == 0) && (((uintptr_t)bt->mask & 3) == 0);
-  a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off;
+  a.taps = pl.taps_fwd; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off; a.ct_zero = 0;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
@@ -889,7 +891,7 @@ static BwdArgs bwd_args(const Plan& pl, const LiveSet& ls) {
   BwdArgs a;
   a.md = pl.md; a.tg = pl.tg; a.cc = pl.ws.cc;
   a.taps = pl.taps_adj; a.taps_stride = pl.taps_stride;
-  a.ct_off = pl.ct_off >= 0 ? pl.ct_off + (pl.KP + 1) * (pl.KP + 1) : -1;
+  a.ct_off = pl.ct_off >= 0 ? pl.ct_off + (pl.KP + 1) * (pl.KP + 1) : -1; a.ct_zero = 0;
   a.G = pl.ws.G; a.grad_part = pl.ws.grad_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   return a;
@@ -900,7 +902,7 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
   a.md = pl.md; a.fg = pl.fg; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
   a.any_unconv = 0;
   for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
-  a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off;
+  a.taps_fwd = pl.taps_fwd; a.taps_adj = pl.taps_adj; a.taps_stride = pl.taps_stride; a.ct_off = pl.ct_off; a.ct_zero = 0;
   a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
   a.G = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
   a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;

@@ -56,6 +56,7 @@ struct FusedArgs {
   const CompConst* cc;
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int ct_off;                // >= 0: both tap sets of the shared PSF at c_tap_pool[ct_off ..] (forward, then adjoint)
+  int ct_zero;               // 0 (see conv_tile_ct)
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                  // [B,H,W]: model_out (mode 0) or back-seed spill (any_unconv)
   float* chi2_part;          // [B]
@@ -129,14 +130,14 @@ __device__ __forceinline__ void conv_rows(const float* __restrict__ gal, int pit
 // outermost, the input row (or the zero row) reloaded for every row pair
 template <int K, int RP, int TC>
 __device__ __forceinline__ void conv_rows_ct(const float* __restrict__ gal, int pitch, int H, int i0, int c0,
-                                             int ct_off, float2 (&acc)[RP][TC]) {
+                                             int ct_off, int ct_zero, float2 (&acc)[RP][TC]) {
   constexpr int NW = ((TC + K - 1) + 3) / 4;
   constexpr int TP = ConvCfg<K>::kTapPitch;
 #pragma unroll 2
   for (int a = 0; a <= K; ++a) {
-    const float2* tp = c_tap_pool + ct_off + a * TP;
 #pragma unroll
     for (int rp = 0; rp < RP; ++rp) {
+      const float2* tp = c_tap_pool + ct_off + a * TP + rp * ct_zero;   // ct_zero = 0: see conv_tile_ct
       const int i = i0 + a + 2 * rp;
       const int r = ((unsigned)i < (unsigned)H) ? i : H;          // outside the cutout: the zero row
       float in[NW * 4];
@@ -239,7 +240,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
 #pragma unroll
             for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
           if (active) {
-            if (CT) conv_rows_ct<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, a.ct_off + phase * TAPN, acc);
+            if (CT) conv_rows_ct<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, a.ct_off + phase * TAPN, a.ct_zero, acc);
             else conv_rows<K, RP, TC>(gal, fg.pitch, fg.H, ty * 2 * RP - h, tx * TC, taps_of(s, g, phase), acc);
           }
           bar_sync(BAR_CONV, kConvThreads);                     // every conv thread is done reading

@@ -51,6 +51,7 @@ struct FwdArgs {
   const CompConst* cc;     // [B, n_comp]
   const float2* taps; long long taps_stride;   // paired flipped taps, float2 per galaxy (0 = shared)
   int ct_off;              // >= 0: the taps of the shared PSF sit at c_tap_pool[ct_off ..] (constant bank)
+  int ct_zero;             // 0 (see conv_tile_ct)
   const float* data; const float* sigma; const uint8_t* mask;
   float* G;                // [B,H,W] workspace (or model_out when RENDER)
   float* chi2_part;        // [B, tiles]
@@ -70,6 +71,7 @@ struct BwdArgs {
   const CompConst* cc;
   const float2* taps; long long taps_stride;   // paired unflipped taps
   int ct_off;              // >= 0: taps at c_tap_pool[ct_off ..]
+  int ct_zero;             // 0 (see conv_tile_ct)
   const float* G;          // [B,H,W]
   float* grad_part;        // [B, tiles, n_comp, kNSum]
   const int* frozen;
@@ -157,15 +159,19 @@ constexpr int kTapPoolN = 7424;                           // float2: 59,392 byte
 __constant__ float2 c_tap_pool[kTapPoolN];
 
 template <int K, int RP, int TC>
-__device__ __forceinline__ void conv_tile_ct(const float* __restrict__ win, int pitch, int ct_off,
+__device__ __forceinline__ void conv_tile_ct(const float* __restrict__ win, int pitch, int ct_off, int ct_zero,
                                              float2 (&acc)[RP][TC]) {
   constexpr int NW = ((TC + K - 1) + 3) / 4;
   constexpr int TP = ConvCfg<K>::kTapPitch;
 #pragma unroll 2
   for (int a = 0; a <= K; ++a) {
-    const float2* tp = c_tap_pool + ct_off + a * TP;
 #pragma unroll
     for (int rp = 0; rp < RP; ++rp) {
+      // ct_zero is 0 at run time.  Without it the compiler keeps the K tap pairs of row a live
+      // across the RP row pairs; beyond K = 33 that exceeds the 63 uniform registers and it
+      // falls back to vector registers and shared-memory-speed code.  An address it cannot
+      // prove equal makes every row pair reload its taps (LDCU is nearly free).
+      const float2* tp = c_tap_pool + ct_off + a * TP + rp * ct_zero;
       float in[NW * 4];
       const float4* row = reinterpret_cast<const float4*>(win + (a + 2 * rp) * pitch);
 #pragma unroll
@@ -330,7 +336,7 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
     for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
   if (active) {
     const float* win = tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC;
-    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, acc);
+    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, a.ct_zero, acc);
     else conv_tile<K, RP, TC>(win, tg.pitch, taps, acc);
   }
 
@@ -524,7 +530,7 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
     for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
   if (active) {
     const float* win = tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC;
-    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, acc);
+    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, a.ct_zero, acc);
     else conv_tile<K, RP, TC>(win, tg.pitch, taps, acc);
   }
 
