@@ -151,6 +151,26 @@ def test_fit_multi_equals_fit_per_batch_bitwise():
             assert np.array_equal(s[key], m[key], equal_nan=True), key
 
 
+def test_constant_tap_pool_exhaustion_falls_back_bitwise():
+    # the paired taps of a shared PSF live in a 59 KB constant-bank pool, 10.8 KB per call in
+    # flight at K = 25: of seven concurrent buckets two find no region and run the shared-memory
+    # taps.  Both forms add the products in the same order, so every bucket must give exactly
+    # what a lone gm_fit gives (which always finds a region), and the pool must recover.
+    b, o = _bucket(2, range(60), 64, 25, 0.0)
+    assert b["psf"].shape[-1] == 25 and len(b["galaxies"]) >= 4
+    single = gpu_fit(b, o)
+    mk = lambda: {"params": dev(b["start"]).clone(), "data": dev(b["data"]), "sigma": dev(b["sigma"]),
+                  "mask": dev(b["mask"]), "psf": dev(b["psf"]), "opts": o}
+    for _ in range(2):                       # second round: regions of the first were handed back
+        outs = gm.gm_fit_multi(b["model"], [mk() for _ in range(7)])
+        torch.cuda.synchronize()
+        for m in outs:
+            for key in ("params", "chi2", "iters_used", "status"):
+                assert np.array_equal(single[key], m[key].cpu().numpy(), equal_nan=True), key
+    again = gpu_fit(b, o)
+    assert np.array_equal(single["params"], again["params"])
+
+
 def test_live_list_after_early_stop_matches_oracle():
     # many more galaxies than stop at the same time: the compacted live list changes every few
     # iterations; per-galaxy results must not depend on it (compare with the oracle, which has none)
