@@ -234,10 +234,11 @@ __device__ __forceinline__ void store_acc(float* dst, int pitch, const float2 (&
   }
 }
 
-// dynamic shared memory: [ tile: rows x pitch floats | taps: (K+1) x (K+1) float2 | red ]
+// dynamic shared memory: [ tile: rows x pitch floats | taps: (K+1) x (K+1) float2 | red ];
+// no tap area when the taps are in the constant bank (ct)
 template <int K>
-__host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int n_red) {
-  return (size_t)tg.rows * tg.pitch * 4 + (size_t)(K + 1) * ConvCfg<K>::kTapPitch * 8 +
+__host__ __device__ inline size_t smem_bytes(const TileGeom& tg, int nwarps, int n_red, bool ct) {
+  return (size_t)tg.rows * tg.pitch * 4 + (ct ? 0 : (size_t)(K + 1) * ConvCfg<K>::kTapPitch * 8) +
          (size_t)nwarps * n_red * 4 + 64;
 }
 
@@ -265,7 +266,7 @@ __global__ void __launch_bounds__(512) k_forward(const FwdArgs a) {
 
   float* tilebuf = reinterpret_cast<float*>(smem_raw);
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
-  float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
+  float* red = reinterpret_cast<float*>(taps + (CT ? 0 : (K + 1) * ConvCfg<K>::kTapPitch));
 
   if (!CT) copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 
@@ -484,7 +485,7 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
 
   float* tilebuf = reinterpret_cast<float*>(smem_raw);
   float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
-  float* red = reinterpret_cast<float*>(taps + (K + 1) * ConvCfg<K>::kTapPitch);
+  float* red = reinterpret_cast<float*>(taps + (CT ? 0 : (K + 1) * ConvCfg<K>::kTapPitch));
 
   if (!CT) copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
 

@@ -25,12 +25,12 @@ static cudaError_t set_smem(Kern kern, size_t bytes) {
 }
 
 // Threads of a tile CTA.  When the tile is so large that only one CTA fits an SM (K = 41 with
-// 128 x 128 tiles) the CTA gets 512 threads: the upper 256 own no output pixels and only
+// 128 x 128 tiles and the taps in shared memory; with the taps in the constant bank two fit) the CTA gets 512 threads: the upper 256 own no output pixels and only
 // help with the render, the tile load and the epilogue, which run with the
 // convolution warps idle and need the extra warps to hide the SFU / memory latency.
 template <int K>
-static int tile_threads(const TileGeom& tg, int nthr) {
-  const size_t one = smem_bytes<K>(tg, 16, kNSum) + 1024;
+static int tile_threads(const TileGeom& tg, int nthr, bool ct) {
+  const size_t one = smem_bytes<K>(tg, 8, kNSum, ct) + 1024;   // + the 1 KB the driver reserves per CTA
   return (2 * one > 233472) ? 512 : nthr;
 }
 
@@ -116,8 +116,8 @@ int GM_CAT(launch_forward_, GM_K)(const FwdArgs& a, int mode, int B, cudaStream_
   constexpr int K = GM_K;
   int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
   if (nthr > 256) return GM_ENOTSUP;
-  nthr = tile_threads<K>(a.tg, nthr);
-  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1);
+  nthr = tile_threads<K>(a.tg, nthr, a.ct_off >= 0);
+  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, 1, a.ct_off >= 0);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
   if (a.ct_off >= 0)
     return a.tg.variant == 1 ? launch_forward_v<K, 3, 12, true>(a, mode, nthr, sm, grid, st, err)
@@ -130,8 +130,8 @@ int GM_CAT(launch_backward_, GM_K)(const BwdArgs& a, int B, cudaStream_t st, cud
   constexpr int K = GM_K;
   int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
   if (nthr > 256) return GM_ENOTSUP;
-  nthr = tile_threads<K>(a.tg, nthr);
-  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum);
+  nthr = tile_threads<K>(a.tg, nthr, a.ct_off >= 0);
+  const size_t sm = smem_bytes<K>(a.tg, nthr / 32, kNSum, a.ct_off >= 0);
   const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
   const bool ct = a.ct_off >= 0;
   if (a.tg.variant == 1 && ct) {
