@@ -244,7 +244,7 @@ __global__ void k_fit_init(int B, int P, const float* __restrict__ params, FitOp
 // a6: one warp per galaxy, lane k = parameter k.  t = 1..n_iter are update steps,
 // t = n_iter + 1 is the closing evaluation (last != 0, no update).
 __global__ void __launch_bounds__(kFinWarps * 32)
-k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* __restrict__ params, int t, int last,
+k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* params, CompConst* cc_next, int t, int last,
            float c1 /*1-b1^t*/, float c2 /*1-b2^t*/, float dec /*decay^(t-1)*/, int* iters, int* status) {
   __shared__ float sh[kFinWarps][GM_MAX_COMP * kNSum];
   const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -304,6 +304,10 @@ k_fit_step(const FinArgs a, const FitOptsDev o, FitState st, float* __restrict__
       params[pk] = o.lg[lane] ? exp10f(u) : u;
     }
   }
+  // a0 of the next evaluation, here instead of in a launch of its own: lane c makes the
+  // constants of component c from the parameters the warp has just written
+  __syncwarp();
+  if (lane < a.md.n_comp) make_comp_const(a.md, lane, params + (size_t)b * P, cc_next + (size_t)b * a.md.n_comp + lane);
 }
 
 // Rebuild the ascending list of galaxies that still iterate (early stop, R:O5, or a
@@ -1151,14 +1155,15 @@ static int fit_iter(FitRun* r, int t) {
   LiveSet ls;
   ls.frozen = r->fs.frozen;
   if (compact) { ls.live = r->fs.live; ls.n_live = r->fs.n_live; }
-  if ((rc = run_prologue(pl, B, r->params, r->fs.frozen, st)) != GM_OK) return rc;
+  // a0: a launch of its own before the first evaluation, then inside k_fit_step
+  if (t == 1 && (rc = run_prologue(pl, B, r->params, r->fs.frozen, st)) != GM_OK) return rc;
   if ((rc = run_eval(pl, r->bt, !last, ls, st)) != GM_OK) return rc;
   const float c1 = (float)(1.0 - std::pow((double)opts->beta1, (double)t));
   const float c2 = (float)(1.0 - std::pow((double)opts->beta2, (double)t));
   const float dec = (float)std::pow((double)opts->lr_decay, (double)(t - 1));
   const int fin_grid = (B + kFinWarps - 1) / kFinWarps;
   k_fit_step<<<fin_grid, kFinWarps * 32, 0, st>>>(fin_args(pl, B, !last, r->chi2_out, nullptr), r->o, r->fs,
-                                                 r->params, t, last, c1, c2, dec, r->iters_used, r->status);
+                                                 r->params, pl.ws.cc, t, last, c1, c2, dec, r->iters_used, r->status);
   ++t_launches;
   GM_CUDA(cudaGetLastError());
   if (compact && !last) {
