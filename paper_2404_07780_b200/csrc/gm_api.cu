@@ -1354,10 +1354,30 @@ extern "C" {
 
 // ---- host-buffer variants ----------------------------------------------------
 namespace {
+// Device buffers of the host-buffer calls come from the device's stream-ordered pool
+// (cudaMallocAsync on the call's stream, cudaFreeAsync on the same stream in the destructor, so
+// a buffer is never released under a kernel that still runs).  The pool keeps up to 8 GB of
+// freed memory for the next call: a plain cudaMalloc / cudaFree pair of the image buffers cost
+// 15-25 ms per call at C1, more than the 134 MB host-to-device copy itself.
+static void keep_pool_memory() {
+  static std::mutex mu;
+  static bool done[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return;
+  std::lock_guard<std::mutex> lk(mu);
+  if (done[dev]) return;
+  cudaMemPool_t pool;
+  if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+    uint64_t keep = 8ull << 30;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+  }
+  done[dev] = true;
+}
 struct DevBuf {
   void* p = nullptr;
-  ~DevBuf() { if (p) cudaFree(p); }
-  cudaError_t alloc(size_t n) { return cudaMalloc(&p, n ? n : 1); }
+  cudaStream_t s = nullptr;
+  ~DevBuf() { if (p) cudaFreeAsync(p, s); }
+  cudaError_t alloc(size_t n, cudaStream_t st) { s = st; return cudaMallocAsync(&p, n ? n : 1, st); }
 };
 struct StreamGuard {
   cudaStream_t s = nullptr;
@@ -1365,8 +1385,8 @@ struct StreamGuard {
 };
 
 struct HostCall {
+  StreamGuard sg;            // first member: destroyed last, after the buffers freed on it
   DevBuf data, sigma, mask, psf, params, ws;
-  StreamGuard sg;
   gm_batch dev;
   size_t ws_bytes = 0;
 };
@@ -1378,34 +1398,35 @@ int stage_in(const gm_model* model, const gm_batch* hb, const float* params, boo
   if (need_data && (!hb->data || !hb->sigma)) return GM_EINVAL;
   hc->ws_bytes = gm_workspace_bytes(model, hb);
   if (hc->ws_bytes == 0) return GM_EINVAL;
+  keep_pool_memory();
   GM_CUDA(cudaStreamCreateWithFlags(&hc->sg.s, cudaStreamNonBlocking));
   cudaStream_t st = hc->sg.s;
   const size_t npx = (size_t)hb->B * hb->H * hb->W;
   const size_t npsf = (hb->psf_stride == 0 ? 1 : (size_t)hb->B) * hb->K * hb->K;
   hc->dev = *hb;
   hc->dev.data = nullptr; hc->dev.sigma = nullptr; hc->dev.mask = nullptr;
-  GM_CUDA(hc->psf.alloc(npsf * 4));
+  GM_CUDA(hc->psf.alloc(npsf * 4, st));
   GM_CUDA(cudaMemcpyAsync(hc->psf.p, hb->psf, npsf * 4, cudaMemcpyHostToDevice, st));
   hc->dev.psf = (const float*)hc->psf.p;
   if (hb->psf_stride != 0) hc->dev.psf_stride = (int64_t)hb->K * hb->K;
   if (hb->psf_stride != 0 && hb->psf_stride != (int64_t)hb->K * hb->K) return GM_EINVAL;
   if (need_data) {
-    GM_CUDA(hc->data.alloc(npx * 4));
-    GM_CUDA(hc->sigma.alloc(npx * 4));
+    GM_CUDA(hc->data.alloc(npx * 4, st));
+    GM_CUDA(hc->sigma.alloc(npx * 4, st));
     GM_CUDA(cudaMemcpyAsync(hc->data.p, hb->data, npx * 4, cudaMemcpyHostToDevice, st));
     GM_CUDA(cudaMemcpyAsync(hc->sigma.p, hb->sigma, npx * 4, cudaMemcpyHostToDevice, st));
     hc->dev.data = (const float*)hc->data.p;
     hc->dev.sigma = (const float*)hc->sigma.p;
     if (hb->mask) {
-      GM_CUDA(hc->mask.alloc(npx));
+      GM_CUDA(hc->mask.alloc(npx, st));
       GM_CUDA(cudaMemcpyAsync(hc->mask.p, hb->mask, npx, cudaMemcpyHostToDevice, st));
       hc->dev.mask = (const uint8_t*)hc->mask.p;
     }
   }
   const size_t npar = (size_t)hb->B * model->n_par * 4;
-  GM_CUDA(hc->params.alloc(npar));
+  GM_CUDA(hc->params.alloc(npar, st));
   GM_CUDA(cudaMemcpyAsync(hc->params.p, params, npar, cudaMemcpyHostToDevice, st));
-  GM_CUDA(hc->ws.alloc(hc->ws_bytes));
+  GM_CUDA(hc->ws.alloc(hc->ws_bytes, st));
   return GM_OK;
 }
 }  // namespace
@@ -1417,7 +1438,7 @@ int gm_render_host(const gm_model* model, const gm_batch* hb, const float* param
   if (rc != GM_OK) return rc;
   const size_t npx = (size_t)hb->B * hb->H * hb->W;
   DevBuf out;
-  GM_CUDA(out.alloc(npx * 4));
+  GM_CUDA(out.alloc(npx * 4, hc.sg.s));
   rc = gm_render(model, &hc.dev, (const float*)hc.params.p, (float*)out.p, hc.ws.p, hc.ws_bytes, hc.sg.s);
   if (rc != GM_OK) return rc;
   const int64_t n = t_launches;
@@ -1434,8 +1455,8 @@ int gm_loss_grad_host(const gm_model* model, const gm_batch* hb, const float* pa
   if (rc != GM_OK) return rc;
   const size_t B = hb->B, P = model->n_par;
   DevBuf dchi2, dgrad;
-  GM_CUDA(dchi2.alloc(B * 4));
-  GM_CUDA(dgrad.alloc(B * P * 4));
+  GM_CUDA(dchi2.alloc(B * 4, hc.sg.s));
+  GM_CUDA(dgrad.alloc(B * P * 4, hc.sg.s));
   rc = gm_loss_grad(model, &hc.dev, (const float*)hc.params.p, (float*)dchi2.p, grad ? (float*)dgrad.p : nullptr,
                     nullptr, nullptr, hc.ws.p, hc.ws_bytes, hc.sg.s);
   if (rc != GM_OK) return rc;
@@ -1453,9 +1474,9 @@ int gm_fit_host(const gm_model* model, const gm_batch* hb, float* params, const 
   if (rc != GM_OK) return rc;
   const size_t B = hb->B, P = model->n_par;
   DevBuf dchi2, dit, dst;
-  GM_CUDA(dchi2.alloc(B * 4));
-  GM_CUDA(dit.alloc(B * 4));
-  GM_CUDA(dst.alloc(B * 4));
+  GM_CUDA(dchi2.alloc(B * 4, hc.sg.s));
+  GM_CUDA(dit.alloc(B * 4, hc.sg.s));
+  GM_CUDA(dst.alloc(B * 4, hc.sg.s));
   rc = gm_fit(model, &hc.dev, (float*)hc.params.p, opts, (float*)dchi2.p, (int32_t*)dit.p, (int32_t*)dst.p,
               hc.ws.p, hc.ws_bytes, hc.sg.s);
   if (rc != GM_OK) return rc;
@@ -1484,9 +1505,9 @@ int gm_fit_multi_host(const gm_model* model, int32_t n_batches, const gm_batch* 
     int rc = stage_in(model, &hbs[i], params[i], true, &hc[i]);
     if (rc != GM_OK) return rc;
     const size_t B = hbs[i].B;
-    GM_CUDA(out[i].chi2.alloc(B * 4));
-    GM_CUDA(out[i].it.alloc(B * 4));
-    GM_CUDA(out[i].st.alloc(B * 4));
+    GM_CUDA(out[i].chi2.alloc(B * 4, hc[i].sg.s));
+    GM_CUDA(out[i].it.alloc(B * 4, hc[i].sg.s));
+    GM_CUDA(out[i].st.alloc(B * 4, hc[i].sg.s));
     dev[i] = hc[i].dev;
     dpar[i] = (float*)hc[i].params.p; dchi2[i] = (float*)out[i].chi2.p;
     dit[i] = (int32_t*)out[i].it.p; dst[i] = (int32_t*)out[i].st.p;
