@@ -117,6 +117,37 @@ def test_shared_and_per_galaxy_psf_agree_bitwise():
     assert torch.equal(a, c)
 
 
+@pytest.mark.parametrize("H,W,K", [(64, 64, 25), (96, 96, 9), (128, 128, 41), (100, 90, 33), (192, 192, 25),
+                                   (256, 256, 41), (140, 200, 15), (37, 45, 7)])
+def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, monkeypatch):
+    # a batch-wide PSF runs the convolution with its taps in the constant bank (FFMA2 with a
+    # uniform-register operand), a per-galaxy PSF or GM_NO_CONST_TAPS with the taps in shared
+    # memory; both add the K^2 products of a pixel in the same order, in k_fused and in the
+    # tile kernels, for every compiled PSF side and both thread tiles
+    model = models.bulge_disk()
+    par, data, sigma, mask, psf = synth(model, 3, H, W, K, seed=7 * H + W + K)
+    def run():
+        img = gm.gm_render(model, dev(par), H, W, dev(psf))
+        out = gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(psf))
+        torch.cuda.synchronize()
+        return [img] + [t for t in out]
+    const = run()
+    monkeypatch.setenv("GM_NO_CONST_TAPS", "1")
+    shared = run()
+    monkeypatch.delenv("GM_NO_CONST_TAPS")
+    rep = np.ascontiguousarray(np.broadcast_to(psf, (3, K, K)))
+    per = [gm.gm_render(model, dev(par), H, W, dev(rep))] + \
+        [t for t in gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(rep))]
+    # the pixels must not move at all; where the taps live may change the kernel that runs
+    # (k_fused slot geometry, tile kernels) and with it the ORDER of the chi^2 / gradient
+    # reductions, so those agree to rounding only
+    for other in (shared, per):
+        assert torch.equal(const[0], other[0])
+        assert_chi2(other[1].cpu().numpy(), const[1].cpu().numpy().astype(np.float64), rtol=2e-6)
+        assert_grad(other[2].cpu().numpy(), const[2].cpu().numpy().astype(np.float64), rtol=1e-5)
+    assert_chi2(const[1].cpu().numpy(), oracle.loss_grad(model, par, data, sigma, mask, psf)[0])
+
+
 # ---- mask / sigma properties on the GPU (reading X1) -------------------------------
 def test_mask_properties():
     model = models.single_sersic()
