@@ -356,9 +356,15 @@ def run_ours(args):
         n_dom = kern[dom]["launches"]
         big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
         traffic = None
-        tf = ROOT / "profiles" / "traffic.json"
+        # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+        # ncu --set full capture summarised in profiles/r01_fused_ncu.md (kernel,bytes per line)
+        tf = ROOT / "profiles" / "r01_traffic.csv"
         if tf.exists() and len(buckets) == 1:
-            traffic = json.loads(tf.read_text()).get(f"{dom}_K{K}_{big['H']}x{big['W']}_B{big['B']}")
+            key = f"{dom}_K{K}_{big['H']}x{big['W']}_B{big['B']}"
+            for line in tf.read_text().splitlines()[1:]:
+                name, _, nbytes = line.partition(",")
+                if name.strip() == key:
+                    traffic = int(nbytes)
         px_bytes = 9 if big["b"]["mask"] is not None else 8
         roofline = {"bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved,
                     "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
