@@ -148,6 +148,31 @@ def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, monkeypatch
     assert_chi2(const[1].cpu().numpy(), oracle.loss_grad(model, par, data, sigma, mask, psf)[0])
 
 
+def test_constant_tap_regions_are_refilled_between_and_across_calls(monkeypatch):
+    # a pool region is reused by the next call with another PSF, and concurrent calls on their own
+    # streams hold different PSFs at the same time: nobody may see somebody else's (or stale) taps
+    model = models.single_sersic()
+    H = W = 64; K = 25
+    par, data, sigma, mask, _ = synth(model, 4, H, W, K, seed=99)
+    psfs = [asymmetric_psf(K, seed=300 + i).astype(np.float32) for i in range(6)]
+    monkeypatch.setenv("GM_NO_CONST_TAPS", "1")
+    want = [gm.gm_render(model, dev(par), H, W, dev(p)).clone() for p in psfs]
+    monkeypatch.delenv("GM_NO_CONST_TAPS")
+    for rnd in range(3):                                   # back to back on one stream
+        for p, w in zip(psfs, want):
+            assert torch.equal(gm.gm_render(model, dev(par), H, W, dev(p)), w)
+    streams = [torch.cuda.Stream() for _ in psfs]          # and all at once
+    torch.cuda.synchronize()
+    outs = []
+    for rnd in range(3):
+        for p, st in zip(psfs, streams):
+            with torch.cuda.stream(st):
+                outs.append(gm.gm_render(model, dev(par), H, W, dev(p)))
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        assert torch.equal(o, want[i % len(psfs)])
+
+
 # ---- mask / sigma properties on the GPU (reading X1) -------------------------------
 def test_mask_properties():
     model = models.single_sersic()
