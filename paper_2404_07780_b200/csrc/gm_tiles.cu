@@ -39,11 +39,12 @@ static int tile_threads(const TileGeom& tg, int nthr, bool ct) {
 // module with its own constant bank).  A region holds the forward + adjoint tap sets of one
 // call; it is filled on the call's stream and handed back by an event recorded on that
 // stream after the call's last launch, so concurrent calls (gm_fit_multi runs one stream per
-// size bucket) never share a region that is still being read.  No region free: the caller
-// runs the shared-memory taps instead.  Nothing here blocks or synchronises.
+// size bucket) never share a region that is still being read; a later call on the SAME stream
+// takes the region over at once.  No region free: the caller runs the shared-memory taps
+// instead.  Nothing here blocks or synchronises.
 // ---------------------------------------------------------------------------
 namespace {
-struct TapRegion { int dev, off, n; cudaEvent_t ev; bool recorded; };
+struct TapRegion { int dev, off, n; cudaEvent_t ev; bool recorded; cudaStream_t st; };
 std::mutex g_pool_mu;
 std::vector<TapRegion> g_pool_used;
 }  // namespace
@@ -54,6 +55,19 @@ int GM_CAT(tap_pool_acquire_, GM_K)(const float2* taps_dev, int n, cudaStream_t 
   int dev = 0;
   GM_TRY(cudaGetDevice(&dev));
   std::lock_guard<std::mutex> lk(g_pool_mu);
+  // A region whose call was enqueued on this very stream can be refilled at once: stream order
+  // puts the copy behind that call's last kernel.  This is what keeps a loop of asynchronous
+  // calls on one stream (or on a few, round robin) in the constant bank however far the host
+  // runs ahead of the device.
+  for (TapRegion& r : g_pool_used) {
+    if (r.dev != dev || !r.recorded || r.st != st || r.n != n) continue;
+    GM_TRY(cudaMemcpyToSymbolAsync(c_tap_pool, taps_dev, (size_t)n * sizeof(float2), (size_t)r.off * sizeof(float2),
+                                   cudaMemcpyDeviceToDevice, st));
+    cudaEventDestroy(r.ev);
+    r.ev = nullptr; r.recorded = false;
+    *off = r.off;
+    return GM_OK;
+  }
   for (size_t i = 0; i < g_pool_used.size();) {           // hand back the regions whose call has finished
     TapRegion& r = g_pool_used[i];
     if (r.recorded && cudaEventQuery(r.ev) == cudaSuccess) {
@@ -74,7 +88,7 @@ int GM_CAT(tap_pool_acquire_, GM_K)(const float2* taps_dev, int n, cudaStream_t 
   if (start + n > kTapPoolN) return GM_OK;
   GM_TRY(cudaMemcpyToSymbolAsync(c_tap_pool, taps_dev, (size_t)n * sizeof(float2), (size_t)start * sizeof(float2),
                                  cudaMemcpyDeviceToDevice, st));
-  g_pool_used.push_back({dev, start, n, nullptr, false});
+  g_pool_used.push_back({dev, start, n, nullptr, false, st});
   *off = start;
   return GM_OK;
 }
@@ -88,6 +102,7 @@ void GM_CAT(tap_pool_release_, GM_K)(int off, cudaStream_t st) {
     if (r.dev != dev || r.off != off || r.recorded) continue;
     if (cudaEventCreateWithFlags(&r.ev, cudaEventDisableTiming) == cudaSuccess && cudaEventRecord(r.ev, st) == cudaSuccess) {
       r.recorded = true;
+      r.st = st;
     } else {                                               // cannot track it: wait once, then free
       cudaStreamSynchronize(st);
       g_pool_used.erase(g_pool_used.begin() + i);
