@@ -251,6 +251,8 @@ def run_ours(args):
         b = configs.make_batch(cfg.cid, gal, render, side=side)
         if not b["galaxies"]:
             continue
+        if args.per_galaxy_psf:                     # the paper's data: one PSF image per galaxy
+            b["psf"] = np.ascontiguousarray(np.broadcast_to(b["psf"], (len(b["galaxies"]),) + b["psf"].shape))
         opts = dict(b["opts"]); opts["n_iter"] = n_iter
         opts["lr_decay"] = 0.01 ** (1.0 / max(n_iter - 1, 1))
         if args.no_early_stop:
@@ -260,7 +262,7 @@ def run_ours(args):
         B, H, W, K = len(b["galaxies"]), b["H"], b["W"], b["K"]
         buckets.append({"b": b, "B": B, "H": H, "W": W, "K": K, "opts": opts, "host": host, "dev": devt,
                         "params": devt[4].clone(),
-                        "ws": torch.empty(gm.gm_workspace_bytes(b["model"], B, H, W, K) + 256,
+                        "ws": torch.empty(gm.gm_workspace_bytes(b["model"], B, H, W, K, args.per_galaxy_psf) + 256,
                                           dtype=torch.uint8, device="cuda")})
     model = buckets[0]["b"]["model"]
     K = buckets[0]["K"]
@@ -439,7 +441,8 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": wl, "global_batch": B * world,
+            "config": {"workload": wl + (", one PSF per galaxy [B,K,K]" if args.per_galaxy_psf else ""),
+                       "global_batch": B * world,
                        "buckets": ("gm_fit_multi, one stream per cutout side" if multi else
                                    "gm_fit per cutout side, one after the other") if len(buckets) > 1 else None,
                        "parallelism": f"dp{world} (independent galaxies, no collective)",
@@ -474,6 +477,8 @@ def main():
     ap.add_argument("--serial-buckets", action="store_true",
                     help="C2: one gm_fit per size bucket, one after the other, instead of gm_fit_multi")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--per-galaxy-psf", action="store_true",
+                    help="pass the PSF as [B,K,K] (taps in shared memory instead of the constant bank)")
     ap.add_argument("--stream-batches", type=int, default=0,
                     help="also stream this many batches through two streams (C4: 65,536 galaxies = 32 x 2048)")
     args = ap.parse_args()

@@ -211,9 +211,9 @@ def gm_profile_read():
     return {"forward": (ms[0], int(n[0])), "backward": (ms[1], int(n[1])), "fused": (ms[2], int(n[2]))}
 
 
-def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) -> int:
+def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int, per_galaxy_psf: bool = False) -> int:
     m = _model_struct(model)
-    b = _Batch(B, H, W, K, None, None, None, None, 0)
+    b = _Batch(B, H, W, K, None, None, None, None, K * K if per_galaxy_psf else 0)
     return int(_lib().gm_workspace_bytes(C.byref(m), C.byref(b)))
 
 
