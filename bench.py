@@ -453,6 +453,28 @@ def run_ours(args):
                             "mean_iters": float(iters.mean()),
                             "median_reduced_chi2": float(np.median(red))},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
+    if len(buckets) == 1 and rank == 0:
+        # BASELINE metric (i) as SURVEY 8(d) words it: B*H*W*reps / t(gm_loss_grad), 3 warm-ups, 20 timed
+        # calls at the start parameters, CUDA events on the launching stream, L2 flushed before each call
+        k = buckets[0]
+        data, sigma, mask, psf, start = k["dev"]
+        chi2 = torch.empty(k["B"], dtype=torch.float32, device="cuda"); grad = torch.empty_like(start)
+        lg = lambda: gm.gm_loss_grad(model, start, data, sigma, mask, psf, chi2=chi2, grad=grad,
+                                     workspace=k["ws"], stream=stream)
+        for _ in range(3):
+            lg()
+        tt = []
+        for _ in range(20):
+            flush.zero_()
+            a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); lg(); z.record(stream)
+            tt.append((a, z))
+        torch.cuda.synchronize()
+        ms = statistics.median(a.elapsed_time(z) for a, z in tt)
+        line["loss_grad"] = {"value": k["B"] * k["H"] * k["W"] / (ms * 1e-3), "unit": UNIT, "ms_per_call": ms,
+                             "calls": 20, "stat": "median",
+                             "frac": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12 / peak_tflops,
+                             "api": "gm_loss_grad (prologue, taps, chi^2 + gradient, finalize: the whole call)"}
     if args.stream_batches > 1 and len(buckets) == 1 and rank == 0:
         line["streamed"] = streamed(buckets[0], model, args.stream_batches)
     if world == 1 and not args.no_cpu:
