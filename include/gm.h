@@ -28,6 +28,16 @@
  *     the legacy default stream), allocate nothing, and never synchronise.  Scratch
  *     comes from the caller: `workspace` (dev, 256-byte aligned) of at least
  *     gm_workspace_bytes(model, batch) bytes.
+ *   - Process-wide state the library keeps (all of it derived, none of it observable in
+ *     results): the nu_n interpolation table, uploaded once per device; a 59 KB
+ *     constant-bank pool per PSF side that holds the paired taps of a batch-wide PSF
+ *     (psf_stride == 0) for the duration of a call -- a region is filled by a
+ *     device-to-device copy on the call's stream and handed back through an event on that
+ *     stream, a later call on the same stream may take it over at once, and when no
+ *     region is free (or the PSF is per galaxy) the taps go through shared memory, bit
+ *     for bit the same result; the environment variable GM_NO_CONST_TAPS forces that
+ *     form.  The *_host entry points take their device buffers from the device's
+ *     stream-ordered memory pool and leave up to 8 GB of it cached for the next call.
  *   - Return value: GM_OK or a negative gm_status; nothing is launched when the
  *     arguments fail validation.  There is no CPU fallback: without a CUDA device
  *     every compute entry point returns GM_ECUDA.
@@ -42,7 +52,7 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   103     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   104     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
