@@ -18,9 +18,13 @@
 //   conv   : C1(a)   | C1(b)   | C2(a)   | C2(b)          | C1(c) ...
 //   helper : P1(b)   | E1(a)   | E1(b)   | E2(a) P1(c)    | E2(b) P1(d) ...
 //
-// so the FP32 pipe never waits for the SFU/ALU work of render, residual and gradient
-// (that work fills the issue slots FFMA2 leaves free).  Hand-off is by named barriers
-// (bar.arrive / bar.sync): full[s] helper -> conv, done[s] conv -> helper.
+// so the FP32 pipe never waits for the memory and SFU latency of render, residual and
+// gradient.  That work is NOT free, though: FFMA2 holds the issue port for both of its
+// cycles, so every helper instruction takes a cycle from the convolution (measured,
+// DESIGN.md section 5) and the helper loops are written to issue as little as possible.
+// Hand-off is by named barriers (bar.arrive / bar.sync): full[s] helper -> conv,
+// done[s] conv -> helper.  The taps of a batch-wide PSF are read from the constant bank
+// through uniform registers (CT, conv_rows_ct); per-galaxy taps from shared memory.
 //
 // Slot layout.  Outside the cutout both convolution inputs are zero (R:C1, R:C2), so a
 // cutout is stored as its H rows of `pitch` floats ([h zeros | W pixels | zeros]) plus ONE
@@ -279,11 +283,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_fused(const FusedArgs a) {
   // The helper loops walk a cutout in groups of four consecutive pixels of a row, one group
   // per lane: group idx -> (row, first column).  The warps of a cutout interleave by 32 groups.
   const int W4 = (fg.W + 3) >> 2;
-#ifdef GM_EXP_NOHELP
-  const int ngrp = 0;
-#else
   const int ngrp = fg.H * W4;
-#endif
   const float inv_w4 = 1.0f / (float)W4;
   const int gstart = lw * 32 + lane, gstep = hpg * 32;
   auto group_row = [&](int idx) -> int { return (int)(((float)idx + 0.5f) * inv_w4); };   // exact: idx < 2^16

@@ -2,19 +2,22 @@
 // SURVEY.md section 8(a)), templated on the PSF side K.
 //
 // One CTA owns a TH x TW tile of one galaxy's cutout.  Each thread owns an
-// 8 x 8 block of output pixels and runs the direct PSF convolution as packed
-// FP32 FMAs (FFMA2 on sm_100a): an accumulator pair holds two vertically adjacent
-// output pixels, the multiplicand pair holds two vertically adjacent PSF taps,
-// and the input sample is the scalar-broadcast operand, so one instruction does
-// two of the 2 K^2 multiply-adds per pixel and half of the issue slots stay free
-// for the shared-memory loads that feed it.
+// 8 x 8 or 6 x 12 block of output pixels (RP row pairs x TC columns) and runs the direct
+// PSF convolution as packed FP32 FMAs (FFMA2 on sm_100a): an accumulator pair holds two
+// vertically adjacent output pixels, the multiplicand pair holds two vertically adjacent
+// PSF taps, and the input sample is the scalar-broadcast operand, so one instruction
+// does two of the 2 K^2 multiply-adds per pixel.  FFMA2 holds the issue port for both of
+// its cycles, so every other instruction of the loop is overhead;
+// with a batch-wide PSF the tap pair is a uniform-register operand filled from the
+// constant bank (CT), which removes the tap loads from the loop.
 //
-//   k_forward<K, RENDER>  a1 render S on tile + halo (shared memory)
+//   k_forward<K, MODE, RP, TC, CT>  a1 render S on tile + halo (shared memory)
 //                         a2 M = PSF (*) S          (R:C1, flipped-tap correlation)
 //                         a3 rho, chi2 partial, G = -2 w rho -> workspace
-//                         (RENDER: write M instead; gm_render)
-//   k_backward<K>         a4 A = PSF (star) G        (R:C2) from the G tile + halo
-//                         a5 per-tile partial sums of A dS/dp (8 per component)
+//                         (FWD_RENDER: write M instead, gm_render; FWD_DERIV: one
+//                         column of the Jacobian, gm_uncertainty)
+//   k_backward<K, RP, TC, CT>       a4 A = PSF (star) G   (R:C2) from the G tile + halo
+//                         a5 per-tile partial sums of A dS/dp (kNSum per component)
 //
 // Reductions are fixed-order (thread -> warp shuffle tree -> warps in order ->
 // tiles in order in k_finalize); no floating-point atomics anywhere.
