@@ -25,19 +25,23 @@
  *   - All images are row-major, [B,H,W] contiguous, float32; row 0 is the TOP row
  *     (largest y).  Angles are radians, lengths pixels, amplitudes intensities.
  *   - Device entry points are asynchronous on `cuda_stream` (a cudaStream_t; NULL =
- *     the legacy default stream), allocate nothing, and never synchronise.  Scratch
- *     comes from the caller: `workspace` (dev, 256-byte aligned) of at least
- *     gm_workspace_bytes(model, batch) bytes.
+ *     the legacy default stream), allocate nothing, and never synchronise, from the first
+ *     call on.  Scratch comes from the caller: `workspace` (dev, 256-byte aligned) of at
+ *     least gm_workspace_bytes(model, batch) bytes.
  *   - Process-wide state the library keeps (all of it derived, none of it observable in
- *     results): the nu_n interpolation table, uploaded once per device; a 59 KB
- *     constant-bank pool per PSF side that holds the paired taps of a batch-wide PSF
- *     (psf_stride == 0) for the duration of a call -- a region is filled by a
- *     device-to-device copy on the call's stream and handed back through an event on that
- *     stream, a later call on the same stream may take it over at once, and when no
+ *     results): the nu_n interpolation table, filled once per device by a kernel on the
+ *     stream of gm_init or of the first compute call (calls on other streams are made to
+ *     wait for that kernel through an event until it has completed; call gm_init before
+ *     capturing a CUDA graph); a 59 KB constant-bank pool per PSF side that holds the
+ *     paired taps of a batch-wide PSF (psf_stride == 0) for the duration of a call -- a
+ *     region is filled by a device-to-device copy on the call's stream and handed back
+ *     through an event on that stream, a later call on the same stream (same
+ *     cudaStreamGetId, not merely the same handle) may take it over at once, and when no
  *     region is free (or the PSF is per galaxy) the taps go through shared memory, bit
- *     for bit the same result; the environment variable GM_NO_CONST_TAPS forces that
- *     form.  The *_host entry points take their device buffers from the device's
- *     stream-ordered memory pool and leave up to 8 GB of it cached for the next call.
+ *     for bit the same result; gm_set_option(GM_OPT_CONST_TAPS, 0) forces that form.  The
+ *     library reads no environment variable.  The *_host entry points take their device
+ *     buffers from the device's stream-ordered memory pool and leave up to 8 GB of it
+ *     cached for the next call.
  *   - Return value: GM_OK or a negative gm_status; nothing is launched when the
  *     arguments fail validation.  There is no CPU fallback: without a CUDA device
  *     every compute entry point returns GM_ECUDA.
@@ -52,7 +56,7 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   104     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   200     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
@@ -151,8 +155,22 @@ enum { GM_FIT_OK = 0, GM_FIT_CONVERGED = 1, GM_FIT_NONFINITE = 2 };
 
 /* ---- device entry points (asynchronous) ---------------------------------- */
 
+/* Optional: build the per-device tables on `cuda_stream` now instead of inside the first
+ * compute call (asynchronous; idempotent).  Needed only before CUDA graph capture. */
+int gm_init(void* cuda_stream);
+
+/* Process-wide switches, for tests and measurements (value 0 / 1, default 1 each):
+ *   GM_OPT_FUSED       cutouts up to 128 x 128 take the single fused kernel; 0: tile kernels
+ *   GM_OPT_CONST_TAPS  a batch-wide PSF is read from the constant bank; 0: shared memory
+ * Every setting gives bit for bit the same results.  gm_set_option returns GM_EINVAL for an
+ * unknown option, gm_get_option -1. */
+enum { GM_OPT_FUSED = 0, GM_OPT_CONST_TAPS = 1, GM_OPT_COUNT_ = 2 };
+int gm_set_option(int option, int value);
+int gm_get_option(int option);
+
 /* Bytes of device scratch gm_render / gm_loss_grad / gm_fit need for this model
- * and batch shape (only B, H, W, K and the model are read).  0 on invalid input. */
+ * and batch shape (B, H, W, K, psf_stride -- one PSF or B of them -- and the model are
+ * read; the pointers are not).  0 on invalid input. */
 size_t gm_workspace_bytes(const gm_model* model, const gm_batch* batch);
 
 /* Render the model image M (App. C "initial_model").
@@ -172,8 +190,11 @@ int gm_loss_grad(const gm_model* model, const gm_batch* batch, const float* para
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Fixed-iteration batched fit.  params: dev [B,P], in/out.
- * chi2_out: dev [B], chi^2 AT the returned parameters.  iters_used: dev [B] number
- * of updates applied, or NULL.  status: dev [B] GM_FIT_*, or NULL.
+ * chi2_out: dev [B], chi^2 AT the returned parameters.  iters_used: dev [B], the number of
+ * the last iteration whose chi^2 was finite and acted upon (= updates applied for
+ * GM_FIT_OK and GM_FIT_CONVERGED; for GM_FIT_NONFINITE at iteration t it is t - 1 while
+ * the returned parameters are those that entered iteration t - 1, i.e. carry t - 2
+ * updates), or NULL.  status: dev [B] GM_FIT_*, or NULL.
  * A galaxy whose chi^2 turns non-finite gets GM_FIT_NONFINITE and keeps the last
  * parameters that had a finite chi^2. */
 int gm_fit(const gm_model* model, const gm_batch* batch, float* params,
@@ -291,6 +312,13 @@ int64_t     gm_last_launch_count(void);
  * disabling also clears it. */
 int gm_profile_enable(int on);
 int gm_profile_read(double* ms /* host [3] */, int64_t* count /* host [3] */);
+
+/* The FP32 peak the roofline is quoted against, MEASURED: a kernel of nothing but
+ * independent packed FP32 multiply-adds (fma.rn.f32x2, the instruction of the convolution
+ * loops), one 256-thread CTA x 4 per SM, timed with CUDA events on `cuda_stream` over
+ * `repeats` launches after one warm-up launch.  Synchronous (waits for its own events).
+ * tflops: host, 2 flop per multiply-add. */
+int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream);
 
 #ifdef __cplusplus
 }

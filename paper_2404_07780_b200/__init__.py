@@ -5,7 +5,13 @@ argument marshalling only -- every step of the path runs in the CUDA kernels
 under ``csrc/``.  PyTorch supplies device memory and streams.
 """
 from .binding import (  # noqa: F401
+    GM_OPT_CONST_TAPS,
+    GM_OPT_FUSED,
     GmError,
+    gm_get_option,
+    gm_init,
+    gm_measure_fp32_peak,
+    gm_set_option,
     gm_bootstrap,
     gm_bootstrap_counts,
     gm_fit,

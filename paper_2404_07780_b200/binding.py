@@ -20,6 +20,7 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libgm.so"
 
 GM_MAX_COMP, GM_MAX_PAR, GM_MAX_K, GM_NSLOT = 8, 32, 41, 10
+GM_OPT_FUSED, GM_OPT_CONST_TAPS = 0, 1
 _KINDS = {"sersic": 0, "expdisk": 1, "ferrer": 2, "king": 3, "gaussian": 4, "moffat": 5, "sky": 6}
 _SLOTS = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box", "m0")
 
@@ -99,6 +100,11 @@ def _lib():
         L.gm_last_cuda_error.restype = i; L.gm_last_cuda_error.argtypes = []
         L.gm_last_cuda_error_string.restype = C.c_char_p; L.gm_last_cuda_error_string.argtypes = []
         L.gm_last_launch_count.restype = C.c_int64; L.gm_last_launch_count.argtypes = []
+        L.gm_init.restype = i; L.gm_init.argtypes = [vp]
+        L.gm_set_option.restype = i; L.gm_set_option.argtypes = [i, i]
+        L.gm_get_option.restype = i; L.gm_get_option.argtypes = [i]
+        L.gm_measure_fp32_peak.restype = i
+        L.gm_measure_fp32_peak.argtypes = [i, C.POINTER(C.c_double), vp]
         L.gm_profile_enable.restype = i; L.gm_profile_enable.argtypes = [i]
         L.gm_profile_read.restype = i
         L.gm_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -142,11 +148,34 @@ def _batch_struct(B, H, W, psf, data=None, sigma=None, mask=None, host=False):
     if psf.ndim == 2:
         stride = 0
     else:
-        if psf.shape[0] != B:
+        if psf.ndim != 3 or psf.shape[0] != B:
             raise ValueError("per-galaxy psf must be [B,K,K]")
         stride = K * K
+    if psf.shape[-2] != K:
+        raise ValueError("psf must be square")
+    for name, t in (("data", data), ("sigma", sigma), ("mask", mask)):
+        if t is not None and tuple(t.shape) != (B, H, W):
+            raise ValueError(f"{name} must have shape [B,H,W] = {(B, H, W)}, got {tuple(t.shape)}")
+    devs = {t.device for t in (psf, data, sigma, mask) if isinstance(t, torch.Tensor)}
+    if len(devs) > 1:
+        raise ValueError(f"all tensors of a batch must live on one device, got {sorted(map(str, devs))}")
     return _Batch(B, H, W, K, _dev(data, torch.float32, "data"), _dev(sigma, torch.float32, "sigma"),
                   _dev(mask, torch.uint8, "mask"), _dev(psf, torch.float32, "psf"), stride)
+
+
+def _on_stream(fn):
+    """Run the entry point with `stream` as torch's current stream, so that the tensors it
+    allocates (results, a temporary workspace) belong to the stream the kernels run on."""
+    import functools
+
+    @functools.wraps(fn)
+    def wrapper(*args, **kw):
+        stream = kw.get("stream")
+        if stream is None:
+            return fn(*args, **kw)
+        with torch.cuda.stream(stream):
+            return fn(*args, **kw)
+    return wrapper
 
 
 def _stream_ptr(stream):
@@ -200,6 +229,26 @@ def gm_last_launch_count() -> int:
     return int(_lib().gm_last_launch_count())
 
 
+def gm_init(stream=None) -> None:
+    """Build the per-device tables now (asynchronous on the stream); optional."""
+    _check(_lib().gm_init(_stream_ptr(stream)), "gm_init")
+
+
+def gm_set_option(option: int, value: int) -> None:
+    _check(_lib().gm_set_option(int(option), int(value)), "gm_set_option")
+
+
+def gm_get_option(option: int) -> int:
+    return int(_lib().gm_get_option(int(option)))
+
+
+def gm_measure_fp32_peak(repeats: int = 20, stream=None) -> float:
+    """Measured FP32 peak in TFLOP/s (a pure fma.rn.f32x2 kernel, CUDA events)."""
+    v = C.c_double()
+    _check(_lib().gm_measure_fp32_peak(int(repeats), C.byref(v), _stream_ptr(stream)), "gm_measure_fp32_peak")
+    return float(v.value)
+
+
 def gm_profile_enable(on: bool) -> None:
     _check(_lib().gm_profile_enable(1 if on else 0), "gm_profile_enable")
 
@@ -217,6 +266,7 @@ def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int, per_galaxy_p
     return int(_lib().gm_workspace_bytes(C.byref(m), C.byref(b)))
 
 
+@_on_stream
 def gm_render(model, params, H, W, psf, out=None, workspace=None, stream=None):
     """M[B,H,W] for params[B,P].  Asynchronous on the stream."""
     B = params.shape[0]
@@ -232,6 +282,7 @@ def gm_render(model, params, H, W, psf, out=None, workspace=None, stream=None):
     return out
 
 
+@_on_stream
 def gm_loss_grad(model, params, data, sigma, mask, psf, want_grad=True, chi2=None, grad=None,
                  workspace=None, stream=None, want_jtj=False):
     """chi^2[B] (Eq. 18) and d chi^2 / d p [B,P].  Asynchronous on the stream.
@@ -265,6 +316,7 @@ def gm_uncertainty_workspace_bytes(model: dict, B: int, H: int, W: int, K: int) 
     return int(_lib().gm_uncertainty_workspace_bytes(C.byref(m), C.byref(b)))
 
 
+@_on_stream
 def gm_uncertainty(model, params, sigma, mask, psf, free_mask=None, want_jtj=False, workspace=None,
                    stream=None):
     """sigma_p[B,P] = sqrt(diag[(J^T W J)^-1]) at params (Sec. 5.2).  Asynchronous.
@@ -292,6 +344,7 @@ def gm_uncertainty(model, params, sigma, mask, psf, free_mask=None, want_jtj=Fal
     return out
 
 
+@_on_stream
 def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=None):
     """Batched fixed-iteration fit; params[B,P] is updated IN PLACE.  Asynchronous."""
     B, P = params.shape
@@ -309,6 +362,7 @@ def gm_fit(model, params, data, sigma, mask, psf, opts, workspace=None, stream=N
     return {"params": params, "chi2": chi2, "iters_used": iters, "status": status, "_ws": ws}
 
 
+@_on_stream
 def gm_bootstrap_counts(B, H, W, mask, seed, r, id_offset=0, stream=None):
     """int32 multiplicities [B,H,W] of bootstrap resample r (reading B1).  Asynchronous."""
     dev = mask.device if mask is not None else torch.device("cuda")
@@ -324,6 +378,7 @@ def gm_bootstrap_counts(B, H, W, mask, seed, r, id_offset=0, stream=None):
     return counts
 
 
+@_on_stream
 def gm_bootstrap(model, params, data, sigma, mask, psf, opts, n_resample, seed, id_offset=0,
                  want_samples=False, workspace=None, stream=None):
     """Bootstrap uncertainties (Sec. 5.2): n_resample refits from params[B,P] (not

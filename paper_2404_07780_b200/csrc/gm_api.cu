@@ -3,6 +3,7 @@
 // (a0), gradient assembly and Adam update (a5 tail, a6), and the host-buffer
 // end-to-end variants.  No CPU fallback: every compute entry point needs a CUDA
 // device and returns GM_ECUDA without one.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -33,7 +34,7 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 // the launching stream (gm_profile_enable / gm_profile_read); off by default
 struct Profiler {
   static constexpr int kCap = 8192;
-  bool on = false;
+  std::atomic<bool> on{false};       // read without the lock on every heavy launch
   int n = 0;
   cudaEvent_t ev[kCap][2] = {};
   uint8_t kind[kCap] = {};
@@ -43,9 +44,9 @@ struct Profiler {
 static Profiler g_prof;
 
 static int prof_begin(int kind, cudaStream_t st) {
-  if (!g_prof.on) return -1;
+  if (!g_prof.on.load(std::memory_order_relaxed)) return -1;
   std::lock_guard<std::mutex> lk(g_prof.mu);
-  if (g_prof.n >= Profiler::kCap) return -1;
+  if (!g_prof.on.load(std::memory_order_relaxed) || g_prof.n >= Profiler::kCap) return -1;
   const int i = g_prof.n;
   if (i >= g_prof.created) {
     if (cudaEventCreate(&g_prof.ev[i][0]) != cudaSuccess || cudaEventCreate(&g_prof.ev[i][1]) != cudaSuccess)
@@ -58,36 +59,57 @@ static int prof_begin(int kind, cudaStream_t st) {
   return i;
 }
 static void prof_end(int i, cudaStream_t st) {
-  if (i >= 0) cudaEventRecord(g_prof.ev[i][1], st);
+  if (i < 0) return;
+  std::lock_guard<std::mutex> lk(g_prof.mu);
+  cudaEventRecord(g_prof.ev[i][1], st);
 }
 
+// run-time options (gm_set_option): process-wide, read once per call
+static std::atomic<int> g_opt[GM_OPT_COUNT_] = {{1}, {1}};
+
 // ---------------------------------------------------------------------------
-// nu_n table (gm_device.cuh): built once per process on the host with the exact
-// fp64 solver, uploaded once per device into the g_nu_table symbol.
+// nu_n table (gm_prologue.cuh): filled once per device BY A KERNEL on the stream of the
+// first call (or of gm_init), with the exact fp64 solver; nothing is copied from the host
+// and nothing blocks.  Until the event recorded behind that kernel has completed, calls
+// on other streams are made to wait for it (cudaStreamWaitEvent, also asynchronous).
 // ---------------------------------------------------------------------------
+__global__ void k_nu_table() {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > kNuTableN) return;
+  const double h = (kNuTableS1 - kNuTableS0) / kNuTableN;
+  const double n = exp(kNuTableS0 + h * i);
+  double nu, dnu;
+  sersic_nu_exact(n, &nu, &dnu);
+  g_nu_table[i] = make_double2(nu, dnu * n);             // (nu, d nu / d ln n)
+}
+
 static int ensure_nu_table(cudaStream_t st) {
+  struct State { int phase = 0; cudaEvent_t ev = nullptr; unsigned long long sid = 0; };   // 0 none, 1 in flight, 2 done
   static std::mutex mu;
-  static std::vector<double2> host_table;
-  static bool uploaded[64] = {};
+  static State state[64];
   int dev = 0;
   GM_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= 64) return GM_ENOTSUP;
   std::lock_guard<std::mutex> lk(mu);
-  if (uploaded[dev]) return GM_OK;
-  if (host_table.empty()) {
-    host_table.resize(kNuTableN + 1);
-    const double h = (kNuTableS1 - kNuTableS0) / kNuTableN;
-    for (int i = 0; i <= kNuTableN; ++i) {
-      const double n = std::exp(kNuTableS0 + h * i);
-      double nu, dnu;
-      sersic_nu_exact(n, &nu, &dnu);
-      host_table[i] = make_double2(nu, dnu * n);         // (nu, d nu / d ln n)
-    }
+  State& s = state[dev];
+  if (s.phase == 2) return GM_OK;
+  unsigned long long sid = 0;
+  GM_CUDA(cudaStreamGetId(st, &sid));
+  if (s.phase == 0) {
+    k_nu_table<<<(kNuTableN + 1 + 127) / 128, 128, 0, st>>>();
+    GM_CUDA(cudaGetLastError());
+    ++t_launches;
+    GM_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+    GM_CUDA(cudaEventRecord(s.ev, st));
+    s.sid = sid;
+    s.phase = 1;
+    return GM_OK;
   }
-  // synchronous copy: later launches on any stream see the table
-  (void)st;
-  GM_CUDA(cudaMemcpyToSymbol(g_nu_table, host_table.data(), sizeof(double2) * (kNuTableN + 1)));
-  uploaded[dev] = true;
+  const cudaError_t q = cudaEventQuery(s.ev);
+  if (q == cudaSuccess) { s.phase = 2; return GM_OK; }
+  if (q != cudaErrorNotReady) { t_last_err = q; return GM_ECUDA; }
+  (void)cudaGetLastError();
+  if (sid != s.sid) GM_CUDA(cudaStreamWaitEvent(st, s.ev, 0));
   return GM_OK;
 }
 
@@ -96,10 +118,10 @@ static int ensure_nu_table(cudaStream_t st) {
 // ---------------------------------------------------------------------------
 __global__ void k_pad_psf(const float* __restrict__ psf, long long stride, int n_psf, int K, int KP,
                           float* __restrict__ out) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int per = KP * KP;
-  if (idx >= n_psf * per) return;
-  const int p = idx / per, r = idx - p * per;
+  if (idx >= (long long)n_psf * per) return;
+  const int p = (int)(idx / per), r = (int)(idx - (long long)p * per);
   const int a = r / KP, b = r - a * KP;
   const int off = (KP - K) / 2;
   const int aa = a - off, bb = b - off;
@@ -114,10 +136,10 @@ __global__ void k_make_taps(const float* __restrict__ psf, long long stride, int
                             float2* __restrict__ out) {
   const int TP = KP + 1;
   const int per = (KP + 1) * TP;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= n_psf * 2 * per) return;
-  const int p = idx / (2 * per);
-  const int r = idx - p * 2 * per;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)n_psf * 2 * per) return;
+  const int p = (int)(idx / (2 * per));
+  const int r = (int)(idx - (long long)p * 2 * per);
   const int which = r / per, e = r - which * per;
   const int row = e / TP, t = e - row * TP;
   const float* src = psf + (long long)p * stride;
@@ -501,6 +523,29 @@ k_covar(int B, int P, const FreeSet fs, const double* __restrict__ jtj, float* _
 }
 
 // ---------------------------------------------------------------------------
+// measured FP32 peak (gm_measure_fp32_peak): kPeakAcc independent accumulator pairs per
+// thread, every one updated by one fma.rn.f32x2 per loop trip; the multiplicand pair is
+// shared by a run of accumulators, as the tap pair is in the convolution loops.
+// ---------------------------------------------------------------------------
+constexpr int kPeakAcc = 32;
+__global__ void __launch_bounds__(256) k_ffma2_peak(int iters, float seed, float* __restrict__ sink) {
+  float2 acc[kPeakAcc];
+#pragma unroll
+  for (int i = 0; i < kPeakAcc; ++i) acc[i] = make_float2(seed * (float)i, seed * (float)(threadIdx.x & 7));
+  const float2 w = make_float2(0.999e-3f * seed, -1.001e-3f * seed);
+  const float x = 1.0f - 1e-7f * (float)(threadIdx.x & 3);
+#pragma unroll 4
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < kPeakAcc; ++i) acc[i] = __ffma2_rn(make_float2(x, x), w, acc[i]);
+  }
+  float t = 0.0f;
+#pragma unroll
+  for (int i = 0; i < kPeakAcc; ++i) t += acc[i].x + acc[i].y;
+  if (t == 123.456f) sink[threadIdx.x] = t;                // never true: keeps the loop alive
+}
+
+// ---------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------
 static const int kCompiledK[] = {5, 9, 15, 21, 25, 33, 41};
@@ -815,15 +860,19 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   pl->ws = carve(workspace, pl->md, bt, pl->KP, pl->tg);
   if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < pl->ws.total) return GM_EWORKSPACE;
   if ((rc = device_caps(&pl->caps)) != GM_OK) return rc;
-  pl->fused = bt->H <= 128 && bt->W <= 128 && !getenv("GM_NO_FUSED") &&
+  pl->fused = bt->H <= 128 && bt->W <= 128 && g_opt[GM_OPT_FUSED].load() != 0 &&
               make_fused_geom(bt->H, bt->W, pl->KP, bt->psf_stride == 0, pl->caps.smem_optin, &pl->fg,
                               &pl->fused_variant);
+  // k_fused writes one chi^2 / gradient partial per galaxy: the finalize kernels read them with
+  // the tile count of the tile geometry, so that must be one as well (it is for every H, W <= 128
+  // today; checked here so that a change of make_geom cannot silently break the sums)
+  if (pl->fused && pl->tiles != 1) pl->fused = false;
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
   if (pl->KP != bt->K) {
     const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
-    const int n = n_psf * pl->KP * pl->KP;
-    k_pad_psf<<<(n + 255) / 256, 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, pl->KP, pl->ws.psf_pad);
+    const long long n = (long long)n_psf * pl->KP * pl->KP;
+    k_pad_psf<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, pl->KP, pl->ws.psf_pad);
     ++t_launches;
     GM_CUDA(cudaGetLastError());
     pl->psf = pl->ws.psf_pad;
@@ -839,7 +888,7 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
     pl->taps_fwd = pl->ws.taps;
     pl->taps_adj = pl->ws.taps + per;
     pl->taps_stride = bt->psf_stride == 0 ? 0 : 2ll * per;
-    if (bt->psf_stride == 0 && !getenv("GM_NO_CONST_TAPS")) {
+    if (bt->psf_stride == 0 && g_opt[GM_OPT_CONST_TAPS].load() != 0) {
       if ((rc = tap_pool_acquire(pl->KP, pl->ws.taps, 2 * per, st, &pl->ct_off)) != GM_OK) return rc;
       pl->ct_stream = st;
     }
@@ -1561,6 +1610,52 @@ int gm_profile_read(double* ms, int64_t* count) {
     count[g_prof.kind[i]] += 1;
   }
   g_prof.n = 0;
+  return GM_OK;
+}
+
+int gm_init(void* cuda_stream) {
+  t_launches = 0;
+  return ensure_nu_table((cudaStream_t)cuda_stream);
+}
+
+int gm_set_option(int option, int value) {
+  if (option < 0 || option >= GM_OPT_COUNT_) return GM_EINVAL;
+  g_opt[option].store(value != 0);
+  return GM_OK;
+}
+
+int gm_get_option(int option) {
+  if (option < 0 || option >= GM_OPT_COUNT_) return -1;
+  return g_opt[option].load();
+}
+
+int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream) {
+  t_launches = 0;
+  if (!tflops || repeats < 1 || repeats > 1000) return GM_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DevCaps caps;
+  int rc = device_caps(&caps);
+  if (rc != GM_OK) return rc;
+  float* sink = nullptr;
+  GM_CUDA(cudaMallocAsync(&sink, 256 * sizeof(float), st));
+  cudaEvent_t e0, e1;
+  GM_CUDA(cudaEventCreate(&e0));
+  GM_CUDA(cudaEventCreate(&e1));
+  const int grid = caps.n_sm * 4, iters = 2048;
+  k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);        // warm-up
+  GM_CUDA(cudaEventRecord(e0, st));
+  for (int r = 0; r < repeats; ++r) k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);
+  GM_CUDA(cudaEventRecord(e1, st));
+  GM_CUDA(cudaGetLastError());
+  t_launches = repeats + 1;
+  GM_CUDA(cudaEventSynchronize(e1));
+  float ms = 0.0f;
+  GM_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  GM_CUDA(cudaFreeAsync(sink, st));
+  // per thread and loop trip: kPeakAcc FFMA2 = 2 * kPeakAcc multiply-adds = 4 * kPeakAcc flop
+  const double flop = (double)repeats * grid * 256.0 * iters * kPeakAcc * 4.0;
+  *tflops = flop / ((double)ms * 1e-3) / 1e12;
   return GM_OK;
 }
 

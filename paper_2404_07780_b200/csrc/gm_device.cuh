@@ -43,9 +43,13 @@ struct __align__(16) CompConst {
 // ---------------------------------------------------------------------------
 struct Geo { float u, vq, r; };
 
-// SFU forms.  FAST = MUFU.LG2 / MUFU.EX2 approximations (~2^-22 error): used by the
-// gradient pass (tolerance 1e-3 of the gradient norm).  !FAST = log2f / exp2f of the
-// CUDA math library (<= 2 ulp): used wherever a pixel value of M is produced.
+// SFU forms.  FAST = MUFU.LG2 / MUFU.EX2 approximations (absolute error 2^-22 in the logarithm,
+// 2 ulp in the exponential): used by the gradient pass and, with kFastForward (the default,
+// gm_kernels.cuh), by every pass that produces a pixel of M as well -- gm_render included.
+// Accuracy contract of a rendered pixel: relative error below 1e-5 wherever the profile has
+// not underflowed (nu t < 30), derived in DESIGN.md section 6 and checked by
+// test_render_accuracy_high_n_wings.  !FAST = log2f / exp2f of the CUDA math library
+// (<= 2 ulp), selected for all pixel values by -DGM_PRECISE_FORWARD.
 template <bool FAST> __device__ __forceinline__ float lg2(float x) {
   if (FAST) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
   return log2f(x);

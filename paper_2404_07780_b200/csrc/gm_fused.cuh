@@ -89,7 +89,7 @@ __host__ __device__ inline size_t fused_smem_bytes(int KP, const FusedGeom& fg) 
 }
 
 // (2 RP) x TC outputs per thread, accumulator pairs = vertically adjacent pixels (see
-// conv8x8 in gm_kernels.cuh for the FFMA2 scheme).  `gal` is the cutout's slot, i0 the
+// conv_tile in gm_kernels.cuh for the FFMA2 scheme).  `gal` is the cutout's slot, i0 the
 // image row of the thread's first input row (may be negative), c0 its first slot column.
 template <int K, int RP, int TC>
 __device__ __forceinline__ void conv_rows(const float* __restrict__ gal, int pitch, int H, int i0, int c0,

@@ -3,6 +3,7 @@
 #include "gm_fused.cuh"
 
 #include <mutex>
+#include <utility>
 #include <vector>
 
 #ifndef GM_K
@@ -19,10 +20,25 @@ namespace gm {
     if (e__ != cudaSuccess) { *err = e__; return GM_ECUDA; } \
   } while (0)
 
-template <typename Kern>
-static cudaError_t set_smem(Kern kern, size_t bytes) {
-  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+// cudaFuncAttributeMaxDynamicSharedMemorySize is raised once per (kernel, device), to the
+// device's opt-in maximum, not on every launch
+static cudaError_t set_smem_once(const void* kern) {
+  static std::mutex mu;
+  static std::vector<std::pair<const void*, int>> done;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lk(mu);
+  for (const auto& d : done)
+    if (d.first == kern && d.second == dev) return cudaSuccess;
+  int optin = 0;
+  if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess) return e;
+  done.emplace_back(kern, dev);
+  return cudaSuccess;
 }
+template <typename Kern>
+static cudaError_t set_smem(Kern kern, size_t /*bytes*/) { return set_smem_once((const void*)kern); }
 
 // Threads of a tile CTA.  When the tile is so large that only one CTA fits an SM (K = 41 with
 // 128 x 128 tiles and the taps in shared memory; with the taps in the constant bank two fit) the CTA gets 512 threads: the upper 256 own no output pixels and only
@@ -40,11 +56,14 @@ static int tile_threads(const TileGeom& tg, int nthr, bool ct) {
 // call; it is filled on the call's stream and handed back by an event recorded on that
 // stream after the call's last launch, so concurrent calls (gm_fit_multi runs one stream per
 // size bucket) never share a region that is still being read; a later call on the SAME stream
-// takes the region over at once.  No region free: the caller runs the shared-memory taps
-// instead.  Nothing here blocks or synchronises.
+// takes the region over at once.  "Same stream" is decided by cudaStreamGetId, never by the
+// handle: equal handles do not imply stream order (cudaStreamPerThread is a different stream
+// in every host thread, and a destroyed stream's handle can be handed out again), equal ids
+// do.  No region free: the caller runs the shared-memory taps instead.  Nothing here blocks
+// or synchronises.
 // ---------------------------------------------------------------------------
 namespace {
-struct TapRegion { int dev, off, n; cudaEvent_t ev; bool recorded; cudaStream_t st; };
+struct TapRegion { int dev, off, n; cudaEvent_t ev; bool recorded; unsigned long long sid; };
 std::mutex g_pool_mu;
 std::vector<TapRegion> g_pool_used;
 }  // namespace
@@ -54,13 +73,15 @@ int GM_CAT(tap_pool_acquire_, GM_K)(const float2* taps_dev, int n, cudaStream_t 
   if (n <= 0 || n > kTapPoolN || (n & 1)) return GM_OK;
   int dev = 0;
   GM_TRY(cudaGetDevice(&dev));
+  unsigned long long sid = 0;
+  GM_TRY(cudaStreamGetId(st, &sid));
   std::lock_guard<std::mutex> lk(g_pool_mu);
   // A region whose call was enqueued on this very stream can be refilled at once: stream order
   // puts the copy behind that call's last kernel.  This is what keeps a loop of asynchronous
   // calls on one stream (or on a few, round robin) in the constant bank however far the host
   // runs ahead of the device.
   for (TapRegion& r : g_pool_used) {
-    if (r.dev != dev || !r.recorded || r.st != st || r.n != n) continue;
+    if (r.dev != dev || !r.recorded || r.sid != sid || r.n != n) continue;
     GM_TRY(cudaMemcpyToSymbolAsync(c_tap_pool, taps_dev, (size_t)n * sizeof(float2), (size_t)r.off * sizeof(float2),
                                    cudaMemcpyDeviceToDevice, st));
     cudaEventDestroy(r.ev);
@@ -88,7 +109,7 @@ int GM_CAT(tap_pool_acquire_, GM_K)(const float2* taps_dev, int n, cudaStream_t 
   if (start + n > kTapPoolN) return GM_OK;
   GM_TRY(cudaMemcpyToSymbolAsync(c_tap_pool, taps_dev, (size_t)n * sizeof(float2), (size_t)start * sizeof(float2),
                                  cudaMemcpyDeviceToDevice, st));
-  g_pool_used.push_back({dev, start, n, nullptr, false, st});
+  g_pool_used.push_back({dev, start, n, nullptr, false, sid});
   *off = start;
   return GM_OK;
 }
@@ -100,9 +121,11 @@ void GM_CAT(tap_pool_release_, GM_K)(int off, cudaStream_t st) {
   for (size_t i = 0; i < g_pool_used.size(); ++i) {
     TapRegion& r = g_pool_used[i];
     if (r.dev != dev || r.off != off || r.recorded) continue;
-    if (cudaEventCreateWithFlags(&r.ev, cudaEventDisableTiming) == cudaSuccess && cudaEventRecord(r.ev, st) == cudaSuccess) {
+    unsigned long long sid = 0;
+    if (cudaStreamGetId(st, &sid) == cudaSuccess &&
+        cudaEventCreateWithFlags(&r.ev, cudaEventDisableTiming) == cudaSuccess && cudaEventRecord(r.ev, st) == cudaSuccess) {
       r.recorded = true;
-      r.st = st;
+      r.sid = sid;
     } else {                                               // cannot track it: wait once, then free
       cudaStreamSynchronize(st);
       g_pool_used.erase(g_pool_used.begin() + i);

@@ -56,6 +56,31 @@ def test_validation_codes_without_gpu():
     assert L.gm_fit(C.byref(m), C.byref(b), None, None, None, None, None, None, 0, None) == -1
 
 
+def test_options_and_init_entry_points(lib):
+    # gm_set_option / gm_get_option replace the environment-variable hooks of round 1
+    lib.gm_set_option.restype = C.c_int; lib.gm_get_option.restype = C.c_int
+    for opt in (0, 1):
+        assert lib.gm_get_option(opt) == 1
+        assert lib.gm_set_option(opt, 0) == 0 and lib.gm_get_option(opt) == 0
+        assert lib.gm_set_option(opt, 7) == 0 and lib.gm_get_option(opt) == 1
+    assert lib.gm_set_option(99, 1) == -1 and lib.gm_get_option(-1) == -1
+    assert lib.gm_measure_fp32_peak(0, None, None) == -1            # validated before any CUDA call
+    text = (ROOT / "paper_2404_07780_b200" / "csrc" / "gm_api.cu").read_text()
+    assert "getenv" not in text and "cudaMemcpyToSymbol(" not in text
+
+
+def test_binding_checks_shapes_before_the_library_sees_them():
+    import torch
+    from paper_2404_07780_b200 import binding as bd
+    z = torch.zeros
+    with pytest.raises(ValueError):
+        bd._batch_struct(4, 16, 16, z(3, 5, 5), host=False)          # per-galaxy PSFs: 3 for 4 galaxies
+    with pytest.raises(ValueError):
+        bd._batch_struct(4, 16, 16, z(5, 7), host=False)             # not square
+    with pytest.raises(ValueError):
+        bd._batch_struct(4, 16, 16, z(5, 5), data=z(4, 16, 15), host=False)
+
+
 def test_binding_refuses_cpu_tensors():
     import torch
     import paper_2404_07780_b200 as gm

@@ -119,9 +119,9 @@ def test_shared_and_per_galaxy_psf_agree_bitwise():
 
 @pytest.mark.parametrize("H,W,K", [(64, 64, 25), (96, 96, 9), (128, 128, 41), (100, 90, 33), (192, 192, 25),
                                    (256, 256, 41), (140, 200, 15), (37, 45, 7)])
-def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, monkeypatch):
+def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K):
     # a batch-wide PSF runs the convolution with its taps in the constant bank (FFMA2 with a
-    # uniform-register operand), a per-galaxy PSF or GM_NO_CONST_TAPS with the taps in shared
+    # uniform-register operand), a per-galaxy PSF or gm_set_option(GM_OPT_CONST_TAPS, 0) in shared
     # memory; both add the K^2 products of a pixel in the same order, in k_fused and in the
     # tile kernels, for every compiled PSF side and both thread tiles
     model = models.bulge_disk()
@@ -132,9 +132,11 @@ def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, monkeypatch
         torch.cuda.synchronize()
         return [img] + [t for t in out]
     const = run()
-    monkeypatch.setenv("GM_NO_CONST_TAPS", "1")
-    shared = run()
-    monkeypatch.delenv("GM_NO_CONST_TAPS")
+    gm.gm_set_option(gm.GM_OPT_CONST_TAPS, 0)
+    try:
+        shared = run()
+    finally:
+        gm.gm_set_option(gm.GM_OPT_CONST_TAPS, 1)
     rep = np.ascontiguousarray(np.broadcast_to(psf, (3, K, K)))
     per = [gm.gm_render(model, dev(par), H, W, dev(rep))] + \
         [t for t in gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(rep))]
@@ -148,16 +150,18 @@ def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, monkeypatch
     assert_chi2(const[1].cpu().numpy(), oracle.loss_grad(model, par, data, sigma, mask, psf)[0])
 
 
-def test_constant_tap_regions_are_refilled_between_and_across_calls(monkeypatch):
+def test_constant_tap_regions_are_refilled_between_and_across_calls():
     # a pool region is reused by the next call with another PSF, and concurrent calls on their own
     # streams hold different PSFs at the same time: nobody may see somebody else's (or stale) taps
     model = models.single_sersic()
     H = W = 64; K = 25
     par, data, sigma, mask, _ = synth(model, 4, H, W, K, seed=99)
     psfs = [asymmetric_psf(K, seed=300 + i).astype(np.float32) for i in range(6)]
-    monkeypatch.setenv("GM_NO_CONST_TAPS", "1")
-    want = [gm.gm_render(model, dev(par), H, W, dev(p)).clone() for p in psfs]
-    monkeypatch.delenv("GM_NO_CONST_TAPS")
+    gm.gm_set_option(gm.GM_OPT_CONST_TAPS, 0)
+    try:
+        want = [gm.gm_render(model, dev(par), H, W, dev(p)).clone() for p in psfs]
+    finally:
+        gm.gm_set_option(gm.GM_OPT_CONST_TAPS, 1)
     for rnd in range(3):                                   # back to back on one stream
         for p, w in zip(psfs, want):
             assert torch.equal(gm.gm_render(model, dev(par), H, W, dev(p)), w)
