@@ -2,17 +2,25 @@
 """bench.py -- throughput of the batched galaxy-fit hot path on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--config 1|3|...] [--sweep]
+                    [--config 2|1|3|4|5] [--no-per-config] ...
 
-One "step" = one pass of the whole hot path over one batch: a full ``gm_fit`` of the
-workload (render -> PSF convolution -> chi^2 -> adjoint convolution -> gradient ->
-Adam update, n_iter times, plus the closing chi^2 evaluation).  The N=1 workload is
-BASELINE.json ``configs[1]`` (C1: 1,024 single-Sersic galaxies, 128x128, 25x25 Moffat
-PSF, 200 iterations).  With N>1 every rank fits its own 1,024 galaxies (weak scaling,
-no data-path collective: galaxies are independent).
+One "step" = one pass of the whole hot path over one batch: a full fit of the workload
+(render -> PSF convolution -> chi^2 -> adjoint convolution -> gradient -> Adam update,
+every iteration, plus the closing chi^2 evaluation).  The headline workload (N = 1) is
+BASELINE.json ``configs[2]`` (C2), the one the target sentence names: 8,289 single-Sersic
+galaxies, cutout sides {64, 96, 128, 192, 256}, 25x25 Moffat PSF, 10 % of the pixels
+masked, fit to convergence (tol 1e-6, patience 10) capped at 500 iterations, all five size
+buckets in one ``gm_fit_multi`` call.  The same JSON line carries, under ``per_config``,
+C1, C3, one 2,048-galaxy batch of C4, P1 (the paper's own shapes: 8,289 cutouts of 128x128
+with 41x41 PSFs) and P1 with one PSF per galaxy, each measured the same way.
+
+With N > 1 (torchrun) the N x 8,289 galaxies are dealt to the ranks by pixel count
+(``sharding.shard_galaxies``), every rank fits its shard (no data-path collective: galaxies
+are independent), and the fitted parameters are all-gathered at the
+end (``sharding.gather_results``, timed separately).
 
 Prints ONE JSON line (rank 0).  metric = galaxy-pixel chi^2+gradient evaluations per
-second = B*H*W*n_iter / step time, whole job.  See DESIGN.md "Measurement".
+second = sum over galaxies of H*W*iterations / step time, whole job.  DESIGN.md section 7.
 """
 from __future__ import annotations
 
@@ -95,17 +103,40 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def workload_name(cfg, B, H, W, K, n_iter):
-    return (f"{cfg.name}: {B} galaxies, {cfg.model_name}, {H}x{W} fp32 cutouts, {K}x{K} "
-            f"{'Moffat' if cfg.psf_kind.startswith('moffat') else 'Gaussian'} PSF, "
-            f"{n_iter}-iteration gm_fit")
+def workload_name(cfg, buckets, n_iter, early, per_galaxy_psf):
+    K = buckets[0]["K"]
+    B = sum(k["B"] for k in buckets)
+    psf = "Moffat" if cfg.psf_kind.startswith("moffat") else "Gaussian"
+    if len(buckets) == 1:
+        k = buckets[0]
+        s = f"{cfg.name}: {B} galaxies, {cfg.model_name}, {k['H']}x{k['W']} fp32 cutouts, {K}x{K} {psf} PSF, "
+    else:
+        s = (f"{cfg.name}: {B} galaxies, {cfg.model_name}, sides " +
+             ", ".join(f"{k['H']}px x{k['B']}" for k in buckets) + f", {K}x{K} {psf} PSF, ")
+    if cfg.mask_frac:
+        s += f"{int(round(100 * cfg.mask_frac))}% masked, "
+    s += (f"fit to convergence (tol {buckets[0]['opts']['tol']:g}, patience {buckets[0]['opts']['patience']}) "
+          f"capped at {n_iter} iterations" if early else f"{n_iter}-iteration fit")
+    if per_galaxy_psf:
+        s += ", one PSF per galaxy [B,K,K]"
+    return s
 
 
 # ---------------------------------------------------------------------------------
+def reference_sample(cfg, n_gal):
+    """`n_gal` galaxies of the config's middle size bucket, truth images by the oracle."""
+    import oracle
+    from gen import configs
+    side = cfg.sides[len(cfg.sides) // 2]
+    cand = list(range(40 * n_gal))
+    gal = [g for g, s in zip(cand, configs.sides_for(cfg, cand)) if s == side][:n_gal]
+    return configs.make_batch(cfg.cid, gal, lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf), side=side)
+
+
 def run_reference(args):
     """--impl reference: the fp64 oracle, as it stands, on the host cores (the other
     place bench.py may execute oracle/).  Each step is a bounded sample of the same
-    workload: `cores` galaxies x a few iterations of C1's shapes."""
+    workload: `cores` galaxies x 3 iterations of the config's middle size bucket."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
@@ -113,11 +144,8 @@ def run_reference(args):
     from gen import configs
     cfg = configs.CONFIGS[args.config]
     cores = oracle.num_threads()
-    n_gal, n_iter = cores, 3
-    side = cfg.sides[len(cfg.sides) // 2]
-    cand = list(range(40 * cores))
-    gal = [g for g, s in zip(cand, configs.sides_for(cfg, cand)) if s == side][:n_gal]
-    b = configs.make_batch(cfg.cid, gal, lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf), side=side)
+    n_iter = 3
+    b = reference_sample(cfg, cores)
     n_gal = len(b["galaxies"])
     opts = configs.fit_options(b["model"], b["H"], b["W"], n_iter)
 
@@ -131,11 +159,12 @@ def run_reference(args):
         step()
     dt = (time.perf_counter() - t0) / args.steps
     value = n_gal * b["H"] * b["W"] * n_iter / dt
-    sample = f"{n_gal} galaxies x {n_iter} iterations of {cfg.name} ({b['H']}x{b['W']}, K={b['K']}) per step"
+    sample = (f"{n_gal} galaxies x {n_iter} iterations of {cfg.name}'s {b['H']}x{b['W']} bucket "
+              f"(K={b['K']}{', masked' if b['mask'] is not None else ''}) per step")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(cfg, cfg.B, b["H"], b["W"], b["K"], cfg.n_iter),
+            "config": {"workload": f"{cfg.name} ({cfg.B} galaxies, {cfg.model_name}, K={cfg.K}; see the ours arm)",
                        "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -144,138 +173,104 @@ def run_reference(args):
     return 0
 
 
-def streamed(k, model, n_batches):
-    """BASELINE config C4 is "streamed in batches": n_batches batches through the device-pointer
-    C ABI on two streams with two sets of device buffers, so that the host-to-device copy of batch
-    i + 1 (from pinned host memory) and the read-back of batch i - 1 overlap the fit of batch i.
-    The same synthetic batch is re-sent every time (its bytes cross the bus every time); wall
-    clock with a device synchronise on both sides."""
-    import torch
-
-    import paper_2404_07780_b200 as gm
-    hd, hs, hm, _, hp = k["host"]
-    psf = k["dev"][3]
-    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
-    sets = [{"data": torch.empty_like(k["dev"][0]), "sigma": torch.empty_like(k["dev"][1]),
-             "mask": None if hm is None else torch.empty_like(k["dev"][2]),
-             "params": torch.empty_like(k["dev"][4]), "ws": torch.empty_like(k["ws"]),
-             "back": torch.empty_like(hp).pin_memory()} for _ in streams]
-
-    def run(n):
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for i in range(n):
-            st, b = streams[i % 2], sets[i % 2]
-            with torch.cuda.stream(st):
-                b["data"].copy_(hd, non_blocking=True)
-                b["sigma"].copy_(hs, non_blocking=True)
-                if hm is not None:
-                    b["mask"].copy_(hm, non_blocking=True)
-                b["params"].copy_(hp, non_blocking=True)
-                gm.gm_fit(model, b["params"], b["data"], b["sigma"], b["mask"], psf, k["opts"],
-                          workspace=b["ws"], stream=st)
-                b["back"].copy_(b["params"], non_blocking=True)
-        torch.cuda.synchronize()
-        return time.perf_counter() - t0
-
-    run(2)                                                              # warm-up
-    sec = run(n_batches)
-    B, H, W = k["B"], k["H"], k["W"]
-    h2d = hd.numel() * 4 + hs.numel() * 4 + (0 if hm is None else hm.numel()) + hp.numel() * 4
-    return {"batches": n_batches, "galaxies": n_batches * B, "seconds": sec,
-            "galaxies_fitted_per_s": n_batches * B / sec,
-            "value": n_batches * B * H * W * k["opts"]["n_iter"] / sec, "unit": UNIT,
-            "h2d_bytes_per_batch": int(h2d), "d2h_bytes_per_batch": int(hp.numel() * 4),
-            "how": "two streams, two device buffer sets, H2D / fit / D2H of consecutive batches overlap; "
-                   "gm_fit through the device-pointer C ABI; fixed iteration count assumed"}
-
-
-def cpu_baseline(cfg, side):
+def cpu_baseline(cfg):
     """The oracle timed on the box's host cores on a bounded sample (~10-30 s)."""
     import oracle
     from gen import configs
     cores = oracle.num_threads()
-    n_gal = 2 * cores
-    cand = list(range(40 * cores))
-    gal = [g for g, s in zip(cand, configs.sides_for(cfg, cand)) if s == side][:n_gal]
-    b = configs.make_batch(cfg.cid, gal, lambda m, p, H, W, psf: oracle.render(m, p, H, W, psf), side=side)
+    b = reference_sample(cfg, 2 * cores)
     n_gal = len(b["galaxies"])
     # size the iteration count from one timed evaluation so the sample takes ~15 s
     t0 = time.perf_counter()
     oracle.loss_grad(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"])
     t_eval = time.perf_counter() - t0
-    n_iter = int(min(max(15.0 / max(t_eval, 1e-3), 2), cfg.n_iter or 200))
+    n_iter = int(min(max(15.0 / max(t_eval, 1e-3), 2), 200))
     opts = configs.fit_options(b["model"], b["H"], b["W"], n_iter)
     t0 = time.perf_counter()
     oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
     dt = time.perf_counter() - t0
     return {"value": n_gal * b["H"] * b["W"] * n_iter / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "galaxies_per_s_at_full_iters": n_gal / (dt * (cfg.n_iter or n_iter) / n_iter),
-            "sample": f"{n_gal} galaxies x {n_iter} iterations of {cfg.name} ({b['H']}x{b['W']}, K={b['K']}), "
+            "sample": f"{n_gal} galaxies x {n_iter} iterations of {cfg.name}'s {b['H']}x{b['W']} bucket (K={b['K']}), "
                       f"{dt:.1f} s, OpenMP over galaxies"}
 
 
 # ---------------------------------------------------------------------------------
-def run_ours(args):
-    import torch
-    import paper_2404_07780_b200 as gm
-    from gen import configs
+class Bench:
+    """One process = one GPU.  Holds torch / the binding / the distributed group."""
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    def __init__(self, args):
+        import torch
+        import paper_2404_07780_b200 as gm
+        self.torch, self.gm, self.args = torch, gm, args
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+        torch.cuda.set_device(self.local)
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            self.dist = dist
+        self.flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+        self.stream = torch.cuda.current_stream()
+        self.workers = min(16, os.cpu_count() or 1)
+        gm.gm_init()
+        # the roofline denominator, measured in this process: a pure FFMA2 kernel (gm.h)
+        self.peak_measured = gm.gm_measure_fp32_peak(10)
+        pk, self.pk_src = peaks()
+        self.pk = pk
+        self.f_mhz = pk.get("sm_max_mhz", 1965.0)
+        self.peak_nominal = SM_COUNT * FP32_LANES * 2 * self.f_mhz * 1e6 / 1e12
 
-    cfg = configs.CONFIGS[args.config]
-    Btot = args.batch or min(cfg.B, 8289)
-    n_iter = args.iters or cfg.n_iter or 200
-    gal = range(rank * Btot, rank * Btot + Btot)   # weak scaling: every rank its own galaxies
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    def render(model, p, H, W, psf):               # truth images from the CUDA path itself
-        out = gm.gm_render(model, torch.from_numpy(p).cuda(), H, W, torch.from_numpy(psf).cuda())
-        torch.cuda.synchronize()
-        return out.cpu().numpy()
+    def render(self, model, p, H, W, psf):
+        """Truth images from the CUDA path itself (never compared with the oracle), in chunks."""
+        torch, gm = self.torch, self.gm
+        out = np.empty((p.shape[0], H, W), dtype=np.float32)
+        dpsf = torch.from_numpy(psf).cuda()
+        step = max(1, (256 << 20) // (H * W * 4))
+        for i in range(0, p.shape[0], step):
+            out[i:i + step] = gm.gm_render(model, torch.from_numpy(p[i:i + step]).cuda(), H, W, dpsf).cpu().numpy()
+        return out
 
-    # one bucket per cutout side (C2: five; every other config: one), each its own gm_batch
-    pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
-    d = lambda t: None if t is None else t.cuda(non_blocking=True)
-    sides = [args.side] if args.side else list(cfg.sides)
-    buckets = []
-    for side in sides:
-        b = configs.make_batch(cfg.cid, gal, render, side=side)
-        if not b["galaxies"]:
-            continue
-        if args.per_galaxy_psf:                     # the paper's data: one PSF image per galaxy (P:45, P:296)
-            b["psf"] = np.ascontiguousarray(np.broadcast_to(b["psf"], (len(b["galaxies"]),) + b["psf"].shape))
-        opts = dict(b["opts"]); opts["n_iter"] = n_iter
-        opts["lr_decay"] = 0.01 ** (1.0 / max(n_iter - 1, 1))
-        if args.no_early_stop:
-            opts["tol"] = 0.0
-        host = tuple(map(pin, (b["data"], b["sigma"], b["mask"], b["psf"], b["start"])))
-        devt = tuple(map(d, host))
-        B, H, W, K = len(b["galaxies"]), b["H"], b["W"], b["K"]
-        buckets.append({"b": b, "B": B, "H": H, "W": W, "K": K, "opts": opts, "host": host, "dev": devt,
-                        "params": devt[4].clone(),
-                        "ws": torch.empty(gm.gm_workspace_bytes(b["model"], B, H, W, K, args.per_galaxy_psf) + 256,
-                                          dtype=torch.uint8, device="cuda")})
-    model = buckets[0]["b"]["model"]
-    K = buckets[0]["K"]
-    B = sum(k["B"] for k in buckets)
-    early = any(k["opts"]["tol"] > 0.0 for k in buckets)
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
-    stream = torch.cuda.current_stream()
+    # -----------------------------------------------------------------------------
+    def make_buckets(self, cfg, gal, n_iter, per_galaxy_psf=False, side=None, early_stop=True):
+        torch, gm = self.torch, self.gm
+        from gen import configs
+        pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
+        d = lambda t: None if t is None else t.cuda(non_blocking=True)
+        drawn = configs.sides_for(cfg, list(gal))
+        buckets = []
+        for s in ([side] if side else list(cfg.sides)):
+            if not (drawn == s).any():
+                continue
+            b = configs.make_batch(cfg.cid, gal, self.render, side=s, workers=self.workers)
+            if per_galaxy_psf:                      # the paper's data: one PSF image per galaxy (P:45, P:296)
+                b["psf"] = np.ascontiguousarray(np.broadcast_to(b["psf"], (len(b["galaxies"]),) + b["psf"].shape))
+            opts = dict(b["opts"]); opts["n_iter"] = n_iter
+            opts["lr_decay"] = 0.01 ** (1.0 / max(n_iter - 1, 1))
+            if not early_stop:
+                opts["tol"] = 0.0
+            host = tuple(map(pin, (b["data"], b["sigma"], b["mask"], b["psf"], b["start"])))
+            devt = tuple(map(d, host))
+            B, H, W, K = len(b["galaxies"]), b["H"], b["W"], b["K"]
+            buckets.append({"model": b["model"], "galaxies": b["galaxies"], "start": b["start"],
+                            "n_used": (None if b["mask"] is None else b["mask"].reshape(B, -1).sum(1)),
+                            "B": B, "H": H, "W": W, "K": K, "opts": opts, "host": host, "dev": devt,
+                            "params": devt[4].clone(),
+                            "ws": torch.empty(gm.gm_workspace_bytes(b["model"], B, H, W, K, per_galaxy_psf) + 256,
+                                              dtype=torch.uint8, device="cuda")})
+        return buckets
 
-    multi = len(buckets) > 1 and not args.serial_buckets
-    side_streams = [torch.cuda.Stream() for _ in buckets] if multi else None
-
-    def step():
-        outs, n = [], 0
+    def step(self, buckets, multi, side_streams):
+        torch, gm, stream = self.torch, self.gm, self.stream
+        model = buckets[0]["model"]
         for k in buckets:
             k["params"].copy_(k["dev"][4])
         if multi:
@@ -292,196 +287,357 @@ def run_ours(args):
                 e = torch.cuda.Event(); e.record(s)
                 stream.wait_event(e)
             return outs, n
+        outs, n = [], 0
         for k in buckets:
-            data, sigma, mask, psf, start = k["dev"]
+            data, sigma, mask, psf, _ = k["dev"]
             outs.append(gm.gm_fit(model, k["params"], data, sigma, mask, psf, k["opts"], workspace=k["ws"],
                                   stream=stream))
             n += gm.gm_last_launch_count()
         return outs, n
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        flush.zero_()
-        outs, _ = step()
-    barrier()
-
-    # ---- timed region: K steps, device time by CUDA events on the launching stream
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    launches = 0
-    gm.gm_profile_enable(True)
-    with ClockSampler(local) as clk:
-        barrier()
-        for s in range(args.steps):
-            flush.zero_()                           # L2 flushed between steps (not timed)
-            ev[s][0].record(stream)
-            outs, n = step()
-            ev[s][1].record(stream)
-            launches += n
-        barrier()
-    prof = gm.gm_profile_read()
-    gm.gm_profile_enable(False)
-    t_ms = sum(a.elapsed_time(z) for a, z in ev)
-    t = torch.tensor([t_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    t_ms = float(t.item())
-    ms_per_step = t_ms / args.steps
-
-    # chi^2+gradient evaluations actually made: iters_used per galaxy (= n_iter without early stop)
-    status = np.concatenate([o["status"].cpu().numpy() for o in outs])
-    iters = np.concatenate([o["iters_used"].cpu().numpy() for o in outs])
-    red = np.concatenate([o["chi2"].cpu().numpy() /
-                          np.maximum(k["H"] * k["W"] if k["b"]["mask"] is None
-                                     else k["b"]["mask"].reshape(k["B"], -1).sum(1), 1)
-                          for o, k in zip(outs, buckets)])
-    evals = float(sum(o["iters_used"].sum().item() * k["H"] * k["W"] for o, k in zip(outs, buckets)))
-    # algorithmic convolution flops of one step: 2 convolutions per evaluation + the closing forward
-    # (status 0: n_iter evaluations + closing forward; stopped early or non-finite: the evaluation
-    # that triggered the stop ran both convolutions but applied no update)
-    def n_convs(o):
+    @staticmethod
+    def conv_flops(o, k):
+        """Algorithmic convolution flops of one bucket's fit: 2 K^2 flops per pixel per convolution
+        actually run (status 0: n_iter evaluations of two convolutions + the closing forward; stopped
+        early or non-finite: the evaluation that triggered the stop ran both but applied no update)."""
         it = o["iters_used"].cpu().numpy().astype(np.float64); st = o["status"].cpu().numpy()
-        return float(np.where(st == 0, 2.0 * it + 1.0, 2.0 * (it + 1.0)).sum())
-    conv_flops = float(sum(n_convs(o) * 2.0 * k["H"] * k["W"] * k["K"] ** 2 for o, k in zip(outs, buckets)))
-    value = world * evals / (ms_per_step * 1e-3)
+        n_fwd = np.where(st == 0, it + 1.0, it + 1.0).sum()
+        n_bwd = np.where(st == 0, it, it + 1.0).sum()
+        per = 2.0 * k["H"] * k["W"] * k["K"] ** 2
+        return n_fwd * per, n_bwd * per
 
-    # ---- e2e: the same step through the host-buffer C-ABI call (copies inside)
-    e2e = None
-    if rank == 0 or world > 1:
-        hps = [k["host"][4].numpy().copy() for k in buckets]
-        hargs = [tuple(None if t is None else t.numpy() for t in k["host"][:4]) for k in buckets]
+    # -----------------------------------------------------------------------------
+    def measure(self, cfg, buckets, steps, warmup, multi, want_e2e=True, serial_profile=False):
+        """Times `steps` steps of the workload; returns the record of that workload."""
+        torch, gm, stream = self.torch, self.gm, self.stream
+        world = self.world
+        model = buckets[0]["model"]
+        K = buckets[0]["K"]
+        B = sum(k["B"] for k in buckets)
+        n_iter = buckets[0]["opts"]["n_iter"]
+        early = any(k["opts"]["tol"] > 0.0 for k in buckets)
+        side_streams = [torch.cuda.Stream() for _ in buckets] if multi else None
 
-        def host_step():
-            for k, hp in zip(buckets, hps):
-                hp[...] = k["b"]["start"]
-            if multi:
-                gm.gm_fit_multi_host(model, [{"params": hp, "data": ha[0], "sigma": ha[1], "mask": ha[2],
-                                              "psf": ha[3], "opts": k["opts"]}
-                                             for k, hp, ha in zip(buckets, hps, hargs)])
-                return
-            for k, hp, ha in zip(buckets, hps, hargs):
-                gm.gm_fit_host(model, hp, *ha, k["opts"])
+        for _ in range(max(warmup, 3)):
+            self.flush.zero_()
+            outs, _ = self.step(buckets, multi, side_streams)
+        self.barrier()
 
-        host_step()                                                   # warm-up
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            host_step()
-        te = torch.tensor([(time.perf_counter() - t0) / args.steps], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        h2d = sum(a.nbytes for ha in hargs for a in ha if a is not None) + sum(hp.nbytes for hp in hps)
-        d2h = sum(hp.nbytes for hp in hps) + 3 * B * 4
-        e2e = {"value": world * evals / float(te.item()), "unit": UNIT, "ms_per_step": float(te.item()) * 1e3,
-               "galaxies_fitted_per_s": world * B / float(te.item()),
-               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-               "api": ("gm_fit_multi_host" if multi else "gm_fit_host") +
-                      " (host buffers; cudaMalloc + H2D + fit + D2H inside the call)"}
+        # ---- timed region: `steps` steps, device time by CUDA events on the launching stream
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        launches = 0
+        gm.gm_profile_enable(True)
+        with ClockSampler(self.local) as clk:
+            self.barrier()
+            for s in range(steps):
+                self.flush.zero_()                  # L2 flushed between steps (not timed)
+                ev[s][0].record(stream)
+                outs, n = self.step(buckets, multi, side_streams)
+                ev[s][1].record(stream)
+                launches += n
+            self.barrier()
+        prof = gm.gm_profile_read()
+        gm.gm_profile_enable(False)
+        t_ms = sum(a.elapsed_time(z) for a, z in ev)
+        t = torch.tensor([t_ms], dtype=torch.float64, device="cuda")
+        if self.dist is not None:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        t_ms = float(t.item())
+        ms_per_step = t_ms / steps
 
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return 0
+        status = np.concatenate([o["status"].cpu().numpy() for o in outs])
+        iters = np.concatenate([o["iters_used"].cpu().numpy() for o in outs])
+        red = np.concatenate([o["chi2"].cpu().numpy() / np.maximum(k["H"] * k["W"] if k["n_used"] is None else k["n_used"], 1)
+                              for o, k in zip(outs, buckets)])
+        # chi^2+gradient evaluations actually made: iters_used per galaxy (= n_iter without early stop)
+        evals = torch.tensor([float(sum(o["iters_used"].sum().item() * k["H"] * k["W"] for o, k in zip(outs, buckets)))],
+                             dtype=torch.float64, device="cuda")
+        ngal = torch.tensor([float(B)], dtype=torch.float64, device="cuda")
+        if self.dist is not None:
+            self.dist.all_reduce(evals); self.dist.all_reduce(ngal)
+        evals_all, B_all = float(evals.item()), float(ngal.item())
+        flops = [self.conv_flops(o, k) for o, k in zip(outs, buckets)]
+        conv_flops = sum(f + b for f, b in flops)
+        value = evals_all / (ms_per_step * 1e-3)
 
-    # ---- roofline of the heavy kernels (all run the same K^2-tap FFMA2 loop)
-    pk, pk_src = peaks()
-    clocks = clk.summary()
-    f_mhz = pk.get("sm_max_mhz", 1965.0)
-    peak_tflops = SM_COUNT * FP32_LANES * 2 * f_mhz * 1e6 / 1e12
-    kern = {name: {"launches": n, "avg_ms": ms / n, "share_of_step": ms / t_ms if world == 1 else None}
-            for name, (ms, n) in prof.items() if n}
-    heavy_ms = sum(ms for ms, n in prof.values() if n)
-    dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
-    roofline = None
-    if dom:
-        # buckets on concurrent streams: per-launch event times overlap one another, so the
-        # kernels' time is the step's own device time, not the sum over launches
-        achieved = (conv_flops / (ms_per_step * 1e-3) if multi else
-                    args.steps * conv_flops / (heavy_ms * 1e-3)) / 1e12
-        n_dom = kern[dom]["launches"]
-        big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
-        traffic = None
-        # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-        # ncu --set full capture summarised in profiles/r01_fused_ncu.md (kernel,bytes per line)
-        tf = ROOT / "profiles" / "r01_traffic.csv"
-        if tf.exists() and len(buckets) == 1:
-            key = f"{dom}_K{K}_{big['H']}x{big['W']}_B{big['B']}"
-            for line in tf.read_text().splitlines()[1:]:
-                name, _, nbytes = line.partition(",")
-                if name.strip() == key:
-                    traffic = int(nbytes)
-        px_bytes = 9 if big["b"]["mask"] is not None else 8
-        roofline = {"bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved,
-                    "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                    "traffic": traffic,
-                    "peak_source": f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 flop x {f_mhz:.0f} MHz "
-                                   f"(sm_max_mhz of {pk_src} MEASURED_PEAKS.json; an FFMA2 loop measured "
-                                   "36.8 TFMA/s = 73.7 TFLOP/s on this pool, DESIGN.md)",
-                    "algorithmic_flops_per_launch": args.steps * conv_flops / max(n_dom, 1)
-                    if len(kern) == 1 else None,
-                    "how": "2*K^2 flops per pixel per convolution x convolutions actually run "
-                           "(2 per chi^2+gradient evaluation + the closing forward) / summed CUDA-event time of the "
-                           "heavy kernels (forward, backward, fused) inside the timed region" +
-                           ("; size buckets run concurrently on one stream each, so the divisor is the step's "
-                            "device time and the per-kernel averages include time shared between streams"
-                            if multi else ""),
-                    "hbm_gbs_algorithmic": (evals * args.steps * px_bytes) / (heavy_ms * 1e-3) / 1e9,
-                    "hbm_peak_gbs": pk.get("hbm_gbs"), "kernels": kern}
-        # whole-step view: the same flops against the step time (small kernels and gaps included)
-        roofline["step_frac"] = (conv_flops / (ms_per_step * 1e-3) / 1e12) / peak_tflops
+        rec = {"workload": workload_name(cfg, buckets, n_iter, early, buckets[0]["dev"][3].dim() == 3),
+               "ms_per_step": ms_per_step, "value": value, "unit": UNIT,
+               "galaxies_fitted_per_s": B_all / (ms_per_step * 1e-3),
+               "fit_summary": {"status_counts": {str(k): int((status == k).sum()) for k in np.unique(status)},
+                               "mean_iters": float(iters.mean()), "median_reduced_chi2": float(np.median(red))},
+               "clocks": clk.summary(), "gpu_launches": int(launches)}
 
-    wl = (workload_name(cfg, B, buckets[0]["H"], buckets[0]["W"], K, n_iter) if len(buckets) == 1 else
-          f"{cfg.name}: {B} galaxies, {cfg.model_name}, sides " +
-          ", ".join(f"{k['H']}px x{k['B']}" for k in buckets) +
-          f", {K}x{K} Moffat PSF, {'10% masked, ' if cfg.mask_frac else ''}gm_fit capped at {n_iter} iterations"
-          + (" with early stop" if early else ""))
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": wl + (", one PSF per galaxy [B,K,K]" if args.per_galaxy_psf else ""),
-                       "global_batch": B * world,
-                       "buckets": ("gm_fit_multi, one stream per cutout side" if multi else
-                                   "gm_fit per cutout side, one after the other") if len(buckets) > 1 else None,
-                       "parallelism": f"dp{world} (independent galaxies, no collective)",
-                       "l2": "flushed between steps (256 MiB write)",
-                       "inputs": "seeded synthetic SDSS-like (gen/configs.py), resident in HBM"},
-            "galaxies_fitted_per_s": world * B / (ms_per_step * 1e-3),
-            "fit_summary": {"status_counts": {str(k): int((status == k).sum()) for k in np.unique(status)},
-                            "mean_iters": float(iters.mean()),
-                            "median_reduced_chi2": float(np.median(red))},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
-    if len(buckets) == 1 and rank == 0:
-        # BASELINE metric (i) as SURVEY 8(d) words it: B*H*W*reps / t(gm_loss_grad), 3 warm-ups, 20 timed
-        # calls at the start parameters, CUDA events on the launching stream, L2 flushed before each call
-        k = buckets[0]
+        # ---- roofline of the heavy kernels (all run the same K^2-tap FFMA2 loop)
+        kinds = {name: (ms, n) for name, (ms, n) in prof.items() if n}
+        if multi and serial_profile and self.rank == 0:
+            # buckets on concurrent streams: per-launch event times overlap one another.  One more
+            # step, bucket after bucket on one stream, gives every kernel its own duration.
+            per_kind_ms = {}; per_kind_n = {}; per_kind_flops = {}
+            for k in buckets:
+                k["params"].copy_(k["dev"][4])
+                gm.gm_profile_enable(True)
+                data, sigma, mask, psf, _ = k["dev"]
+                o = gm.gm_fit(model, k["params"], data, sigma, mask, psf, k["opts"], workspace=k["ws"], stream=stream)
+                torch.cuda.synchronize()
+                pr = gm.gm_profile_read()
+                gm.gm_profile_enable(False)
+                f_fwd, f_bwd = self.conv_flops(o, k)
+                ran = {name for name, (ms, n) in pr.items() if n}
+                for name, (ms, n) in pr.items():
+                    if not n:
+                        continue
+                    per_kind_ms[name] = per_kind_ms.get(name, 0.0) + ms
+                    per_kind_n[name] = per_kind_n.get(name, 0) + n
+                    fl = (f_fwd + f_bwd) if name == "fused" else (f_fwd if name == "forward" else f_bwd)
+                    per_kind_flops[name] = per_kind_flops.get(name, 0.0) + fl
+                    k.setdefault("serial", {})[name] = {"launches": n, "avg_ms": ms / n,
+                                                        "frac_measured": fl / (ms * 1e-3) / 1e12 / self.peak_measured}
+                assert ran, "no heavy kernel ran"
+            kern = {name: {"launches": per_kind_n[name], "avg_ms": per_kind_ms[name] / per_kind_n[name],
+                           "tflops": per_kind_flops[name] / (per_kind_ms[name] * 1e-3) / 1e12}
+                    for name in per_kind_ms}
+            dom = max(kern, key=lambda n: per_kind_ms[n])
+            achieved = kern[dom]["tflops"]
+            how_t = ("one extra step with the buckets one after the other on one stream (per-launch CUDA events do not "
+                     "overlap there); the timed steps run the buckets concurrently")
+            rec["buckets"] = [{"side": k["H"], "galaxies": k["B"], "kernels": k.get("serial")} for k in buckets]
+        else:
+            heavy_ms = sum(ms for ms, n in kinds.values())
+            kern = {name: {"launches": n, "avg_ms": ms / n} for name, (ms, n) in kinds.items()}
+            dom = max(kern, key=lambda n: kern[n]["avg_ms"] * kern[n]["launches"]) if kern else None
+            achieved = steps * conv_flops / (heavy_ms * 1e-3) / 1e12 if heavy_ms else None
+            how_t = "summed CUDA-event time of the heavy kernels (forward, backward, fused) inside the timed region"
+            for name in kern:
+                kern[name]["share_of_step"] = kinds[name][0] / t_ms if world == 1 else None
+        if dom:
+            big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
+            px_bytes = 9 if big["dev"][2] is not None else 8
+            rec["roofline"] = {
+                "bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved, "peak": self.peak_measured,
+                "unit": "TFLOP/s", "frac": achieved / self.peak_measured,
+                "peak_source": "measured in this process: gm_measure_fp32_peak, a pure fma.rn.f32x2 kernel (include/gm.h)",
+                "peak_nominal": self.peak_nominal, "frac_of_nominal": achieved / self.peak_nominal,
+                "peak_nominal_source": f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 flop x {self.f_mhz:.0f} MHz "
+                                       f"(sm_max_mhz of {self.pk_src} MEASURED_PEAKS.json)",
+                "traffic": traffic_from_profiles(dom, K, big),
+                "algorithmic_bytes_per_px_eval": px_bytes,
+                "how": "2*K^2 flops per pixel per convolution x convolutions actually run (2 per chi^2+gradient "
+                       "evaluation + the closing forward) / " + how_t,
+                "hbm_peak_gbs": self.pk.get("hbm_gbs"), "kernels": kern,
+                # whole-step view: the same flops against the step time (small kernels and gaps included)
+                "step_frac": (conv_flops / (ms_per_step * 1e-3) / 1e12) / self.peak_measured}
+
+        # ---- e2e: the same step through the host-buffer C-ABI call (copies inside)
+        if want_e2e:
+            hps = [k["host"][4].numpy().copy() for k in buckets]
+            hargs = [tuple(None if t is None else t.numpy() for t in k["host"][:4]) for k in buckets]
+
+            def host_step():
+                for k, hp in zip(buckets, hps):
+                    hp[...] = k["start"]
+                if len(buckets) > 1:
+                    gm.gm_fit_multi_host(model, [{"params": hp, "data": ha[0], "sigma": ha[1], "mask": ha[2],
+                                                  "psf": ha[3], "opts": k["opts"]}
+                                                 for k, hp, ha in zip(buckets, hps, hargs)])
+                    return
+                for k, hp, ha in zip(buckets, hps, hargs):
+                    gm.gm_fit_host(model, hp, *ha, k["opts"])
+
+            host_step()                                                   # warm-up
+            self.barrier()
+            t0 = time.perf_counter()
+            for _ in range(steps):
+                host_step()
+            te = torch.tensor([(time.perf_counter() - t0) / steps], dtype=torch.float64, device="cuda")
+            if self.dist is not None:
+                self.dist.all_reduce(te, op=self.dist.ReduceOp.MAX)
+            h2d = sum(a.nbytes for ha in hargs for a in ha if a is not None) + sum(hp.nbytes for hp in hps)
+            d2h = sum(hp.nbytes for hp in hps) + 3 * B * 4
+            rec["e2e"] = {"value": evals_all / float(te.item()), "unit": UNIT, "ms_per_step": float(te.item()) * 1e3,
+                          "galaxies_fitted_per_s": B_all / float(te.item()),
+                          "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                          "api": ("gm_fit_multi_host" if len(buckets) > 1 else "gm_fit_host") +
+                                 " (host buffers; device allocation + H2D + fit + D2H inside the call)"}
+        rec["_outs"] = outs
+        return rec
+
+    def loss_grad_line(self, k):
+        """BASELINE metric (i) as SURVEY 8(d) words it: B*H*W*reps / t(gm_loss_grad): 3 warm-ups, 20 timed
+        calls at the start parameters, CUDA events on the launching stream, L2 flushed before each call."""
+        torch, gm, stream = self.torch, self.gm, self.stream
         data, sigma, mask, psf, start = k["dev"]
         chi2 = torch.empty(k["B"], dtype=torch.float32, device="cuda"); grad = torch.empty_like(start)
-        lg = lambda: gm.gm_loss_grad(model, start, data, sigma, mask, psf, chi2=chi2, grad=grad,
+        lg = lambda: gm.gm_loss_grad(k["model"], start, data, sigma, mask, psf, chi2=chi2, grad=grad,
                                      workspace=k["ws"], stream=stream)
         for _ in range(3):
             lg()
         tt = []
         for _ in range(20):
-            flush.zero_()
+            self.flush.zero_()
             a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream); lg(); z.record(stream)
             tt.append((a, z))
         torch.cuda.synchronize()
         ms = statistics.median(a.elapsed_time(z) for a, z in tt)
-        line["loss_grad"] = {"value": k["B"] * k["H"] * k["W"] / (ms * 1e-3), "unit": UNIT, "ms_per_call": ms,
-                             "calls": 20, "stat": "median",
-                             "frac": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12 / peak_tflops,
-                             "api": "gm_loss_grad (prologue, taps, chi^2 + gradient, finalize: the whole call)"}
-    if args.stream_batches > 1 and len(buckets) == 1 and rank == 0:
-        line["streamed"] = streamed(buckets[0], model, args.stream_batches)
-    if world == 1 and not args.no_cpu:
-        line["cpu_baseline"] = cpu_baseline(cfg, buckets[len(buckets) // 2]["H"])
+        return {"value": k["B"] * k["H"] * k["W"] / (ms * 1e-3), "unit": UNIT, "ms_per_call": ms, "calls": 20,
+                "stat": "median",
+                "frac": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12 / self.peak_measured,
+                "api": "gm_loss_grad (prologue, taps, chi^2 + gradient, finalize: the whole call)"}
+
+    def streamed(self, k, n_batches):
+        """BASELINE config C4 is "streamed in batches": n_batches batches through the device-pointer
+        C ABI on two streams with two sets of device buffers, so that the host-to-device copy of batch
+        i + 1 (from pinned host memory) and the read-back of batch i - 1 overlap the fit of batch i.
+        The same synthetic batch is re-sent every time (its bytes cross the bus every time); wall
+        clock with a device synchronise on both sides."""
+        torch, gm = self.torch, self.gm
+        hd, hs, hm, _, hp = k["host"]
+        psf = k["dev"][3]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        sets = [{"data": torch.empty_like(k["dev"][0]), "sigma": torch.empty_like(k["dev"][1]),
+                 "mask": None if hm is None else torch.empty_like(k["dev"][2]),
+                 "params": torch.empty_like(k["dev"][4]), "ws": torch.empty_like(k["ws"]),
+                 "back": torch.empty_like(hp).pin_memory()} for _ in streams]
+
+        def run(n):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for i in range(n):
+                st, b = streams[i % 2], sets[i % 2]
+                with torch.cuda.stream(st):
+                    b["data"].copy_(hd, non_blocking=True)
+                    b["sigma"].copy_(hs, non_blocking=True)
+                    if hm is not None:
+                        b["mask"].copy_(hm, non_blocking=True)
+                    b["params"].copy_(hp, non_blocking=True)
+                    gm.gm_fit(k["model"], b["params"], b["data"], b["sigma"], b["mask"], psf, k["opts"],
+                              workspace=b["ws"], stream=st)
+                    b["back"].copy_(b["params"], non_blocking=True)
+            torch.cuda.synchronize()
+            return time.perf_counter() - t0
+
+        run(2)                                                              # warm-up
+        sec = run(n_batches)
+        B, H, W = k["B"], k["H"], k["W"]
+        h2d = hd.numel() * 4 + hs.numel() * 4 + (0 if hm is None else hm.numel()) + hp.numel() * 4
+        return {"batches": n_batches, "galaxies": n_batches * B, "seconds": sec,
+                "galaxies_fitted_per_s": n_batches * B / sec,
+                "value": n_batches * B * H * W * k["opts"]["n_iter"] / sec, "unit": UNIT,
+                "h2d_bytes_per_batch": int(h2d), "d2h_bytes_per_batch": int(hp.numel() * 4),
+                "how": "two streams, two device buffer sets, H2D / fit / D2H of consecutive batches overlap; "
+                       "gm_fit through the device-pointer C ABI; fixed iteration count assumed"}
+
+
+def traffic_from_profiles(dom, K, big):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu
+    --set full captures summarised under profiles/ (kernel_K.._HxW_B..,bytes per line); None when that
+    kernel / shape was not captured."""
+    key = f"{dom}_K{K}_{big['H']}x{big['W']}_B{big['B']}"
+    for name in ("r02_traffic.csv", "r01_traffic.csv"):
+        tf = ROOT / "profiles" / name
+        if not tf.exists():
+            continue
+        for line in tf.read_text().splitlines()[1:]:
+            k, _, nbytes = line.partition(",")
+            if k.strip() == key:
+                return int(nbytes.split(",")[0])
+    return None
+
+
+# ---------------------------------------------------------------------------------
+SUB_CONFIGS = (  # key, config id, galaxies, per-galaxy PSF
+    ("C1", 1, None, False),
+    ("C3", 3, None, False),
+    ("C4_batch2048", 4, 2048, False),
+    ("P1", 5, None, False),
+    ("P1_per_galaxy_psf", 5, None, True),
+)
+
+
+def run_ours(args):
+    from gen import configs
+    from paper_2404_07780_b200.sharding import gather_results, shard_galaxies
+    bn = Bench(args)
+    torch = bn.torch
+    cfg = configs.CONFIGS[args.config]
+    Btot = args.batch or cfg.B
+    n_iter = args.iters or cfg.n_iter or 200
+
+    # galaxies of this rank: the world x Btot galaxies dealt out by pixel count (LPT), no collective
+    # in the loop; at world = 1 this is galaxies 0 .. Btot-1 in order
+    all_gal = np.arange(bn.world * Btot)
+    px = configs.sides_for(cfg, all_gal).astype(np.int64) ** 2
+    shards = shard_galaxies(px, bn.world)
+    mine = all_gal[shards[bn.rank]]
+    buckets = bn.make_buckets(cfg, list(mine), n_iter, args.per_galaxy_psf, args.side or None, not args.no_early_stop)
+    multi = len(buckets) > 1 and not args.serial_buckets
+    rec = bn.measure(cfg, buckets, args.steps, args.warmup, multi, want_e2e=True, serial_profile=True)
+    outs = rec.pop("_outs")
+
+    gather = None
+    if bn.world > 1:
+        # final gather of the fitted parameters and chi^2 in the original galaxy order (8(e))
+        order = np.concatenate([np.searchsorted(all_gal, np.asarray(k["galaxies"])) for k in buckets])
+        par = torch.cat([o["params"] for o in outs]); chi = torch.cat([o["chi2"] for o in outs])
+        bn.barrier()
+        t0 = time.perf_counter()
+        full_p, full_c = gather_results(order, par, chi, len(all_gal))
+        torch.cuda.synchronize()
+        gather = {"ms": (time.perf_counter() - t0) * 1e3, "rows": int(full_p.shape[0]),
+                  "finite": bool(torch.isfinite(full_c).all().item())}
+
+    if bn.rank != 0:
+        if bn.dist is not None:
+            bn.dist.destroy_process_group()
+        return 0
+
+    line = {"metric": METRIC, "value": rec["value"], "unit": UNIT, "n_gpus": bn.world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": rec["workload"], "global_batch": Btot * bn.world,
+                       "buckets": ("gm_fit_multi, one stream per cutout side" if multi else
+                                   "gm_fit per cutout side, one after the other") if len(buckets) > 1 else None,
+                       "parallelism": f"dp{bn.world} (galaxies dealt by pixel count, no collective in the loop, "
+                                      "final all-gather of params/chi2)" if bn.world > 1 else "single GPU",
+                       "l2": "flushed between steps (256 MiB write)",
+                       "inputs": "seeded synthetic SDSS-like (gen/configs.py), resident in HBM"},
+            "galaxies_fitted_per_s": rec["galaxies_fitted_per_s"], "fit_summary": rec["fit_summary"],
+            "clocks": rec["clocks"], "e2e": rec.get("e2e"), "gpu_launches": rec["gpu_launches"],
+            "roofline": rec.get("roofline"), "buckets": rec.get("buckets"),
+            "fp32_peak": {"measured_tflops": bn.peak_measured, "nominal_tflops": bn.peak_nominal}}
+    if gather:
+        line["gather"] = gather
+    if len(buckets) == 1:
+        line["loss_grad"] = bn.loss_grad_line(buckets[0])
+        if args.stream_batches > 1:
+            line["streamed"] = bn.streamed(buckets[0], args.stream_batches)
+    del buckets, outs
+    torch.cuda.empty_cache()
+
+    if bn.world == 1 and not args.no_per_config and args.config == 2 and not args.side:
+        per = {}
+        sub_steps = max(1, min(args.steps, 2))
+        for key, cid, nb, pg in SUB_CONFIGS:
+            c = configs.CONFIGS[cid]
+            B = nb or c.B
+            bk = bn.make_buckets(c, list(range(B)), c.n_iter or 200, pg, None, True)
+            r = bn.measure(c, bk, sub_steps, 3, False, want_e2e=True)
+            r.pop("_outs")
+            rf = r.pop("roofline", None) or {}
+            r.update({"steps": sub_steps, "frac": rf.get("frac"), "frac_of_nominal": rf.get("frac_of_nominal"),
+                      "step_frac": rf.get("step_frac"), "achieved_tflops": rf.get("achieved"),
+                      "traffic": rf.get("traffic"), "kernels": rf.get("kernels")})
+            if key == "C1":
+                r["loss_grad"] = bn.loss_grad_line(bk[0])
+            per[key] = r
+            del bk
+            torch.cuda.empty_cache()
+        line["per_config"] = per
+    if bn.world == 1 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(cfg)
     print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    if bn.dist is not None:
+        bn.dist.destroy_process_group()
     return 0
 
 
@@ -491,16 +647,18 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = C1)")
+    ap.add_argument("--config", type=int, default=2,
+                    help="BASELINE.json config index (default 2 = C2, the 8,289-galaxy target; 5 = P1)")
     ap.add_argument("--batch", type=int, default=0, help="galaxies per GPU (default: the config's)")
-    ap.add_argument("--side", type=int, default=0, help="cutout side for the mixed-size config C2")
+    ap.add_argument("--side", type=int, default=0, help="only this cutout side of the mixed-size config C2")
     ap.add_argument("--iters", type=int, default=0, help="override the iteration count")
     ap.add_argument("--no-early-stop", action="store_true")
     ap.add_argument("--serial-buckets", action="store_true",
                     help="C2: one gm_fit per size bucket, one after the other, instead of gm_fit_multi")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sub-records (C1, C3, C4, P1)")
     ap.add_argument("--per-galaxy-psf", action="store_true",
-                    help="pass the PSF as [B,K,K] (taps in shared memory instead of the constant bank)")
+                    help="pass the PSF as [B,K,K] (the paper's data layout, P:45)")
     ap.add_argument("--stream-batches", type=int, default=0,
                     help="also stream this many batches through two streams (C4: 65,536 galaxies = 32 x 2048)")
     args = ap.parse_args()

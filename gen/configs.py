@@ -195,12 +195,13 @@ def _noise_one(cfg: Config, g: int, M: np.ndarray, Ie: float):
     return D, sigma, mask
 
 
-def make_batch(cid: int, galaxies, render, side: int | None = None) -> dict:
+def make_batch(cid: int, galaxies, render, side: int | None = None, workers: int = 1) -> dict:
     """Inputs for the given galaxy indices of config ``cid`` (one cutout side).
 
     ``render(model, params_f32[B,P], H, W, psf_f32) -> ndarray[B,H,W]`` supplies the
     noiseless model.  For C2, ``side`` selects the size bucket; galaxies whose
-    drawn side differs are dropped.
+    drawn side differs are dropped.  ``workers`` > 1 draws the noise of different galaxies in
+    threads (every galaxy has its own generator, so the result does not depend on it).
     """
     cfg = CONFIGS[cid]
     galaxies = list(galaxies)
@@ -220,9 +221,17 @@ def make_batch(cid: int, galaxies, render, side: int | None = None) -> dict:
     sigma = np.empty((B, H, W), dtype=np.float32)
     mask = np.empty((B, H, W), dtype=np.uint8)
     amp_idx = model["roles"].index("amp")
-    for row, g in enumerate(galaxies):
-        D, s, m = _noise_one(cfg, g, M[row], float(truth[row, amp_idx]))
+    def noise(row):
+        D, s, m = _noise_one(cfg, galaxies[row], M[row], float(truth[row, amp_idx]))
         data[row] = D; sigma[row] = s; mask[row] = m
+
+    if workers > 1 and B > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=workers) as ex:
+            list(ex.map(noise, range(B)))
+    else:
+        for row in range(B):
+            noise(row)
     start = start_params(cfg, model, truth.astype(np.float64), galaxies, H, W).astype(np.float32)
     return {"cfg": cfg, "model": model, "galaxies": galaxies, "H": H, "W": W, "K": cfg.K,
             "psf": psf, "truth": truth, "start": start, "data": data, "sigma": sigma,

@@ -1641,7 +1641,7 @@ int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream) {
   cudaEvent_t e0, e1;
   GM_CUDA(cudaEventCreate(&e0));
   GM_CUDA(cudaEventCreate(&e1));
-  const int grid = caps.n_sm * 4, iters = 2048;
+  const int grid = caps.n_sm * 4, iters = 256;
   k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);        // warm-up
   GM_CUDA(cudaEventRecord(e0, st));
   for (int r = 0; r < repeats; ++r) k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);

@@ -1,0 +1,166 @@
+"""Fit parity of gm_fit / gm_fit_multi against the oracle's fit, config by config.
+
+Shared by tests/test_gpu_fit_configs.py (the -m gpu tests) and tests/parity_report.py (the
+script that writes profiles/r02_parity.md).  Calls only ``oracle/`` and the binding.
+
+Criterion (BASELINE.json north_star, SURVEY 8(c) M1 + the S/N note of 8(d)): every fitted
+parameter within 1e-3 relative of the oracle's (theta modulo pi, skipped when q > 0.95).
+Where a galaxy misses that on some parameter -- the fit of a faint galaxy ends in a flat
+valley of chi^2, where fp32 and fp64 trajectories drift apart along the valley -- the two
+end points must be THE SAME FIT in everything that is well conditioned, judged by the
+oracle alone at both parameter sets:
+  * chi^2_oracle(p_gpu) and chi^2_oracle(p_oracle) agree within CHI2_RTOL (1e-5);
+  * the model images oracle.render(p_gpu) and oracle.render(p_oracle) agree within
+    IMG_SIGMA_TOL of the noise sigma on every used pixel (the data cannot tell them apart).
+A galaxy that fails both the parameter criterion and this check is a parity failure.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle
+import paper_2404_07780_b200 as gm
+from gen import configs
+
+PAR_RTOL = 1e-3
+CHI2_RTOL = 1e-5
+IMG_SIGMA_TOL = 0.05     # |M(p_gpu) - M(p_orc)| <= 0.05 sigma per pixel: far below the noise
+
+
+def dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def oracle_render(model, p, H, W, psf):
+    return oracle.render(model, p, H, W, psf)
+
+
+def param_ok(model, gpu, orc, rtol=PAR_RTOL):
+    """[B,P] bool: parameter within rtol of the oracle's (reading M1 for theta)."""
+    ok = np.ones(gpu.shape, dtype=bool)
+    roles = model["roles"]
+    comps = model["components"]
+    for k, role in enumerate(roles):
+        if role == "theta":
+            d = np.abs(((gpu[:, k] - orc[:, k]) + np.pi / 2) % np.pi - np.pi / 2)
+            ok[:, k] = d <= rtol * np.maximum(np.abs(orc[:, k]), 1.0)
+            # theta is unconstrained when its component is round: find that component's q
+            qk = [c["slots"].get("q") for c in comps if c["slots"].get("theta") == k]
+            if qk and qk[0] is not None:
+                ok[:, k] |= orc[:, qk[0]] > 0.95
+        else:
+            ok[:, k] = np.abs(gpu[:, k] - orc[:, k]) <= rtol * np.abs(orc[:, k])
+    return ok
+
+
+def rel_dev(model, gpu, orc):
+    """[B,P] relative deviation (theta: absolute, modulo pi, against max(|theta|, 1))."""
+    out = np.abs(gpu - orc) / np.maximum(np.abs(orc), 1e-300)
+    for k, role in enumerate(model["roles"]):
+        if role == "theta":
+            d = np.abs(((gpu[:, k] - orc[:, k]) + np.pi / 2) % np.pi - np.pi / 2)
+            out[:, k] = d / np.maximum(np.abs(orc[:, k]), 1.0)
+    return out
+
+
+def same_fit_check(b, gpu_params, orc_params, rows):
+    """For the galaxies `rows`: (chi2 relative difference, max |dM| / sigma over used pixels),
+    both from the oracle evaluated at the two parameter sets."""
+    if len(rows) == 0:
+        return np.zeros(0), np.zeros(0)
+    sub = lambda a: None if a is None else a[rows]
+    psf = b["psf"] if b["psf"].ndim == 2 else b["psf"][rows]
+    pg = gpu_params[rows].astype(np.float64); po = orc_params[rows].astype(np.float64)
+    cg, _ = oracle.loss_grad(b["model"], pg, sub(b["data"]), sub(b["sigma"]), sub(b["mask"]), psf)
+    co, _ = oracle.loss_grad(b["model"], po, sub(b["data"]), sub(b["sigma"]), sub(b["mask"]), psf)
+    H, W = b["data"].shape[1:]
+    mg = oracle.render(b["model"], pg, H, W, psf)
+    mo = oracle.render(b["model"], po, H, W, psf)
+    used = np.ones(mg.shape, dtype=bool) if b["mask"] is None else (b["mask"][rows] != 0)
+    dm = np.where(used, np.abs(mg - mo) / b["sigma"][rows].astype(np.float64), 0.0)
+    return np.abs(cg - co) / np.abs(co), dm.reshape(len(rows), -1).max(axis=1)
+
+
+def judge(b, gpu, orc):
+    """Compare one bucket's GPU fit with the oracle's.  -> dict of arrays / numbers."""
+    model = b["model"]
+    gp = gpu["params"].astype(np.float64); op = orc["params"]
+    ok = param_ok(model, gp, op)
+    dev_ = rel_dev(model, gp, op)
+    miss = np.flatnonzero(~ok.all(axis=1))
+    dchi, dimg = same_fit_check(b, gp, op, miss)
+    valid = (dchi <= CHI2_RTOL) & (dimg <= IMG_SIGMA_TOL)
+    chi_rel = np.abs(gpu["chi2"].astype(np.float64) - orc["chi2"]) / np.abs(orc["chi2"])
+    return {"ok": ok, "dev": dev_, "miss": miss, "miss_dchi2": dchi, "miss_dimg_sigma": dimg,
+            "miss_valid": valid, "chi2_rel": chi_rel,
+            "status_equal": np.array_equal(gpu["status"], orc["status"]),
+            "iters_gpu": gpu["iters_used"], "iters_orc": orc["iters_used"]}
+
+
+def assert_parity(name, j, floor):
+    """The complete check: every galaxy either meets 1e-3 on every parameter or is the same fit
+    by the oracle's chi^2 and image; and the per-parameter pass rate is at least `floor`."""
+    bad = j["miss"][~j["miss_valid"]]
+    assert len(bad) == 0, (f"{name}: galaxies {bad.tolist()} miss {PAR_RTOL:g} on a parameter AND differ as fits: "
+                           f"d chi2 {j['miss_dchi2'][~j['miss_valid']]}, d image / sigma {j['miss_dimg_sigma'][~j['miss_valid']]}")
+    rate = j["ok"].mean()
+    assert rate >= floor, f"{name}: parameter pass rate {rate:.4f} < {floor}"
+
+
+# ---- the configurations ---------------------------------------------------------
+def _np_out(out):
+    return {k: v.cpu().numpy() for k, v in out.items() if not k.startswith("_")}
+
+
+def gpu_fit(b, opts):
+    p = dev(b["start"]).clone()
+    out = gm.gm_fit(b["model"], p, dev(b["data"]), dev(b["sigma"]), dev(b["mask"]), dev(b["psf"]), opts)
+    torch.cuda.synchronize()
+    return _np_out(out)
+
+
+def gpu_fit_multi(buckets):
+    batches = [{"params": dev(b["start"]).clone(), "data": dev(b["data"]), "sigma": dev(b["sigma"]),
+                "mask": dev(b["mask"]), "psf": dev(b["psf"]), "opts": o} for b, o in buckets]
+    outs = gm.gm_fit_multi(buckets[0][0]["model"], batches)
+    torch.cuda.synchronize()
+    return [_np_out(o) for o in outs]
+
+
+def oracle_fit(b, opts):
+    return oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
+
+
+def case_c0(n_gal=16, n_iter=150):
+    b = configs.make_batch(0, range(n_gal), oracle_render)
+    return b, configs.fit_options(b["model"], b["H"], b["W"], n_iter)
+
+
+def case_c1(sample):
+    """C1 exactly (200 iterations, no early stop) for the galaxy indices `sample`."""
+    b = configs.make_batch(1, sample, oracle_render)
+    return b, b["opts"]
+
+
+def case_c2(gal, sides=(64, 96, 128, 192, 256)):
+    """C2 exactly (mask on, tol 1e-6, patience 10, cap 500): one (batch, opts) per cutout side."""
+    out = []
+    drawn = configs.sides_for(configs.CONFIGS[2], list(gal))
+    for side in sides:
+        if (drawn == side).any():
+            b = configs.make_batch(2, gal, oracle_render, side=side)
+            out.append((b, b["opts"]))
+    return out
+
+
+def case_c3(n_gal=16, n_iter=100):
+    """C3's model and shapes (bulge + disk, P = 11, 128 x 128, K = 25), n_iter iterations."""
+    b = configs.make_batch(3, range(n_gal), oracle_render)
+    return b, configs.fit_options(b["model"], b["H"], b["W"], n_iter)
+
+
+def case_c4(n_gal=4, n_iter=30):
+    """C4's model and shapes (Sersic + Ferrer + Moffat, P = 16, 256 x 256, K = 41)."""
+    b = configs.make_batch(4, range(n_gal), oracle_render)
+    return b, configs.fit_options(b["model"], b["H"], b["W"], n_iter)

@@ -7,7 +7,7 @@ import oracle
 import paper_2404_07780_b200 as gm
 from gen import configs, models
 from gen.psf import gaussian_psf
-from gpu_util import PAR_RTOL, assert_chi2, dev, oracle_render
+from gpu_util import assert_chi2, dev, oracle_render
 
 pytestmark = pytest.mark.gpu
 
@@ -17,22 +17,6 @@ def gpu_fit(b, opts, start=None):
     out = gm.gm_fit(b["model"], p, dev(b["data"]), dev(b["sigma"]), dev(b["mask"]), dev(b["psf"]), opts)
     torch.cuda.synchronize()
     return {k: v.cpu().numpy() for k, v in out.items() if not k.startswith("_")}
-
-
-def theta_close(a, b, rtol):
-    d = np.abs(((a - b) + np.pi / 2) % np.pi - np.pi / 2)      # theta is defined modulo pi (reading M1)
-    return d <= rtol * np.maximum(np.abs(b), 1.0)
-
-
-def compare_params(model, gpu, orc, rtol=PAR_RTOL):
-    ok = np.ones(gpu.shape, dtype=bool)
-    for k, role in enumerate(model["roles"]):
-        if role == "theta":
-            ok[:, k] = theta_close(gpu[:, k], orc[:, k], rtol)
-            ok[:, k] |= orc[:, [i for i, r in enumerate(model["roles"]) if r == "q"][0]] > 0.95
-        else:
-            ok[:, k] = np.abs(gpu[:, k] - orc[:, k]) <= rtol * np.abs(orc[:, k])
-    return ok
 
 
 def test_first_steps_match_oracle_closely():
@@ -46,22 +30,18 @@ def test_first_steps_match_oracle_closely():
     assert (g["iters_used"] == 3).all() and (g["status"] == 0).all()
 
 
-def test_fit_c0_like_fixed_iterations():
+def test_chi2_out_is_chi2_at_the_returned_parameters():
     b = configs.make_batch(0, range(16), oracle_render)
-    opts = configs.fit_options(b["model"], 64, 64, 150)
+    opts = configs.fit_options(b["model"], 64, 64, 40)
     g = gpu_fit(b, opts)
-    o = oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
-    ok = compare_params(b["model"], g["params"], o["params"])
-    assert ok.mean() >= 0.97, f"parameter pass rate {ok.mean():.3f}\n{ok}"
-    assert_chi2(g["chi2"], o["chi2"], rtol=1e-4)
-    # chi2_out is chi^2 at the returned parameters
     c, _ = gm.gm_loss_grad(b["model"], dev(g["params"]), dev(b["data"]), dev(b["sigma"]), None, dev(b["psf"]))
     assert_chi2(g["chi2"], c.cpu().numpy().astype(np.float64), rtol=1e-6)
 
 
 def test_fit_bulge_disk_small():
-    def render(model, p, H, W, psf):
-        return oracle.render(model, p, H, W, psf)
+    # tied centre, two components, small cutout: long fits of the full-size configurations are
+    # in test_gpu_fit_configs.py with the complete same-fit criterion
+    import fit_parity as fp
     cfg = configs.CONFIGS[3]
     model = configs.get_model(cfg)
     H = W = 48
@@ -73,13 +53,12 @@ def test_fit_bulge_disk_small():
     sigma = np.full(M.shape, 0.02, dtype=np.float32)
     data = (M + 0.02 * rng.normal(size=M.shape)).astype(np.float32)
     start = configs.start_params(cfg, model, truth.astype(np.float64), gal, H, W).astype(np.float32)
-    b = {"model": model, "start": start, "data": data, "sigma": sigma, "mask": None, "psf": psf}
+    b = {"model": model, "start": start, "data": data, "sigma": sigma, "mask": None, "psf": psf,
+         "galaxies": list(gal), "H": H, "W": W, "K": 9}
     opts = configs.fit_options(model, H, W, 100)
     g = gpu_fit(b, opts)
     o = oracle.fit(model, start, data, sigma, None, psf, opts)
-    assert_chi2(g["chi2"], o["chi2"], rtol=1e-3)
-    ok = compare_params(model, g["params"], o["params"], rtol=5e-3)
-    assert ok.mean() >= 0.9, f"{ok.mean()}\n{ok}"
+    fp.assert_parity("bulge+disk 48 px", fp.judge(b, g, o), floor=0.9)
 
 
 def test_early_stop_fixed_parameter_and_nonfinite():

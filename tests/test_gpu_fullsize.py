@@ -11,7 +11,7 @@ import oracle
 import paper_2404_07780_b200 as gm
 from gen import configs
 from gpu_util import assert_chi2, assert_grad, assert_pixels, dev, oracle_render
-from test_gpu_fit import compare_params
+import fit_parity as fp
 
 pytestmark = pytest.mark.gpu
 
@@ -45,11 +45,15 @@ def test_c1_full_batch_fit_sampled():
     assert (out["status"].cpu().numpy() == 0).all() and (out["iters_used"].cpu().numpy() == 200).all()
     sample = np.arange(0, 1024, 43)                                # 24 galaxies across the batch
     o = oracle.fit(b["model"], b["start"][sample], b["data"][sample], b["sigma"][sample], None, b["psf"], opts)
-    # chi^2 at the fitted point is well conditioned; parameters sit in flat valleys for the
-    # faint galaxies (SURVEY 8(d) S/N note), so they are judged as a pass rate
+    # chi^2 at the fitted point is well conditioned; parameters of faint galaxies sit in flat
+    # valleys (SURVEY 8(d) S/N note): whoever misses 1e-3 must be the same fit by the oracle's
+    # chi^2 and model image (tests/fit_parity.py)
     assert_chi2(gc[sample], o["chi2"], rtol=1e-4)
-    ok = compare_params(b["model"], gp[sample], o["params"])
-    assert ok.mean() >= 0.9, f"parameter pass rate {ok.mean():.3f}"
+    sub = dict(b, start=b["start"][sample], data=b["data"][sample], sigma=b["sigma"][sample],
+               galaxies=[b["galaxies"][i] for i in sample])
+    g_s = {"params": gp[sample], "chi2": gc[sample], "status": out["status"].cpu().numpy()[sample],
+           "iters_used": out["iters_used"].cpu().numpy()[sample]}
+    fp.assert_parity("C1 full batch", fp.judge(sub, g_s, o), floor=0.90)
     # the fit must not depend on the batch a galaxy sits in (galaxies are independent)
     p2 = dev(b["start"][sample]).clone()
     out2 = gm.gm_fit(b["model"], p2, dev(b["data"][sample]), dev(b["sigma"][sample]), None, dev(b["psf"]), opts)
