@@ -271,6 +271,23 @@ int gm_bootstrap(const gm_model* model, const gm_batch* batch, const float* para
                  float* mean, float* samples, void* workspace, size_t workspace_bytes,
                  void* cuda_stream);
 
+/* The PSF convolution on its own, with a choice of engine (the paper leaves the
+ * convolution algorithm open):  out = PSF (*) in, true convolution, PSF centre (K-1)/2, zero
+ * fill outside the cutout, same size (R:C1); adjoint != 0: the correlation with the same PSF (R:C2).
+ *   GM_CONV_FFMA2   the FP32 direct convolution of the fit path (packed FFMA2 loop); any H, W, odd
+ *                   K <= GM_MAX_K
+ *   GM_CONV_TENSOR  tcgen05 tensor cores: every fp32 operand is scaled by an exact power of two and
+ *                   split into two fp16 halves (22 significant bits), three MMAs per product accumulate
+ *                   hi*hi + lo*hi + hi*lo in fp32 in tensor memory (the dropped lo*lo term is 2^-22
+ *                   relative); Toeplitz band blocks of the PSF stream through shared memory.  H = W = 128
+ *                   only (GM_ENOTSUP otherwise); inputs must be finite.
+ * batch: B, H, W, K, psf, psf_stride are read and batch->data is the INPUT image, dev [B,H,W].
+ * out: dev [B,H,W].  workspace: gm_conv_workspace_bytes(engine, batch).  Asynchronous. */
+enum { GM_CONV_FFMA2 = 0, GM_CONV_TENSOR = 1 };
+size_t gm_conv_workspace_bytes(int engine, const gm_batch* batch);
+int gm_conv(int engine, int adjoint, const gm_batch* batch, float* out, void* workspace,
+            size_t workspace_bytes, void* cuda_stream);
+
 /* ---- host-buffer entry points (synchronous, end to end) -------------------- */
 /* Same operations with every pointer of `batch` and every array argument in HOST
  * memory (pinned memory makes the copies faster, pageable works).  The call
@@ -315,7 +332,7 @@ int gm_profile_read(double* ms /* host [3] */, int64_t* count /* host [3] */);
 
 /* The FP32 peak the roofline is quoted against, MEASURED: a kernel of nothing but
  * independent packed FP32 multiply-adds (fma.rn.f32x2, the instruction of the convolution
- * loops), one 256-thread CTA x 4 per SM, timed with CUDA events on `cuda_stream` over
+ * loops), three 256-thread CTAs per SM in one wave, timed with CUDA events on `cuda_stream` over
  * `repeats` launches after one warm-up launch.  Synchronous (waits for its own events).
  * tflops: host, 2 flop per multiply-add. */
 int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream);

@@ -5,6 +5,8 @@ argument marshalling only -- every step of the path runs in the CUDA kernels
 under ``csrc/``.  PyTorch supplies device memory and streams.
 """
 from .binding import (  # noqa: F401
+    GM_CONV_FFMA2,
+    GM_CONV_TENSOR,
     GM_OPT_CONST_TAPS,
     GM_OPT_FUSED,
     GmError,
@@ -14,6 +16,7 @@ from .binding import (  # noqa: F401
     gm_set_option,
     gm_bootstrap,
     gm_bootstrap_counts,
+    gm_conv,
     gm_fit,
     gm_fit_host,
     gm_fit_multi,

@@ -21,6 +21,7 @@ _LIB_PATH = _PKG / "libgm.so"
 
 GM_MAX_COMP, GM_MAX_PAR, GM_MAX_K, GM_NSLOT = 8, 32, 41, 10
 GM_OPT_FUSED, GM_OPT_CONST_TAPS = 0, 1
+GM_CONV_FFMA2, GM_CONV_TENSOR = 0, 1
 _KINDS = {"sersic": 0, "expdisk": 1, "ferrer": 2, "king": 3, "gaussian": 4, "moffat": 5, "sky": 6}
 _SLOTS = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box", "m0")
 
@@ -100,6 +101,8 @@ def _lib():
         L.gm_last_cuda_error.restype = i; L.gm_last_cuda_error.argtypes = []
         L.gm_last_cuda_error_string.restype = C.c_char_p; L.gm_last_cuda_error_string.argtypes = []
         L.gm_last_launch_count.restype = C.c_int64; L.gm_last_launch_count.argtypes = []
+        L.gm_conv_workspace_bytes.restype = sz; L.gm_conv_workspace_bytes.argtypes = [i, bp]
+        L.gm_conv.restype = i; L.gm_conv.argtypes = [i, i, bp, vp, vp, sz, vp]
         L.gm_init.restype = i; L.gm_init.argtypes = [vp]
         L.gm_set_option.restype = i; L.gm_set_option.argtypes = [i, i]
         L.gm_get_option.restype = i; L.gm_get_option.argtypes = [i]
@@ -279,6 +282,27 @@ def gm_render(model, params, H, W, psf, out=None, workspace=None, stream=None):
                           _dev(out, torch.float32, "out"), wp, wn, _stream_ptr(stream))
     _check(rc, "gm_render")
     out._gm_ws = ws
+    return out
+
+
+@_on_stream
+def gm_conv(image, psf, engine=GM_CONV_FFMA2, adjoint=False, out=None, workspace=None, stream=None):
+    """out[B,H,W] = psf (*) image (true convolution, zero fill, same size; adjoint: correlation) with the
+    FFMA2 loop or on the tensor cores (include/gm.h gm_conv).  Asynchronous on the stream."""
+    B, H, W = image.shape
+    b = _batch_struct(B, H, W, psf, data=image)
+    need = _lib().gm_conv_workspace_bytes(int(engine), C.byref(b))
+    if need == 0:
+        raise GmError(-2, "gm_conv_workspace_bytes")
+    if workspace is None:
+        workspace = torch.empty(need + 256, dtype=torch.uint8, device=image.device)
+    off = (-workspace.data_ptr()) % 256
+    if out is None:
+        out = torch.empty_like(image)
+    rc = _lib().gm_conv(int(engine), int(bool(adjoint)), C.byref(b), _dev(out, torch.float32, "out"),
+                        workspace.data_ptr() + off, workspace.numel() - off, _stream_ptr(stream))
+    _check(rc, "gm_conv")
+    out._gm_ws = workspace
     return out
 
 

@@ -48,6 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     nvcc = _nvcc()
     jobs = [([nvcc, *NVCC_FLAGS, "-c", str(CSRC / "gm_api.cu"), "-o", str(OBJ / "gm_api.o")], "gm_api")]
+    jobs.append(([nvcc, *NVCC_FLAGS, f"-I{INCLUDE}", "-c", str(CSRC / "gm_tc.cu"), "-o", str(OBJ / "gm_tc.o")], "gm_tc"))
     for k in KS:
         jobs.append(([nvcc, *NVCC_FLAGS, f"-DGM_K={k}", "-c", str(CSRC / "gm_tiles.cu"),
                       "-o", str(OBJ / f"gm_tiles_{k}.o")], f"gm_tiles K={k}"))
@@ -63,7 +64,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
         list(ex.map(run, jobs))
-    objs = [str(OBJ / "gm_api.o")] + [str(OBJ / f"gm_tiles_{k}.o") for k in KS]
+    objs = [str(OBJ / "gm_api.o"), str(OBJ / "gm_tc.o")] + [str(OBJ / f"gm_tiles_{k}.o") for k in KS]
     tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
     r = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *objs],
                        capture_output=True, text=True)

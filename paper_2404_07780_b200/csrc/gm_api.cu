@@ -528,7 +528,7 @@ k_covar(int B, int P, const FreeSet fs, const double* __restrict__ jtj, float* _
 // shared by a run of accumulators, as the tap pair is in the convolution loops.
 // ---------------------------------------------------------------------------
 constexpr int kPeakAcc = 32;
-__global__ void __launch_bounds__(256) k_ffma2_peak(int iters, float seed, float* __restrict__ sink) {
+__global__ void __launch_bounds__(256, 3) k_ffma2_peak(int iters, float seed, float* __restrict__ sink) {
   float2 acc[kPeakAcc];
 #pragma unroll
   for (int i = 0; i < kPeakAcc; ++i) acc[i] = make_float2(seed * (float)i, seed * (float)(threadIdx.x & 7));
@@ -681,6 +681,7 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   int launch_backward_##K(const BwdArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
   int launch_fused_##K(const FusedArgs& a, int variant, int n_sm, size_t smem_limit, cudaStream_t st,         \
                        cudaError_t* err);                                                     \
+  int launch_conv_##K(const ConvTileArgs& a, int B, cudaStream_t st, cudaError_t* err);                 \
   int tap_pool_acquire_##K(const float2* taps_dev, int n, cudaStream_t st, int* off, cudaError_t* err); \
   void tap_pool_release_##K(int off, cudaStream_t st);
 GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33) GM_DECL_K(41)
@@ -721,6 +722,32 @@ static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
     default: return GM_ENOTSUP;
   }
   prof_end(pi, st);
+  if (rc == GM_OK) ++t_launches;
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+
+namespace tc {          // gm_tc.cu
+extern int g_tc_dbg;
+int padded_side(int K);
+size_t table_bytes(int KP);
+int conv(int KP, int B, const float* in, float* out, const float* psf, long long psf_stride, int K, int flip, uint8_t* tab,
+         float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches);
+}  // namespace tc
+
+static int dispatch_conv(int KP, const ConvTileArgs& a, int B, cudaStream_t st) {
+  int rc;
+  cudaError_t err = cudaSuccess;
+  switch (KP) {
+    case 5: rc = launch_conv_5(a, B, st, &err); break;
+    case 9: rc = launch_conv_9(a, B, st, &err); break;
+    case 15: rc = launch_conv_15(a, B, st, &err); break;
+    case 21: rc = launch_conv_21(a, B, st, &err); break;
+    case 25: rc = launch_conv_25(a, B, st, &err); break;
+    case 33: rc = launch_conv_33(a, B, st, &err); break;
+    case 41: rc = launch_conv_41(a, B, st, &err); break;
+    default: return GM_ENOTSUP;
+  }
   if (rc == GM_OK) ++t_launches;
   if (rc == GM_ECUDA) t_last_err = err;
   return rc;
@@ -1114,6 +1141,84 @@ int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params,
     if ((rc = jtj_to_float(uw, (size_t)bt->B * pl.md.n_par * pl.md.n_par, jtj, st)) != GM_OK) return rc;
   }
   return GM_OK;
+}
+
+// ---- gm_conv: the convolution alone, FFMA2 or tensor-core engine ------------
+static bool conv_args_ok(const gm_batch* bt) {
+  return bt && bt->B >= 1 && bt->H >= 1 && bt->W >= 1 && bt->K >= 1 && bt->K <= GM_MAX_K && (bt->K & 1) && bt->psf_stride >= 0;
+}
+
+size_t gm_conv_workspace_bytes(int engine, const gm_batch* bt) {
+  if (!conv_args_ok(bt)) return 0;
+  const size_t n_psf = bt->psf_stride == 0 ? 1 : (size_t)bt->B;
+  if (engine == GM_CONV_TENSOR) {
+    const int KP = tc::padded_side(bt->K);
+    if (KP < 0) return 0;
+    return align_up(n_psf * tc::table_bytes(KP), 256) + align_up(n_psf * 4, 256);
+  }
+  if (engine != GM_CONV_FFMA2) return 0;
+  const int KP = padded_K(bt->K);
+  if (KP < 0) return 0;
+  return align_up(n_psf * KP * KP * 4, 256) + align_up(n_psf * 2 * (size_t)(KP + 1) * (KP + 1) * sizeof(float2), 256);
+}
+
+int gm_conv(int engine, int adjoint, const gm_batch* bt, float* out, void* workspace, size_t workspace_bytes,
+            void* cuda_stream) {
+  t_launches = 0;
+  if (!conv_args_ok(bt) || !bt->data || !bt->psf || !out) return GM_EINVAL;
+  if (engine != GM_CONV_FFMA2 && engine != GM_CONV_TENSOR) return GM_EINVAL;
+  const size_t need = gm_conv_workspace_bytes(engine, bt);
+  if (need == 0) return GM_ENOTSUP;
+  if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return GM_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DevCaps caps;
+  int rc = device_caps(&caps);
+  if (rc != GM_OK) return rc;
+  const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
+  if (engine == GM_CONV_TENSOR) {
+    if (bt->H != 128 || bt->W != 128) return GM_ENOTSUP;
+    const int KP = tc::padded_side(bt->K);
+    uint8_t* tab = (uint8_t*)workspace;
+    float* bscale = (float*)((char*)workspace + align_up((size_t)n_psf * tc::table_bytes(KP), 256));
+    cudaError_t err = cudaSuccess;
+    int launches = 0;
+    rc = tc::conv(KP, bt->B, bt->data, out, bt->psf, bt->psf_stride, bt->K, adjoint ? 0 : 1, tab, bscale, caps.n_sm, st,
+                  &err, &launches);
+    t_launches += launches;
+    if (rc == GM_ECUDA) t_last_err = err;
+    return rc;
+  }
+  const int KP = padded_K(bt->K);
+  float* psf_pad = (float*)workspace;
+  float2* taps = (float2*)((char*)workspace + align_up((size_t)n_psf * KP * KP * 4, 256));
+  const float* psf = bt->psf;
+  long long stride = bt->psf_stride;
+  if (KP != bt->K) {
+    const long long n = (long long)n_psf * KP * KP;
+    k_pad_psf<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, KP, psf_pad);
+    ++t_launches;
+    GM_CUDA(cudaGetLastError());
+    psf = psf_pad;
+    stride = bt->psf_stride == 0 ? 0 : (long long)KP * KP;
+  }
+  const int per = (KP + 1) * (KP + 1);
+  const long long n = (long long)n_psf * 2 * per;
+  k_make_taps<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(psf, stride, n_psf, KP, taps);
+  ++t_launches;
+  GM_CUDA(cudaGetLastError());
+  int ct_off = -1;
+  if (bt->psf_stride == 0 && g_opt[GM_OPT_CONST_TAPS].load() != 0)
+    if ((rc = tap_pool_acquire(KP, taps, 2 * per, st, &ct_off)) != GM_OK) return rc;
+  ConvTileArgs a;
+  a.tg = make_geom(bt->H, bt->W, KP);
+  a.taps = taps + (adjoint ? per : 0);
+  a.taps_stride = bt->psf_stride == 0 ? 0 : 2ll * per;
+  a.ct_off = ct_off >= 0 ? ct_off + (adjoint ? per : 0) : -1;
+  a.ct_zero = 0;
+  a.in = bt->data; a.out = out;
+  rc = dispatch_conv(KP, a, bt->B, st);
+  if (ct_off >= 0) tap_pool_release(KP, ct_off, st);
+  return rc;
 }
 
 int gm_uncertainty(const gm_model* model, const gm_batch* bt, const float* params,
@@ -1619,6 +1724,7 @@ int gm_init(void* cuda_stream) {
 }
 
 int gm_set_option(int option, int value) {
+  if (option == 99) { tc::g_tc_dbg = value; return GM_OK; }   // PROBE ONLY
   if (option < 0 || option >= GM_OPT_COUNT_) return GM_EINVAL;
   g_opt[option].store(value != 0);
   return GM_OK;
@@ -1641,7 +1747,9 @@ int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream) {
   cudaEvent_t e0, e1;
   GM_CUDA(cudaEventCreate(&e0));
   GM_CUDA(cudaEventCreate(&e1));
-  const int grid = caps.n_sm * 4, iters = 256;
+  // 3 CTAs per SM, all resident in ONE wave (74 registers x 768 threads): a fourth CTA per SM would
+  // start a second, unevenly placed wave and understate the peak by 15 %
+  const int grid = caps.n_sm * 3, iters = 1024;
   k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);        // warm-up
   GM_CUDA(cudaEventRecord(e0, st));
   for (int r = 0; r < repeats; ++r) k_ffma2_peak<<<grid, 256, 0, st>>>(iters, 1.0f, sink);

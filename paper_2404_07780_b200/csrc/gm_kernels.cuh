@@ -607,4 +607,62 @@ __global__ void __launch_bounds__(512) k_backward(const BwdArgs a) {
   }
 }
 
+// ---------------------------------------------------------------------------
+// gm_conv, engine GM_CONV_FFMA2: the convolution loop above on its own (out = PSF (*) in
+// with the flipped taps, or the adjoint with the taps as given), one tile per CTA.  It is
+// the FP32 side of the comparison with the tensor-core engine (gm_tc.cuh).
+// ---------------------------------------------------------------------------
+struct ConvTileArgs {
+  TileGeom tg;
+  const float2* taps; long long taps_stride;
+  int ct_off, ct_zero;
+  const float* in;         // [B,H,W]
+  float* out;              // [B,H,W]
+};
+
+template <int K, int RP, int TC, bool CT>
+__global__ void __launch_bounds__(512) k_conv_ffma2(const ConvTileArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const TileGeom& tg = a.tg;
+  const int tiles = tg.tiles_x * tg.tiles_y;
+  const int b = blockIdx.x / tiles, tile = blockIdx.x - b * tiles;
+  const int tile_y = tile / tg.tiles_x, tile_x = tile - tile_y * tg.tiles_x;
+  const int i0 = tile_y * tg.TH, j0 = tile_x * tg.TW;
+  constexpr int h = (K - 1) / 2;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  float* tilebuf = reinterpret_cast<float*>(smem_raw);
+  float2* taps = reinterpret_cast<float2*>(tilebuf + (size_t)tg.rows * tg.pitch);
+  if (!CT) copy_taps<K>(taps, a.taps + (long long)b * a.taps_stride, tid, nthr);
+  const float* src = a.in + (size_t)b * tg.H * tg.W;
+  for (int idx = tid; idx < tg.rows * tg.pitch; idx += nthr) {       // tile + halo, zero outside the cutout
+    const int yy = idx / tg.pitch, xx = idx - yy * tg.pitch;
+    const int i = i0 - h + yy, j = j0 - h + xx;
+    const bool ok = i >= 0 && i < tg.H && j >= 0 && j < tg.W;
+    cp_async_zfill4(tilebuf + idx, src + (ok ? (size_t)i * tg.W + j : 0), ok);
+  }
+  cp_async_wait_all();
+  __syncthreads();
+  const int ty = tid / tg.ntx, tx = tid - ty * tg.ntx;
+  const bool active = ty < tg.nty;
+  float2 acc[RP][TC];
+#pragma unroll
+  for (int rp = 0; rp < RP; ++rp)
+#pragma unroll
+    for (int c = 0; c < TC; ++c) acc[rp][c] = make_float2(0.0f, 0.0f);
+  if (active) {
+    const float* win = tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC;
+    if (CT) conv_tile_ct<K, RP, TC>(win, tg.pitch, a.ct_off, a.ct_zero, acc);
+    else conv_tile<K, RP, TC>(win, tg.pitch, taps, acc);
+  }
+  __syncthreads();
+  if (active) store_acc<RP, TC>(tilebuf + (size_t)(ty * 2 * RP) * tg.pitch + tx * TC, tg.pitch, acc);
+  __syncthreads();
+  float* dst = a.out + (size_t)b * tg.H * tg.W;
+  for (int idx = tid; idx < tg.TH * tg.TW; idx += nthr) {
+    const int yy = idx / tg.TW, xx = idx - yy * tg.TW;
+    const int i = i0 + yy, j = j0 + xx;
+    if (i < tg.H && j < tg.W) dst[(size_t)i * tg.W + j] = tilebuf[(size_t)yy * tg.pitch + xx];
+  }
+}
+
 }  // namespace gm

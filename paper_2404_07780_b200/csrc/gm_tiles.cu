@@ -215,4 +215,29 @@ int GM_CAT(launch_fused_, GM_K)(const FusedArgs& a, int variant, int n_sm, size_
   return GM_OK;
 }
 
+// gm_conv, FFMA2 engine
+int GM_CAT(launch_conv_, GM_K)(const ConvTileArgs& a, int B, cudaStream_t st, cudaError_t* err) {
+  constexpr int K = GM_K;
+  int nthr = (a.tg.ntx * a.tg.nty + 31) / 32 * 32;
+  if (nthr > 256) return GM_ENOTSUP;
+  const bool ct = a.ct_off >= 0;
+  const size_t sm = smem_bytes<K>(a.tg, 8, 1, ct);
+  const unsigned grid = (unsigned)((size_t)B * a.tg.tiles_x * a.tg.tiles_y);
+  if (a.tg.variant == 1 && ct) {
+    GM_TRY(set_smem(k_conv_ffma2<K, 3, 12, true>, sm));
+    k_conv_ffma2<K, 3, 12, true><<<grid, nthr, sm, st>>>(a);
+  } else if (a.tg.variant == 1) {
+    GM_TRY(set_smem(k_conv_ffma2<K, 3, 12, false>, sm));
+    k_conv_ffma2<K, 3, 12, false><<<grid, nthr, sm, st>>>(a);
+  } else if (ct) {
+    GM_TRY(set_smem(k_conv_ffma2<K, 4, 8, true>, sm));
+    k_conv_ffma2<K, 4, 8, true><<<grid, nthr, sm, st>>>(a);
+  } else {
+    GM_TRY(set_smem(k_conv_ffma2<K, 4, 8, false>, sm));
+    k_conv_ffma2<K, 4, 8, false><<<grid, nthr, sm, st>>>(a);
+  }
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
 }  // namespace gm

@@ -132,6 +132,51 @@ def oracle_fit(b, opts):
     return oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
 
 
+def oracle_fit_at_iters(b, opts, iters):
+    """The oracle's fit of every galaxy with exactly iters[g] updates and no early stop: the
+    oracle's trajectory read at the iteration where the GPU path stopped that galaxy.
+
+    The early-stop rule (reading O5) is a threshold on |chi2_t - chi2_(t-1)| / chi2_t at tol = 1e-6,
+    i.e. at the resolution of an fp32 chi^2: the iteration at which it fires is not unique between
+    an fp32 and an fp64 evaluation (it differs by up to a few tens of iterations, both valid), while
+    the parameters still drift along the flat valley.  So the trajectory is compared at EQUAL
+    iteration counts, and the stop decision separately (stop_decision_ok)."""
+    from concurrent.futures import ThreadPoolExecutor
+    iters = np.asarray(iters)
+    P = b["start"].shape[1]
+    out = {"params": np.empty((len(iters), P)), "chi2": np.empty(len(iters)),
+           "iters_used": np.zeros(len(iters), dtype=np.int32), "status": np.zeros(len(iters), dtype=np.int32)}
+    groups = {}
+    for g, t in enumerate(iters):
+        groups.setdefault(int(t), []).append(g)
+    n_thr = oracle.num_threads()
+
+    def run(item):
+        t, rows = item
+        o = dict(opts); o["n_iter"] = t; o["tol"] = 0.0
+        sub = lambda a: None if a is None else a[rows]
+        psf = b["psf"] if b["psf"].ndim == 2 else b["psf"][rows]
+        r = oracle.fit(b["model"], b["start"][rows], sub(b["data"]), sub(b["sigma"]), sub(b["mask"]), psf, o)
+        for k in out:
+            out[k][rows] = r[k]
+
+    oracle.set_num_threads(1)                              # one galaxy group per Python thread instead
+    try:
+        with ThreadPoolExecutor(max_workers=n_thr) as ex:
+            list(ex.map(run, sorted(groups.items(), key=lambda it: -it[0] * len(it[1]))))
+    finally:
+        oracle.set_num_threads(n_thr)
+    return out
+
+
+def stop_decision_ok(gpu, orc, patience):
+    """Early stop (reading O5): same status per galaxy, and stop iterations that differ by no more
+    than max(2 * patience, 25 % of the oracle's count)."""
+    dt = np.abs(gpu["iters_used"].astype(np.int64) - orc["iters_used"])
+    lim = np.maximum(2 * patience, 0.25 * orc["iters_used"])
+    return np.array_equal(gpu["status"], orc["status"]) and bool(np.all(dt <= lim)), dt
+
+
 def case_c0(n_gal=16, n_iter=150):
     b = configs.make_batch(0, range(n_gal), oracle_render)
     return b, configs.fit_options(b["model"], b["H"], b["W"], n_iter)

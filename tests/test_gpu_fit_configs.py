@@ -18,7 +18,7 @@ def _chi2_at_oracle_params_close(j, rtol):
 def test_c0_fixed_150_iterations():
     b, opts = fp.case_c0()
     j = fp.judge(b, fp.gpu_fit(b, opts), fp.oracle_fit(b, opts))
-    fp.assert_parity("C0", j, floor=0.97)
+    fp.assert_parity("C0", j, floor=0.99)
     _chi2_at_oracle_params_close(j, 1e-4)
 
 
@@ -26,24 +26,27 @@ def test_c1_200_iterations_sample():
     sample = list(range(0, 1024, 43))
     b, opts = fp.case_c1(sample)
     j = fp.judge(b, fp.gpu_fit(b, opts), fp.oracle_fit(b, opts))
-    fp.assert_parity("C1", j, floor=0.90)
+    fp.assert_parity("C1", j, floor=0.95)
     _chi2_at_oracle_params_close(j, 1e-4)
 
 
 def test_c2_every_bucket_through_fit_multi_early_stop_masked():
     # mask on, tol 1e-6 / patience 10, cap 500, all five sides in ONE gm_fit_multi call: the
-    # 64 / 96 / 128 px buckets run k_fused with the live list, 192 / 256 px the tile kernels
+    # 64 / 96 / 128 px buckets run k_fused with the live list, 192 / 256 px the tile kernels.
+    # The iteration at which the stop rule fires is not unique at tol = 1e-6 (fit_parity.py), so
+    # (1) the oracle's own early-stop run must agree in status and, loosely, in iteration count,
+    # (2) the oracle's trajectory read at the GPU's iteration count must be the GPU's parameters.
     buckets = fp.case_c2(range(60))
     assert sorted(b["H"] for b, _ in buckets) == [64, 96, 128, 192, 256]
     outs = fp.gpu_fit_multi(buckets)
     stopped = 0
     for (b, opts), g in zip(buckets, outs):
         assert b["mask"] is not None and opts["tol"] > 0 and opts["n_iter"] == 500
-        o = fp.oracle_fit(b, opts)
+        ok, dt = fp.stop_decision_ok(g, fp.oracle_fit(b, opts), opts["patience"])
+        assert ok, f"C2/{b['H']}px: stop decisions differ, |d iterations| = {dt}"
+        o = fp.oracle_fit_at_iters(b, opts, g["iters_used"])
         j = fp.judge(b, g, o)
-        fp.assert_parity(f"C2/{b['H']}px", j, floor=0.85)
-        # early-stop decisions sit at the fp32 resolution of chi^2 (tol 1e-6): iteration counts may
-        # differ (reading O5), the fits may not
+        fp.assert_parity(f"C2/{b['H']}px", j, floor=0.95)
         _chi2_at_oracle_params_close(j, 1e-4)
         stopped += int((g["status"] == 1).sum())
     assert stopped > 0, "early stop never triggered: the test would not cover the live list"
@@ -53,7 +56,7 @@ def test_c3_bulge_disk_128px_k25():
     b, opts = fp.case_c3(16, 100)
     assert b["model"]["n_par"] == 11 and b["H"] == 128 and b["K"] == 25
     j = fp.judge(b, fp.gpu_fit(b, opts), fp.oracle_fit(b, opts))
-    fp.assert_parity("C3", j, floor=0.90)
+    fp.assert_parity("C3", j, floor=0.99)
     _chi2_at_oracle_params_close(j, 1e-4)
 
 
@@ -61,5 +64,5 @@ def test_c4_three_components_256px_k41():
     b, opts = fp.case_c4(4, 30)
     assert b["model"]["n_par"] == 16 and b["H"] == 256 and b["K"] == 41
     j = fp.judge(b, fp.gpu_fit(b, opts), fp.oracle_fit(b, opts))
-    fp.assert_parity("C4", j, floor=0.90)
+    fp.assert_parity("C4", j, floor=0.99)
     _chi2_at_oracle_params_close(j, 1e-4)
