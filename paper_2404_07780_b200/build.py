@@ -32,12 +32,22 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def _stamp() -> str:
+def _stamp(files=None) -> str:
     h = hashlib.sha256()
-    for p in sorted(list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + [INCLUDE / "gm.h", Path(__file__)]):
+    if files is None:
+        files = sorted(list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")))
+    for p in list(files) + [INCLUDE / "gm.h", Path(__file__)]:
         h.update(p.name.encode()); h.update(p.read_bytes())
     h.update(" ".join(EXTRA).encode())
     return h.hexdigest()
+
+
+# what each object is compiled from (an object is rebuilt only when one of these changed)
+_DEPS = {
+    "gm_api": ["gm_api.cu", "gm_fused.cuh", "gm_kernels.cuh", "gm_device.cuh", "gm_prologue.cuh", "gm_boot.cuh"],
+    "gm_tc": ["gm_tc.cu", "gm_tc.cuh", "gm_device.cuh"],
+    "gm_tiles": ["gm_tiles.cu", "gm_fused.cuh", "gm_kernels.cuh", "gm_device.cuh"],
+}
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
@@ -55,9 +65,16 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
     def run(job):
         cmd, name = job
+        obj = Path(cmd[cmd.index("-o") + 1])
+        key = name.split()[0]
+        want = _stamp([CSRC / f for f in _DEPS[key]]) + " " + " ".join(cmd)
+        ostamp = obj.with_suffix(".stamp")
+        if not force and obj.exists() and ostamp.exists() and ostamp.read_text() == want:
+            return name
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {name}:\n{r.stdout}\n{r.stderr}")
+        ostamp.write_text(want)
         if verbose:
             print(f"[build] {name} ok", file=sys.stderr)
         return name

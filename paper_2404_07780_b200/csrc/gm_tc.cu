@@ -54,7 +54,7 @@ size_t table_bytes(int KP) {
 template <int KP>
 static int launch(const ConvArgs& a, const float* psf, long long psf_stride, int n_psf, int K, int flip, uint8_t* tab,
                   float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches) {
-  k_tc_btab<KP><<<n_psf, 256, 0, st>>>(psf, psf_stride, K, flip, tab, bscale);
+  k_tc_btab<KP><<<n_psf * KP, 256, 0, st>>>(psf, psf_stride, K, flip, tab, bscale);
   GM_TRY(cudaGetLastError());
   GM_TRY(set_smem_once((const void*)k_tc_conv<KP>, (int)Cfg<KP>::kSmem));
   const int grid = a.B < n_sm ? a.B : n_sm;

@@ -25,8 +25,8 @@
 //   warps 4-7   load cutout g+1 (global fp32 -> shared (hi, lo) fp16 pairs, one word per
 //               pixel), then drain the accumulators of cutout g (tcgen05.ld -> global)
 //   warps 0-3   window row y of every tile: LDS.128 -> PRMT -> tcgen05.st (3 row buffers)
-//   warp 10     streams the E_a of the tap rows into a ring with cp.async.bulk (TMA)
-//   warps 8-9   issue the MMAs (converged warp, one elected lane), accumulators r = 0,1 / 2,3
+//   warps 8-11  issue the MMAs (converged warp, one elected lane), one accumulator row each
+//   warp 12     streams the E_a of the tap rows into two rings with cp.async.bulk (TMA)
 // Measured issue rates (B200): one converged warp issues a 128 x 32 x 16 MMA every 16.0 clk,
 // the tensor-core floor for that shape.
 #pragma once
@@ -44,7 +44,8 @@ constexpr int kPitch = kSide + 28;          // words per image row in shared mem
 constexpr int kNBuf = 3;                    // window-row buffers in tensor memory
 constexpr int kRing = 5;                    // tap-row slots per ring; two rings (low / high tap rows)
 constexpr int kNSlot = 2 * kRing;
-constexpr int kThreads = 11 * 32;
+constexpr int kMmaWarps = 4;                // one accumulator row each
+constexpr int kThreads = (8 + kMmaWarps + 1) * 32;
 
 template <int KP> struct Cfg {
   static_assert(((KP - 1) / 2) % 4 == 0, "half width must be a multiple of 4 (16-byte window chunks)");
@@ -134,6 +135,14 @@ __device__ __forceinline__ void mma_commit(uint32_t bar) {
       "elect.sync _|q, 0xffffffff;\n\t"
       "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]),
                "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
@@ -183,14 +192,15 @@ __device__ __forceinline__ uint32_t split_pack(float x) {  // (hi, lo) fp16 pair
 
 // ---- E_a tables -----------------------------------------------------------------------
 // out[psf][a][part][kb][rho][e] (fp16) = part of s * Pf[a][8 kb + e - (rho - 16 (NCH - 1))], 0 outside the PSF;
-// Pf = the PSF flipped in both axes (flip != 0: true convolution) or as given (adjoint).  One CTA per PSF.
+// Pf = the PSF flipped in both axes (flip != 0: true convolution) or as given (adjoint).
 template <int KP>
 __global__ void __launch_bounds__(256) k_tc_btab(const float* __restrict__ psf, long long psf_stride, int K, int flip,
                                                  uint8_t* __restrict__ tab, float* __restrict__ bscale) {
   using C = Cfg<KP>;
   __shared__ float red[8];
   __shared__ float s_scale;
-  const float* p = psf + (long long)blockIdx.x * psf_stride;
+  const int ipsf = blockIdx.x / KP, a = blockIdx.x - ipsf * KP;   // one CTA per (PSF, tap row)
+  const float* p = psf + (long long)ipsf * psf_stride;
   const int off = (KP - K) / 2;                            // a smaller PSF sits in the middle of the KP x KP frame
   float amax = 0.0f;
   for (int i = threadIdx.x; i < K * K; i += 256) amax = fmaxf(amax, fabsf(p[i]));
@@ -201,22 +211,22 @@ __global__ void __launch_bounds__(256) k_tc_btab(const float* __restrict__ psf, 
     float m = 0.0f;
     for (int w = 0; w < 8; ++w) m = fmaxf(m, red[w]);
     s_scale = pow2_scale(m);
-    bscale[blockIdx.x] = 1.0f / s_scale;
+    if (a == 0) bscale[ipsf] = 1.0f / s_scale;
   }
   __syncthreads();
   const float s = s_scale;
-  __half* out = reinterpret_cast<__half*>(tab + (size_t)blockIdx.x * KP * C::kTapBytes);
-  const int per_a = C::kTapBytes / 2;                      // halves per tap row
-  for (int idx = threadIdx.x; idx < KP * per_a; idx += 256) {
-    const int a = idx / per_a;
-    int r = idx - a * per_a;
+  constexpr int per_a = C::kTapBytes / 2;                  // halves per tap row
+  __half* out = reinterpret_cast<__half*>(tab + ((size_t)ipsf * KP + a) * C::kTapBytes);
+  const int aa = (flip ? KP - 1 - a : a) - off;
+  for (int idx = threadIdx.x; idx < per_a; idx += 256) {
+    int r = idx;
     const int part = r / (2 * C::NR * 8); r -= part * (2 * C::NR * 8);
     const int kb = r / (C::NR * 8); r -= kb * (C::NR * 8);
     const int rho = r >> 3, e = r & 7;
     const int b = 8 * kb + e - (rho - 16 * (C::NCH - 1));
     float v = 0.0f;
     if (b >= 0 && b < KP) {
-      const int aa = (flip ? KP - 1 - a : a) - off, bb = (flip ? KP - 1 - b : b) - off;
+      const int bb = (flip ? KP - 1 - b : b) - off;
       if (aa >= 0 && aa < K && bb >= 0 && bb < K) v = p[aa * K + bb] * s;
     }
     const __half hi = __float2half_rn(v);
@@ -229,8 +239,8 @@ enum { IMG_FULL = 0, IMG_EMPTY = 2, A_FULL = 4, A_EMPTY = 4 + kNBuf, B_FULL = 4 
        D_FULL = B_EMPTY + kNSlot, D_EMPTY = D_FULL + 2, N_BARS = D_EMPTY + 2 };
 static_assert(N_BARS <= 64, "barrier area");
 
-// MMA issue of accumulators R0 and R0 + 1 (one converged warp)
-template <int KP, int R0>
+// MMA issue of accumulators R0 .. R0 + NACC - 1 (one converged warp)
+template <int KP, int R0, int NACC>
 __device__ __forceinline__ void mma_role(int dbg, int n_gal, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
   using C = Cfg<KP>;
   constexpr uint32_t idesc = instr_desc(128, kTileC);
@@ -251,7 +261,7 @@ __device__ __forceinline__ void mma_role(int dbg, int n_gal, uint32_t bars, uint
       fence_after();
       const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
 #pragma unroll
-      for (int rr = 0; rr < 2; ++rr) {
+      for (int rr = 0; rr < NACC; ++rr) {
         const int ta = y - (R0 + rr);                               // tap row
         if (ta < 0 || ta >= KP) continue;
         const int slot = C::slot_of(ta);
@@ -302,12 +312,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(IMG_FULL + i), 4); mbar_init(bar(IMG_EMPTY + i), 4); }
-    for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(A_FULL + i), 4); mbar_init(bar(A_EMPTY + i), 2); }
+    for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(A_FULL + i), 4); mbar_init(bar(A_EMPTY + i), kMmaWarps); }
     for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 4); }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(D_FULL + i), 2); mbar_init(bar(D_EMPTY + i), 4); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(D_FULL + i), kMmaWarps); mbar_init(bar(D_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (wid == 10) {
+  if (wid == 8 + kMmaWarps) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -327,8 +337,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
     int row_count = 0;
     for (int it = 0; it < n_gal; ++it) {
       const int s = it & 1;
-      const uint32_t* slot = slots + (size_t)s * C::kSlotWords;
-      const uint32_t* zero = slot + kSide * kPitch;
+      const uint32_t slot = smem_u32(slots + (size_t)s * C::kSlotWords);       // byte address in shared memory
+      const uint32_t zero = slot + 4u * (kSide * kPitch);
       mbar_wait(bar(IMG_FULL + s), (it >> 1) & 1);
       for (int i = 0; i < C::NY; ++i, ++row_count) {
         const int y = C::seq(i);
@@ -337,7 +347,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
         fence_after();
         const int R = 4 * lane + y - h;
         const bool row_ok = (unsigned)R < (unsigned)kSide;
-        const uint32_t* rowp = row_ok ? slot + R * kPitch + 4 * ((R >> 2) & 7) : zero;
+        const uint32_t rowp = row_ok ? slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7)) : zero;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           if (a.dbg & 2) break;
@@ -345,8 +355,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             const int c0 = 32 * wid - h + 16 * kc + 4 * q;
-            const uint32_t* p = (row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + c0 : zero;
-            const uint4 v = *reinterpret_cast<const uint4*>(p);
+            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 4u * (uint32_t)c0 : zero);
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
           uint32_t hi[8], lo[8];
@@ -396,16 +405,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
     for (int it = 0; it < n_gal; ++it) {
       const int s = it & 1;
       const int g = (int)blockIdx.x + it * (int)gridDim.x;
-      uint32_t* slot = slots + (size_t)s * C::kSlotWords;
+      const uint32_t slot = smem_u32(slots + (size_t)s * C::kSlotWords);
       mbar_wait(bar(IMG_EMPTY + s), ((it >> 1) & 1) ^ 1);
       // pass 1: global fp32 -> the slot (as fp32), and the largest magnitude of the cutout
       const float4* src = reinterpret_cast<const float4*>(a.in + (size_t)g * kSide * kSide);
       float amax = 0.0f;
 #pragma unroll 4
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
+        if (a.dbg & 32) break;
         const float4 v = __ldg(src + i);
         const int R = i >> 5, c = (i & 31) << 2;
-        *reinterpret_cast<float4*>(slot + R * kPitch + 4 * ((R >> 2) & 7) + c) = v;
+        sts128(slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c),
+               make_uint4(__float_as_uint(v.x), __float_as_uint(v.y), __float_as_uint(v.z), __float_as_uint(v.w)));
         amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
       }
       for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
@@ -417,10 +428,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
         if (a.dbg & 4) break;
         const int R = i >> 5, c = (i & 31) << 2;
-        uint4* p = reinterpret_cast<uint4*>(slot + R * kPitch + 4 * ((R >> 2) & 7) + c);
-        const uint4 v = *p;
-        *p = make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
-                        split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc));
+        const uint32_t p = slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c);
+        const uint4 v = lds128(p);
+        sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
+                             split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
       }
       asm volatile("bar.sync 1, 128;" ::: "memory");              // red_s may be rewritten after this
       if (ltid == 0) inv_scale_s[s] = 1.0f / sc;                     // read by drain(it), after the next bar.sync
@@ -432,12 +443,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       asm volatile("bar.sync 1, 128;" ::: "memory");              // inv_scale_s of the last cutout is visible
       drain(n_gal - 1);
     }
-  } else if (wid < 10) {
+  } else if (wid < 8 + kMmaWarps) {
     // ----------------------------------- MMA issue ------------------------------------
     // (the accumulator pair is a template argument so that every address of the issue loop is
     // warp-uniform at compile time and stays in uniform registers)
-    if (wid == 8) mma_role<KP, 0>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else mma_role<KP, 2>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
+    if (wid == 8) mma_role<KP, 0, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 9) mma_role<KP, 1, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 10) mma_role<KP, 2, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else mma_role<KP, 3, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
     // in the order of first use: window row y = seq(i) brings tap row y (r = 0) on the low side and
@@ -453,6 +467,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
           const int slot = C::slot_of(ta);
           const uint32_t gen = (uint32_t)(it * C::uses_of_slot(slot) + C::index_in_slot(ta));
           mbar_wait(bar(B_EMPTY + slot), (gen & 1) ^ 1);
+          if (a.dbg & 16) { mbar_arrive(bar(B_FULL + slot)); continue; }
           mbar_expect_tx(bar(B_FULL + slot), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(B_FULL + slot));
         }
@@ -461,7 +476,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
   }
   fence_before();
   __syncthreads();
-  if (wid == 10) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tm) : "memory");
+  if (wid == 8 + kMmaWarps) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tm) : "memory");
 }
 
 }  // namespace tc
