@@ -162,9 +162,13 @@ int gm_init(void* cuda_stream);
 /* Process-wide switches, for tests and measurements (value 0 / 1, default 1 each):
  *   GM_OPT_FUSED       cutouts up to 128 x 128 take the single fused kernel; 0: tile kernels
  *   GM_OPT_CONST_TAPS  a batch-wide PSF is read from the constant bank; 0: shared memory
- * Every setting gives bit for bit the same results.  gm_set_option returns GM_EINVAL for an
- * unknown option, gm_get_option -1. */
-enum { GM_OPT_FUSED = 0, GM_OPT_CONST_TAPS = 1, GM_OPT_COUNT_ = 2 };
+ *   GM_OPT_TENSOR      128 x 128 cutouts whose components all go through the PSF run both convolutions
+ *                      on the tensor cores (fp16 hi/lo split of the fp32 operands, see gm_conv); 0: the
+ *                      FP32 (FFMA2) convolution everywhere
+ * The first two give bit for bit the same results; GM_OPT_TENSOR changes the convolution arithmetic
+ * (pixels agree to a few 1e-6 relative, inside every documented tolerance).  gm_set_option returns
+ * GM_EINVAL for an unknown option, gm_get_option -1. */
+enum { GM_OPT_FUSED = 0, GM_OPT_CONST_TAPS = 1, GM_OPT_TENSOR = 2, GM_OPT_COUNT_ = 3 };
 int gm_set_option(int option, int value);
 int gm_get_option(int option);
 

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     GM_CONV_TENSOR,
     GM_OPT_CONST_TAPS,
     GM_OPT_FUSED,
+    GM_OPT_TENSOR,
     GmError,
     gm_get_option,
     gm_init,

@@ -20,7 +20,7 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libgm.so"
 
 GM_MAX_COMP, GM_MAX_PAR, GM_MAX_K, GM_NSLOT = 8, 32, 41, 10
-GM_OPT_FUSED, GM_OPT_CONST_TAPS = 0, 1
+GM_OPT_FUSED, GM_OPT_CONST_TAPS, GM_OPT_TENSOR = 0, 1, 2
 GM_CONV_FFMA2, GM_CONV_TENSOR = 0, 1
 _KINDS = {"sersic": 0, "expdisk": 1, "ferrer": 2, "king": 3, "gaussian": 4, "moffat": 5, "sky": 6}
 _SLOTS = ("xc", "yc", "theta", "q", "amp", "s0", "s1", "s2", "box", "m0")

@@ -44,8 +44,9 @@ def _stamp(files=None) -> str:
 
 # what each object is compiled from (an object is rebuilt only when one of these changed)
 _DEPS = {
-    "gm_api": ["gm_api.cu", "gm_fused.cuh", "gm_kernels.cuh", "gm_device.cuh", "gm_prologue.cuh", "gm_boot.cuh"],
-    "gm_tc": ["gm_tc.cu", "gm_tc.cuh", "gm_device.cuh"],
+    "gm_api": ["gm_api.cu", "gm_fused.cuh", "gm_kernels.cuh", "gm_device.cuh", "gm_prologue.cuh", "gm_boot.cuh",
+               "gm_tc.cuh", "gm_tc_fused.cuh"],
+    "gm_tc": ["gm_tc.cu", "gm_tc.cuh", "gm_tc_fused.cuh", "gm_kernels.cuh", "gm_device.cuh"],
     "gm_tiles": ["gm_tiles.cu", "gm_fused.cuh", "gm_kernels.cuh", "gm_device.cuh"],
 }
 

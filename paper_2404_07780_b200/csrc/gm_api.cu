@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "gm_fused.cuh"
+#include "gm_tc_fused.cuh"
 #include "gm_prologue.cuh"
 #include "gm_boot.cuh"
 
@@ -29,6 +30,18 @@ static thread_local int64_t t_launches = 0;
   } while (0)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+namespace tc {          // gm_tc.cu
+extern int g_tc_dbg;
+int padded_side(int K);
+size_t table_bytes(int KP);
+int conv(int KP, int B, const float* in, float* out, const float* psf, long long psf_stride, int K, int flip, uint8_t* tab,
+         float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches);
+int build_tables(int KP, const float* psf, long long psf_stride, int n_psf, int K, uint8_t* tab_fwd, uint8_t* tab_adj,
+                 float* bscale, cudaStream_t st, cudaError_t* err, int* launches);
+int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);
+}  // namespace tc
+
 
 // optional per-launch timing of the two tile kernels with CUDA events recorded on
 // the launching stream (gm_profile_enable / gm_profile_read); off by default
@@ -65,7 +78,7 @@ static void prof_end(int i, cudaStream_t st) {
 }
 
 // run-time options (gm_set_option): process-wide, read once per call
-static std::atomic<int> g_opt[GM_OPT_COUNT_] = {{1}, {1}};
+static std::atomic<int> g_opt[GM_OPT_COUNT_] = {{1}, {1}, {1}};
 
 // ---------------------------------------------------------------------------
 // nu_n table (gm_prologue.cuh): filled once per device BY A KERNEL on the stream of the
@@ -643,8 +656,15 @@ struct Workspace {
   float2* taps;
   float *u, *m, *s, *p_prev, *chi2_prev;
   int *calm, *frozen, *live, *n_live;
+  uint8_t *tc_fwd, *tc_adj;  // E_a tables of the tensor-core path (128 x 128 cutouts only)
+  float* tc_scale;
   size_t total;
 };
+
+// padded PSF side of the tensor-core path for this batch, or -1 when that path does not apply
+static int tc_side(const gm_batch* bt) {
+  return (bt->H == tc::kSide && bt->W == tc::kSide) ? tc::padded_side(bt->K) : -1;
+}
 
 static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int KP, const TileGeom& tg) {
   Workspace w;
@@ -671,6 +691,11 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   w.frozen = (int*)take(B * 4);
   w.live = (int*)take(B * 4);
   w.n_live = (int*)take(4);
+  const int KT = tc_side(bt);
+  const size_t tcb = KT > 0 ? n_psf * tc::table_bytes(KT) : 0;
+  w.tc_fwd = (uint8_t*)take(tcb);
+  w.tc_adj = (uint8_t*)take(tcb);
+  w.tc_scale = (float*)take(KT > 0 ? n_psf * 4 : 0);
   w.total = off;
   return w;
 }
@@ -727,13 +752,6 @@ static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
   return rc;
 }
 
-namespace tc {          // gm_tc.cu
-extern int g_tc_dbg;
-int padded_side(int K);
-size_t table_bytes(int KP);
-int conv(int KP, int B, const float* in, float* out, const float* psf, long long psf_stride, int K, int flip, uint8_t* tab,
-         float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches);
-}  // namespace tc
 
 static int dispatch_conv(int KP, const ConvTileArgs& a, int B, cudaStream_t st) {
   int rc;
@@ -833,6 +851,7 @@ struct Plan {
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int tiles;
   bool fused;                // whole cutouts per CTA and two slots fit: k_fused path
+  bool tc = false; int KT = -1;   // 128 x 128 cutouts, every component convolved: both convolutions on the tensor cores
   FusedGeom fg; int fused_variant;
   DevCaps caps;
   // lease of a region of the constant-bank tap pool (shared PSF only); handed back, by an event
@@ -920,6 +939,25 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
       pl->ct_stream = st;
     }
   }
+  // Tensor-core path (gm_tc_fused.cuh): 128 x 128 cutouts whose components all go through the PSF.  It
+  // needs the E_a tables of the PSF(s), forward and adjoint; the FFMA2 taps above stay available for the
+  // Jacobian columns of the covariance row.
+  pl->KT = tc_side(bt);
+  pl->tc = pl->KT > 0 && g_opt[GM_OPT_TENSOR].load() != 0;
+  for (int c = 0; c < pl->md.n_comp && pl->tc; ++c) pl->tc = pl->md.conv[c] != 0;
+  if (pl->tc) {
+    const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma;
+    if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = false;          // 128-bit row accesses
+  }
+  if (pl->tc) {
+    cudaError_t err = cudaSuccess;
+    int launches = 0;
+    rc = tc::build_tables(pl->KT, bt->psf, bt->psf_stride, bt->psf_stride == 0 ? 1 : bt->B, bt->K, pl->ws.tc_fwd, pl->ws.tc_adj,
+                          pl->ws.tc_scale, st, &err, &launches);
+    t_launches += launches;
+    if (rc == GM_ECUDA) t_last_err = err;
+    if (rc != GM_OK) return rc;
+  }
   // One cutout per slot (sides above 96) with the taps in shared memory (per-galaxy PSFs, or no
   // free region of the constant pool): k_fused and the tile kernels run the same loop at the
   // same rate (0.70 against 0.71 of the FP32 peak at 128 x 128, K = 25), but k_fused hands whole
@@ -991,9 +1029,28 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
   return a;
 }
 
+static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out, const LiveSet& ls, cudaStream_t st) {
+  tc::FusedTcArgs a;
+  a.md = pl.md; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
+  a.btab_fwd = pl.ws.tc_fwd; a.btab_adj = pl.ws.tc_adj;
+  a.btab_stride = bt->psf_stride == 0 ? 0 : (long long)tc::table_bytes(pl.KT);
+  a.bscale = pl.ws.tc_scale;
+  a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
+  a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+  a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
+  cudaError_t err = cudaSuccess;
+  const int pi = prof_begin(2, st);
+  const int rc = tc::launch_fused(pl.KT, a, pl.caps.n_sm, st, &err);
+  prof_end(pi, st);
+  if (rc == GM_OK) ++t_launches;
+  if (rc == GM_ECUDA) t_last_err = err;
+  return rc;
+}
+
 // one evaluation of every (non-frozen) galaxy: chi^2 partials and, if wanted, gradient partials
 static int run_eval(const Plan& pl, const gm_batch* bt, bool with_grad, const LiveSet& ls, cudaStream_t st) {
   int rc;
+  if (pl.tc) return dispatch_tc(pl, bt, with_grad ? 2 : 1, nullptr, ls, st);
   if (pl.fused)
     return dispatch_fused(pl.KP, fused_args(pl, bt, with_grad ? 2 : 1, pl.ws.G, ls), pl.fused_variant,
                           pl.caps.n_sm, pl.caps.smem_optin, st);
@@ -1108,6 +1165,7 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
   if (rc != GM_OK) return rc;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
+  if (pl.tc && (((uintptr_t)model_out & 15) == 0)) return dispatch_tc(pl, bt, 0, model_out, LiveSet{}, st);
   if (pl.fused)
     return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, LiveSet{}), pl.fused_variant, pl.caps.n_sm,
                           pl.caps.smem_optin, st);

@@ -1,6 +1,6 @@
 // gm_tc.cu -- launchers of the tensor-core convolution engine (gm_tc.cuh), one
 // instantiation per padded PSF side whose half width is a multiple of 4.
-#include "gm_tc.cuh"
+#include "gm_tc_fused.cuh"
 
 #include <mutex>
 #include <utility>
@@ -79,6 +79,44 @@ int conv(int KP, int B, const float* in, float* out, const float* psf, long long
     case 25: return launch<25>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
     case 33: return launch<33>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
     case 41: return launch<41>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
+    default: return GM_ENOTSUP;
+  }
+}
+
+// both E_a tables of every PSF (forward: flipped taps, adjoint: taps as given) and the PSF scales
+int build_tables(int KP, const float* psf, long long psf_stride, int n_psf, int K, uint8_t* tab_fwd, uint8_t* tab_adj,
+                 float* bscale, cudaStream_t st, cudaError_t* err, int* launches) {
+  switch (KP) {
+#define GM_TC_CASE(S)                                                                     \
+    case S:                                                                                 \
+      k_tc_btab<S><<<n_psf * S, 256, 0, st>>>(psf, psf_stride, K, 1, tab_fwd, bscale);      \
+      k_tc_btab<S><<<n_psf * S, 256, 0, st>>>(psf, psf_stride, K, 0, tab_adj, bscale);      \
+      break;
+    GM_TC_CASE(9) GM_TC_CASE(17) GM_TC_CASE(25) GM_TC_CASE(33) GM_TC_CASE(41)
+#undef GM_TC_CASE
+    default: return GM_ENOTSUP;
+  }
+  GM_TRY(cudaGetLastError());
+  *launches += 2;
+  return GM_OK;
+}
+
+template <int KP>
+static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  GM_TRY(set_smem_once((const void*)k_tc_fused<KP>, (int)FusedCfg<KP>::kSmem));
+  const int grid = a.B < n_sm ? a.B : n_sm;
+  k_tc_fused<KP><<<grid, kFusedThreadsTc, FusedCfg<KP>::kSmem, st>>>(a);
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
+int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  switch (KP) {
+    case 9: return launch_fused_t<9>(a, n_sm, st, err);
+    case 17: return launch_fused_t<17>(a, n_sm, st, err);
+    case 25: return launch_fused_t<25>(a, n_sm, st, err);
+    case 33: return launch_fused_t<33>(a, n_sm, st, err);
+    case 41: return launch_fused_t<41>(a, n_sm, st, err);
     default: return GM_ENOTSUP;
   }
 }

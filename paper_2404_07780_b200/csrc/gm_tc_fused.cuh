@@ -1,0 +1,460 @@
+// gm_tc_fused.cuh -- steps a1..a5 of the hot path for 128 x 128 cutouts with BOTH convolutions on the
+// tensor cores (the engine of gm_tc.cuh): one persistent CTA per SM, two cutouts in flight, nothing but
+// chi^2 and the kNSum partial sums per component leaving the SM (mode 0 writes the model image).
+//
+// Roles (17 warps, all hand-offs by mbarrier / named barrier):
+//   warps 0-3    window rows of the current job: shared memory -> tensor memory (A operand)
+//   warps 4-11   helpers: a1 render S into a slot, scale + split into (hi, lo) fp16 pairs; after the forward
+//                convolution drain M (tensor memory -> slot, fp32), a3 residual / chi^2 / G in place, scale +
+//                split G; after the adjoint convolution drain A, a5 gradient sums
+//   warps 12-15  MMA issue, one accumulator row of the 4 x 32 tiles each
+//   warp 16      streams the Toeplitz band blocks E_a (forward or adjoint table) through the two rings
+// A JOB is one convolution of one cutout.  Jobs run in the order C1(a) C1(b) C2(a) C2(b) (cutouts a, b in
+// slots 0, 1), so the helpers always work on the slot the tensor cores are not reading: the same
+// schedule as k_fused (gm_fused.cuh), with the FFMA2 loop replaced by tcgen05.mma.
+#pragma once
+#include "gm_kernels.cuh"
+#include "gm_tc.cuh"
+
+namespace gm {
+namespace tc {
+
+constexpr int kHelpWarpsTc = 8;
+constexpr int kFusedThreadsTc = (4 + kHelpWarpsTc + kMmaWarps + 1) * 32;     // 544
+constexpr int kHN = 32 * kHelpWarpsTc;
+
+struct FusedTcArgs {
+  ModelDesc md;
+  int B;
+  int mode;                  // 0 render (write M), 1 chi^2 only, 2 chi^2 + gradient
+  const CompConst* cc;
+  const uint8_t* btab_fwd; const uint8_t* btab_adj;   // E_a tables of the flipped PSF and of the PSF as given
+  long long btab_stride;     // bytes between the tables of consecutive galaxies (0: one PSF for the batch)
+  const float* bscale;       // [n_psf] 1 / (power-of-two scale of the PSF)
+  const float* data; const float* sigma; const uint8_t* mask;
+  float* out;                // mode 0: model image [B,128,128]
+  float* chi2_part;          // [B]
+  float* grad_part;          // [B, n_comp, kNSum]
+  const int* frozen;
+  const int* live; const int* n_live;
+};
+
+enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kNSlot,
+       F_N_BARS = F_B_EMPTY + kNSlot };
+static_assert(F_N_BARS <= 64, "barrier area");
+
+template <int KP> struct FusedCfg {
+  using C = Cfg<KP>;
+  // [1 KB: barriers, tensor-memory address, reduction scratch | tap-row rings | 2 slots]
+  static constexpr size_t kSmem = 1024 + 1024 + (size_t)kNSlot * C::kTapBytes + 2 * (size_t)C::kSlotWords * 4;
+};
+
+// the jobs of one CTA in tensor-core order; f(item, phase, slot)
+template <typename F>
+__device__ __forceinline__ void for_each_job(int n_items, int phases, F&& f) {
+  for (int m = 0; 2 * m < n_items; ++m)
+    for (int ph = 0; ph < phases; ++ph)
+      for (int s = 0; s < 2; ++s) {
+        const int item = 2 * m + s;
+        if (item < n_items) f(item, ph, s);
+      }
+}
+
+// MMA issue of accumulator row R0 for every job (one converged warp)
+template <int KP, int R0>
+__device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
+  using C = Cfg<KP>;
+  constexpr uint32_t idesc = instr_desc(128, kTileC);
+  constexpr uint32_t desc_hi = (uint32_t)(smem_desc(0, C::NR * 16, 128) >> 32);
+  constexpr uint32_t desc_lo0 = (uint32_t)(smem_desc(0, C::NR * 16, 128) & 0xffffffffu);
+  auto bar = [&](int i) -> uint32_t { return bars + 8u * (uint32_t)i; };
+  int row_count = 0, jc = 0;
+  for_each_job(n_items, phases, [&](int, int, int s) {
+    uint32_t started = 0;
+    const uint32_t dcol = tD + (uint32_t)(s * C::kDCols + R0 * kTileC);
+#pragma unroll 1
+    for (int i = 0; i < C::NY; ++i, ++row_count) {
+      const int y = C::seq(i);
+      const int buf = row_count % kNBuf;
+      mbar_wait(bar(F_A_FULL + buf), (row_count / kNBuf) & 1);
+      fence_after();
+      const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
+      const int ta = y - R0;
+      if (ta >= 0 && ta < KP) {
+        const int slot = C::slot_of(ta);
+        mbar_wait(bar(F_B_FULL + slot), (uint32_t)(jc * C::uses_of_slot(slot) + C::index_in_slot(ta)) & 1);
+        fence_after();
+        const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
+#pragma unroll
+        for (int kc = 0; kc < C::NCH; ++kc) {
+          const uint32_t b_hi = lo0 + (uint32_t)(16 * (C::NCH - 1 - kc));
+          const uint32_t b_lo = b_hi + (uint32_t)(2 * C::NR);
+          mma_f16_ts2(dcol, acol + kc * 16, b_hi, desc_hi, idesc, kc ? 1u : started);    // hi * hi (the first MMA overwrites)
+          mma_f16_ts2(dcol, acol + kc * 16 + 8, b_hi, desc_hi, idesc, 1);                 // lo * hi
+          mma_f16_ts2(dcol, acol + kc * 16, b_lo, desc_hi, idesc, 1);                     // hi * lo
+        }
+        started = 1;
+        mma_commit(bar(F_B_EMPTY + slot));
+      }
+      mma_commit(bar(F_A_EMPTY + buf));
+    }
+    mma_commit(bar(F_D_FULL + s));
+    ++jc;
+  });
+}
+
+template <int KP>
+__global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcArgs a) {
+  using C = Cfg<KP>;
+  constexpr int h = C::h;
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(base);
+  uint32_t* tmem_base_s = reinterpret_cast<uint32_t*>(base + 512);
+  float* red = reinterpret_cast<float*>(base + 528);                // [kHelpWarpsTc * kNSum] sums, then [8] maxima
+  float* redmax = red + kHelpWarpsTc * kNSum;
+  unsigned char* ring = base + 1024;
+  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)kNSlot * C::kTapBytes);
+  static_assert(528 + (kHelpWarpsTc * kNSum + 8) * 4 <= 1024, "header area");
+  auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
+
+  const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
+  if (tid == 0) {
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
+    for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
+    for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
+  if (wid == kLastWarp) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int i = tid; i < 2 * C::kSlotWords; i += kFusedThreadsTc) slots[i] = 0u;    // zero rows (and skew gaps)
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tm = __shfl_sync(0xffffffffu, *tmem_base_s, 0);
+  const uint32_t tD = tm, tA = tm + 2 * C::kDCols;
+
+  const bool with_grad = a.mode == 2;
+  const int phases = with_grad ? 2 : 1;
+  const int n_gal = a.live ? *a.n_live : a.B;
+  const int n_items = (n_gal - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  auto galaxy = [&](int item) -> int {                     // -1: a galaxy that no longer iterates
+    const int i = (int)blockIdx.x + item * (int)gridDim.x;
+    const int b = a.live ? a.live[i] : i;
+    return (a.frozen && a.frozen[b]) ? -1 : b;
+  };
+
+  if (wid < 4) {
+    // ------------------------- window rows -> tensor memory --------------------------
+    const uint32_t lane_base = (uint32_t)(32 * wid) << 16;
+    int row_count = 0, cnt[2] = {0, 0};
+    for_each_job(n_items, phases, [&](int, int, int s) {
+      const uint32_t slot = smem_u32(slots + (size_t)s * C::kSlotWords);
+      const uint32_t zero = slot + 4u * (kSide * kPitch);
+      mbar_wait(bar(F_IN_FULL + s), cnt[s] & 1);
+      ++cnt[s];
+      for (int i = 0; i < C::NY; ++i, ++row_count) {
+        const int y = C::seq(i);
+        const int buf = row_count % kNBuf;
+        mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
+        fence_after();
+        const int R = 4 * lane + y - h;
+        const bool row_ok = (unsigned)R < (unsigned)kSide;
+        const uint32_t rowp = row_ok ? slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7)) : zero;
+#pragma unroll
+        for (int kc = 0; kc < C::NCH; ++kc) {
+          uint32_t w[16];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int c0 = 32 * wid - h + 16 * kc + 4 * q;
+            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 4u * (uint32_t)c0 : zero);
+            w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+          }
+          uint32_t hi[8], lo[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            hi[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x5410);
+            lo[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x7632);
+          }
+          const uint32_t col = tA + (uint32_t)(buf * C::kACols + kc * 16) + lane_base;
+          tmem_st8(col, hi);
+          tmem_st8(col + 8, lo);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(F_A_FULL + buf));
+      }
+    });
+  } else if (wid < 4 + kHelpWarpsTc) {
+    // ------------------------------------ helpers -------------------------------------
+    const int hw = wid - 4, htid = tid - 128;
+    const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
+    float inv_sc[2] = {1.0f, 1.0f};                       // 1 / scale of what is in slot s (every thread holds the same)
+    int cnt_d[2] = {0, 0};
+    auto slot_addr = [&](int s) -> uint32_t { return smem_u32(slots + (size_t)s * C::kSlotWords); };
+    auto px_addr = [&](uint32_t slot, int R, int c) -> uint32_t {
+      return slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c);
+    };
+    auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
+    constexpr int kGroups = kSide * kSide / 4;            // groups of four pixels of a row; a warp walks one row at a time
+
+    // fp32 values in the slot -> (hi, lo) fp16 pairs of value * 2^e, e from the largest magnitude `amax`
+    // (every thread passes its own maximum; converts the groups it owns)
+    auto scale_and_split = [&](uint32_t slot, float amax) -> float {
+      for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      if (lane == 0) redmax[hw] = amax;
+      help_sync();
+      float m = redmax[0];
+#pragma unroll
+      for (int w = 1; w < kHelpWarpsTc; ++w) m = fmaxf(m, redmax[w]);
+      const float sc = pow2_scale(m);
+#pragma unroll 2
+      for (int idx = htid; idx < kGroups; idx += kHN) {
+        const uint32_t p = px_addr(slot, idx >> 5, (idx & 31) << 2);
+        const uint4 v = lds128(p);
+        sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
+                             split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
+      }
+      help_sync();                                         // redmax may be rewritten
+      return 1.0f / sc;
+    };
+    auto signal_input = [&](int s) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(F_IN_FULL + s));
+    };
+
+    // a1: S of the cutout (all components go through the PSF on this path) -> slot s
+    auto produce = [&](int item, int s) {
+      const int b = galaxy(item);
+      const uint32_t slot = slot_addr(s);
+      float amax = 0.0f;
+      if (b >= 0) {
+        const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+        for (int c = 0; c < a.md.n_comp; ++c) {
+          const CompConst cc = ccb[c];
+          const bool box = a.md.box[c] != 0;
+          const bool first = c == 0, last = c == a.md.n_comp - 1;
+          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+            for (int idx = htid; idx < kGroups; idx += kHN) {
+              const int R = idx >> 5, x = (idx & 31) << 2;
+              float v[4];
+              value4<KIND, kFastForward>(cc, box, (float)x + 0.5f, (float)kSide - 0.5f - (float)R, v);   // R:G1
+              const uint32_t p = px_addr(slot, R, x);
+              if (!first) {
+                const uint4 q = lds128(p);
+                v[0] += __uint_as_float(q.x); v[1] += __uint_as_float(q.y); v[2] += __uint_as_float(q.z); v[3] += __uint_as_float(q.w);
+              }
+              if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
+              sts128(p, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
+            }
+          });
+        }
+      } else {
+        for (int idx = htid; idx < kGroups; idx += kHN) sts128(px_addr(slot, idx >> 5, (idx & 31) << 2), make_uint4(0u, 0u, 0u, 0u));
+      }
+      inv_sc[s] = scale_and_split(slot, amax);
+      signal_input(s);
+    };
+
+    // accumulators of the job on slot s -> the slot, as fp32 (tile m = lane m: rows 4 t + r, columns 32 q ..)
+    auto drain = [&](int item, int s) {
+      const int b = galaxy(item);
+      const uint32_t slot = slot_addr(s);
+      mbar_wait(bar(F_D_FULL + s), cnt_d[s] & 1);
+      ++cnt_d[s];
+      fence_after();
+      const float inv = inv_sc[s] * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
+      const int q = hw & 3, r_first = 2 * (hw >> 2);
+#pragma unroll 1
+      for (int r = r_first; r < r_first + 2; ++r) {
+        uint32_t v[32];
+        tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        const uint32_t p = px_addr(slot, 4 * lane + r, 32 * q);
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+          sts128(p + 16u * k, make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+                                         __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
+      }
+      fence_before();
+      help_sync();                                         // the whole image is in the slot
+    };
+
+    // a3: M (slot, fp32) -> chi^2 and G in place, then G as fp16 pairs for the adjoint convolution; mode 0 writes M out
+    auto residual = [&](int item, int s) {
+      const int b = galaxy(item);
+      const uint32_t slot = slot_addr(s);
+      float chi2 = 0.0f, amax = 0.0f;
+      if (b >= 0) {
+        const size_t img = (size_t)b * kSide * kSide;
+        if (a.mode == 0) {
+          for (int idx = htid; idx < kGroups; idx += kHN) {
+            const uint4 v = lds128(px_addr(slot, idx >> 5, (idx & 31) << 2));
+            *reinterpret_cast<float4*>(a.out + img + 4 * (size_t)idx) =
+                make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
+          }
+        } else {
+          // branch free; the weight and the residual are SELECTED for unused pixels, never multiplied by 0 (R:X1)
+          auto one = [&](float m, float d, float sg, bool used) -> float {
+            float w = rcp_fast(sg * sg), rho = d - m;
+            w = used ? w : 0.0f;
+            rho = used ? rho : 0.0f;
+            const float t = w * rho;
+            chi2 = fmaf(t, rho, chi2);
+            const float g = -2.0f * t;
+            amax = fmaxf(amax, fabsf(g));
+            return g;
+          };
+          const float4* dptr = reinterpret_cast<const float4*>(a.data + img);
+          const float4* sptr = reinterpret_cast<const float4*>(a.sigma + img);
+          auto pass = [&]<bool MASKED>() {
+            const uchar4* kptr = MASKED ? reinterpret_cast<const uchar4*>(a.mask + img) : nullptr;
+#pragma unroll 2
+            for (int idx = htid; idx < kGroups; idx += kHN) {
+              const uint32_t p = px_addr(slot, idx >> 5, (idx & 31) << 2);
+              const float4 d4 = dptr[idx], s4 = sptr[idx];
+              uchar4 k4 = make_uchar4(1, 1, 1, 1);
+              if (MASKED) k4 = kptr[idx];
+              const uint4 m4 = lds128(p);
+              uint4 g;
+              g.x = __float_as_uint(one(__uint_as_float(m4.x), d4.x, s4.x, !MASKED || k4.x != 0));
+              g.y = __float_as_uint(one(__uint_as_float(m4.y), d4.y, s4.y, !MASKED || k4.y != 0));
+              g.z = __float_as_uint(one(__uint_as_float(m4.z), d4.z, s4.z, !MASKED || k4.z != 0));
+              g.w = __float_as_uint(one(__uint_as_float(m4.w), d4.w, s4.w, !MASKED || k4.w != 0));
+              if (with_grad) sts128(p, g);
+            }
+          };
+          if (a.mask) pass.template operator()<true>();
+          else pass.template operator()<false>();
+        }
+      }
+      if (a.mode != 0) {
+        chi2 = warp_sum(chi2);
+        if (lane == 0) red[hw] = chi2;
+        if (!isfinite(amax)) amax = 0.0f;                  // a non-finite chi^2 is reported through chi2_part; keep the scale sane
+        if (with_grad) {
+          inv_sc[s] = scale_and_split(slot_addr(s), amax); // its first barrier also publishes red[]
+        } else {
+          help_sync();
+        }
+        if (htid == 0 && b >= 0) {
+          float t = 0.0f;
+          for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
+          a.chi2_part[b] = t;
+        }
+        help_sync();                                       // red[] may be rewritten
+      }
+    };
+
+    // a5: the partial sums of every component from A (slot, fp32)
+    auto gradient = [&](int item, int s) {
+      const int b = galaxy(item);
+      const uint32_t slot = slot_addr(s);
+      for (int c = 0; c < a.md.n_comp; ++c) {
+        float sm[kNSum];
+#pragma unroll
+        for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
+        if (b >= 0) {
+          const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
+          const bool box = a.md.box[c] != 0;
+          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+            if (box) {                                     // Eq. 2 with B != 0: per-pixel geometry
+              for (int idx = htid; idx < kGroups; idx += kHN) {
+                const int R = idx >> 5, x = (idx & 31) << 2;
+                const uint4 q = lds128(px_addr(slot, R, x));
+                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                  grad_accumulate<KIND>(cc, true, seed[k], (float)(x + k) + 0.5f, (float)kSide - 0.5f - (float)R, sm);
+              }
+            } else {
+              GradAcc<KIND> acc;
+              acc.init();
+              for (int idx = htid; idx < kGroups; idx += kHN) {
+                const int R = idx >> 5, x = (idx & 31) << 2;
+                const uint4 q = lds128(px_addr(slot, R, x));
+                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+                grad_add4<KIND>(acc, cc, seed, (float)x + 0.5f, (float)kSide - 0.5f - (float)R);
+              }
+              acc.finish(cc, sm);
+            }
+          });
+          if (!box) sm[8] = sm[2];
+        }
+#pragma unroll
+        for (int k = 0; k < kNSum; ++k) {
+          const float v = warp_sum(sm[k]);
+          if (lane == 0) red[hw * kNSum + k] = v;
+        }
+        help_sync();
+        if (htid < kNSum && b >= 0) {
+          float t = 0.0f;
+          for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
+          a.grad_part[((size_t)b * a.md.n_comp + c) * kNSum + htid] = t;
+        }
+        help_sync();
+      }
+    };
+
+    auto feed = [&](int item, int s) { if (item < n_items) produce(item, s); };
+    feed(0, 0);
+    feed(1, 1);
+    for (int m = 0; 2 * m < n_items; ++m) {
+      for (int s = 0; s < 2; ++s) {                       // after C1: residual
+        const int item = 2 * m + s;
+        if (item >= n_items) continue;
+        drain(item, s);
+        residual(item, s);
+        if (with_grad) signal_input(s);                    // G is in place: the adjoint convolution may start
+        else feed(item + 2, s);
+      }
+      if (with_grad) {
+        for (int s = 0; s < 2; ++s) {                     // after C2: gradient, then the next cutout
+          const int item = 2 * m + s;
+          if (item >= n_items) continue;
+          drain(item, s);
+          gradient(item, s);
+          feed(item + 2, s);
+        }
+      }
+    }
+  } else if (wid < kLastWarp) {
+    // ----------------------------------- MMA issue ------------------------------------
+    static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
+    const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2>(n_items, phases, b0, r0, tD, tA);
+    else fused_mma_role<KP, 3>(n_items, phases, b0, r0, tD, tA);
+  } else {
+    // ------------------------------- tap-row producer --------------------------------
+    if (lane == 0) {
+      int jc = 0;
+      for_each_job(n_items, phases, [&](int item, int ph, int) {
+        const int b = galaxy(item);
+        const uint8_t* tab = (ph ? a.btab_adj : a.btab_fwd) + (size_t)(b >= 0 ? b : 0) * a.btab_stride;
+        for (int i = 0; i < C::NY; ++i) {
+          const int y = C::seq(i);
+          const int ta = (i & 1) ? y - (kTileR - 1) : y;
+          if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
+          const int slot = C::slot_of(ta);
+          const uint32_t gen = (uint32_t)(jc * C::uses_of_slot(slot) + C::index_in_slot(ta));
+          mbar_wait(bar(F_B_EMPTY + slot), (gen & 1) ^ 1);
+          mbar_expect_tx(bar(F_B_FULL + slot), C::kTapBytes);
+          bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + slot));
+        }
+        ++jc;
+      });
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (wid == kLastWarp) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tm) : "memory");
+}
+
+}  // namespace tc
+}  // namespace gm

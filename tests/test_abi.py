@@ -59,7 +59,7 @@ def test_validation_codes_without_gpu():
 def test_options_and_init_entry_points(lib):
     # gm_set_option / gm_get_option replace the environment-variable hooks of round 1
     lib.gm_set_option.restype = C.c_int; lib.gm_get_option.restype = C.c_int
-    for opt in (0, 1):
+    for opt in (0, 1, 2):
         assert lib.gm_get_option(opt) == 1
         assert lib.gm_set_option(opt, 0) == 0 and lib.gm_get_option(opt) == 0
         assert lib.gm_set_option(opt, 7) == 0 and lib.gm_get_option(opt) == 1

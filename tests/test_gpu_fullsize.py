@@ -23,7 +23,17 @@ def _loss_grad(b):
     return chi2.cpu().numpy(), grad.cpu().numpy()
 
 
-def test_c1_full_batch_loss_grad_every_galaxy():
+@pytest.fixture(params=["tensor", "ffma2"])
+def engine(request):
+    """128 x 128 cutouts run both convolutions on the tensor cores by default (gm_tc_fused.cuh);
+    gm_set_option(GM_OPT_TENSOR, 0) keeps them on the FP32 FFMA2 path (k_fused).  Both must meet the
+    tolerances."""
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 1 if request.param == "tensor" else 0)
+    yield request.param
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
+
+
+def test_c1_full_batch_loss_grad_every_galaxy(engine):
     # C1 as bench.py runs it: B = 1024, 128x128, K = 25, one gm_loss_grad call
     b = configs.make_batch(1, range(1024), oracle_render)
     chi2, grad = _loss_grad(b)
@@ -73,7 +83,7 @@ def test_c2_buckets_masked(side):
     assert_grad(grad, og)
 
 
-def test_c3_bulge_disk_full_batch():
+def test_c3_bulge_disk_full_batch(engine):
     # C3: B = 4096, P = 11; data for all galaxies from the oracle, gradient checked on a sample
     b = configs.make_batch(3, range(4096), oracle_render)
     chi2, grad = _loss_grad(b)
