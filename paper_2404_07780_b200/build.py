@@ -20,6 +20,7 @@ LIB = PKG / "libgm.so"
 INCLUDE = PKG.parent / "include"
 
 KS = (5, 9, 15, 21, 25, 33, 41)          # keep in sync with kCompiledK in gm_api.cu
+TC_KS = (9, 17, 25, 33, 41)              # tensor-core engine: padded sides with (K - 1) / 2 a multiple of 4
 EXTRA = os.environ.get("GM_NVCC_EXTRA", "").split()
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++20",
               "-Xcompiler", "-fPIC", *EXTRA]
@@ -59,7 +60,9 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     nvcc = _nvcc()
     jobs = [([nvcc, *NVCC_FLAGS, "-c", str(CSRC / "gm_api.cu"), "-o", str(OBJ / "gm_api.o")], "gm_api")]
-    jobs.append(([nvcc, *NVCC_FLAGS, f"-I{INCLUDE}", "-c", str(CSRC / "gm_tc.cu"), "-o", str(OBJ / "gm_tc.o")], "gm_tc"))
+    for k in TC_KS:
+        jobs.append(([nvcc, *NVCC_FLAGS, f"-I{INCLUDE}", f"-DGM_TC_K={k}", "-c", str(CSRC / "gm_tc.cu"),
+                      "-o", str(OBJ / f"gm_tc_{k}.o")], f"gm_tc K={k}"))
     for k in KS:
         jobs.append(([nvcc, *NVCC_FLAGS, f"-DGM_K={k}", "-c", str(CSRC / "gm_tiles.cu"),
                       "-o", str(OBJ / f"gm_tiles_{k}.o")], f"gm_tiles K={k}"))
@@ -82,7 +85,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
         list(ex.map(run, jobs))
-    objs = [str(OBJ / "gm_api.o"), str(OBJ / "gm_tc.o")] + [str(OBJ / f"gm_tiles_{k}.o") for k in KS]
+    objs = [str(OBJ / "gm_api.o")] + [str(OBJ / f"gm_tc_{k}.o") for k in TC_KS] + [str(OBJ / f"gm_tiles_{k}.o") for k in KS]
     tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
     r = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *objs],
                        capture_output=True, text=True)

@@ -31,15 +31,65 @@ static thread_local int64_t t_launches = 0;
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-namespace tc {          // gm_tc.cu
-extern int g_tc_dbg;
-int padded_side(int K);
-size_t table_bytes(int KP);
-int conv(int KP, int B, const float* in, float* out, const float* psf, long long psf_stride, int K, int flip, uint8_t* tab,
-         float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches);
-int build_tables(int KP, const float* psf, long long psf_stride, int n_psf, int K, uint8_t* tab_fwd, uint8_t* tab_adj,
-                 float* bscale, cudaStream_t st, cudaError_t* err, int* launches);
-int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);
+namespace tc {          // gm_tc.cu, one object per padded PSF side
+#define GM_DECL_TC(K)                                                                                                   \
+  size_t table_bytes_##K();                                                                                             \
+  int build_table_##K(const float* psf, long long psf_stride, int n_psf, int Kin, int flip, uint8_t* tab, float* bscale, \
+                      cudaStream_t st, cudaError_t* err);                                                              \
+  int launch_conv_tc_##K(const ConvArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);                               \
+  int launch_fused_tc_##K(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);                           \
+  int launch_tile_tc_##K(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err);
+GM_DECL_TC(9) GM_DECL_TC(17) GM_DECL_TC(25) GM_DECL_TC(33) GM_DECL_TC(41)
+#undef GM_DECL_TC
+
+#define GM_TC_SWITCH(KP, CALL)       \
+  switch (KP) {                      \
+    case 9: return CALL(9);          \
+    case 17: return CALL(17);        \
+    case 25: return CALL(25);        \
+    case 33: return CALL(33);        \
+    case 41: return CALL(41);        \
+    default: break;                  \
+  }
+
+static int padded_side(int K) {
+  static const int sides[] = {9, 17, 25, 33, 41};
+  for (int s : sides)
+    if (K <= s) return s;
+  return -1;
+}
+static size_t table_bytes(int KP) {
+#define GM_C(K) table_bytes_##K()
+  GM_TC_SWITCH(KP, GM_C)
+#undef GM_C
+  return 0;
+}
+static int build_table(int KP, const float* psf, long long psf_stride, int n_psf, int K, int flip, uint8_t* tab, float* bscale,
+                       cudaStream_t st, cudaError_t* err) {
+#define GM_C(S) build_table_##S(psf, psf_stride, n_psf, K, flip, tab, bscale, st, err)
+  GM_TC_SWITCH(KP, GM_C)
+#undef GM_C
+  return GM_ENOTSUP;
+}
+static int launch_conv(int KP, const ConvArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+#define GM_C(S) launch_conv_tc_##S(a, n_sm, st, err)
+  GM_TC_SWITCH(KP, GM_C)
+#undef GM_C
+  return GM_ENOTSUP;
+}
+static int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+#define GM_C(S) launch_fused_tc_##S(a, n_sm, st, err)
+  GM_TC_SWITCH(KP, GM_C)
+#undef GM_C
+  return GM_ENOTSUP;
+}
+static int launch_tile(int KP, const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err) {
+#define GM_C(S) launch_tile_tc_##S(a, trb, bwd, n_sm, st, err)
+  GM_TC_SWITCH(KP, GM_C)
+#undef GM_C
+  return GM_ENOTSUP;
+}
+static bool has_tile_kernels(int KP) { return KP == 25 || KP == 41; }
 }  // namespace tc
 
 
@@ -661,9 +711,27 @@ struct Workspace {
   size_t total;
 };
 
-// padded PSF side of the tensor-core path for this batch, or -1 when that path does not apply
-static int tc_side(const gm_batch* bt) {
-  return (bt->H == tc::kSide && bt->W == tc::kSide) ? tc::padded_side(bt->K) : -1;
+// Super-tiles of the tensor-core tile kernels for an H x W cutout: 128 lanes of 4 x 32 pixels arranged as
+// trb x (128 / trb) tiles (128 x 128, 64 x 256 or 256 x 64 pixels), whichever covers the cutout with the fewest.
+static void tc_tile_geom(int H, int W, int* trb, int* tx, int* ty) {
+  static const int cand[3] = {32, 16, 64};
+  long long best = -1;
+  for (int c : cand) {
+    const int TH = tc::kTileR * c, TW = tc::kTileC * (128 / c);
+    const int ny = (H + TH - 1) / TH, nx = (W + TW - 1) / TW;
+    if (best < 0 || (long long)nx * ny < best) { best = (long long)nx * ny; *trb = c; *tx = nx; *ty = ny; }
+  }
+}
+
+// which tensor-core path the SHAPE of the batch allows (the model and the options decide later):
+// 1 = k_tc_fused (128 x 128), 2 = k_tc_tile (larger, W a multiple of 4, PSF side with tile kernels), 0 = none;
+// *KT = padded PSF side of that engine
+static int tc_kind(const gm_batch* bt, int* KT) {
+  *KT = tc::padded_side(bt->K);
+  if (*KT < 0) return 0;
+  if (bt->H == tc::kSide && bt->W == tc::kSide) return 1;
+  if ((bt->H > tc::kSide || bt->W > tc::kSide) && (bt->W & 3) == 0 && tc::has_tile_kernels(*KT)) return 2;
+  return 0;
 }
 
 static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int KP, const TileGeom& tg) {
@@ -674,7 +742,15 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
     off += align_up(bytes, 256);
     return p;
   };
-  const size_t B = bt->B, P = md.n_par, tiles = (size_t)tg.tiles_x * tg.tiles_y;
+  const size_t B = bt->B, P = md.n_par;
+  size_t tiles = (size_t)tg.tiles_x * tg.tiles_y;
+  int KT = -1;
+  const int tck = tc_kind(bt, &KT);
+  if (tck == 2) {                                          // the tensor-core tile kernels may cut the cutout differently
+    int trb, tx, ty;
+    tc_tile_geom(bt->H, bt->W, &trb, &tx, &ty);
+    if ((size_t)tx * ty > tiles) tiles = (size_t)tx * ty;
+  }
   w.cc = (CompConst*)take(B * md.n_comp * sizeof(CompConst));
   w.G = (float*)take(B * bt->H * bt->W * 4);
   w.chi2_part = (float*)take(B * tiles * 4);
@@ -691,11 +767,10 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   w.frozen = (int*)take(B * 4);
   w.live = (int*)take(B * 4);
   w.n_live = (int*)take(4);
-  const int KT = tc_side(bt);
-  const size_t tcb = KT > 0 ? n_psf * tc::table_bytes(KT) : 0;
+  const size_t tcb = tck ? n_psf * tc::table_bytes(KT) : 0;
   w.tc_fwd = (uint8_t*)take(tcb);
   w.tc_adj = (uint8_t*)take(tcb);
-  w.tc_scale = (float*)take(KT > 0 ? n_psf * 4 : 0);
+  w.tc_scale = (float*)take(tck ? n_psf * 4 : 0);
   w.total = off;
   return w;
 }
@@ -851,7 +926,8 @@ struct Plan {
   const float2* taps_fwd; const float2* taps_adj; long long taps_stride;
   int tiles;
   bool fused;                // whole cutouts per CTA and two slots fit: k_fused path
-  bool tc = false; int KT = -1;   // 128 x 128 cutouts, every component convolved: both convolutions on the tensor cores
+  int tc = 0; int KT = -1;        // tensor-core path: 1 = k_tc_fused (128 x 128), 2 = k_tc_tile (larger cutouts), 0 = none
+  int tc_trb = 32, tc_tx = 1, tc_ty = 1;
   FusedGeom fg; int fused_variant;
   DevCaps caps;
   // lease of a region of the constant-bank tap pool (shared PSF only); handed back, by an event
@@ -942,21 +1018,25 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   // Tensor-core path (gm_tc_fused.cuh): 128 x 128 cutouts whose components all go through the PSF.  It
   // needs the E_a tables of the PSF(s), forward and adjoint; the FFMA2 taps above stay available for the
   // Jacobian columns of the covariance row.
-  pl->KT = tc_side(bt);
-  pl->tc = pl->KT > 0 && g_opt[GM_OPT_TENSOR].load() != 0;
-  for (int c = 0; c < pl->md.n_comp && pl->tc; ++c) pl->tc = pl->md.conv[c] != 0;
+  pl->tc = g_opt[GM_OPT_TENSOR].load() != 0 ? tc_kind(bt, &pl->KT) : 0;
+  for (int c = 0; c < pl->md.n_comp && pl->tc; ++c)
+    if (pl->md.conv[c] == 0) pl->tc = 0;
   if (pl->tc) {
     const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma;
-    if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = false;          // 128-bit row accesses
+    if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = 0;              // 128-bit row accesses
   }
   if (pl->tc) {
     cudaError_t err = cudaSuccess;
-    int launches = 0;
-    rc = tc::build_tables(pl->KT, bt->psf, bt->psf_stride, bt->psf_stride == 0 ? 1 : bt->B, bt->K, pl->ws.tc_fwd, pl->ws.tc_adj,
-                          pl->ws.tc_scale, st, &err, &launches);
-    t_launches += launches;
+    const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
+    rc = tc::build_table(pl->KT, bt->psf, bt->psf_stride, n_psf, bt->K, 1, pl->ws.tc_fwd, pl->ws.tc_scale, st, &err);
+    if (rc == GM_OK) rc = tc::build_table(pl->KT, bt->psf, bt->psf_stride, n_psf, bt->K, 0, pl->ws.tc_adj, pl->ws.tc_scale, st, &err);
+    t_launches += 2;
     if (rc == GM_ECUDA) t_last_err = err;
     if (rc != GM_OK) return rc;
+    if (pl->tc == 2) {                                     // the partial sums are per super-tile on this path
+      tc_tile_geom(bt->H, bt->W, &pl->tc_trb, &pl->tc_tx, &pl->tc_ty);
+      pl->tiles = pl->tc_tx * pl->tc_ty;
+    }
   }
   // One cutout per slot (sides above 96) with the taps in shared memory (per-galaxy PSFs, or no
   // free region of the constant pool): k_fused and the tile kernels run the same loop at the
@@ -1030,19 +1110,39 @@ static FusedArgs fused_args(const Plan& pl, const gm_batch* bt, int mode, float*
 }
 
 static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out, const LiveSet& ls, cudaStream_t st) {
-  tc::FusedTcArgs a;
-  a.md = pl.md; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
-  a.btab_fwd = pl.ws.tc_fwd; a.btab_adj = pl.ws.tc_adj;
-  a.btab_stride = bt->psf_stride == 0 ? 0 : (long long)tc::table_bytes(pl.KT);
-  a.bscale = pl.ws.tc_scale;
-  a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
-  a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
-  a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
   cudaError_t err = cudaSuccess;
-  const int pi = prof_begin(2, st);
-  const int rc = tc::launch_fused(pl.KT, a, pl.caps.n_sm, st, &err);
-  prof_end(pi, st);
-  if (rc == GM_OK) ++t_launches;
+  int rc;
+  const long long stride = bt->psf_stride == 0 ? 0 : (long long)tc::table_bytes(pl.KT);
+  if (pl.tc == 1) {
+    tc::FusedTcArgs a;
+    a.md = pl.md; a.B = bt->B; a.mode = mode; a.cc = pl.ws.cc;
+    a.btab_fwd = pl.ws.tc_fwd; a.btab_adj = pl.ws.tc_adj; a.btab_stride = stride; a.bscale = pl.ws.tc_scale;
+    a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
+    a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+    a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
+    const int pi = prof_begin(2, st);
+    rc = tc::launch_fused(pl.KT, a, pl.caps.n_sm, st, &err);
+    prof_end(pi, st);
+    if (rc == GM_OK) ++t_launches;
+  } else {
+    tc::TileTcArgs a;
+    a.md = pl.md; a.B = bt->B; a.H = bt->H; a.W = bt->W; a.tiles_x = pl.tc_tx; a.tiles_y = pl.tc_ty; a.mode = mode;
+    a.cc = pl.ws.cc; a.btab = pl.ws.tc_fwd; a.btab_stride = stride; a.bscale = pl.ws.tc_scale;
+    a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
+    a.out = out; a.gbuf = pl.ws.G; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+    a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
+    int pi = prof_begin(0, st);
+    rc = tc::launch_tile(pl.KT, a, pl.tc_trb, 0, pl.caps.n_sm, st, &err);
+    prof_end(pi, st);
+    if (rc == GM_OK) ++t_launches;
+    if (rc == GM_OK && mode == 2) {
+      a.btab = pl.ws.tc_adj;
+      pi = prof_begin(1, st);
+      rc = tc::launch_tile(pl.KT, a, pl.tc_trb, 1, pl.caps.n_sm, st, &err);
+      prof_end(pi, st);
+      if (rc == GM_OK) ++t_launches;
+    }
+  }
   if (rc == GM_ECUDA) t_last_err = err;
   return rc;
 }
@@ -1239,10 +1339,15 @@ int gm_conv(int engine, int adjoint, const gm_batch* bt, float* out, void* works
     uint8_t* tab = (uint8_t*)workspace;
     float* bscale = (float*)((char*)workspace + align_up((size_t)n_psf * tc::table_bytes(KP), 256));
     cudaError_t err = cudaSuccess;
-    int launches = 0;
-    rc = tc::conv(KP, bt->B, bt->data, out, bt->psf, bt->psf_stride, bt->K, adjoint ? 0 : 1, tab, bscale, caps.n_sm, st,
-                  &err, &launches);
-    t_launches += launches;
+    rc = tc::build_table(KP, bt->psf, bt->psf_stride, n_psf, bt->K, adjoint ? 0 : 1, tab, bscale, st, &err);
+    if (rc == GM_OK) {
+      ++t_launches;
+      tc::ConvArgs a;
+      a.B = bt->B; a.in = bt->data; a.out = out; a.btab = tab; a.bscale = bscale;
+      a.btab_stride = bt->psf_stride ? (long long)tc::table_bytes(KP) : 0;
+      rc = tc::launch_conv(KP, a, caps.n_sm, st, &err);
+      if (rc == GM_OK) ++t_launches;
+    }
     if (rc == GM_ECUDA) t_last_err = err;
     return rc;
   }
@@ -1782,7 +1887,6 @@ int gm_init(void* cuda_stream) {
 }
 
 int gm_set_option(int option, int value) {
-  if (option == 99) { tc::g_tc_dbg = value; return GM_OK; }   // PROBE ONLY
   if (option < 0 || option >= GM_OPT_COUNT_) return GM_EINVAL;
   g_opt[option].store(value != 0);
   return GM_OK;

@@ -1,5 +1,5 @@
-// gm_tc.cu -- launchers of the tensor-core convolution engine (gm_tc.cuh), one
-// instantiation per padded PSF side whose half width is a multiple of 4.
+// gm_tc.cu -- launchers of the tensor-core engine (gm_tc.cuh, gm_tc_fused.cuh) for ONE padded PSF
+// side, -DGM_TC_K=<9|17|25|33|41> (half width a multiple of 4).  Compiled once per side (build.py).
 #include "gm_tc_fused.cuh"
 
 #include <mutex>
@@ -7,6 +7,12 @@
 #include <vector>
 
 #include "gm.h"
+
+#ifndef GM_TC_K
+#error "compile with -DGM_TC_K=<padded PSF side>"
+#endif
+#define GM_CAT_(a, b) a##b
+#define GM_CAT(a, b) GM_CAT_(a, b)
 
 namespace gm {
 namespace tc {
@@ -16,6 +22,8 @@ namespace tc {
     cudaError_t e__ = (expr);                          \
     if (e__ != cudaSuccess) { *err = e__; return GM_ECUDA; } \
   } while (0)
+
+constexpr int KP = GM_TC_K;
 
 static cudaError_t set_smem_once(const void* kern, int bytes) {
   static std::mutex mu;
@@ -31,78 +39,27 @@ static cudaError_t set_smem_once(const void* kern, int bytes) {
   return cudaSuccess;
 }
 
-int g_tc_dbg = 0;   // PROBE ONLY
+size_t GM_CAT(table_bytes_, GM_TC_K)() { return (size_t)KP * Cfg<KP>::kTapBytes; }
 
-int padded_side(int K) {
-  static const int sides[] = {9, 17, 25, 33, 41};
-  for (int s : sides)
-    if (K <= s) return s;
-  return -1;
-}
-
-size_t table_bytes(int KP) {
-  switch (KP) {
-    case 9: return (size_t)9 * Cfg<9>::kTapBytes;
-    case 17: return (size_t)17 * Cfg<17>::kTapBytes;
-    case 25: return (size_t)25 * Cfg<25>::kTapBytes;
-    case 33: return (size_t)33 * Cfg<33>::kTapBytes;
-    case 41: return (size_t)41 * Cfg<41>::kTapBytes;
-    default: return 0;
-  }
-}
-
-template <int KP>
-static int launch(const ConvArgs& a, const float* psf, long long psf_stride, int n_psf, int K, int flip, uint8_t* tab,
-                  float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches) {
+// the E_a table of every PSF (flip = 1: flipped taps, the forward convolution; 0: the adjoint) and the PSF scales
+int GM_CAT(build_table_, GM_TC_K)(const float* psf, long long psf_stride, int n_psf, int K, int flip, uint8_t* tab, float* bscale,
+                                 cudaStream_t st, cudaError_t* err) {
   k_tc_btab<KP><<<n_psf * KP, 256, 0, st>>>(psf, psf_stride, K, flip, tab, bscale);
   GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
+// gm_conv, tensor engine: B cutouts of 128 x 128
+int GM_CAT(launch_conv_tc_, GM_TC_K)(const ConvArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
   GM_TRY(set_smem_once((const void*)k_tc_conv<KP>, (int)Cfg<KP>::kSmem));
   const int grid = a.B < n_sm ? a.B : n_sm;
   k_tc_conv<KP><<<grid, kThreads, Cfg<KP>::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
-  *launches += 2;
   return GM_OK;
 }
 
-// out = PSF (*) in (flip = 1) or the adjoint (flip = 0) for B cutouts of 128 x 128; tab / bscale: device scratch of
-// n_psf * table_bytes(KP) bytes and n_psf floats
-int conv(int KP, int B, const float* in, float* out, const float* psf, long long psf_stride, int K, int flip, uint8_t* tab,
-         float* bscale, int n_sm, cudaStream_t st, cudaError_t* err, int* launches) {
-  ConvArgs a;
-  a.dbg = g_tc_dbg;
-  a.B = B; a.in = in; a.out = out; a.btab = tab; a.bscale = bscale;
-  a.btab_stride = psf_stride ? (long long)table_bytes(KP) : 0;
-  const int n_psf = psf_stride ? B : 1;
-  switch (KP) {
-    case 9: return launch<9>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
-    case 17: return launch<17>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
-    case 25: return launch<25>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
-    case 33: return launch<33>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
-    case 41: return launch<41>(a, psf, psf_stride, n_psf, K, flip, tab, bscale, n_sm, st, err, launches);
-    default: return GM_ENOTSUP;
-  }
-}
-
-// both E_a tables of every PSF (forward: flipped taps, adjoint: taps as given) and the PSF scales
-int build_tables(int KP, const float* psf, long long psf_stride, int n_psf, int K, uint8_t* tab_fwd, uint8_t* tab_adj,
-                 float* bscale, cudaStream_t st, cudaError_t* err, int* launches) {
-  switch (KP) {
-#define GM_TC_CASE(S)                                                                     \
-    case S:                                                                                 \
-      k_tc_btab<S><<<n_psf * S, 256, 0, st>>>(psf, psf_stride, K, 1, tab_fwd, bscale);      \
-      k_tc_btab<S><<<n_psf * S, 256, 0, st>>>(psf, psf_stride, K, 0, tab_adj, bscale);      \
-      break;
-    GM_TC_CASE(9) GM_TC_CASE(17) GM_TC_CASE(25) GM_TC_CASE(33) GM_TC_CASE(41)
-#undef GM_TC_CASE
-    default: return GM_ENOTSUP;
-  }
-  GM_TRY(cudaGetLastError());
-  *launches += 2;
-  return GM_OK;
-}
-
-template <int KP>
-static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+// a1 .. a5 of 128 x 128 cutouts in one launch
+int GM_CAT(launch_fused_tc_, GM_TC_K)(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
   GM_TRY(set_smem_once((const void*)k_tc_fused<KP>, (int)FusedCfg<KP>::kSmem));
   const int grid = a.B < n_sm ? a.B : n_sm;
   k_tc_fused<KP><<<grid, kFusedThreadsTc, FusedCfg<KP>::kSmem, st>>>(a);
@@ -110,15 +67,29 @@ static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaE
   return GM_OK;
 }
 
-int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
-  switch (KP) {
-    case 9: return launch_fused_t<9>(a, n_sm, st, err);
-    case 17: return launch_fused_t<17>(a, n_sm, st, err);
-    case 25: return launch_fused_t<25>(a, n_sm, st, err);
-    case 33: return launch_fused_t<33>(a, n_sm, st, err);
-    case 41: return launch_fused_t<41>(a, n_sm, st, err);
+// larger cutouts, super-tiles of trb x (128 / trb) tiles; bwd = 0: forward kernel, 1: backward kernel
+template <int TRB, bool BWD>
+static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  GM_TRY(set_smem_once((const void*)k_tc_tile<KP, TRB, BWD>, (int)TileCfg<KP, TRB>::kSmem));
+  const long long items = (long long)a.B * a.tiles_x * a.tiles_y;
+  const int grid = items < n_sm ? (int)items : n_sm;
+  k_tc_tile<KP, TRB, BWD><<<grid, kFusedThreadsTc, TileCfg<KP, TRB>::kSmem, st>>>(a);
+  GM_TRY(cudaGetLastError());
+  return GM_OK;
+}
+
+int GM_CAT(launch_tile_tc_, GM_TC_K)(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err) {
+#if GM_TC_K == 25 || GM_TC_K == 41
+  switch (trb) {
+    case 16: return bwd ? launch_tile_t<16, true>(a, n_sm, st, err) : launch_tile_t<16, false>(a, n_sm, st, err);
+    case 32: return bwd ? launch_tile_t<32, true>(a, n_sm, st, err) : launch_tile_t<32, false>(a, n_sm, st, err);
+    case 64: return bwd ? launch_tile_t<64, true>(a, n_sm, st, err) : launch_tile_t<64, false>(a, n_sm, st, err);
     default: return GM_ENOTSUP;
   }
+#else
+  (void)a; (void)trb; (void)bwd; (void)n_sm; (void)st; (void)err;
+  return GM_ENOTSUP;                        // the super-tile kernels are built for the PSF sides of the configs (25, 41)
+#endif
 }
 
 }  // namespace tc

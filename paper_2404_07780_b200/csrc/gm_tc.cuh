@@ -83,7 +83,6 @@ struct ConvArgs {
   const uint8_t* btab;        // [n_psf][KP tap rows][kTapBytes]: E_a of every tap row (k_tc_btab)
   const float* bscale;        // [n_psf]: 1 / (power-of-two scale of the PSF)
   long long btab_stride;      // bytes between the tables of consecutive cutouts (0: one PSF for all)
-  int dbg;                    // PROBE ONLY: 1 skip MMAs, 2 skip window loads/stores, 4 skip conversion, 8 skip drain stores
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------
@@ -241,7 +240,7 @@ static_assert(N_BARS <= 64, "barrier area");
 
 // MMA issue of accumulators R0 .. R0 + NACC - 1 (one converged warp)
 template <int KP, int R0, int NACC>
-__device__ __forceinline__ void mma_role(int dbg, int n_gal, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
+__device__ __forceinline__ void mma_role(int n_gal, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
   using C = Cfg<KP>;
   constexpr uint32_t idesc = instr_desc(128, kTileC);
   constexpr uint32_t desc_hi = (uint32_t)(smem_desc(0, C::NR * 16, 128) >> 32);
@@ -270,7 +269,7 @@ __device__ __forceinline__ void mma_role(int dbg, int n_gal, uint32_t bars, uint
         const uint32_t dcol = tD + (uint32_t)(d * C::kDCols + (R0 + rr) * kTileC);
         // start-address field of the hi part's chunk 0 (+ the constant LBO field); parts and chunks differ by constants
         const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
-        if (!(dbg & 1)) {
+        {
 #pragma unroll
           for (int kc = 0; kc < C::NCH; ++kc) {
             const uint32_t b_hi = lo0 + (uint32_t)(16 * (C::NCH - 1 - kc));          // 16 rows of 16 bytes per chunk step
@@ -350,7 +349,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
         const uint32_t rowp = row_ok ? slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7)) : zero;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
-          if (a.dbg & 2) break;
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
@@ -395,7 +393,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
         float4* dst = reinterpret_cast<float4*>(outp + (size_t)(4 * lane + r) * kSide + 32 * lw);
 #pragma unroll
         for (int q = 0; q < 8; ++q)
-          if (!(a.dbg & 8)) dst[q] = make_float4(__uint_as_float(v[4 * q]) * inv, __uint_as_float(v[4 * q + 1]) * inv,
+          dst[q] = make_float4(__uint_as_float(v[4 * q]) * inv, __uint_as_float(v[4 * q + 1]) * inv,
                                __uint_as_float(v[4 * q + 2]) * inv, __uint_as_float(v[4 * q + 3]) * inv);
       }
       fence_before();
@@ -412,7 +410,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       float amax = 0.0f;
 #pragma unroll 4
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
-        if (a.dbg & 32) break;
         const float4 v = __ldg(src + i);
         const int R = i >> 5, c = (i & 31) << 2;
         sts128(slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c),
@@ -426,7 +423,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       // pass 2: every thread turns its own pixels into (hi, lo) fp16 pairs in place
 #pragma unroll 4
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
-        if (a.dbg & 4) break;
         const int R = i >> 5, c = (i & 31) << 2;
         const uint32_t p = slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c);
         const uint4 v = lds128(p);
@@ -448,10 +444,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
     // (the accumulator pair is a template argument so that every address of the issue loop is
     // warp-uniform at compile time and stays in uniform registers)
     static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
-    if (wid == 8) mma_role<KP, 0, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else if (wid == 9) mma_role<KP, 1, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else if (wid == 10) mma_role<KP, 2, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else mma_role<KP, 3, 1>(a.dbg, n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    if (wid == 8) mma_role<KP, 0, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 9) mma_role<KP, 1, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 10) mma_role<KP, 2, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else mma_role<KP, 3, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
     // in the order of first use: window row y = seq(i) brings tap row y (r = 0) on the low side and
@@ -467,7 +463,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
           const int slot = C::slot_of(ta);
           const uint32_t gen = (uint32_t)(it * C::uses_of_slot(slot) + C::index_in_slot(ta));
           mbar_wait(bar(B_EMPTY + slot), (gen & 1) ^ 1);
-          if (a.dbg & 16) { mbar_arrive(bar(B_FULL + slot)); continue; }
           mbar_expect_tx(bar(B_FULL + slot), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(B_FULL + slot));
         }

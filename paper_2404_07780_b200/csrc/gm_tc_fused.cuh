@@ -456,5 +456,353 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   if (wid == kLastWarp) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tm) : "memory");
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Cutouts above 128 px: the same engine on SUPER-TILES of 128 lanes (128 x 128 or 64 x 256 / 256 x 64
+// pixels, whichever covers the cutout with the fewest), G through global memory between the forward and
+// the backward kernel as in the FFMA2 tile kernels (k_forward / k_backward).  One shared-memory slot holds
+// the super-tile plus its halo, so the phases of an item run one after the other:
+//   k_tc_tile<KP, TRB, false>  a1 render S on tile + halo -> scale, split -> C1 -> drain M -> a3 residual,
+//                              G to global, chi^2 partial (mode 0: M to global)
+//   k_tc_tile<KP, TRB, true>   G tile + halo from global -> scale, split -> C2 -> drain A -> a5 partial sums
+// ---------------------------------------------------------------------------------------------------
+struct TileTcArgs {
+  ModelDesc md;
+  int B, H, W;
+  int tiles_x, tiles_y;      // super-tiles per cutout
+  int mode;                  // forward kernel: 0 render (write M to out), 1 / 2 chi^2 (G to gbuf when 2)
+  const CompConst* cc;
+  const uint8_t* btab; long long btab_stride; const float* bscale;
+  const float* data; const float* sigma; const uint8_t* mask;
+  float* out;                // mode 0: model image
+  float* gbuf;               // [B,H,W] back-seed G: written by the forward kernel, read by the backward kernel
+  float* chi2_part;          // [B, tiles]
+  float* grad_part;          // [B, tiles, n_comp, kNSum]
+  const int* frozen; const int* live; const int* n_live;
+};
+
+template <int KP, int TRB> struct TileCfg {
+  using C = Cfg<KP>;
+  static constexpr int TCB = 128 / TRB;                       // tile columns of a super-tile
+  static constexpr int TH = kTileR * TRB, TW = kTileC * TCB;  // pixels of a super-tile
+  static constexpr int RR = TH + KP - 1;                      // slot rows: tile + halo
+  static constexpr int RW = TW + KP - 1;                      // columns that carry data
+  static constexpr int kPitchT = TW - kTileC + 16 * C::NCH + 28;   // + window padding of the last tile column + skew
+  static_assert(kPitchT % 4 == 0 && (kPitchT / 4) % 2 == 1, "rows 4 apart must land 16 banks apart");
+  static constexpr int kSlotWordsT = RR * kPitchT;
+  static constexpr size_t kSmem = 1024 + 1024 + (size_t)kNSlot * C::kTapBytes + (size_t)kSlotWordsT * 4;
+};
+
+template <int KP, int TRB, bool BWD>
+__global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs a) {
+  using C = Cfg<KP>;
+  using T = TileCfg<KP, TRB>;
+  constexpr int h = C::h;
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(base);
+  uint32_t* tmem_base_s = reinterpret_cast<uint32_t*>(base + 512);
+  float* red = reinterpret_cast<float*>(base + 528);
+  float* redmax = red + kHelpWarpsTc * kNSum;
+  unsigned char* ring = base + 1024;
+  uint32_t* slotw = reinterpret_cast<uint32_t*>(ring + (size_t)kNSlot * C::kTapBytes);
+  auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
+
+  const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
+  if (tid == 0) {
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
+    for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
+    for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
+  if (wid == kLastWarp) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int i = tid; i < T::kSlotWordsT; i += kFusedThreadsTc) slotw[i] = 0u;        // padding columns stay zero
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tm = __shfl_sync(0xffffffffu, *tmem_base_s, 0);
+  const uint32_t tD = tm, tA = tm + 2 * C::kDCols;
+  const uint32_t slot = smem_u32(slotw);
+
+  // items of this CTA: (galaxy of the list, super-tile), entries blockIdx.x, + gridDim.x, ...
+  const int tiles = a.tiles_x * a.tiles_y;
+  const int n_gal = a.live ? *a.n_live : a.B;
+  const int n_all = n_gal * tiles;
+  const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  auto item_of = [&](int it, int& b, int& tile) {
+    const int e = (int)blockIdx.x + it * (int)gridDim.x;
+    const int g = e / tiles;
+    tile = e - g * tiles;
+    b = a.live ? a.live[g] : g;
+    if (a.frozen && a.frozen[b]) b = -1;
+  };
+
+  if (wid < 4) {
+    // ------------------------- window rows -> tensor memory --------------------------
+    const uint32_t lane_base = (uint32_t)(32 * wid) << 16;
+    const int m = 32 * wid + lane, tr = m % TRB, tc = m / TRB;     // this lane's tile of the super-tile
+    int row_count = 0;
+    for (int it = 0; it < n_items; ++it) {
+      const int s = it & 1;
+      mbar_wait(bar(F_IN_FULL + s), (it >> 1) & 1);
+      for (int i = 0; i < C::NY; ++i, ++row_count) {
+        const int y = C::seq(i);
+        const int buf = row_count % kNBuf;
+        mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
+        fence_after();
+        const int R = 4 * tr + y;                                  // slot row (row 0 = image row i0 - h)
+        const uint32_t rowp = slot + 4u * (uint32_t)(R * T::kPitchT + 4 * ((R >> 2) & 7) + kTileC * tc);
+#pragma unroll
+        for (int kc = 0; kc < C::NCH; ++kc) {
+          uint32_t w[16];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint4 v = lds128(rowp + 4u * (uint32_t)(16 * kc + 4 * q));
+            w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+          }
+          uint32_t hi[8], lo[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            hi[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x5410);
+            lo[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x7632);
+          }
+          const uint32_t col = tA + (uint32_t)(buf * C::kACols + kc * 16) + lane_base;
+          tmem_st8(col, hi);
+          tmem_st8(col + 8, lo);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(F_A_FULL + buf));
+      }
+    }
+  } else if (wid < 4 + kHelpWarpsTc) {
+    // ------------------------------------ helpers -------------------------------------
+    const int hw = wid - 4, htid = tid - 128;
+    const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
+    auto px_addr = [&](int R, int c) -> uint32_t { return slot + 4u * (uint32_t)(R * T::kPitchT + 4 * ((R >> 2) & 7) + c); };
+    auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
+    constexpr int RW4 = T::RW / 4, kRegionGroups = T::RR * RW4;      // groups of four pixels of the tile + halo
+    constexpr int TW4 = T::TW / 4, kTileGroups = T::TH * TW4;        // ... of the tile itself
+    const float inv_rw4 = 1.0f / (float)RW4;
+
+    auto scale_and_split = [&](float amax) -> float {
+      for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+      if (lane == 0) redmax[hw] = amax;
+      help_sync();
+      float mx = redmax[0];
+#pragma unroll
+      for (int w = 1; w < kHelpWarpsTc; ++w) mx = fmaxf(mx, redmax[w]);
+      const float sc = pow2_scale(mx);
+#pragma unroll 2
+      for (int idx = htid; idx < kRegionGroups; idx += kHN) {
+        const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
+        const uint32_t p = px_addr(R, x);
+        const uint4 v = lds128(p);
+        sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
+                             split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
+      }
+      help_sync();
+      return 1.0f / sc;
+    };
+
+    for (int it = 0; it < n_items; ++it) {
+      const int s = it & 1;
+      int b, tile;
+      item_of(it, b, tile);
+      const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
+      const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;          // tile origin in the cutout
+      const size_t img = (size_t)(b >= 0 ? b : 0) * a.H * a.W;
+      float amax = 0.0f;
+
+      // ---- fill the slot: S (forward) or G (backward) on the tile + halo, zero outside the cutout
+      if (!BWD) {
+        const CompConst* ccb = a.cc + (size_t)(b >= 0 ? b : 0) * a.md.n_comp;
+        for (int c = 0; c < a.md.n_comp; ++c) {
+          const CompConst cc = ccb[c];
+          const bool box = a.md.box[c] != 0;
+          const bool first = c == 0, last = c == a.md.n_comp - 1;
+          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+            for (int idx = htid; idx < kRegionGroups; idx += kHN) {
+              const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
+              const int i = i0 - h + R, j = j0 - h + x;
+              const uint32_t p = px_addr(R, x);
+              float v[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+              if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) {        // W % 4 == 0: whole group in or out
+                value4<KIND, kFastForward>(cc, box, (float)j + 0.5f, (float)a.H - 0.5f - (float)i, v);   // R:G1
+                if (!first) {
+                  const uint4 q = lds128(p);
+                  v[0] += __uint_as_float(q.x); v[1] += __uint_as_float(q.y); v[2] += __uint_as_float(q.z); v[3] += __uint_as_float(q.w);
+                }
+                if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
+              }
+              sts128(p, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
+            }
+          });
+        }
+      } else {
+        const float* gsrc = a.gbuf + img;
+        for (int idx = htid; idx < kRegionGroups; idx += kHN) {
+          const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
+          const int i = i0 - h + R, j = j0 - h + x;
+          float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) {
+            v = *reinterpret_cast<const float4*>(gsrc + (size_t)i * a.W + j);
+            amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+          }
+          sts128(px_addr(R, x), make_uint4(__float_as_uint(v.x), __float_as_uint(v.y), __float_as_uint(v.z), __float_as_uint(v.w)));
+        }
+      }
+      if (!isfinite(amax)) amax = 0.0f;
+      const float inv_sc = scale_and_split(amax);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(F_IN_FULL + s));
+
+      // ---- drain the accumulators into the (now free) slot, top-left aligned: pixel (R, c) of the tile
+      mbar_wait(bar(F_D_FULL + s), (it >> 1) & 1);
+      fence_after();
+      {
+        const float inv = inv_sc * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
+        const int q = hw & 3, r_first = 2 * (hw >> 2);
+        const int m = 32 * q + lane, tr = m % TRB, tc = m / TRB;
+#pragma unroll 1
+        for (int r = r_first; r < r_first + 2; ++r) {
+          uint32_t v[32];
+          tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          const uint32_t p = px_addr(4 * tr + r, kTileC * tc);
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            sts128(p + 16u * k, make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+                                           __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
+        }
+        fence_before();
+        help_sync();
+      }
+
+      if (!BWD) {
+        // ---- a3 on the tile: residual, chi^2 partial, G to global (mode 0: M to global)
+        float chi2 = 0.0f;
+        if (b >= 0) {
+          auto one = [&](float mm, float d, float sg, bool used) -> float {
+            float w = rcp_fast(sg * sg), rho = d - mm;
+            w = used ? w : 0.0f;
+            rho = used ? rho : 0.0f;
+            const float t = w * rho;
+            chi2 = fmaf(t, rho, chi2);
+            return -2.0f * t;
+          };
+#pragma unroll 2
+          for (int idx = htid; idx < kTileGroups; idx += kHN) {
+            const int R = idx / TW4, x = (idx - R * TW4) << 2;
+            const int i = i0 + R, j = j0 + x;
+            if (i >= a.H || j >= a.W) continue;
+            const size_t o = img + (size_t)i * a.W + j;
+            const uint4 m4 = lds128(px_addr(R, x));
+            if (a.mode == 0) {
+              *reinterpret_cast<float4*>(a.out + o) = make_float4(__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w));
+            } else {
+              const float4 d4 = *reinterpret_cast<const float4*>(a.data + o), s4 = *reinterpret_cast<const float4*>(a.sigma + o);
+              uchar4 k4 = make_uchar4(1, 1, 1, 1);
+              if (a.mask) k4 = *reinterpret_cast<const uchar4*>(a.mask + o);
+              float4 g;
+              g.x = one(__uint_as_float(m4.x), d4.x, s4.x, k4.x != 0);
+              g.y = one(__uint_as_float(m4.y), d4.y, s4.y, k4.y != 0);
+              g.z = one(__uint_as_float(m4.z), d4.z, s4.z, k4.z != 0);
+              g.w = one(__uint_as_float(m4.w), d4.w, s4.w, k4.w != 0);
+              if (a.mode == 2) *reinterpret_cast<float4*>(a.gbuf + o) = g;
+            }
+          }
+        }
+        if (a.mode != 0) {
+          chi2 = warp_sum(chi2);
+          if (lane == 0) red[hw] = chi2;
+          help_sync();
+          if (htid == 0 && b >= 0) {
+            float t = 0.0f;
+            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
+            a.chi2_part[(size_t)b * tiles + tile] = t;
+          }
+        }
+        help_sync();                                       // every read of the slot is done before the next fill
+      } else {
+        // ---- a5 on the tile: the partial sums of every component from A
+        for (int c = 0; c < a.md.n_comp; ++c) {
+          float sm[kNSum];
+#pragma unroll
+          for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
+          if (b >= 0) {
+            const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
+            const bool box = a.md.box[c] != 0;
+            dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+              GradAcc<KIND> acc;
+              acc.init();
+              for (int idx = htid; idx < kTileGroups; idx += kHN) {
+                const int R = idx / TW4, x = (idx - R * TW4) << 2;
+                const int i = i0 + R, j = j0 + x;
+                if (i >= a.H || j >= a.W) continue;
+                const uint4 q = lds128(px_addr(R, x));
+                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+                if (box) {
+#pragma unroll
+                  for (int k = 0; k < 4; ++k)
+                    grad_accumulate<KIND>(cc, true, seed[k], (float)(j + k) + 0.5f, (float)a.H - 0.5f - (float)i, sm);
+                } else {
+                  grad_add4<KIND>(acc, cc, seed, (float)j + 0.5f, (float)a.H - 0.5f - (float)i);
+                }
+              }
+              if (!box) { acc.finish(cc, sm); sm[8] = sm[2]; }
+            });
+          }
+#pragma unroll
+          for (int k = 0; k < kNSum; ++k) {
+            const float v = warp_sum(sm[k]);
+            if (lane == 0) red[hw * kNSum + k] = v;
+          }
+          help_sync();
+          if (htid < kNSum && b >= 0) {
+            float t = 0.0f;
+            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
+            a.grad_part[(((size_t)b * tiles + tile) * a.md.n_comp + c) * kNSum + htid] = t;
+          }
+          help_sync();
+        }
+      }
+    }
+  } else if (wid < kLastWarp) {
+    // ----------------------------------- MMA issue ------------------------------------
+    const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2>(n_items, 1, b0, r0, tD, tA);
+    else fused_mma_role<KP, 3>(n_items, 1, b0, r0, tD, tA);
+  } else {
+    // ------------------------------- tap-row producer --------------------------------
+    if (lane == 0) {
+      for (int it = 0; it < n_items; ++it) {
+        int b, tile;
+        item_of(it, b, tile);
+        const uint8_t* tab = a.btab + (size_t)(b >= 0 ? b : 0) * a.btab_stride;
+        for (int i = 0; i < C::NY; ++i) {
+          const int y = C::seq(i);
+          const int ta = (i & 1) ? y - (kTileR - 1) : y;
+          if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
+          const int sl = C::slot_of(ta);
+          const uint32_t gen = (uint32_t)(it * C::uses_of_slot(sl) + C::index_in_slot(ta));
+          mbar_wait(bar(F_B_EMPTY + sl), (gen & 1) ^ 1);
+          mbar_expect_tx(bar(F_B_FULL + sl), C::kTapBytes);
+          bulk_g2s(smem_u32(ring + (size_t)sl * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + sl));
+        }
+      }
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (wid == kLastWarp) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tm) : "memory");
+}
+
 }  // namespace tc
 }  // namespace gm
