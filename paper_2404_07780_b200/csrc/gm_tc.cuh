@@ -40,10 +40,16 @@ namespace tc {
 
 constexpr int kTileR = 4, kTileC = 32;      // output tile of one lane
 constexpr int kSide = 128;                  // cutout side this engine is built for (128 lanes)
-constexpr int kPitch = kSide + 28;          // words per image row in shared memory (room for the skew of 0 .. 28)
+constexpr int kPitch = kSide;               // words per image row in shared memory (16-byte chunks XOR-swizzled, see swz)
 constexpr int kNBuf = 3;                    // window-row buffers in tensor memory
-constexpr int kRing = 5;                    // tap-row slots per ring; two rings (low / high tap rows)
-constexpr int kNSlot = 2 * kRing;
+constexpr int kMaxRing = 8;                 // tap-row slots per ring at most; two rings (low / high tap rows)
+constexpr int kMaxSlots = 2 * kMaxRing;
+constexpr size_t kSmemLimit = 232448;       // 227 KB of dynamic shared memory per CTA
+
+// Word offset of pixel (row R, column c), c a multiple of 4, in an image stored with `pitch` words per row
+// (a multiple of 32): the 16-byte chunk index is XORed with bits 2..4 of the row, so that the eight lanes of
+// a shared-memory wavefront, which read the same chunk of rows 4 apart, hit eight different bank groups.
+__host__ __device__ constexpr int swz(int R, int c, int pitch) { return R * pitch + ((((c >> 2) ^ ((R >> 2) & 7))) << 2); }
 constexpr int kMmaWarps = 4;                // one accumulator row each
 constexpr int kThreads = (8 + kMmaWarps + 1) * 32;
 
@@ -57,6 +63,11 @@ template <int KP> struct Cfg {
   static constexpr int kACols = NCH * 16;                     // tensor-memory columns of one row buffer
   static constexpr int kDCols = kTileR * kTileC;              // 128 accumulator columns per cutout
   static constexpr int kSlotWords = (kSide + 1) * kPitch;     // image rows + the zero row
+  // tap-row ring depth: what two image slots leave of the shared memory, at least 5 (4 tap rows are live per side)
+  static constexpr int kRing = ((kSmemLimit - 2048 - 2 * (size_t)kSlotWords * 4) / (2 * (size_t)kTapBytes)) >= (size_t)kMaxRing
+                                   ? kMaxRing : (int)((kSmemLimit - 2048 - 2 * (size_t)kSlotWords * 4) / (2 * (size_t)kTapBytes));
+  static_assert(kRing >= 5, "tap-row rings");
+  static constexpr int kNSlot = 2 * kRing;
   // Window rows are visited OUTSIDE-IN (0, NY-1, 1, NY-2, ...): the tensor core adds every MMA into the
   // fp32 accumulator with truncation, a loss of half an ulp OF THE RUNNING SUM per step, so the tap rows
   // near the PSF centre, which carry most of the sum, must come last (measured: relative bias of a
@@ -67,12 +78,14 @@ template <int KP> struct Cfg {
   static constexpr int kNHigh = KP - kNLow;                   // tap rows KP-1 down to kNLow
   __host__ __device__ static constexpr int seq(int i) { return (i & 1) ? NY - 1 - (i >> 1) : (i >> 1); }
   // ring slot of tap row ta and how many tap rows of one cutout were in that slot before it / in total
-  __host__ __device__ static constexpr int slot_of(int ta) { return ta < kNLow ? ta % kRing : kRing + (KP - 1 - ta) % kRing; }
-  __host__ __device__ static constexpr int index_in_slot(int ta) { return ta < kNLow ? ta / kRing : (KP - 1 - ta) / kRing; }
-  __host__ __device__ static constexpr int uses_of_slot(int s) {
-    return s < kRing ? (kNLow - s + kRing - 1) / kRing : (kNHigh - (s - kRing) + kRing - 1) / kRing;
+  // (RING = slots per ring of the kernel at hand)
+  template <int RING> __host__ __device__ static constexpr int slot_of(int ta) { return ta < kNLow ? ta % RING : RING + (KP - 1 - ta) % RING; }
+  template <int RING> __host__ __device__ static constexpr int index_in_slot(int ta) { return ta < kNLow ? ta / RING : (KP - 1 - ta) / RING; }
+  template <int RING> __host__ __device__ static constexpr int uses_of_slot(int s) {
+    return s < RING ? (kNLow - s + RING - 1) / RING : (kNHigh - (s - RING) + RING - 1) / RING;
   }
-  static constexpr size_t kSmem = 1024 + 2 * (size_t)kSlotWords * 4 + (size_t)kNSlot * kTapBytes + 512;
+  static constexpr size_t kSmem = 2048 + 2 * (size_t)kSlotWords * 4 + (size_t)kNSlot * kTapBytes;
+  static_assert(kSmem <= kSmemLimit, "shared memory");
   static_assert(2 * kDCols + kNBuf * kACols <= 512, "tensor memory");
 };
 
@@ -234,8 +247,8 @@ __global__ void __launch_bounds__(256) k_tc_btab(const float* __restrict__ psf, 
 }
 
 // barrier indices of k_tc_conv (8 bytes each, from the start of the CTA's barrier area)
-enum { IMG_FULL = 0, IMG_EMPTY = 2, A_FULL = 4, A_EMPTY = 4 + kNBuf, B_FULL = 4 + 2 * kNBuf, B_EMPTY = B_FULL + kNSlot,
-       D_FULL = B_EMPTY + kNSlot, D_EMPTY = D_FULL + 2, N_BARS = D_EMPTY + 2 };
+enum { IMG_FULL = 0, IMG_EMPTY = 2, A_FULL = 4, A_EMPTY = 4 + kNBuf, B_FULL = 4 + 2 * kNBuf, B_EMPTY = B_FULL + kMaxSlots,
+       D_FULL = B_EMPTY + kMaxSlots, D_EMPTY = D_FULL + 2, N_BARS = D_EMPTY + 2 };
 static_assert(N_BARS <= 64, "barrier area");
 
 // MMA issue of accumulators R0 .. R0 + NACC - 1 (one converged warp)
@@ -263,8 +276,8 @@ __device__ __forceinline__ void mma_role(int n_gal, uint32_t bars, uint32_t ring
       for (int rr = 0; rr < NACC; ++rr) {
         const int ta = y - (R0 + rr);                               // tap row
         if (ta < 0 || ta >= KP) continue;
-        const int slot = C::slot_of(ta);
-        mbar_wait(bar(B_FULL + slot), (uint32_t)(it * C::uses_of_slot(slot) + C::index_in_slot(ta)) & 1);
+        const int slot = C::template slot_of<C::kRing>(ta);
+        mbar_wait(bar(B_FULL + slot), (uint32_t)(it * C::template uses_of_slot<C::kRing>(slot) + C::template index_in_slot<C::kRing>(ta)) & 1);
         fence_after();
         const uint32_t dcol = tD + (uint32_t)(d * C::kDCols + (R0 + rr) * kTileC);
         // start-address field of the hi part's chunk 0 (+ the constant LBO field); parts and chunks differ by constants
@@ -301,7 +314,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
   float* inv_scale_s = reinterpret_cast<float*>(base + 528);          // [2]
   float* red_s = reinterpret_cast<float*>(base + 544);                // [4]
   unsigned char* ring = base + 1024;
-  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)kNSlot * C::kTapBytes);
+  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)C::kNSlot * C::kTapBytes);
 
   static_assert(C::NY % 2 == 0, "outside-in order pairs the window rows");
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
@@ -312,7 +325,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(IMG_FULL + i), 4); mbar_init(bar(IMG_EMPTY + i), 4); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(A_FULL + i), 4); mbar_init(bar(A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 4); }
+    for (int i = 0; i < C::kNSlot; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 4); }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(D_FULL + i), kMmaWarps); mbar_init(bar(D_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -346,14 +359,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
         fence_after();
         const int R = 4 * lane + y - h;
         const bool row_ok = (unsigned)R < (unsigned)kSide;
-        const uint32_t rowp = row_ok ? slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7)) : zero;
+        const uint32_t rowp = slot + 4u * (uint32_t)(R * kPitch);
+        const int sw = (R >> 2) & 7;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             const int c0 = 32 * wid - h + 16 * kc + 4 * q;
-            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 4u * (uint32_t)c0 : zero);
+            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
           uint32_t hi[8], lo[8];
@@ -412,7 +426,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
         const float4 v = __ldg(src + i);
         const int R = i >> 5, c = (i & 31) << 2;
-        sts128(slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c),
+        sts128(slot + 4u * (uint32_t)swz(R, c, kPitch),
                make_uint4(__float_as_uint(v.x), __float_as_uint(v.y), __float_as_uint(v.z), __float_as_uint(v.w)));
         amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
       }
@@ -424,7 +438,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
 #pragma unroll 4
       for (int i = ltid; i < kSide * kSide / 4; i += 128) {
         const int R = i >> 5, c = (i & 31) << 2;
-        const uint32_t p = slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c);
+        const uint32_t p = slot + 4u * (uint32_t)swz(R, c, kPitch);
         const uint4 v = lds128(p);
         sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
                              split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
@@ -460,8 +474,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
           const int y = C::seq(i);
           const int ta = (i & 1) ? y - (kTileR - 1) : y;
           if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
-          const int slot = C::slot_of(ta);
-          const uint32_t gen = (uint32_t)(it * C::uses_of_slot(slot) + C::index_in_slot(ta));
+          const int slot = C::template slot_of<C::kRing>(ta);
+          const uint32_t gen = (uint32_t)(it * C::template uses_of_slot<C::kRing>(slot) + C::template index_in_slot<C::kRing>(ta));
           mbar_wait(bar(B_EMPTY + slot), (gen & 1) ^ 1);
           mbar_expect_tx(bar(B_FULL + slot), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(B_FULL + slot));

@@ -39,14 +39,15 @@ struct FusedTcArgs {
   const int* live; const int* n_live;
 };
 
-enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kNSlot,
-       F_N_BARS = F_B_EMPTY + kNSlot };
+enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kMaxSlots,
+       F_N_BARS = F_B_EMPTY + kMaxSlots };
 static_assert(F_N_BARS <= 64, "barrier area");
 
 template <int KP> struct FusedCfg {
   using C = Cfg<KP>;
   // [1 KB: barriers, tensor-memory address, reduction scratch | tap-row rings | 2 slots]
-  static constexpr size_t kSmem = 1024 + 1024 + (size_t)kNSlot * C::kTapBytes + 2 * (size_t)C::kSlotWords * 4;
+  static constexpr size_t kSmem = 1024 + 1024 + (size_t)C::kNSlot * C::kTapBytes + 2 * (size_t)C::kSlotWords * 4;
+  static_assert(kSmem <= kSmemLimit, "shared memory");
 };
 
 // the jobs of one CTA in tensor-core order; f(item, phase, slot)
@@ -60,8 +61,8 @@ __device__ __forceinline__ void for_each_job(int n_items, int phases, F&& f) {
       }
 }
 
-// MMA issue of accumulator row R0 for every job (one converged warp)
-template <int KP, int R0>
+// MMA issue of accumulator row R0 for every job (one converged warp); RING = tap-row slots per ring
+template <int KP, int R0, int RING>
 __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
   using C = Cfg<KP>;
   constexpr uint32_t idesc = instr_desc(128, kTileC);
@@ -81,8 +82,8 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
       const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
       const int ta = y - R0;
       if (ta >= 0 && ta < KP) {
-        const int slot = C::slot_of(ta);
-        mbar_wait(bar(F_B_FULL + slot), (uint32_t)(jc * C::uses_of_slot(slot) + C::index_in_slot(ta)) & 1);
+        const int slot = C::template slot_of<RING>(ta);
+        mbar_wait(bar(F_B_FULL + slot), (uint32_t)(jc * C::template uses_of_slot<RING>(slot) + C::template index_in_slot<RING>(ta)) & 1);
         fence_after();
         const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
 #pragma unroll
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   float* red = reinterpret_cast<float*>(base + 528);                // [kHelpWarpsTc * kNSum] sums, then [8] maxima
   float* redmax = red + kHelpWarpsTc * kNSum;
   unsigned char* ring = base + 1024;
-  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)kNSlot * C::kTapBytes);
+  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)C::kNSlot * C::kTapBytes);
   static_assert(528 + (kHelpWarpsTc * kNSum + 8) * 4 <= 1024, "header area");
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
@@ -122,7 +123,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    for (int i = 0; i < C::kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
@@ -130,7 +131,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = tid; i < 2 * C::kSlotWords; i += kFusedThreadsTc) slots[i] = 0u;    // zero rows (and skew gaps)
+  for (int i = tid; i < 2 * C::kSlotWords; i += kFusedThreadsTc) slots[i] = 0u;    // the zero rows
   fence_before();
   __syncthreads();
   fence_after();
@@ -163,14 +164,15 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         fence_after();
         const int R = 4 * lane + y - h;
         const bool row_ok = (unsigned)R < (unsigned)kSide;
-        const uint32_t rowp = row_ok ? slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7)) : zero;
+        const uint32_t rowp = slot + 4u * (uint32_t)(R * kPitch);
+        const int sw = (R >> 2) & 7;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             const int c0 = 32 * wid - h + 16 * kc + 4 * q;
-            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 4u * (uint32_t)c0 : zero);
+            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
           uint32_t hi[8], lo[8];
@@ -196,9 +198,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     float inv_sc[2] = {1.0f, 1.0f};                       // 1 / scale of what is in slot s (every thread holds the same)
     int cnt_d[2] = {0, 0};
     auto slot_addr = [&](int s) -> uint32_t { return smem_u32(slots + (size_t)s * C::kSlotWords); };
-    auto px_addr = [&](uint32_t slot, int R, int c) -> uint32_t {
-      return slot + 4u * (uint32_t)(R * kPitch + 4 * ((R >> 2) & 7) + c);
-    };
+    auto px_addr = [&](uint32_t slot, int R, int c) -> uint32_t { return slot + 4u * (uint32_t)swz(R, c, kPitch); };
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
     constexpr int kGroups = kSide * kSide / 4;            // groups of four pixels of a row; a warp walks one row at a time
 
@@ -274,10 +274,9 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         uint32_t v[32];
         tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        const uint32_t p = px_addr(slot, 4 * lane + r, 32 * q);
 #pragma unroll
         for (int k = 0; k < 8; ++k)
-          sts128(p + 16u * k, make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+          sts128(px_addr(slot, 4 * lane + r, 32 * q + 4 * k), make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
                                          __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
       }
       fence_before();
@@ -426,10 +425,10 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     // ----------------------------------- MMA issue ------------------------------------
     static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0>(n_items, phases, b0, r0, tD, tA);
-    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1>(n_items, phases, b0, r0, tD, tA);
-    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2>(n_items, phases, b0, r0, tD, tA);
-    else fused_mma_role<KP, 3>(n_items, phases, b0, r0, tD, tA);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, C::kRing>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, C::kRing>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, C::kRing>(n_items, phases, b0, r0, tD, tA);
+    else fused_mma_role<KP, 3, C::kRing>(n_items, phases, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
     if (lane == 0) {
@@ -441,8 +440,8 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
           const int y = C::seq(i);
           const int ta = (i & 1) ? y - (kTileR - 1) : y;
           if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
-          const int slot = C::slot_of(ta);
-          const uint32_t gen = (uint32_t)(jc * C::uses_of_slot(slot) + C::index_in_slot(ta));
+          const int slot = C::template slot_of<C::kRing>(ta);
+          const uint32_t gen = (uint32_t)(jc * C::template uses_of_slot<C::kRing>(slot) + C::template index_in_slot<C::kRing>(ta));
           mbar_wait(bar(F_B_EMPTY + slot), (gen & 1) ^ 1);
           mbar_expect_tx(bar(F_B_FULL + slot), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + slot));
@@ -486,10 +485,13 @@ template <int KP, int TRB> struct TileCfg {
   static constexpr int TH = kTileR * TRB, TW = kTileC * TCB;  // pixels of a super-tile
   static constexpr int RR = TH + KP - 1;                      // slot rows: tile + halo
   static constexpr int RW = TW + KP - 1;                      // columns that carry data
-  static constexpr int kPitchT = TW - kTileC + 16 * C::NCH + 28;   // + window padding of the last tile column + skew
-  static_assert(kPitchT % 4 == 0 && (kPitchT / 4) % 2 == 1, "rows 4 apart must land 16 banks apart");
+  static constexpr int kPitchT = (TW - kTileC + 16 * C::NCH + 31) / 32 * 32;   // + window padding of the last tile column, whole swizzle groups
   static constexpr int kSlotWordsT = RR * kPitchT;
-  static constexpr size_t kSmem = 1024 + 1024 + (size_t)kNSlot * C::kTapBytes + (size_t)kSlotWordsT * 4;
+  static constexpr int kRingT = ((kSmemLimit - 2048 - (size_t)kSlotWordsT * 4) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
+                                    ? kMaxRing : (int)((kSmemLimit - 2048 - (size_t)kSlotWordsT * 4) / (2 * (size_t)C::kTapBytes));
+  static_assert(kRingT >= 5, "tap-row rings");
+  static constexpr size_t kSmem = 1024 + 1024 + (size_t)(2 * kRingT) * C::kTapBytes + (size_t)kSlotWordsT * 4;
+  static_assert(kSmem <= kSmemLimit, "shared memory");
 };
 
 template <int KP, int TRB, bool BWD>
@@ -504,14 +506,14 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
   float* red = reinterpret_cast<float*>(base + 528);
   float* redmax = red + kHelpWarpsTc * kNSum;
   unsigned char* ring = base + 1024;
-  uint32_t* slotw = reinterpret_cast<uint32_t*>(ring + (size_t)kNSlot * C::kTapBytes);
+  uint32_t* slotw = reinterpret_cast<uint32_t*>(ring + (size_t)(2 * T::kRingT) * C::kTapBytes);
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    for (int i = 0; i < 2 * T::kRingT; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
@@ -554,13 +556,14 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
         mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
         fence_after();
         const int R = 4 * tr + y;                                  // slot row (row 0 = image row i0 - h)
-        const uint32_t rowp = slot + 4u * (uint32_t)(R * T::kPitchT + 4 * ((R >> 2) & 7) + kTileC * tc);
+        const uint32_t rowp = slot + 4u * (uint32_t)(R * T::kPitchT);
+        const int sw = (R >> 2) & 7;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
-            const uint4 v = lds128(rowp + 4u * (uint32_t)(16 * kc + 4 * q));
+            const uint4 v = lds128(rowp + 16u * (uint32_t)((8 * tc + 4 * kc + q) ^ sw));
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
           uint32_t hi[8], lo[8];
@@ -583,7 +586,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
     // ------------------------------------ helpers -------------------------------------
     const int hw = wid - 4, htid = tid - 128;
     const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
-    auto px_addr = [&](int R, int c) -> uint32_t { return slot + 4u * (uint32_t)(R * T::kPitchT + 4 * ((R >> 2) & 7) + c); };
+    auto px_addr = [&](int R, int c) -> uint32_t { return slot + 4u * (uint32_t)swz(R, c, T::kPitchT); };
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
     constexpr int RW4 = T::RW / 4, kRegionGroups = T::RR * RW4;      // groups of four pixels of the tile + halo
     constexpr int TW4 = T::TW / 4, kTileGroups = T::TH * TW4;        // ... of the tile itself
@@ -673,10 +676,9 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
           uint32_t v[32];
           tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
           asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          const uint32_t p = px_addr(4 * tr + r, kTileC * tc);
 #pragma unroll
           for (int k = 0; k < 8; ++k)
-            sts128(p + 16u * k, make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+            sts128(px_addr(4 * tr + r, kTileC * tc + 4 * k), make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
                                            __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
         }
         fence_before();
@@ -775,10 +777,10 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
   } else if (wid < kLastWarp) {
     // ----------------------------------- MMA issue ------------------------------------
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0>(n_items, 1, b0, r0, tD, tA);
-    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1>(n_items, 1, b0, r0, tD, tA);
-    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2>(n_items, 1, b0, r0, tD, tA);
-    else fused_mma_role<KP, 3>(n_items, 1, b0, r0, tD, tA);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    else fused_mma_role<KP, 3, T::kRingT>(n_items, 1, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
     if (lane == 0) {
@@ -790,8 +792,8 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
           const int y = C::seq(i);
           const int ta = (i & 1) ? y - (kTileR - 1) : y;
           if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
-          const int sl = C::slot_of(ta);
-          const uint32_t gen = (uint32_t)(it * C::uses_of_slot(sl) + C::index_in_slot(ta));
+          const int sl = C::template slot_of<T::kRingT>(ta);
+          const uint32_t gen = (uint32_t)(it * C::template uses_of_slot<T::kRingT>(sl) + C::template index_in_slot<T::kRingT>(ta));
           mbar_wait(bar(F_B_EMPTY + sl), (gen & 1) ^ 1);
           mbar_expect_tx(bar(F_B_FULL + sl), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)sl * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + sl));
