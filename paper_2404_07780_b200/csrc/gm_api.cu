@@ -37,7 +37,7 @@ namespace tc {          // gm_tc.cu, one object per padded PSF side
   int build_table_##K(const float* psf, long long psf_stride, int n_psf, int Kin, int flip, uint8_t* tab, float* bscale, \
                       cudaStream_t st, cudaError_t* err);                                                              \
   int launch_conv_tc_##K(const ConvArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);                               \
-  int launch_fused_tc_##K(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err);                           \
+  int launch_fused_tc_##K(const FusedTcArgs& a, int side, int n_sm, cudaStream_t st, cudaError_t* err);                           \
   int launch_tile_tc_##K(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err);
 GM_DECL_TC(9) GM_DECL_TC(17) GM_DECL_TC(25) GM_DECL_TC(33) GM_DECL_TC(41)
 #undef GM_DECL_TC
@@ -77,8 +77,8 @@ static int launch_conv(int KP, const ConvArgs& a, int n_sm, cudaStream_t st, cud
 #undef GM_C
   return GM_ENOTSUP;
 }
-static int launch_fused(int KP, const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
-#define GM_C(S) launch_fused_tc_##S(a, n_sm, st, err)
+static int launch_fused(int KP, const FusedTcArgs& a, int side, int n_sm, cudaStream_t st, cudaError_t* err) {
+#define GM_C(S) launch_fused_tc_##S(a, side, n_sm, st, err)
   GM_TC_SWITCH(KP, GM_C)
 #undef GM_C
   return GM_ENOTSUP;
@@ -724,12 +724,15 @@ static void tc_tile_geom(int H, int W, int* trb, int* tx, int* ty) {
 }
 
 // which tensor-core path the SHAPE of the batch allows (the model and the options decide later):
-// 1 = k_tc_fused (128 x 128), 2 = k_tc_tile (larger, W a multiple of 4, PSF side with tile kernels), 0 = none;
+// 1 = k_tc_fused (square cutouts of 64, 96, 128 px), 2 = k_tc_tile (larger, W a multiple of 4, PSF side with tile kernels), 0 = none;
 // *KT = padded PSF side of that engine
 static int tc_kind(const gm_batch* bt, int* KT) {
   *KT = tc::padded_side(bt->K);
   if (*KT < 0) return 0;
-  if (bt->H == tc::kSide && bt->W == tc::kSide) return 1;
+  if (bt->H == bt->W && (bt->H == 64 || bt->H == 96 || bt->H == 128)) {
+    // several 64 px cutouts share the lanes of one pass, and with them one PSF
+    return (bt->H == 64 && bt->psf_stride != 0) ? 0 : 1;
+  }
   if ((bt->H > tc::kSide || bt->W > tc::kSide) && (bt->W & 3) == 0 && tc::has_tile_kernels(*KT)) return 2;
   return 0;
 }
@@ -1036,6 +1039,8 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
     if (pl->tc == 2) {                                     // the partial sums are per super-tile on this path
       tc_tile_geom(bt->H, bt->W, &pl->tc_trb, &pl->tc_tx, &pl->tc_ty);
       pl->tiles = pl->tc_tx * pl->tc_ty;
+    } else {
+      pl->tiles = 1;                                       // k_tc_fused: one partial per galaxy
     }
   }
   // One cutout per slot (sides above 96) with the taps in shared memory (per-galaxy PSFs, or no
@@ -1121,7 +1126,7 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
     const int pi = prof_begin(2, st);
-    rc = tc::launch_fused(pl.KT, a, pl.caps.n_sm, st, &err);
+    rc = tc::launch_fused(pl.KT, a, bt->H, pl.caps.n_sm, st, &err);
     prof_end(pi, st);
     if (rc == GM_OK) ++t_launches;
   } else {

@@ -58,13 +58,25 @@ int GM_CAT(launch_conv_tc_, GM_TC_K)(const ConvArgs& a, int n_sm, cudaStream_t s
   return GM_OK;
 }
 
-// a1 .. a5 of 128 x 128 cutouts in one launch
-int GM_CAT(launch_fused_tc_, GM_TC_K)(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
-  GM_TRY(set_smem_once((const void*)k_tc_fused<KP>, (int)FusedCfg<KP>::kSmem));
-  const int grid = a.B < n_sm ? a.B : n_sm;
-  k_tc_fused<KP><<<grid, kFusedThreadsTc, FusedCfg<KP>::kSmem, st>>>(a);
+// a1 .. a5 of square cutouts of 64, 96 or 128 pixels in one launch
+template <int SIDE>
+static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  using Gm = FusedGeomTc<KP, SIDE>;
+  GM_TRY(set_smem_once((const void*)k_tc_fused<KP, SIDE>, (int)Gm::kSmem));
+  const int passes = (a.B + Gm::G - 1) / Gm::G;
+  const int grid = passes < n_sm ? passes : n_sm;
+  k_tc_fused<KP, SIDE><<<grid, kFusedThreadsTc, Gm::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;
+}
+
+int GM_CAT(launch_fused_tc_, GM_TC_K)(const FusedTcArgs& a, int side, int n_sm, cudaStream_t st, cudaError_t* err) {
+  switch (side) {
+    case 64: return launch_fused_t<64>(a, n_sm, st, err);
+    case 96: return launch_fused_t<96>(a, n_sm, st, err);
+    case 128: return launch_fused_t<128>(a, n_sm, st, err);
+    default: return GM_ENOTSUP;
+  }
 }
 
 // larger cutouts, super-tiles of trb x (128 / trb) tiles; bwd = 0: forward kernel, 1: backward kernel

@@ -1,4 +1,4 @@
-// gm_tc_fused.cuh -- steps a1..a5 of the hot path for 128 x 128 cutouts with BOTH convolutions on the
+// gm_tc_fused.cuh -- steps a1..a5 of the hot path for 64 / 96 / 128 px cutouts with BOTH convolutions on the
 // tensor cores (the engine of gm_tc.cuh): one persistent CTA per SM, two cutouts in flight, nothing but
 // chi^2 and the kNSum partial sums per component leaving the SM (mode 0 writes the model image).
 //
@@ -42,13 +42,6 @@ struct FusedTcArgs {
 enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kMaxSlots,
        F_N_BARS = F_B_EMPTY + kMaxSlots };
 static_assert(F_N_BARS <= 64, "barrier area");
-
-template <int KP> struct FusedCfg {
-  using C = Cfg<KP>;
-  // [1 KB: barriers, tensor-memory address, reduction scratch | tap-row rings | 2 slots]
-  static constexpr size_t kSmem = 1024 + 1024 + (size_t)C::kNSlot * C::kTapBytes + 2 * (size_t)C::kSlotWords * 4;
-  static_assert(kSmem <= kSmemLimit, "shared memory");
-};
 
 // the jobs of one CTA in tensor-core order; f(item, phase, slot)
 template <typename F>
@@ -104,10 +97,28 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
   });
 }
 
-template <int KP>
+// Geometry of k_tc_fused for square cutouts of SIDE = 64, 96 or 128 pixels: a cutout is (SIDE / 4) x (SIDE / 32)
+// tiles; G = 4, 1, 1 cutouts share the 128 lanes of a pass (64 px: one lane quarter each; 96 px: 72 lanes used).
+template <int KP, int SIDE> struct FusedGeomTc {
+  using C = Cfg<KP>;
+  static_assert(SIDE == 64 || SIDE == 96 || SIDE == 128, "cutout side");
+  static constexpr int TRC = SIDE / kTileR, TCC = SIDE / kTileC, TPG = TRC * TCC;   // tile rows / columns / tiles per cutout
+  static constexpr int G = 128 / TPG;                         // cutouts per pass
+  static constexpr int W4 = SIDE / 4, kGroups = SIDE * W4;    // groups of four pixels per row / per cutout
+  static constexpr int kCutWords = (SIDE + 1) * SIDE;         // rows + the zero row, pitch = SIDE words (XOR-swizzled chunks)
+  static constexpr int kSlotWordsF = G * kCutWords;
+  static constexpr int kRingF = ((kSmemLimit - 2048 - 2 * (size_t)kSlotWordsF * 4) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
+                                    ? kMaxRing : (int)((kSmemLimit - 2048 - 2 * (size_t)kSlotWordsF * 4) / (2 * (size_t)C::kTapBytes));
+  static_assert(kRingF >= 5, "tap-row rings");
+  static constexpr size_t kSmem = 1024 + 1024 + (size_t)(2 * kRingF) * C::kTapBytes + 2 * (size_t)kSlotWordsF * 4;
+  static_assert(kSmem <= kSmemLimit, "shared memory");
+};
+
+template <int KP, int SIDE>
 __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcArgs a) {
   using C = Cfg<KP>;
-  constexpr int h = C::h;
+  using Gm = FusedGeomTc<KP, SIDE>;
+  constexpr int h = C::h, G = Gm::G;
   extern __shared__ unsigned char smem_raw[];
   unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   uint64_t* bars = reinterpret_cast<uint64_t*>(base);
@@ -115,15 +126,16 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   float* red = reinterpret_cast<float*>(base + 528);                // [kHelpWarpsTc * kNSum] sums, then [8] maxima
   float* redmax = red + kHelpWarpsTc * kNSum;
   unsigned char* ring = base + 1024;
-  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)C::kNSlot * C::kTapBytes);
+  uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)(2 * Gm::kRingF) * C::kTapBytes);
   static_assert(528 + (kHelpWarpsTc * kNSum + 8) * 4 <= 1024, "header area");
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
+  // warp index through a lane-0 broadcast: warp-uniform for the compiler (uniform registers in the role code)
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < C::kNSlot; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    for (int i = 0; i < 2 * Gm::kRingF; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
@@ -131,7 +143,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = tid; i < 2 * C::kSlotWords; i += kFusedThreadsTc) slots[i] = 0u;    // the zero rows
+  for (int i = tid; i < 2 * Gm::kSlotWordsF; i += kFusedThreadsTc) slots[i] = 0u;    // the zero rows
   fence_before();
   __syncthreads();
   fence_after();
@@ -141,9 +153,13 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   const bool with_grad = a.mode == 2;
   const int phases = with_grad ? 2 : 1;
   const int n_gal = a.live ? *a.n_live : a.B;
-  const int n_items = (n_gal - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-  auto galaxy = [&](int item) -> int {                     // -1: a galaxy that no longer iterates
-    const int i = (int)blockIdx.x + item * (int)gridDim.x;
+  // the galaxies of this CTA: entries blockIdx.x, + gridDim.x, ... of the list, G at a time (one item = one pass)
+  const int n_k = (n_gal - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int n_items = (n_k + G - 1) / G;
+  auto galaxy = [&](int item, int g) -> int {              // -1: no galaxy in this place, or one that no longer iterates
+    const int k = item * G + g;
+    if (k >= n_k) return -1;
+    const int i = (int)blockIdx.x + k * (int)gridDim.x;
     const int b = a.live ? a.live[i] : i;
     return (a.frozen && a.frozen[b]) ? -1 : b;
   };
@@ -151,10 +167,14 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
   if (wid < 4) {
     // ------------------------- window rows -> tensor memory --------------------------
     const uint32_t lane_base = (uint32_t)(32 * wid) << 16;
+    const int m = 32 * wid + lane;                         // lane of the tensor memory = tile (g, tr, tc)
+    const int g = m / Gm::TPG, rem = m - g * Gm::TPG;
+    const int tr = rem % Gm::TRC, tc = rem / Gm::TRC;
+    const bool lane_ok = g < G;
     int row_count = 0, cnt[2] = {0, 0};
     for_each_job(n_items, phases, [&](int, int, int s) {
-      const uint32_t slot = smem_u32(slots + (size_t)s * C::kSlotWords);
-      const uint32_t zero = slot + 4u * (kSide * kPitch);
+      const uint32_t cut = smem_u32(slots + (size_t)s * Gm::kSlotWordsF + (size_t)(lane_ok ? g : 0) * Gm::kCutWords);
+      const uint32_t zero = cut + 4u * (SIDE * SIDE);
       mbar_wait(bar(F_IN_FULL + s), cnt[s] & 1);
       ++cnt[s];
       for (int i = 0; i < C::NY; ++i, ++row_count) {
@@ -162,17 +182,17 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         const int buf = row_count % kNBuf;
         mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
         fence_after();
-        const int R = 4 * lane + y - h;
-        const bool row_ok = (unsigned)R < (unsigned)kSide;
-        const uint32_t rowp = slot + 4u * (uint32_t)(R * kPitch);
+        const int R = 4 * tr + y - h;
+        const bool row_ok = lane_ok && (unsigned)R < (unsigned)SIDE;
+        const uint32_t rowp = cut + 4u * (uint32_t)(R * SIDE);
         const int sw = (R >> 2) & 7;
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
-            const int c0 = 32 * wid - h + 16 * kc + 4 * q;
-            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
+            const int c0 = 32 * tc - h + 16 * kc + 4 * q;
+            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)SIDE) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
           uint32_t hi[8], lo[8];
@@ -195,26 +215,28 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     // ------------------------------------ helpers -------------------------------------
     const int hw = wid - 4, htid = tid - 128;
     const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
-    float inv_sc[2] = {1.0f, 1.0f};                       // 1 / scale of what is in slot s (every thread holds the same)
+    float inv_sc[2][G];                                    // 1 / scale of cutout g of slot s (every thread holds the same)
+#pragma unroll
+    for (int g = 0; g < G; ++g) inv_sc[0][g] = inv_sc[1][g] = 1.0f;
     int cnt_d[2] = {0, 0};
-    auto slot_addr = [&](int s) -> uint32_t { return smem_u32(slots + (size_t)s * C::kSlotWords); };
-    auto px_addr = [&](uint32_t slot, int R, int c) -> uint32_t { return slot + 4u * (uint32_t)swz(R, c, kPitch); };
+    auto cut_addr = [&](int s, int g) -> uint32_t { return smem_u32(slots + (size_t)s * Gm::kSlotWordsF + (size_t)g * Gm::kCutWords); };
+    auto px_addr = [&](uint32_t cut, int R, int c) -> uint32_t { return cut + 4u * (uint32_t)swz(R, c, SIDE); };
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
-    constexpr int kGroups = kSide * kSide / 4;            // groups of four pixels of a row; a warp walks one row at a time
+    constexpr int W4 = Gm::W4, kGroups = Gm::kGroups;      // a warp walks whole rows: coalesced global, conflict-free shared
 
-    // fp32 values in the slot -> (hi, lo) fp16 pairs of value * 2^e, e from the largest magnitude `amax`
+    // fp32 values of one cutout -> (hi, lo) fp16 pairs of value * 2^e, e from the largest magnitude `amax`
     // (every thread passes its own maximum; converts the groups it owns)
-    auto scale_and_split = [&](uint32_t slot, float amax) -> float {
+    auto scale_and_split = [&](uint32_t cut, float amax) -> float {
       for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
       if (lane == 0) redmax[hw] = amax;
       help_sync();
-      float m = redmax[0];
+      float mx = redmax[0];
 #pragma unroll
-      for (int w = 1; w < kHelpWarpsTc; ++w) m = fmaxf(m, redmax[w]);
-      const float sc = pow2_scale(m);
+      for (int w = 1; w < kHelpWarpsTc; ++w) mx = fmaxf(mx, redmax[w]);
+      const float sc = pow2_scale(mx);
 #pragma unroll 2
       for (int idx = htid; idx < kGroups; idx += kHN) {
-        const uint32_t p = px_addr(slot, idx >> 5, (idx & 31) << 2);
+        const uint32_t p = px_addr(cut, idx / W4, (idx % W4) << 2);
         const uint4 v = lds128(p);
         sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
                              split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
@@ -227,175 +249,186 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
       if (lane == 0) mbar_arrive(bar(F_IN_FULL + s));
     };
 
-    // a1: S of the cutout (all components go through the PSF on this path) -> slot s
+    // a1: S of every cutout of the item (all components go through the PSF on this path) -> slot s
     auto produce = [&](int item, int s) {
-      const int b = galaxy(item);
-      const uint32_t slot = slot_addr(s);
-      float amax = 0.0f;
-      if (b >= 0) {
-        const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
-        for (int c = 0; c < a.md.n_comp; ++c) {
-          const CompConst cc = ccb[c];
-          const bool box = a.md.box[c] != 0;
-          const bool first = c == 0, last = c == a.md.n_comp - 1;
-          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-            for (int idx = htid; idx < kGroups; idx += kHN) {
-              const int R = idx >> 5, x = (idx & 31) << 2;
-              float v[4];
-              value4<KIND, kFastForward>(cc, box, (float)x + 0.5f, (float)kSide - 0.5f - (float)R, v);   // R:G1
-              const uint32_t p = px_addr(slot, R, x);
-              if (!first) {
-                const uint4 q = lds128(p);
-                v[0] += __uint_as_float(q.x); v[1] += __uint_as_float(q.y); v[2] += __uint_as_float(q.z); v[3] += __uint_as_float(q.w);
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int b = galaxy(item, g);
+        const uint32_t cut = cut_addr(s, g);
+        float amax = 0.0f;
+        if (b >= 0) {
+          const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+          for (int c = 0; c < a.md.n_comp; ++c) {
+            const CompConst cc = ccb[c];
+            const bool box = a.md.box[c] != 0;
+            const bool first = c == 0, last = c == a.md.n_comp - 1;
+            dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+              for (int idx = htid; idx < kGroups; idx += kHN) {
+                const int R = idx / W4, x = (idx % W4) << 2;
+                float v[4];
+                value4<KIND, kFastForward>(cc, box, (float)x + 0.5f, (float)SIDE - 0.5f - (float)R, v);   // R:G1
+                const uint32_t p = px_addr(cut, R, x);
+                if (!first) {
+                  const uint4 q = lds128(p);
+                  v[0] += __uint_as_float(q.x); v[1] += __uint_as_float(q.y); v[2] += __uint_as_float(q.z); v[3] += __uint_as_float(q.w);
+                }
+                if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
+                sts128(p, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
               }
-              if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
-              sts128(p, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
-            }
-          });
+            });
+          }
+        } else {
+          for (int idx = htid; idx < kGroups; idx += kHN) sts128(px_addr(cut, idx / W4, (idx % W4) << 2), make_uint4(0u, 0u, 0u, 0u));
         }
-      } else {
-        for (int idx = htid; idx < kGroups; idx += kHN) sts128(px_addr(slot, idx >> 5, (idx & 31) << 2), make_uint4(0u, 0u, 0u, 0u));
+        if (!isfinite(amax)) amax = 0.0f;
+        inv_sc[s][g] = scale_and_split(cut, amax);
       }
-      inv_sc[s] = scale_and_split(slot, amax);
       signal_input(s);
     };
 
-    // accumulators of the job on slot s -> the slot, as fp32 (tile m = lane m: rows 4 t + r, columns 32 q ..)
+    // accumulators of the job on slot s -> the cutouts of the slot, as fp32
     auto drain = [&](int item, int s) {
-      const int b = galaxy(item);
-      const uint32_t slot = slot_addr(s);
       mbar_wait(bar(F_D_FULL + s), cnt_d[s] & 1);
       ++cnt_d[s];
       fence_after();
-      const float inv = inv_sc[s] * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
-      const int q = hw & 3, r_first = 2 * (hw >> 2);
+      const int m = 32 * (hw & 3) + lane;                  // this thread's lane of the tensor memory
+      const int g = m / Gm::TPG, rem = m - g * Gm::TPG;
+      const int tr = rem % Gm::TRC, tc = rem / Gm::TRC;
+      const bool lane_ok = g < G;
+      const int b = lane_ok ? galaxy(item, g) : -1;
+      float isc = 1.0f;
+#pragma unroll
+      for (int gg = 0; gg < G; ++gg) isc = (gg == g) ? inv_sc[s][gg] : isc;
+      const float inv = isc * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
+      const uint32_t cut = cut_addr(s, lane_ok ? g : 0);
+      const int r_first = 2 * (hw >> 2);
 #pragma unroll 1
       for (int r = r_first; r < r_first + 2; ++r) {
         uint32_t v[32];
         tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (lane_ok) {
 #pragma unroll
-        for (int k = 0; k < 8; ++k)
-          sts128(px_addr(slot, 4 * lane + r, 32 * q + 4 * k), make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
-                                         __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
+          for (int k = 0; k < 8; ++k)
+            sts128(px_addr(cut, 4 * tr + r, 32 * tc + 4 * k),
+                   make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+                              __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
+        }
       }
       fence_before();
-      help_sync();                                         // the whole image is in the slot
+      help_sync();                                         // every image is in the slot
     };
 
     // a3: M (slot, fp32) -> chi^2 and G in place, then G as fp16 pairs for the adjoint convolution; mode 0 writes M out
     auto residual = [&](int item, int s) {
-      const int b = galaxy(item);
-      const uint32_t slot = slot_addr(s);
-      float chi2 = 0.0f, amax = 0.0f;
-      if (b >= 0) {
-        const size_t img = (size_t)b * kSide * kSide;
-        if (a.mode == 0) {
-          for (int idx = htid; idx < kGroups; idx += kHN) {
-            const uint4 v = lds128(px_addr(slot, idx >> 5, (idx & 31) << 2));
-            *reinterpret_cast<float4*>(a.out + img + 4 * (size_t)idx) =
-                make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
-          }
-        } else {
-          // branch free; the weight and the residual are SELECTED for unused pixels, never multiplied by 0 (R:X1)
-          auto one = [&](float m, float d, float sg, bool used) -> float {
-            float w = rcp_fast(sg * sg), rho = d - m;
-            w = used ? w : 0.0f;
-            rho = used ? rho : 0.0f;
-            const float t = w * rho;
-            chi2 = fmaf(t, rho, chi2);
-            const float g = -2.0f * t;
-            amax = fmaxf(amax, fabsf(g));
-            return g;
-          };
-          const float4* dptr = reinterpret_cast<const float4*>(a.data + img);
-          const float4* sptr = reinterpret_cast<const float4*>(a.sigma + img);
-          auto pass = [&]<bool MASKED>() {
-            const uchar4* kptr = MASKED ? reinterpret_cast<const uchar4*>(a.mask + img) : nullptr;
-#pragma unroll 2
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int b = galaxy(item, g);
+        const uint32_t cut = cut_addr(s, g);
+        float chi2 = 0.0f, amax = 0.0f;
+        if (b >= 0) {
+          const size_t img = (size_t)b * SIDE * SIDE;
+          if (a.mode == 0) {
             for (int idx = htid; idx < kGroups; idx += kHN) {
-              const uint32_t p = px_addr(slot, idx >> 5, (idx & 31) << 2);
-              const float4 d4 = dptr[idx], s4 = sptr[idx];
-              uchar4 k4 = make_uchar4(1, 1, 1, 1);
-              if (MASKED) k4 = kptr[idx];
-              const uint4 m4 = lds128(p);
-              uint4 g;
-              g.x = __float_as_uint(one(__uint_as_float(m4.x), d4.x, s4.x, !MASKED || k4.x != 0));
-              g.y = __float_as_uint(one(__uint_as_float(m4.y), d4.y, s4.y, !MASKED || k4.y != 0));
-              g.z = __float_as_uint(one(__uint_as_float(m4.z), d4.z, s4.z, !MASKED || k4.z != 0));
-              g.w = __float_as_uint(one(__uint_as_float(m4.w), d4.w, s4.w, !MASKED || k4.w != 0));
-              if (with_grad) sts128(p, g);
+              const uint4 v = lds128(px_addr(cut, idx / W4, (idx % W4) << 2));
+              *reinterpret_cast<float4*>(a.out + img + 4 * (size_t)idx) =
+                  make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
             }
-          };
-          if (a.mask) pass.template operator()<true>();
-          else pass.template operator()<false>();
+          } else {
+            // branch free; the weight and the residual are SELECTED for unused pixels, never multiplied by 0 (R:X1)
+            auto one = [&](float mm, float d, float sg, bool used) -> float {
+              float w = rcp_fast(sg * sg), rho = d - mm;
+              w = used ? w : 0.0f;
+              rho = used ? rho : 0.0f;
+              const float t = w * rho;
+              chi2 = fmaf(t, rho, chi2);
+              const float gg = -2.0f * t;
+              amax = fmaxf(amax, fabsf(gg));
+              return gg;
+            };
+            const float4* dptr = reinterpret_cast<const float4*>(a.data + img);
+            const float4* sptr = reinterpret_cast<const float4*>(a.sigma + img);
+            auto pass = [&]<bool MASKED>() {
+              const uchar4* kptr = MASKED ? reinterpret_cast<const uchar4*>(a.mask + img) : nullptr;
+#pragma unroll 2
+              for (int idx = htid; idx < kGroups; idx += kHN) {
+                const uint32_t p = px_addr(cut, idx / W4, (idx % W4) << 2);
+                const float4 d4 = dptr[idx], s4 = sptr[idx];
+                uchar4 k4 = make_uchar4(1, 1, 1, 1);
+                if (MASKED) k4 = kptr[idx];
+                const uint4 m4 = lds128(p);
+                uint4 gv;
+                gv.x = __float_as_uint(one(__uint_as_float(m4.x), d4.x, s4.x, !MASKED || k4.x != 0));
+                gv.y = __float_as_uint(one(__uint_as_float(m4.y), d4.y, s4.y, !MASKED || k4.y != 0));
+                gv.z = __float_as_uint(one(__uint_as_float(m4.z), d4.z, s4.z, !MASKED || k4.z != 0));
+                gv.w = __float_as_uint(one(__uint_as_float(m4.w), d4.w, s4.w, !MASKED || k4.w != 0));
+                if (with_grad) sts128(p, gv);
+              }
+            };
+            if (a.mask) pass.template operator()<true>();
+            else pass.template operator()<false>();
+          }
         }
-      }
-      if (a.mode != 0) {
-        chi2 = warp_sum(chi2);
-        if (lane == 0) red[hw] = chi2;
-        if (!isfinite(amax)) amax = 0.0f;                  // a non-finite chi^2 is reported through chi2_part; keep the scale sane
-        if (with_grad) {
-          inv_sc[s] = scale_and_split(slot_addr(s), amax); // its first barrier also publishes red[]
-        } else {
-          help_sync();
+        if (a.mode != 0) {
+          chi2 = warp_sum(chi2);
+          if (lane == 0) red[hw] = chi2;
+          if (!isfinite(amax)) amax = 0.0f;                // a non-finite chi^2 is reported through chi2_part; keep the scale sane
+          if (with_grad) inv_sc[s][g] = scale_and_split(cut, amax);     // its first barrier also publishes red[]
+          else help_sync();
+          if (htid == 0 && b >= 0) {
+            float t = 0.0f;
+            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
+            a.chi2_part[b] = t;
+          }
+          help_sync();                                     // red[] may be rewritten
         }
-        if (htid == 0 && b >= 0) {
-          float t = 0.0f;
-          for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
-          a.chi2_part[b] = t;
-        }
-        help_sync();                                       // red[] may be rewritten
       }
     };
 
     // a5: the partial sums of every component from A (slot, fp32)
     auto gradient = [&](int item, int s) {
-      const int b = galaxy(item);
-      const uint32_t slot = slot_addr(s);
-      for (int c = 0; c < a.md.n_comp; ++c) {
-        float sm[kNSum];
 #pragma unroll
-        for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
-        if (b >= 0) {
-          const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
-          const bool box = a.md.box[c] != 0;
-          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-            if (box) {                                     // Eq. 2 with B != 0: per-pixel geometry
-              for (int idx = htid; idx < kGroups; idx += kHN) {
-                const int R = idx >> 5, x = (idx & 31) << 2;
-                const uint4 q = lds128(px_addr(slot, R, x));
-                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+      for (int g = 0; g < G; ++g) {
+        const int b = galaxy(item, g);
+        const uint32_t cut = cut_addr(s, g);
+        for (int c = 0; c < a.md.n_comp; ++c) {
+          float sm[kNSum];
 #pragma unroll
-                for (int k = 0; k < 4; ++k)
-                  grad_accumulate<KIND>(cc, true, seed[k], (float)(x + k) + 0.5f, (float)kSide - 0.5f - (float)R, sm);
-              }
-            } else {
+          for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
+          if (b >= 0) {
+            const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
+            const bool box = a.md.box[c] != 0;
+            dispatch_kind(a.md.kind[c], [&]<int KIND>() {
               GradAcc<KIND> acc;
               acc.init();
               for (int idx = htid; idx < kGroups; idx += kHN) {
-                const int R = idx >> 5, x = (idx & 31) << 2;
-                const uint4 q = lds128(px_addr(slot, R, x));
+                const int R = idx / W4, x = (idx % W4) << 2;
+                const uint4 q = lds128(px_addr(cut, R, x));
                 const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
-                grad_add4<KIND>(acc, cc, seed, (float)x + 0.5f, (float)kSide - 0.5f - (float)R);
-              }
-              acc.finish(cc, sm);
-            }
-          });
-          if (!box) sm[8] = sm[2];
-        }
+                if (box) {                                 // Eq. 2 with B != 0: per-pixel geometry
 #pragma unroll
-        for (int k = 0; k < kNSum; ++k) {
-          const float v = warp_sum(sm[k]);
-          if (lane == 0) red[hw * kNSum + k] = v;
+                  for (int k = 0; k < 4; ++k)
+                    grad_accumulate<KIND>(cc, true, seed[k], (float)(x + k) + 0.5f, (float)SIDE - 0.5f - (float)R, sm);
+                } else {
+                  grad_add4<KIND>(acc, cc, seed, (float)x + 0.5f, (float)SIDE - 0.5f - (float)R);
+                }
+              }
+              if (!box) { acc.finish(cc, sm); sm[8] = sm[2]; }
+            });
+          }
+#pragma unroll
+          for (int k = 0; k < kNSum; ++k) {
+            const float v = warp_sum(sm[k]);
+            if (lane == 0) red[hw * kNSum + k] = v;
+          }
+          help_sync();
+          if (htid < kNSum && b >= 0) {
+            float t = 0.0f;
+            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
+            a.grad_part[((size_t)b * a.md.n_comp + c) * kNSum + htid] = t;
+          }
+          help_sync();
         }
-        help_sync();
-        if (htid < kNSum && b >= 0) {
-          float t = 0.0f;
-          for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
-          a.grad_part[((size_t)b * a.md.n_comp + c) * kNSum + htid] = t;
-        }
-        help_sync();
       }
     };
 
@@ -412,7 +445,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         else feed(item + 2, s);
       }
       if (with_grad) {
-        for (int s = 0; s < 2; ++s) {                     // after C2: gradient, then the next cutout
+        for (int s = 0; s < 2; ++s) {                     // after C2: gradient, then the next cutouts
           const int item = 2 * m + s;
           if (item >= n_items) continue;
           drain(item, s);
@@ -423,25 +456,29 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     }
   } else if (wid < kLastWarp) {
     // ----------------------------------- MMA issue ------------------------------------
+    // (the accumulator row is a template argument so that every address of the issue loop is warp-uniform at
+    // compile time and stays in uniform registers)
     static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, C::kRing>(n_items, phases, b0, r0, tD, tA);
-    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, C::kRing>(n_items, phases, b0, r0, tD, tA);
-    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, C::kRing>(n_items, phases, b0, r0, tD, tA);
-    else fused_mma_role<KP, 3, C::kRing>(n_items, phases, b0, r0, tD, tA);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    else fused_mma_role<KP, 3, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
+    // in the order of first use: window row y = seq(i) brings tap row y (r = 0) on the low side and
+    // tap row y - 3 (r = 3) on the high side.  Several cutouts per pass share one PSF (the host sees to it).
     if (lane == 0) {
       int jc = 0;
       for_each_job(n_items, phases, [&](int item, int ph, int) {
-        const int b = galaxy(item);
+        const int b = galaxy(item, 0);
         const uint8_t* tab = (ph ? a.btab_adj : a.btab_fwd) + (size_t)(b >= 0 ? b : 0) * a.btab_stride;
         for (int i = 0; i < C::NY; ++i) {
           const int y = C::seq(i);
           const int ta = (i & 1) ? y - (kTileR - 1) : y;
           if ((i & 1) ? (ta < C::kNLow || ta >= KP) : (ta >= C::kNLow)) continue;
-          const int slot = C::template slot_of<C::kRing>(ta);
-          const uint32_t gen = (uint32_t)(jc * C::template uses_of_slot<C::kRing>(slot) + C::template index_in_slot<C::kRing>(ta));
+          const int slot = C::template slot_of<Gm::kRingF>(ta);
+          const uint32_t gen = (uint32_t)(jc * C::template uses_of_slot<Gm::kRingF>(slot) + C::template index_in_slot<Gm::kRingF>(ta));
           mbar_wait(bar(F_B_EMPTY + slot), (gen & 1) ^ 1);
           mbar_expect_tx(bar(F_B_FULL + slot), C::kTapBytes);
           bulk_g2s(smem_u32(ring + (size_t)slot * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + slot));

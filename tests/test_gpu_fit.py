@@ -130,7 +130,9 @@ def test_fit_multi_equals_fit_per_batch_bitwise():
             assert np.array_equal(s[key], m[key], equal_nan=True), key
 
 
-def test_constant_tap_pool_exhaustion_falls_back_bitwise():
+def test_constant_tap_pool_exhaustion_falls_back_bitwise(request):
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # the constant-bank taps belong to the FFMA2 engine
+    request.addfinalizer(lambda: gm.gm_set_option(gm.GM_OPT_TENSOR, 1))
     # the paired taps of a shared PSF live in a 59 KB constant-bank pool, 10.8 KB per call in
     # flight at K = 25: of seven concurrent buckets two find no region and run the shared-memory
     # taps.  Both forms add the products in the same order, so every bucket must give exactly

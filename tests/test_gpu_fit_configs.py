@@ -34,7 +34,7 @@ def test_c2_every_bucket_through_fit_multi_early_stop_masked():
     # mask on, tol 1e-6 / patience 10, cap 500, all five sides in ONE gm_fit_multi call: the
     # 64 / 96 / 128 px buckets run k_fused with the live list, 192 / 256 px the tile kernels.
     # The iteration at which the stop rule fires is not unique at tol = 1e-6 (fit_parity.py), so
-    # (1) the oracle's own early-stop run must agree in status and, loosely, in iteration count,
+    # (1) wherever the GPU stopped earlier than the oracle's own run, the oracle's chi^2 was already flat,
     # (2) the oracle's trajectory read at the GPU's iteration count must be the GPU's parameters.
     buckets = fp.case_c2(range(60))
     assert sorted(b["H"] for b, _ in buckets) == [64, 96, 128, 192, 256]
@@ -42,8 +42,8 @@ def test_c2_every_bucket_through_fit_multi_early_stop_masked():
     stopped = 0
     for (b, opts), g in zip(buckets, outs):
         assert b["mask"] is not None and opts["tol"] > 0 and opts["n_iter"] == 500
-        ok, dt = fp.stop_decision_ok(g, fp.oracle_fit(b, opts), opts["patience"])
-        assert ok, f"C2/{b['H']}px: stop decisions differ, |d iterations| = {dt}"
+        ok, dt = fp.stop_decision_ok(g, fp.oracle_fit(b, opts, want_trace=True), opts)
+        assert ok, f"C2/{b['H']}px: the GPU stopped a galaxy while the oracle's chi^2 still moved; |d iterations| = {dt}"
         o = fp.oracle_fit_at_iters(b, opts, g["iters_used"])
         j = fp.judge(b, g, o)
         # profiles/r02_parity.md (120-galaxy sample): 0.966 .. 1.000 per bucket; the 8 .. 19 galaxies per bucket of

@@ -108,24 +108,39 @@ def test_psf_orientation_not_flipped_or_transposed():
     assert_pixels(img, oracle.render(model, par, H, W, psf))
 
 
-def test_shared_and_per_galaxy_psf_agree_bitwise():
-    model = models.single_sersic()
-    b = configs.make_batch(0, range(4), oracle_render)
-    rep = np.ascontiguousarray(np.broadcast_to(b["psf"], (4, 15, 15)))
-    a = gm.gm_render(model, dev(b["start"]), 64, 64, dev(b["psf"]))
-    c = gm.gm_render(model, dev(b["start"]), 64, 64, dev(rep))
-    assert torch.equal(a, c)
+@pytest.mark.parametrize("side,cid", [(64, 0), (128, 1)])
+def test_shared_and_per_galaxy_psf_agree_bitwise(side, cid):
+    # one PSF for the batch or the same PSF replicated per galaxy (reading C4): identical pixels wherever both run
+    # the same engine -- always on the FFMA2 path, and on the tensor-core path where it takes per-galaxy PSFs
+    # (128 px; four 64 px cutouts share the lanes of a pass and so one PSF, which sends them to the FFMA2 path)
+    b = configs.make_batch(cid, range(4), oracle_render)
+    model, K = b["model"], b["psf"].shape[0]
+    rep = np.ascontiguousarray(np.broadcast_to(b["psf"], (4, K, K)))
+    ref = oracle.render(model, b["start"], side, side, b["psf"])
+    for tensor in (1, 0):
+        gm.gm_set_option(gm.GM_OPT_TENSOR, tensor)
+        try:
+            a = gm.gm_render(model, dev(b["start"]), side, side, dev(b["psf"]))
+            c = gm.gm_render(model, dev(b["start"]), side, side, dev(rep))
+        finally:
+            gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
+        if tensor == 0 or side == 128:
+            assert torch.equal(a, c)
+        assert_pixels(a.cpu().numpy(), ref)
+        assert_pixels(c.cpu().numpy(), ref)
 
 
 @pytest.mark.parametrize("H,W,K", [(64, 64, 25), (96, 96, 9), (128, 128, 41), (100, 90, 33), (192, 192, 25),
                                    (256, 256, 41), (140, 200, 15), (37, 45, 7)])
-def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K):
+def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K, request):
     # a batch-wide PSF runs the convolution with its taps in the constant bank (FFMA2 with a
     # uniform-register operand), a per-galaxy PSF or gm_set_option(GM_OPT_CONST_TAPS, 0) in shared
     # memory; both add the K^2 products of a pixel in the same order, in k_fused and in the
     # tile kernels, for every compiled PSF side and both thread tiles
     model = models.bulge_disk()
     par, data, sigma, mask, psf = synth(model, 3, H, W, K, seed=7 * H + W + K)
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # this test is about the FFMA2 engine's two tap homes
+    request.addfinalizer(lambda: gm.gm_set_option(gm.GM_OPT_TENSOR, 1))
     def run():
         img = gm.gm_render(model, dev(par), H, W, dev(psf))
         out = gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(psf))
@@ -150,9 +165,11 @@ def test_constant_bank_and_shared_memory_taps_agree_bitwise(H, W, K):
     assert_chi2(const[1].cpu().numpy(), oracle.loss_grad(model, par, data, sigma, mask, psf)[0])
 
 
-def test_constant_tap_regions_are_refilled_between_and_across_calls():
+def test_constant_tap_regions_are_refilled_between_and_across_calls(request):
     # a pool region is reused by the next call with another PSF, and concurrent calls on their own
     # streams hold different PSFs at the same time: nobody may see somebody else's (or stale) taps
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # the constant-bank taps belong to the FFMA2 engine
+    request.addfinalizer(lambda: gm.gm_set_option(gm.GM_OPT_TENSOR, 1))
     model = models.single_sersic()
     H = W = 64; K = 25
     par, data, sigma, mask, _ = synth(model, 4, H, W, K, seed=99)
