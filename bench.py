@@ -223,6 +223,24 @@ class Bench:
         self.pk = pk
         self.f_mhz = pk.get("sm_max_mhz", 1965.0)
         self.peak_nominal = SM_COUNT * FP32_LANES * 2 * self.f_mhz * 1e6 / 1e12
+        self.peak_tensor = pk.get("bf16_tflops_sustained") or pk["bf16_tflops"]
+
+    @staticmethod
+    def mma_inflation(name, k):
+        """MMA flops the tensor-core kernels issue per algorithmic convolution flop (1 for the FFMA2 kernels).
+        One pass = 128 lanes of 4 x 32 output pixels; per pass and convolution KT tap rows x 4 accumulator rows x
+        NCH 16-column chunks x 3 split terms MMAs of 128 x 32 x 16 (gm_tc.cuh)."""
+        if not name.startswith("tc_"):
+            return 1.0
+        K, H, W = k["K"], k["H"], k["W"]
+        KT = next(t for t in (9, 17, 25, 33, 41) if t >= K)
+        nch = (32 + KT - 1 + 15) // 16
+        per_pass = KT * 4 * nch * 3 * (2.0 * 128 * 32 * 16)
+        if name == "tc_fused":
+            passes = {64: 0.25, 96: 1.0, 128: 1.0}[H]                     # per cutout
+        else:
+            passes = min(-(-H // (4 * c)) * -(-W // (32 * (128 // c))) for c in (32, 16, 64))
+        return passes * per_pass / (2.0 * H * W * K * K)
 
     def barrier(self):
         if self.dist is not None:
@@ -367,12 +385,18 @@ class Bench:
                                "mean_iters": float(iters.mean()), "median_reduced_chi2": float(np.median(red))},
                "clocks": clk.summary(), "gpu_launches": int(launches)}
 
-        # ---- roofline of the heavy kernels (all run the same K^2-tap FFMA2 loop)
+        # ---- roofline of the heavy kernels: algorithmic convolution flops (2 K^2 per pixel per convolution,
+        # SURVEY 8(d)) against the pipe that binds the kernel: the tensor pipe for the tcgen05 kernels (k_tc_*),
+        # the FP32 FMA pipe for the FFMA2 kernels
+        def flops_of(name, f_fwd, f_bwd):
+            return (f_fwd + f_bwd) if name.endswith("fused") else (f_fwd if name.endswith("forward") else f_bwd)
+
         kinds = {name: (ms, n) for name, (ms, n) in prof.items() if n}
+        kern, dom, achieved, issued = {}, None, None, None
         if multi and serial_profile and self.rank == 0:
             # buckets on concurrent streams: per-launch event times overlap one another.  One more
             # step, bucket after bucket on one stream, gives every kernel its own duration.
-            per_kind_ms = {}; per_kind_n = {}; per_kind_flops = {}
+            per_kind_ms = {}; per_kind_n = {}; per_kind_flops = {}; per_kind_issued = {}
             for k in buckets:
                 k["params"].copy_(k["dev"][4])
                 gm.gm_profile_enable(True)
@@ -386,46 +410,65 @@ class Bench:
                 for name, (ms, n) in pr.items():
                     if not n:
                         continue
+                    fl = flops_of(name, f_fwd, f_bwd)
                     per_kind_ms[name] = per_kind_ms.get(name, 0.0) + ms
                     per_kind_n[name] = per_kind_n.get(name, 0) + n
-                    fl = (f_fwd + f_bwd) if name == "fused" else (f_fwd if name == "forward" else f_bwd)
                     per_kind_flops[name] = per_kind_flops.get(name, 0.0) + fl
+                    per_kind_issued[name] = per_kind_issued.get(name, 0.0) + fl * self.mma_inflation(name, k)
+                    pk_k = self.peak_tensor if name.startswith("tc_") else self.peak_measured
                     k.setdefault("serial", {})[name] = {"launches": n, "avg_ms": ms / n,
-                                                        "frac_measured": fl / (ms * 1e-3) / 1e12 / self.peak_measured}
+                                                        "tflops": fl / (ms * 1e-3) / 1e12,
+                                                        "frac": fl / (ms * 1e-3) / 1e12 / pk_k,
+                                                        "bound": "tensor" if name.startswith("tc_") else "alu"}
                 assert ran, "no heavy kernel ran"
             kern = {name: {"launches": per_kind_n[name], "avg_ms": per_kind_ms[name] / per_kind_n[name],
                            "tflops": per_kind_flops[name] / (per_kind_ms[name] * 1e-3) / 1e12}
                     for name in per_kind_ms}
             dom = max(kern, key=lambda n: per_kind_ms[n])
             achieved = kern[dom]["tflops"]
+            issued = per_kind_issued[dom] / (per_kind_ms[dom] * 1e-3) / 1e12
             how_t = ("one extra step with the buckets one after the other on one stream (per-launch CUDA events do not "
                      "overlap there); the timed steps run the buckets concurrently")
             rec["buckets"] = [{"side": k["H"], "galaxies": k["B"], "kernels": k.get("serial")} for k in buckets]
-        else:
-            heavy_ms = sum(ms for ms, n in kinds.values())
+        elif kinds:
             kern = {name: {"launches": n, "avg_ms": ms / n} for name, (ms, n) in kinds.items()}
-            dom = max(kern, key=lambda n: kern[n]["avg_ms"] * kern[n]["launches"]) if kern else None
-            achieved = steps * conv_flops / (heavy_ms * 1e-3) / 1e12 if heavy_ms else None
-            how_t = "summed CUDA-event time of the heavy kernels (forward, backward, fused) inside the timed region"
+            dom = max(kern, key=lambda n: kinds[n][0])
+            # the kernels of one family run the same loop: their flops over their summed time
+            fam = [n for n in kinds if n.startswith("tc_") == dom.startswith("tc_")]
+            fam_ms = sum(kinds[n][0] for n in fam)
+            fam_fl = sum(flops_of(n, fwd, bwd) for n in fam for fwd, bwd in flops) * steps
+            achieved = fam_fl / (fam_ms * 1e-3) / 1e12
+            issued = sum(flops_of(n, fwd, bwd) * self.mma_inflation(n, k) for n in fam
+                         for (fwd, bwd), k in zip(flops, buckets)) * steps / (fam_ms * 1e-3) / 1e12
+            how_t = "summed CUDA-event time of those kernels inside the timed region"
             for name in kern:
                 kern[name]["share_of_step"] = kinds[name][0] / t_ms if world == 1 else None
         if dom:
             big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
             px_bytes = 9 if big["dev"][2] is not None else 8
+            tensor = dom.startswith("tc_")
+            peak = self.peak_tensor if tensor else self.peak_measured
             rec["roofline"] = {
-                "bound": "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved, "peak": self.peak_measured,
-                "unit": "TFLOP/s", "frac": achieved / self.peak_measured,
-                "peak_source": "measured in this process: gm_measure_fp32_peak, a pure fma.rn.f32x2 kernel (include/gm.h)",
-                "peak_nominal": self.peak_nominal, "frac_of_nominal": achieved / self.peak_nominal,
-                "peak_nominal_source": f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 flop x {self.f_mhz:.0f} MHz "
-                                       f"(sm_max_mhz of {self.pk_src} MEASURED_PEAKS.json)",
+                "bound": "tensor" if tensor else "alu", "kernel": f"k_{dom}<K={K}>", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak,
+                "peak_source": (f"{self.pk_src} MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 GEMM back to back; fp16 "
+                                "runs at the bf16 rate); the kernel is timed inside a long step, so the sustained figure")
+                if tensor else "measured in this process: gm_measure_fp32_peak, a pure fma.rn.f32x2 kernel (include/gm.h)",
                 "traffic": traffic_from_profiles(dom, K, big),
                 "algorithmic_bytes_per_px_eval": px_bytes,
                 "how": "2*K^2 flops per pixel per convolution x convolutions actually run (2 per chi^2+gradient "
                        "evaluation + the closing forward) / " + how_t,
                 "hbm_peak_gbs": self.pk.get("hbm_gbs"), "kernels": kern,
+                # the same flops against the FP32 FMA pipe, the bound of the direct (FFMA2) convolution this engine replaces
+                "fp32_peak": self.peak_measured, "frac_of_fp32_peak": achieved / self.peak_measured,
+                "fp32_peak_nominal": self.peak_nominal,
                 # whole-step view: the same flops against the step time (small kernels and gaps included)
-                "step_frac": (conv_flops / (ms_per_step * 1e-3) / 1e12) / self.peak_measured}
+                "step_frac": (conv_flops / (ms_per_step * 1e-3) / 1e12) / peak}
+            if tensor:
+                # what the tensor pipe is asked to do for those flops: 3 fp16 MMAs per product (hi*hi + lo*hi + hi*lo)
+                # on Toeplitz band blocks: issued MMA flops / the same time / the same peak
+                rec["roofline"].update({"mma_issued_tflops": issued, "mma_issued_frac": issued / peak,
+                                        "mma_flops_per_algorithmic_flop": issued / achieved})
 
         # ---- e2e: the same step through the host-buffer C-ABI call (copies inside)
         if want_e2e:
@@ -481,7 +524,8 @@ class Bench:
         ms = statistics.median(a.elapsed_time(z) for a, z in tt)
         return {"value": k["B"] * k["H"] * k["W"] / (ms * 1e-3), "unit": UNIT, "ms_per_call": ms, "calls": 20,
                 "stat": "median",
-                "frac": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12 / self.peak_measured,
+                "tflops": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12,
+                "frac_of_fp32_peak": 2 * 2.0 * k["B"] * k["H"] * k["W"] * k["K"] ** 2 / (ms * 1e-3) / 1e12 / self.peak_measured,
                 "api": "gm_loss_grad (prologue, taps, chi^2 + gradient, finalize: the whole call)"}
 
     def streamed(self, k, n_batches):
@@ -624,7 +668,9 @@ def run_ours(args):
             r = bn.measure(c, bk, sub_steps, 3, False, want_e2e=True)
             r.pop("_outs")
             rf = r.pop("roofline", None) or {}
-            r.update({"steps": sub_steps, "frac": rf.get("frac"), "frac_of_nominal": rf.get("frac_of_nominal"),
+            r.update({"steps": sub_steps, "bound": rf.get("bound"), "kernel": rf.get("kernel"), "frac": rf.get("frac"),
+                      "peak": rf.get("peak"), "frac_of_fp32_peak": rf.get("frac_of_fp32_peak"),
+                      "mma_issued_frac": rf.get("mma_issued_frac"),
                       "step_frac": rf.get("step_frac"), "achieved_tflops": rf.get("achieved"),
                       "traffic": rf.get("traffic"), "kernels": rf.get("kernels")})
             if key == "C1":

@@ -325,14 +325,30 @@ int64_t     gm_last_launch_count(void);
 /* ---- measurement hooks (used by bench.py for the roofline line) ---------------- */
 /* While enabled, every launch of the heavy kernels is bracketed by CUDA events
  * recorded on the launching stream (at most 8192 launches are kept):
- *   [0] forward tile kernel  (render + PSF convolution + residual)
- *   [1] backward tile kernel (adjoint convolution + gradient sums)
- *   [2] fused kernel         (all of the above for cutouts that fit one CTA)
+ *   [GM_PROF_FORWARD]     k_forward   FFMA2 tile kernel (render + PSF convolution + residual)
+ *   [GM_PROF_BACKWARD]    k_backward  FFMA2 tile kernel (adjoint convolution + gradient sums)
+ *   [GM_PROF_FUSED]       k_fused     FFMA2, all of the above for cutouts that fit one CTA
+ *   [GM_PROF_TC_FORWARD]  k_tc_tile   tensor-core forward kernel of cutouts above 128 px
+ *   [GM_PROF_TC_BACKWARD] k_tc_tile   tensor-core backward kernel
+ *   [GM_PROF_TC_FUSED]    k_tc_fused  tensor cores, 64 / 96 / 128 px cutouts in one launch
  * gm_profile_read waits for them, returns the summed durations in milliseconds and
  * the launch counts per kind, and clears the list.  Off by default; enabling or
  * disabling also clears it. */
 int gm_profile_enable(int on);
-int gm_profile_read(double* ms /* host [3] */, int64_t* count /* host [3] */);
+enum { GM_PROF_FORWARD = 0, GM_PROF_BACKWARD = 1, GM_PROF_FUSED = 2, GM_PROF_TC_FORWARD = 3, GM_PROF_TC_BACKWARD = 4,
+       GM_PROF_TC_FUSED = 5, GM_PROF_KINDS = 6 };
+int gm_profile_read(double* ms /* host [GM_PROF_KINDS] */, int64_t* count /* host [GM_PROF_KINDS] */);
+
+/* Phase trace of k_tc_fused (the tensor-core kernel of 64 / 96 / 128 px cutouts).  While `device_buf`
+ * (device memory, GM_TRACE_ROLES * GM_TRACE_CAP uint64, zeroed by the caller) is set, CTA 0 of every
+ * launch appends one record per phase boundary to the list of its role, from the start of the list:
+ * record = (tag << 56 | item << 48 | clock64 & (2^48 - 1)); roles: 0 helper warps (render, drain,
+ * residual, gradient), 1 MMA issue (first window row ready / last MMA issued, per convolution),
+ * 2 unused.  Tags in gm_tc_fused.cuh (TR_*).  nullptr switches it off (default).  Not thread safe
+ * against concurrent launches; a measurement hook, one launch at a time. */
+#define GM_TRACE_ROLES 3
+#define GM_TRACE_CAP   2048
+int gm_trace_set(unsigned long long* device_buf);
 
 /* The FP32 peak the roofline is quoted against, MEASURED: a kernel of nothing but
  * independent packed FP32 multiply-adds (fma.rn.f32x2, the instruction of the convolution

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     gm_init,
     gm_measure_fp32_peak,
     gm_set_option,
+    gm_trace_set,
     gm_bootstrap,
     gm_bootstrap_counts,
     gm_conv,

@@ -107,6 +107,7 @@ def _lib():
         L.gm_set_option.restype = i; L.gm_set_option.argtypes = [i, i]
         L.gm_get_option.restype = i; L.gm_get_option.argtypes = [i]
         L.gm_measure_fp32_peak.restype = i
+        L.gm_trace_set.restype = i; L.gm_trace_set.argtypes = [vp]
         L.gm_measure_fp32_peak.argtypes = [i, C.POINTER(C.c_double), vp]
         L.gm_profile_enable.restype = i; L.gm_profile_enable.argtypes = [i]
         L.gm_profile_read.restype = i
@@ -245,6 +246,16 @@ def gm_get_option(option: int) -> int:
     return int(_lib().gm_get_option(int(option)))
 
 
+TRACE_ROLES, TRACE_CAP = 3, 2048                      # GM_TRACE_ROLES, GM_TRACE_CAP
+
+
+def gm_trace_set(buf) -> None:
+    """Phase trace of k_tc_fused into `buf` (int64 CUDA tensor of TRACE_ROLES * TRACE_CAP zeros), or None: off."""
+    if buf is not None and (not buf.is_cuda or buf.dtype != torch.int64 or buf.numel() < TRACE_ROLES * TRACE_CAP):
+        raise ValueError("gm_trace_set: int64 CUDA tensor of TRACE_ROLES * TRACE_CAP elements")
+    _check(_lib().gm_trace_set(None if buf is None else C.c_void_p(buf.data_ptr())), "gm_trace_set")
+
+
 def gm_measure_fp32_peak(repeats: int = 20, stream=None) -> float:
     """Measured FP32 peak in TFLOP/s (a pure fma.rn.f32x2 kernel, CUDA events)."""
     v = C.c_double()
@@ -256,11 +267,14 @@ def gm_profile_enable(on: bool) -> None:
     _check(_lib().gm_profile_enable(1 if on else 0), "gm_profile_enable")
 
 
+PROF_KINDS = ("forward", "backward", "fused", "tc_forward", "tc_backward", "tc_fused")   # GM_PROF_*
+
+
 def gm_profile_read():
-    """-> {"forward"|"backward"|"fused": (ms, launches)} since the last read."""
-    ms = (C.c_double * 3)(); n = (C.c_int64 * 3)()
+    """-> {kind: (ms, launches)} since the last read; kinds as GM_PROF_* of include/gm.h."""
+    ms = (C.c_double * len(PROF_KINDS))(); n = (C.c_int64 * len(PROF_KINDS))()
     _check(_lib().gm_profile_read(ms, n), "gm_profile_read")
-    return {"forward": (ms[0], int(n[0])), "backward": (ms[1], int(n[1])), "fused": (ms[2], int(n[2]))}
+    return {name: (ms[i], int(n[i])) for i, name in enumerate(PROF_KINDS)}
 
 
 def gm_workspace_bytes(model: dict, B: int, H: int, W: int, K: int, per_galaxy_psf: bool = False) -> int:

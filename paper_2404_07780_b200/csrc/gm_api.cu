@@ -127,6 +127,9 @@ static void prof_end(int i, cudaStream_t st) {
   cudaEventRecord(g_prof.ev[i][1], st);
 }
 
+// phase trace of the tensor-core fused kernel (gm_trace_set): device buffer or nullptr
+static std::atomic<unsigned long long*> g_trace{nullptr};
+
 // run-time options (gm_set_option): process-wide, read once per call
 static std::atomic<int> g_opt[GM_OPT_COUNT_] = {{1}, {1}, {1}};
 
@@ -793,7 +796,7 @@ GM_DECL_K(5) GM_DECL_K(9) GM_DECL_K(15) GM_DECL_K(21) GM_DECL_K(25) GM_DECL_K(33
 static int dispatch_forward(int KP, const FwdArgs& a, int mode, int B, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
-  const int pi = prof_begin(0, st);
+  const int pi = prof_begin(GM_PROF_FORWARD, st);
   switch (KP) {
     case 5: rc = launch_forward_5(a, mode, B, st, &err); break;
     case 9: rc = launch_forward_9(a, mode, B, st, &err); break;
@@ -813,7 +816,7 @@ static int dispatch_forward(int KP, const FwdArgs& a, int mode, int B, cudaStrea
 static int dispatch_backward(int KP, const BwdArgs& a, int B, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
-  const int pi = prof_begin(1, st);
+  const int pi = prof_begin(GM_PROF_BACKWARD, st);
   switch (KP) {
     case 5: rc = launch_backward_5(a, B, st, &err); break;
     case 9: rc = launch_backward_9(a, B, st, &err); break;
@@ -852,7 +855,7 @@ static int dispatch_conv(int KP, const ConvTileArgs& a, int B, cudaStream_t st) 
 static int dispatch_fused(int KP, const FusedArgs& a, int v, int n_sm, size_t lim, cudaStream_t st) {
   int rc;
   cudaError_t err = cudaSuccess;
-  const int pi = prof_begin(2, st);
+  const int pi = prof_begin(GM_PROF_FUSED, st);
   switch (KP) {
     case 5: rc = launch_fused_5(a, v, n_sm, lim, st, &err); break;
     case 9: rc = launch_fused_9(a, v, n_sm, lim, st, &err); break;
@@ -1125,7 +1128,8 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
     a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
-    const int pi = prof_begin(2, st);
+    a.trace = g_trace.load();
+    const int pi = prof_begin(GM_PROF_TC_FUSED, st);
     rc = tc::launch_fused(pl.KT, a, bt->H, pl.caps.n_sm, st, &err);
     prof_end(pi, st);
     if (rc == GM_OK) ++t_launches;
@@ -1136,13 +1140,13 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
     a.out = out; a.gbuf = pl.ws.G; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
-    int pi = prof_begin(0, st);
+    int pi = prof_begin(GM_PROF_TC_FORWARD, st);
     rc = tc::launch_tile(pl.KT, a, pl.tc_trb, 0, pl.caps.n_sm, st, &err);
     prof_end(pi, st);
     if (rc == GM_OK) ++t_launches;
     if (rc == GM_OK && mode == 2) {
       a.btab = pl.ws.tc_adj;
-      pi = prof_begin(1, st);
+      pi = prof_begin(GM_PROF_TC_BACKWARD, st);
       rc = tc::launch_tile(pl.KT, a, pl.tc_trb, 1, pl.caps.n_sm, st, &err);
       prof_end(pi, st);
       if (rc == GM_OK) ++t_launches;
@@ -1873,8 +1877,7 @@ int gm_profile_enable(int on) {
 int gm_profile_read(double* ms, int64_t* count) {
   if (!ms || !count) return GM_EINVAL;
   std::lock_guard<std::mutex> lk(g_prof.mu);
-  ms[0] = ms[1] = ms[2] = 0.0;
-  count[0] = count[1] = count[2] = 0;
+  for (int k = 0; k < GM_PROF_KINDS; ++k) { ms[k] = 0.0; count[k] = 0; }
   for (int i = 0; i < g_prof.n; ++i) {
     GM_CUDA(cudaEventSynchronize(g_prof.ev[i][1]));
     float t = 0.0f;
@@ -1900,6 +1903,11 @@ int gm_set_option(int option, int value) {
 int gm_get_option(int option) {
   if (option < 0 || option >= GM_OPT_COUNT_) return -1;
   return g_opt[option].load();
+}
+
+int gm_trace_set(unsigned long long* device_buf) {
+  g_trace.store(device_buf);
+  return GM_OK;
 }
 
 int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream) {

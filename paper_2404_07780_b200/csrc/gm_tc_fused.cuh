@@ -37,6 +37,27 @@ struct FusedTcArgs {
   float* grad_part;          // [B, n_comp, kNSum]
   const int* frozen;
   const int* live; const int* n_live;
+  unsigned long long* trace; // gm_trace_set: phase time stamps of CTA 0 (measurement hook), or nullptr
+};
+
+// ---- phase trace (gm_trace_set, include/gm.h): CTA 0 appends (tag << 48 | clock64) records, one list per role ----
+constexpr int kTraceCap = 2048;                 // records per role
+enum { TR_HELPER = 0, TR_MMA = 1, TR_WINDOW = 2, TR_ROLES = 3 };
+enum { TR_PRODUCE = 1, TR_PRODUCE_END, TR_DRAIN_WAIT, TR_DRAIN, TR_RESIDUAL, TR_RESIDUAL_END, TR_GRADIENT, TR_GRADIENT_END,
+       TR_JOB, TR_JOB_END };
+struct Tracer {
+  unsigned long long* p = nullptr;
+  int n = 0;
+  __device__ __forceinline__ void init(unsigned long long* base, int role, bool me) {
+    p = (base && blockIdx.x == 0 && me) ? base + (size_t)role * kTraceCap : nullptr;
+  }
+  __device__ __forceinline__ void ev(int tag, int item) {
+    if (p && n < kTraceCap) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
+      p[n++] = ((unsigned long long)((tag << 8) | (item & 255)) << 48) | (t & 0xffffffffffffull);
+    }
+  }
 };
 
 enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kMaxSlots,
@@ -56,22 +77,27 @@ __device__ __forceinline__ void for_each_job(int n_items, int phases, F&& f) {
 
 // MMA issue of accumulator row R0 for every job (one converged warp); RING = tap-row slots per ring
 template <int KP, int R0, int RING>
-__device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
+__device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA,
+                                               unsigned long long* trace = nullptr) {
   using C = Cfg<KP>;
   constexpr uint32_t idesc = instr_desc(128, kTileC);
   constexpr uint32_t desc_hi = (uint32_t)(smem_desc(0, C::NR * 16, 128) >> 32);
   constexpr uint32_t desc_lo0 = (uint32_t)(smem_desc(0, C::NR * 16, 128) & 0xffffffffu);
   auto bar = [&](int i) -> uint32_t { return bars + 8u * (uint32_t)i; };
   int row_count = 0, jc = 0;
-  for_each_job(n_items, phases, [&](int, int, int s) {
+  Tracer tr;
+  tr.init(trace, TR_MMA, R0 == 0 && (threadIdx.x & 31) == 0);
+  for_each_job(n_items, phases, [&](int item, int ph, int s) {
     uint32_t started = 0;
     const uint32_t dcol = tD + (uint32_t)(s * C::kDCols + R0 * kTileC);
+    bool first_row = true;
 #pragma unroll 1
     for (int i = 0; i < C::NY; ++i, ++row_count) {
       const int y = C::seq(i);
       const int buf = row_count % kNBuf;
       mbar_wait(bar(F_A_FULL + buf), (row_count / kNBuf) & 1);
       fence_after();
+      if (first_row) { tr.ev(TR_JOB, 2 * item + ph); first_row = false; }      // the first window row of the job is there
       const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
       const int ta = y - R0;
       if (ta >= 0 && ta < KP) {
@@ -93,6 +119,7 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
       mma_commit(bar(F_A_EMPTY + buf));
     }
     mma_commit(bar(F_D_FULL + s));
+    tr.ev(TR_JOB_END, 2 * item + ph);                      // the last MMA of the job is issued (not yet complete)
     ++jc;
   });
 }
@@ -219,6 +246,8 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
 #pragma unroll
     for (int g = 0; g < G; ++g) inv_sc[0][g] = inv_sc[1][g] = 1.0f;
     int cnt_d[2] = {0, 0};
+    Tracer tr;
+    tr.init(a.trace, TR_HELPER, htid == 0);
     auto cut_addr = [&](int s, int g) -> uint32_t { return smem_u32(slots + (size_t)s * Gm::kSlotWordsF + (size_t)g * Gm::kCutWords); };
     auto px_addr = [&](uint32_t cut, int R, int c) -> uint32_t { return cut + 4u * (uint32_t)swz(R, c, SIDE); };
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
@@ -251,6 +280,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
 
     // a1: S of every cutout of the item (all components go through the PSF on this path) -> slot s
     auto produce = [&](int item, int s) {
+      tr.ev(TR_PRODUCE, item);
 #pragma unroll
       for (int g = 0; g < G; ++g) {
         const int b = galaxy(item, g);
@@ -284,13 +314,16 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         inv_sc[s][g] = scale_and_split(cut, amax);
       }
       signal_input(s);
+      tr.ev(TR_PRODUCE_END, item);
     };
 
     // accumulators of the job on slot s -> the cutouts of the slot, as fp32
     auto drain = [&](int item, int s) {
+      tr.ev(TR_DRAIN_WAIT, item);
       mbar_wait(bar(F_D_FULL + s), cnt_d[s] & 1);
       ++cnt_d[s];
       fence_after();
+      tr.ev(TR_DRAIN, item);
       const int m = 32 * (hw & 3) + lane;                  // this thread's lane of the tensor memory
       const int g = m / Gm::TPG, rem = m - g * Gm::TPG;
       const int tr = rem % Gm::TRC, tc = rem / Gm::TRC;
@@ -440,16 +473,20 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         const int item = 2 * m + s;
         if (item >= n_items) continue;
         drain(item, s);
+        tr.ev(TR_RESIDUAL, item);
         residual(item, s);
         if (with_grad) signal_input(s);                    // G is in place: the adjoint convolution may start
-        else feed(item + 2, s);
+        tr.ev(TR_RESIDUAL_END, item);
+        if (!with_grad) feed(item + 2, s);
       }
       if (with_grad) {
         for (int s = 0; s < 2; ++s) {                     // after C2: gradient, then the next cutouts
           const int item = 2 * m + s;
           if (item >= n_items) continue;
           drain(item, s);
+          tr.ev(TR_GRADIENT, item);
           gradient(item, s);
+          tr.ev(TR_GRADIENT_END, item);
           feed(item + 2, s);
         }
       }
@@ -460,7 +497,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     // compile time and stays in uniform registers)
     static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, Gm::kRingF>(n_items, phases, b0, r0, tD, tA, a.trace);
     else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
     else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
     else fused_mma_role<KP, 3, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
