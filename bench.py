@@ -234,12 +234,13 @@ class Bench:
             return 1.0
         K, H, W = k["K"], k["H"], k["W"]
         KT = next(t for t in (9, 17, 25, 33, 41) if t >= K)
-        nch = (32 + KT - 1 + 15) // 16
-        per_pass = KT * 4 * nch * 3 * (2.0 * 128 * 32 * 16)
+        TR, TC = 4, 32                                                    # kTileR, kTileC of gm_tc.cuh
+        nch = (TC + KT - 1 + 15) // 16
+        per_pass = KT * TR * nch * 3 * (2.0 * 128 * TC * 16)
         if name == "tc_fused":
             passes = {64: 0.25, 96: 1.0, 128: 1.0}[H]                     # per cutout
         else:
-            passes = min(-(-H // (4 * c)) * -(-W // (32 * (128 // c))) for c in (32, 16, 64))
+            passes = min(-(-H // (TR * c)) * -(-W // (TC * (128 // c))) for c in (128 // TR, 64 // TR))
         return passes * per_pass / (2.0 * H * W * K * K)
 
     def barrier(self):

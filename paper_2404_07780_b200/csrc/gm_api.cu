@@ -714,10 +714,10 @@ struct Workspace {
   size_t total;
 };
 
-// Super-tiles of the tensor-core tile kernels for an H x W cutout: 128 lanes of 4 x 32 pixels arranged as
-// trb x (128 / trb) tiles (128 x 128, 64 x 256 or 256 x 64 pixels), whichever covers the cutout with the fewest.
+// Super-tiles of the tensor-core tile kernels for an H x W cutout: the 128 lanes arranged as trb x (128 / trb)
+// tiles (128 x 128 or 64 x 256 pixels), whichever covers the cutout with the fewest.
 static void tc_tile_geom(int H, int W, int* trb, int* tx, int* ty) {
-  static const int cand[3] = {32, 16, 64};
+  static const int cand[2] = {128 / tc::kTileR, 64 / tc::kTileR};
   long long best = -1;
   for (int c : cand) {
     const int TH = tc::kTileR * c, TW = tc::kTileC * (128 / c);
@@ -933,7 +933,7 @@ struct Plan {
   int tiles;
   bool fused;                // whole cutouts per CTA and two slots fit: k_fused path
   int tc = 0; int KT = -1;        // tensor-core path: 1 = k_tc_fused (128 x 128), 2 = k_tc_tile (larger cutouts), 0 = none
-  int tc_trb = 32, tc_tx = 1, tc_ty = 1;
+  int tc_trb = 128 / tc::kTileR, tc_tx = 1, tc_ty = 1;
   FusedGeom fg; int fused_variant;
   DevCaps caps;
   // lease of a region of the constant-bank tap pool (shared PSF only); handed back, by an event

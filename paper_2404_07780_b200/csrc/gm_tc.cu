@@ -65,7 +65,7 @@ static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaE
   GM_TRY(set_smem_once((const void*)k_tc_fused<KP, SIDE>, (int)Gm::kSmem));
   const int passes = (a.B + Gm::G - 1) / Gm::G;
   const int grid = passes < n_sm ? passes : n_sm;
-  k_tc_fused<KP, SIDE><<<grid, kFusedThreadsTc, Gm::kSmem, st>>>(a);
+  k_tc_fused<KP, SIDE><<<grid, Roles<kFusedHW>::kThreads, Gm::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;
 }
@@ -85,7 +85,7 @@ static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaErr
   GM_TRY(set_smem_once((const void*)k_tc_tile<KP, TRB, BWD>, (int)TileCfg<KP, TRB>::kSmem));
   const long long items = (long long)a.B * a.tiles_x * a.tiles_y;
   const int grid = items < n_sm ? (int)items : n_sm;
-  k_tc_tile<KP, TRB, BWD><<<grid, kFusedThreadsTc, TileCfg<KP, TRB>::kSmem, st>>>(a);
+  k_tc_tile<KP, TRB, BWD><<<grid, Roles<kTileHW>::kThreads, TileCfg<KP, TRB>::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;
 }
@@ -93,9 +93,8 @@ static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaErr
 int GM_CAT(launch_tile_tc_, GM_TC_K)(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err) {
 #if GM_TC_K == 25 || GM_TC_K == 41
   switch (trb) {
-    case 16: return bwd ? launch_tile_t<16, true>(a, n_sm, st, err) : launch_tile_t<16, false>(a, n_sm, st, err);
-    case 32: return bwd ? launch_tile_t<32, true>(a, n_sm, st, err) : launch_tile_t<32, false>(a, n_sm, st, err);
-    case 64: return bwd ? launch_tile_t<64, true>(a, n_sm, st, err) : launch_tile_t<64, false>(a, n_sm, st, err);
+    case 128 / kTileR: return bwd ? launch_tile_t<128 / kTileR, true>(a, n_sm, st, err) : launch_tile_t<128 / kTileR, false>(a, n_sm, st, err);   // 128 x 128
+    case 64 / kTileR: return bwd ? launch_tile_t<64 / kTileR, true>(a, n_sm, st, err) : launch_tile_t<64 / kTileR, false>(a, n_sm, st, err);      // 64 x 256
     default: return GM_ENOTSUP;
   }
 #else

@@ -3,8 +3,8 @@
 // engine behind gm_conv (include/gm.h), judged against the same oracle as the FFMA2 loop.
 //
 // Formulation.  M[i,j] = sum_{a,b} P[a,b] S[i+a-h, j+b-h] (P = the flipped PSF, R:C1).  The image
-// is cut into TILES of 4 rows x 32 columns; tile m of a 128 x 128 cutout is LANE m of the
-// tensor memory (128 lanes = the M dimension of one MMA).  For window row y (0 .. 4+K-2) of
+// is cut into TILES of kTileR x kTileC = 4 rows x 32 columns; tile m of a 128 x 128 cutout is LANE m
+// of the tensor memory (128 lanes = the M dimension of one MMA).  For window row y (0 .. kTileR+K-2) of
 // every tile at once and output row r of the tile, tap row a = y - r contributes
 //
 //     D_r[m, j] += sum_c  A_y[m, c] * T_a[c, j],   T_a[c, j] = P[a, c - j]   (a Toeplitz band),
@@ -14,6 +14,13 @@
 // D_r = 32 fp32 columns of tensor memory.  T_a[c0 + r', j] depends on (r' - (j - c0)) only, so all
 // chunks c0 of a tap row are 32-row windows of ONE 16-column matrix E_a stored once per tap row
 // (canonical K-major no-swizzle layout, 16-byte rows: a window is just a start address).
+//
+// Tile shape (measured, profiles/r02_tc_engine.md).  The band wastes (N + K - 1) / K of the tensor work, so a
+// narrower tile looks better on paper, and the code builds with 8 x 16 tiles (N = 16, the smallest N of an
+// M = 128 MMA).  On the B200 a 128 x 16 x 16 MMA takes ~13 cycles, not the 8 its size suggests (128 x 32 x 16:
+// 16.0), so the 1.5x more MMAs of N = 16 made every configuration slower (C1 50 -> 58 ms, P1 682 -> 883 ms),
+// and the 8-row tile leaves up to 7 tap rows after an accumulator's centre row, which triples the truncation
+// bias of the accumulator (below).  4 x 32 stays.
 //
 // Precision.  fp32 operands are split into two fp16 halves after an exact power-of-two scaling
 // per image and per PSF, x = hi + lo with hi = fp16(x), lo = fp16(x - hi) (22 significant
@@ -27,8 +34,8 @@
 //   warps 0-3   window row y of every tile: LDS.128 -> PRMT -> tcgen05.st (3 row buffers)
 //   warps 8-11  issue the MMAs (converged warp, one elected lane), one accumulator row each
 //   warp 12     streams the E_a of the tap rows into two rings with cp.async.bulk (TMA)
-// Measured issue rates (B200): one converged warp issues a 128 x 32 x 16 MMA every 16.0 clk,
-// the tensor-core floor for that shape.
+// Measured issue rates (B200): one converged warp issues a 128 x 32 x 16 MMA every 16.0 clk, the tensor-core
+// floor for that shape; four warps issue, one accumulator row each.
 #pragma once
 #include <cuda_fp16.h>
 #include <cstdint>
@@ -38,19 +45,22 @@
 namespace gm {
 namespace tc {
 
-constexpr int kTileR = 4, kTileC = 32;      // output tile of one lane
+constexpr int kTileR = 4, kTileC = 32;      // output tile of one lane (8 x 16 also builds: measured slower, see above)
+constexpr int kRowsPerLd = 32 / kTileC;     // accumulator rows in one 32-column tensor-memory load
 constexpr int kSide = 128;                  // cutout side this engine is built for (128 lanes)
 constexpr int kPitch = kSide;               // words per image row in shared memory (16-byte chunks XOR-swizzled, see swz)
 constexpr int kNBuf = 3;                    // window-row buffers in tensor memory
-constexpr int kMaxRing = 8;                 // tap-row slots per ring at most; two rings (low / high tap rows)
+constexpr int kMaxRing = 12;                // tap-row slots per ring at most; two rings (low / high tap rows)
 constexpr int kMaxSlots = 2 * kMaxRing;
 constexpr size_t kSmemLimit = 232448;       // 227 KB of dynamic shared memory per CTA
 
 // Word offset of pixel (row R, column c), c a multiple of 4, in an image stored with `pitch` words per row
-// (a multiple of 32): the 16-byte chunk index is XORed with bits 2..4 of the row, so that the eight lanes of
-// a shared-memory wavefront, which read the same chunk of rows 4 apart, hit eight different bank groups.
-__host__ __device__ constexpr int swz(int R, int c, int pitch) { return R * pitch + ((((c >> 2) ^ ((R >> 2) & 7))) << 2); }
-constexpr int kMmaWarps = 4;                // one accumulator row each
+// (a multiple of 32): the 16-byte chunk index is XORed with three bits of row / kTileR, so that the eight lanes of
+// a shared-memory wavefront, which read the same chunk of rows kTileR apart, hit eight different bank groups.
+__host__ __device__ constexpr int swz_of(int R) { return (R / kTileR) & 7; }
+__host__ __device__ constexpr int swz(int R, int c, int pitch) { return R * pitch + ((((c >> 2) ^ swz_of(R))) << 2); }
+constexpr int kMmaWarps = 4;                // accumulator rows w, w + 4, ... each (one row at kTileR = 4)
+constexpr int kAccPerWarp = kTileR / kMmaWarps;
 constexpr int kThreads = (8 + kMmaWarps + 1) * 32;
 
 template <int KP> struct Cfg {
@@ -58,23 +68,28 @@ template <int KP> struct Cfg {
   static constexpr int h = (KP - 1) / 2;
   static constexpr int NCH = (kTileC + KP - 1 + 15) / 16;     // 16-column chunks of a window row
   static constexpr int NY = kTileR + KP - 1;                  // window rows
-  static constexpr int NR = 16 * NCH + 16;                    // rows of E_a
+  static constexpr int NR = 16 * (NCH - 1) + kTileC;          // rows of E_a
   static constexpr int kTapBytes = 2 * 2 * NR * 16;           // (hi, lo) x 2 k-blocks x NR rows x 8 halves
   static constexpr int kACols = NCH * 16;                     // tensor-memory columns of one row buffer
   static constexpr int kDCols = kTileR * kTileC;              // 128 accumulator columns per cutout
   static constexpr int kSlotWords = (kSide + 1) * kPitch;     // image rows + the zero row
-  // tap-row ring depth: what two image slots leave of the shared memory, at least 5 (4 tap rows are live per side)
+  // tap-row ring depth: what two image slots leave of the shared memory, at least kTileR + 1 (kTileR tap rows are live per side)
   static constexpr int kRing = ((kSmemLimit - 2048 - 2 * (size_t)kSlotWords * 4) / (2 * (size_t)kTapBytes)) >= (size_t)kMaxRing
                                    ? kMaxRing : (int)((kSmemLimit - 2048 - 2 * (size_t)kSlotWords * 4) / (2 * (size_t)kTapBytes));
-  static_assert(kRing >= 5, "tap-row rings");
+  static_assert(kRing >= kTileR + 1, "tap-row rings");
   static constexpr int kNSlot = 2 * kRing;
   // Window rows are visited OUTSIDE-IN (0, NY-1, 1, NY-2, ...): the tensor core adds every MMA into the
   // fp32 accumulator with truncation, a loss of half an ulp OF THE RUNNING SUM per step, so the tap rows
   // near the PSF centre, which carry most of the sum, must come last (measured: relative bias of a
-  // convolved pixel -1.2e-5 in row order at K = 41).  Tap rows below kSplit live in the low ring
-  // (ascending use), the others in the high ring (descending use).
+  // convolved pixel -1.2e-5 in row order at K = 41).  A tap row serves window rows ta .. ta + kTileR - 1; it lives
+  // in the LOW ring when its first use in that order is on the ascending side (window row ta at step 2 ta), in the
+  // HIGH ring when it is on the descending side (window row ta + kTileR - 1 at step 2 (NY - ta - kTileR) + 1), i.e.
+  // from ta = NY / 2 - kTileR / 2 + 1 on.  The tap-row producer issues every row at the step of its first use, and
+  // with more than kTileR - 1 slots per ring the previous tenant of a slot has seen its last use by then: the MMA
+  // warps never wait for a row whose slot they still hold (they did, with the rings split at NY / 2 and 8-row tiles).
   static constexpr int kSplit = NY / 2;
-  static constexpr int kNLow = kSplit < KP ? kSplit : KP;     // tap rows 0 .. kNLow-1
+  static constexpr int kNLowRaw = kSplit - kTileR / 2 + 1;
+  static constexpr int kNLow = kNLowRaw < 0 ? 0 : (kNLowRaw < KP ? kNLowRaw : KP);     // tap rows 0 .. kNLow-1
   static constexpr int kNHigh = KP - kNLow;                   // tap rows KP-1 down to kNLow
   __host__ __device__ static constexpr int seq(int i) { return (i & 1) ? NY - 1 - (i >> 1) : (i >> 1); }
   // ring slot of tap row ta and how many tap rows of one cutout were in that slot before it / in total
@@ -251,7 +266,7 @@ enum { IMG_FULL = 0, IMG_EMPTY = 2, A_FULL = 4, A_EMPTY = 4 + kNBuf, B_FULL = 4 
        D_FULL = B_EMPTY + kMaxSlots, D_EMPTY = D_FULL + 2, N_BARS = D_EMPTY + 2 };
 static_assert(N_BARS <= 64, "barrier area");
 
-// MMA issue of accumulators R0 .. R0 + NACC - 1 (one converged warp)
+// MMA issue of accumulator rows R0, R0 + kMmaWarps, ... (NACC of them; one converged warp)
 template <int KP, int R0, int NACC>
 __device__ __forceinline__ void mma_role(int n_gal, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA) {
   using C = Cfg<KP>;
@@ -274,12 +289,12 @@ __device__ __forceinline__ void mma_role(int n_gal, uint32_t bars, uint32_t ring
       const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
 #pragma unroll
       for (int rr = 0; rr < NACC; ++rr) {
-        const int ta = y - (R0 + rr);                               // tap row
+        const int ta = y - (R0 + kMmaWarps * rr);                   // tap row
         if (ta < 0 || ta >= KP) continue;
         const int slot = C::template slot_of<C::kRing>(ta);
         mbar_wait(bar(B_FULL + slot), (uint32_t)(it * C::template uses_of_slot<C::kRing>(slot) + C::template index_in_slot<C::kRing>(ta)) & 1);
         fence_after();
-        const uint32_t dcol = tD + (uint32_t)(d * C::kDCols + (R0 + rr) * kTileC);
+        const uint32_t dcol = tD + (uint32_t)(d * C::kDCols + (R0 + kMmaWarps * rr) * kTileC);
         // start-address field of the hi part's chunk 0 (+ the constant LBO field); parts and chunks differ by constants
         const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
         {
@@ -325,7 +340,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(IMG_FULL + i), 4); mbar_init(bar(IMG_EMPTY + i), 4); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(A_FULL + i), 4); mbar_init(bar(A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < C::kNSlot; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 4); }
+    for (int i = 0; i < C::kNSlot; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), kTileR); }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(D_FULL + i), kMmaWarps); mbar_init(bar(D_EMPTY + i), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -344,8 +359,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
 
   if (wid < 4) {
     // ------------------------- window rows -> tensor memory --------------------------
-    // lane t of warp w owns tile (row block t, column block w): image rows 4t .. 4t+3, columns 32w .. 32w+31
+    // tensor-memory lane m = 32 w + t owns tile (row block m % kTRC, column block m / kTRC) of kTileR x kTileC pixels
     const uint32_t lane_base = (uint32_t)(32 * wid) << 16;
+    constexpr int kTRC = kSide / kTileR;
+    const int m = 32 * wid + lane, tr = m % kTRC, tc = m / kTRC;
     int row_count = 0;
     for (int it = 0; it < n_gal; ++it) {
       const int s = it & 1;
@@ -357,16 +374,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
         const int buf = row_count % kNBuf;
         mbar_wait(bar(A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
         fence_after();
-        const int R = 4 * lane + y - h;
+        const int R = kTileR * tr + y - h;
         const bool row_ok = (unsigned)R < (unsigned)kSide;
         const uint32_t rowp = slot + 4u * (uint32_t)(R * kPitch);
-        const int sw = (R >> 2) & 7;
+        const int sw = swz_of(R);
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           uint32_t w[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
-            const int c0 = 32 * wid - h + 16 * kc + 4 * q;
+            const int c0 = kTileC * tc - h + 16 * kc + 4 * q;
             const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)kSide) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
             w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
           }
@@ -399,16 +416,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
       fence_after();
       const float inv = inv_scale_s[d] * a.bscale[a.btab_stride ? g : 0];
       float* outp = a.out + (size_t)g * kSide * kSide;
+      constexpr int kTRC = kSide / kTileR;
+      const int m = 32 * lw + lane, tr = m % kTRC, tc = m / kTRC;
 #pragma unroll 1
-      for (int r = 0; r < kTileR; ++r) {
+      for (int q = 0; q < C::kDCols / 32; ++q) {                     // 32 columns = kRowsPerLd accumulator rows
         uint32_t v[32];
-        tmem_ld32(tD + (uint32_t)(d * C::kDCols + r * kTileC) + lane_base, v);
+        tmem_ld32(tD + (uint32_t)(d * C::kDCols + 32 * q) + lane_base, v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        float4* dst = reinterpret_cast<float4*>(outp + (size_t)(4 * lane + r) * kSide + 32 * lw);
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
-          dst[q] = make_float4(__uint_as_float(v[4 * q]) * inv, __uint_as_float(v[4 * q + 1]) * inv,
-                               __uint_as_float(v[4 * q + 2]) * inv, __uint_as_float(v[4 * q + 3]) * inv);
+        for (int k = 0; k < 8; ++k) {
+          const int r = kRowsPerLd * q + (4 * k) / kTileC, c = (4 * k) % kTileC;
+          *reinterpret_cast<float4*>(outp + (size_t)(kTileR * tr + r) * kSide + kTileC * tc + c) =
+              make_float4(__uint_as_float(v[4 * k]) * inv, __uint_as_float(v[4 * k + 1]) * inv,
+                          __uint_as_float(v[4 * k + 2]) * inv, __uint_as_float(v[4 * k + 3]) * inv);
+        }
       }
       fence_before();
       __syncwarp();
@@ -457,11 +478,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_tc_conv(const ConvArgs a) {
     // ----------------------------------- MMA issue ------------------------------------
     // (the accumulator pair is a template argument so that every address of the issue loop is
     // warp-uniform at compile time and stays in uniform registers)
-    static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
-    if (wid == 8) mma_role<KP, 0, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else if (wid == 9) mma_role<KP, 1, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else if (wid == 10) mma_role<KP, 2, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
-    else mma_role<KP, 3, 1>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    static_assert(kMmaWarps == 4, "accumulator rows w, w + 4 per MMA warp");
+    if (wid == 8) mma_role<KP, 0, kAccPerWarp>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 9) mma_role<KP, 1, kAccPerWarp>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else if (wid == 10) mma_role<KP, 2, kAccPerWarp>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
+    else mma_role<KP, 3, kAccPerWarp>(n_gal, smem_u32(bars), smem_u32(ring), tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
     // in the order of first use: window row y = seq(i) brings tap row y (r = 0) on the low side and

@@ -2,13 +2,13 @@
 // tensor cores (the engine of gm_tc.cuh): one persistent CTA per SM, two cutouts in flight, nothing but
 // chi^2 and the kNSum partial sums per component leaving the SM (mode 0 writes the model image).
 //
-// Roles (17 warps, all hand-offs by mbarrier / named barrier):
-//   warps 0-3    window rows of the current job: shared memory -> tensor memory (A operand)
-//   warps 4-11   helpers: a1 render S into a slot, scale + split into (hi, lo) fp16 pairs; after the forward
-//                convolution drain M (tensor memory -> slot, fp32), a3 residual / chi^2 / G in place, scale +
-//                split G; after the adjoint convolution drain A, a5 gradient sums
-//   warps 12-15  MMA issue, one accumulator row of the 4 x 32 tiles each
-//   warp 16      streams the Toeplitz band blocks E_a (forward or adjoint table) through the two rings
+// Roles (4 + HW + 4 + 1 warps, all hand-offs by mbarrier / named barrier):
+//   warps 0-3        window rows of the current job: shared memory -> tensor memory (A operand)
+//   HW helper warps  a1 render S into a slot, scale + split into (hi, lo) fp16 pairs; after the forward
+//                    convolution drain M (tensor memory -> slot, fp32), a3 residual / chi^2 / G in place, scale +
+//                    split G; after the adjoint convolution drain A, a5 gradient sums
+//   4 MMA warps      MMA issue, one accumulator row of the 4 x 32 tiles each
+//   last warp        streams the Toeplitz band blocks E_a (forward or adjoint table) through the two rings
 // A JOB is one convolution of one cutout.  Jobs run in the order C1(a) C1(b) C2(a) C2(b) (cutouts a, b in
 // slots 0, 1), so the helpers always work on the slot the tensor cores are not reading: the same
 // schedule as k_fused (gm_fused.cuh), with the FFMA2 loop replaced by tcgen05.mma.
@@ -19,9 +19,21 @@
 namespace gm {
 namespace tc {
 
-constexpr int kHelpWarpsTc = 8;
-constexpr int kFusedThreadsTc = (4 + kHelpWarpsTc + kMmaWarps + 1) * 32;     // 544
-constexpr int kHN = 32 * kHelpWarpsTc;
+// Helper warps: k_tc_fused overlaps them with the tensor pipe of the other slot, and more than 8 only add traffic
+// on the shared-memory pipe that binds it (measured: 16 warps K = 41 +18 %, K = 25 +1 %); the one-slot super-tile
+// kernels run their fill phase alone, where 16 warps are 1.5x faster (C4 -13 %, C2 -8 %).
+template <int HW> struct Roles {
+  static_assert(HW == 8 || HW == 16, "helper warps: a multiple of 4 (tensor-memory lane quarters)");
+  static constexpr int kHelp = HW;
+  static constexpr int kThreads = (4 + HW + kMmaWarps + 1) * 32;
+  static constexpr int kHN = 32 * HW;
+  static constexpr int kLdPerWarp = 4 / (HW / 4);             // 32-column accumulator loads (of 4 per lane) one helper warp drains
+  static constexpr int kLastWarp = 4 + HW + kMmaWarps;
+  // header of the shared memory: 64 barriers, the tensor-memory base, reduction scratch [HW * kNSum] + [HW] maxima
+  static constexpr int kHeaderBytes = (528 + (HW * kNSum + HW) * 4 + 127) / 128 * 128;
+};
+constexpr int kAlignSlack = 128;                              // the dynamic shared memory is re-aligned to 128 bytes
+constexpr int kFusedHW = 8, kTileHW = 16;
 
 struct FusedTcArgs {
   ModelDesc md;
@@ -61,7 +73,7 @@ struct Tracer {
 };
 
 enum { F_IN_FULL = 0, F_D_FULL = 2, F_A_FULL = 4, F_A_EMPTY = 4 + kNBuf, F_B_FULL = 4 + 2 * kNBuf, F_B_EMPTY = F_B_FULL + kMaxSlots,
-       F_N_BARS = F_B_EMPTY + kMaxSlots };
+       F_SLOT_FREE = F_B_EMPTY + kMaxSlots, F_N_BARS = F_SLOT_FREE + 1 };
 static_assert(F_N_BARS <= 64, "barrier area");
 
 // the jobs of one CTA in tensor-core order; f(item, phase, slot)
@@ -75,7 +87,7 @@ __device__ __forceinline__ void for_each_job(int n_items, int phases, F&& f) {
       }
 }
 
-// MMA issue of accumulator row R0 for every job (one converged warp); RING = tap-row slots per ring
+// MMA issue of accumulator rows R0 and R0 + kMmaWarps for every job (one converged warp); RING = tap-row slots per ring
 template <int KP, int R0, int RING>
 __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA,
                                                unsigned long long* trace = nullptr) {
@@ -88,8 +100,7 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
   Tracer tr;
   tr.init(trace, TR_MMA, R0 == 0 && (threadIdx.x & 31) == 0);
   for_each_job(n_items, phases, [&](int item, int ph, int s) {
-    uint32_t started = 0;
-    const uint32_t dcol = tD + (uint32_t)(s * C::kDCols + R0 * kTileC);
+    uint32_t started = 0;                                  // bit rr: accumulator row R0 + kMmaWarps rr holds a sum already
     bool first_row = true;
 #pragma unroll 1
     for (int i = 0; i < C::NY; ++i, ++row_count) {
@@ -99,21 +110,24 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
       fence_after();
       if (first_row) { tr.ev(TR_JOB, 2 * item + ph); first_row = false; }      // the first window row of the job is there
       const uint32_t acol = tA + (uint32_t)(buf * C::kACols);
-      const int ta = y - R0;
-      if (ta >= 0 && ta < KP) {
+#pragma unroll
+      for (int rr = 0; rr < kAccPerWarp; ++rr) {
+        const int ta = y - (R0 + kMmaWarps * rr);
+        if (ta < 0 || ta >= KP) continue;
         const int slot = C::template slot_of<RING>(ta);
         mbar_wait(bar(F_B_FULL + slot), (uint32_t)(jc * C::template uses_of_slot<RING>(slot) + C::template index_in_slot<RING>(ta)) & 1);
         fence_after();
+        const uint32_t dcol = tD + (uint32_t)(s * C::kDCols + (R0 + kMmaWarps * rr) * kTileC);
         const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
 #pragma unroll
         for (int kc = 0; kc < C::NCH; ++kc) {
           const uint32_t b_hi = lo0 + (uint32_t)(16 * (C::NCH - 1 - kc));
           const uint32_t b_lo = b_hi + (uint32_t)(2 * C::NR);
-          mma_f16_ts2(dcol, acol + kc * 16, b_hi, desc_hi, idesc, kc ? 1u : started);    // hi * hi (the first MMA overwrites)
-          mma_f16_ts2(dcol, acol + kc * 16 + 8, b_hi, desc_hi, idesc, 1);                 // lo * hi
-          mma_f16_ts2(dcol, acol + kc * 16, b_lo, desc_hi, idesc, 1);                     // hi * lo
+          mma_f16_ts2(dcol, acol + kc * 16, b_hi, desc_hi, idesc, kc ? 1u : ((started >> rr) & 1u));   // hi * hi (the first MMA overwrites)
+          mma_f16_ts2(dcol, acol + kc * 16 + 8, b_hi, desc_hi, idesc, 1);                                // lo * hi
+          mma_f16_ts2(dcol, acol + kc * 16, b_lo, desc_hi, idesc, 1);                                    // hi * lo
         }
-        started = 1;
+        started |= 1u << rr;
         mma_commit(bar(F_B_EMPTY + slot));
       }
       mma_commit(bar(F_A_EMPTY + buf));
@@ -124,7 +138,34 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
   });
 }
 
-// Geometry of k_tc_fused for square cutouts of SIDE = 64, 96 or 128 pixels: a cutout is (SIDE / 4) x (SIDE / 32)
+// one window row of a lane's tile: NCH chunks of 16 columns, shared memory (hi, lo) words -> tensor memory.
+// chunk0 = 16-byte chunk index of the window's first column in the row at `rowp` (may be negative / beyond n_chunks:
+// those chunks and rows with !row_ok read the zero row); sw = swizzle of the row.
+template <int KP>
+__device__ __forceinline__ void stage_window_row(uint32_t rowp, uint32_t zero, bool row_ok, int chunk0, int n_chunks, int sw,
+                                                 uint32_t tcol) {
+  using C = Cfg<KP>;
+#pragma unroll
+  for (int kc = 0; kc < C::NCH; ++kc) {
+    uint32_t w[16];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int ch = chunk0 + 4 * kc + q;
+      const uint4 v = lds128((row_ok && (unsigned)ch < (unsigned)n_chunks) ? rowp + 16u * (uint32_t)(ch ^ sw) : zero);
+      w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+    }
+    uint32_t hi[8], lo[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      hi[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x5410);
+      lo[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x7632);
+    }
+    tmem_st8(tcol + kc * 16, hi);
+    tmem_st8(tcol + kc * 16 + 8, lo);
+  }
+}
+
+// Geometry of k_tc_fused for square cutouts of SIDE = 64, 96 or 128 pixels: a cutout is (SIDE / kTileR) x (SIDE / kTileC)
 // tiles; G = 4, 1, 1 cutouts share the 128 lanes of a pass (64 px: one lane quarter each; 96 px: 72 lanes used).
 template <int KP, int SIDE> struct FusedGeomTc {
   using C = Cfg<KP>;
@@ -134,43 +175,44 @@ template <int KP, int SIDE> struct FusedGeomTc {
   static constexpr int W4 = SIDE / 4, kGroups = SIDE * W4;    // groups of four pixels per row / per cutout
   static constexpr int kCutWords = (SIDE + 1) * SIDE;         // rows + the zero row, pitch = SIDE words (XOR-swizzled chunks)
   static constexpr int kSlotWordsF = G * kCutWords;
-  static constexpr int kRingF = ((kSmemLimit - 2048 - 2 * (size_t)kSlotWordsF * 4) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
-                                    ? kMaxRing : (int)((kSmemLimit - 2048 - 2 * (size_t)kSlotWordsF * 4) / (2 * (size_t)C::kTapBytes));
-  static_assert(kRingF >= 5, "tap-row rings");
-  static constexpr size_t kSmem = 1024 + 1024 + (size_t)(2 * kRingF) * C::kTapBytes + 2 * (size_t)kSlotWordsF * 4;
+  static constexpr size_t kFixed = kAlignSlack + Roles<kFusedHW>::kHeaderBytes + 2 * (size_t)kSlotWordsF * 4;     // alignment slack, header, slots
+  static constexpr int kRingF = ((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
+                                    ? kMaxRing : (int)((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes));
+  static_assert(kRingF >= kTileR + 1, "tap-row rings");
+  static constexpr size_t kSmem = kFixed + (size_t)(2 * kRingF) * C::kTapBytes;
   static_assert(kSmem <= kSmemLimit, "shared memory");
 };
 
 template <int KP, int SIDE>
-__global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcArgs a) {
+__global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const FusedTcArgs a) {
   using C = Cfg<KP>;
   using Gm = FusedGeomTc<KP, SIDE>;
-  constexpr int h = C::h, G = Gm::G;
+  using Ro = Roles<kFusedHW>;
+  constexpr int h = C::h, G = Gm::G, kHN = Ro::kHN, kHelp = Ro::kHelp;
   extern __shared__ unsigned char smem_raw[];
-  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + (kAlignSlack - 1)) & ~(uintptr_t)(kAlignSlack - 1));
   uint64_t* bars = reinterpret_cast<uint64_t*>(base);
   uint32_t* tmem_base_s = reinterpret_cast<uint32_t*>(base + 512);
-  float* red = reinterpret_cast<float*>(base + 528);                // [kHelpWarpsTc * kNSum] sums, then [8] maxima
-  float* redmax = red + kHelpWarpsTc * kNSum;
-  unsigned char* ring = base + 1024;
+  float* red = reinterpret_cast<float*>(base + 528);                // [kHelp * kNSum] sums, then [kHelp] maxima
+  float* redmax = red + kHelp * kNSum;
+  unsigned char* ring = base + Ro::kHeaderBytes;
   uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)(2 * Gm::kRingF) * C::kTapBytes);
-  static_assert(528 + (kHelpWarpsTc * kNSum + 8) * 4 <= 1024, "header area");
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
   // warp index through a lane-0 broadcast: warp-uniform for the compiler (uniform registers in the role code)
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelp); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < 2 * Gm::kRingF; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    for (int i = 0; i < 2 * Gm::kRingF; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), kTileR); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
+  constexpr int kLastWarp = Ro::kLastWarp;
   if (wid == kLastWarp) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = tid; i < 2 * Gm::kSlotWordsF; i += kFusedThreadsTc) slots[i] = 0u;    // the zero rows
+  for (int i = tid; i < 2 * Gm::kSlotWordsF; i += Ro::kThreads) slots[i] = 0u;    // the zero rows
   fence_before();
   __syncthreads();
   fence_after();
@@ -209,36 +251,17 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
         const int buf = row_count % kNBuf;
         mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
         fence_after();
-        const int R = 4 * tr + y - h;
+        const int R = kTileR * tr + y - h;
         const bool row_ok = lane_ok && (unsigned)R < (unsigned)SIDE;
-        const uint32_t rowp = cut + 4u * (uint32_t)(R * SIDE);
-        const int sw = (R >> 2) & 7;
-#pragma unroll
-        for (int kc = 0; kc < C::NCH; ++kc) {
-          uint32_t w[16];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int c0 = 32 * tc - h + 16 * kc + 4 * q;
-            const uint4 v = lds128((row_ok && (unsigned)c0 < (unsigned)SIDE) ? rowp + 16u * (uint32_t)((c0 >> 2) ^ sw) : zero);
-            w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
-          }
-          uint32_t hi[8], lo[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            hi[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x5410);
-            lo[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x7632);
-          }
-          const uint32_t col = tA + (uint32_t)(buf * C::kACols + kc * 16) + lane_base;
-          tmem_st8(col, hi);
-          tmem_st8(col + 8, lo);
-        }
+        stage_window_row<KP>(cut + 4u * (uint32_t)(R * SIDE), zero, row_ok, (kTileC * tc - h) >> 2, SIDE / 4, swz_of(R),
+                             tA + (uint32_t)(buf * C::kACols) + lane_base);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(F_A_FULL + buf));
       }
     });
-  } else if (wid < 4 + kHelpWarpsTc) {
+  } else if (wid < 4 + kHelp) {
     // ------------------------------------ helpers -------------------------------------
     const int hw = wid - 4, htid = tid - 128;
     const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
@@ -261,7 +284,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
       help_sync();
       float mx = redmax[0];
 #pragma unroll
-      for (int w = 1; w < kHelpWarpsTc; ++w) mx = fmaxf(mx, redmax[w]);
+      for (int w = 1; w < kHelp; ++w) mx = fmaxf(mx, redmax[w]);
       const float sc = pow2_scale(mx);
 #pragma unroll 2
       for (int idx = htid; idx < kGroups; idx += kHN) {
@@ -326,7 +349,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
       tr.ev(TR_DRAIN, item);
       const int m = 32 * (hw & 3) + lane;                  // this thread's lane of the tensor memory
       const int g = m / Gm::TPG, rem = m - g * Gm::TPG;
-      const int tr = rem % Gm::TRC, tc = rem / Gm::TRC;
+      const int tr_ = rem % Gm::TRC, tc = rem / Gm::TRC;
       const bool lane_ok = g < G;
       const int b = lane_ok ? galaxy(item, g) : -1;
       float isc = 1.0f;
@@ -334,16 +357,16 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
       for (int gg = 0; gg < G; ++gg) isc = (gg == g) ? inv_sc[s][gg] : isc;
       const float inv = isc * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
       const uint32_t cut = cut_addr(s, lane_ok ? g : 0);
-      const int r_first = 2 * (hw >> 2);
+      const int q_first = Ro::kLdPerWarp * (hw >> 2);
 #pragma unroll 1
-      for (int r = r_first; r < r_first + 2; ++r) {
+      for (int q = q_first; q < q_first + Ro::kLdPerWarp; ++q) {    // 32 columns = kRowsPerLd accumulator rows
         uint32_t v[32];
-        tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
+        tmem_ld32(tD + (uint32_t)(s * C::kDCols + 32 * q) + lane_base, v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (lane_ok) {
 #pragma unroll
           for (int k = 0; k < 8; ++k)
-            sts128(px_addr(cut, 4 * tr + r, 32 * tc + 4 * k),
+            sts128(px_addr(cut, kTileR * tr_ + kRowsPerLd * q + (4 * k) / kTileC, kTileC * tc + (4 * k) % kTileC),
                    make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
                               __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
         }
@@ -383,7 +406,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
             const float4* sptr = reinterpret_cast<const float4*>(a.sigma + img);
             auto pass = [&]<bool MASKED>() {
               const uchar4* kptr = MASKED ? reinterpret_cast<const uchar4*>(a.mask + img) : nullptr;
-#pragma unroll 2
+#pragma unroll 4
               for (int idx = htid; idx < kGroups; idx += kHN) {
                 const uint32_t p = px_addr(cut, idx / W4, (idx % W4) << 2);
                 const float4 d4 = dptr[idx], s4 = sptr[idx];
@@ -410,7 +433,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
           else help_sync();
           if (htid == 0 && b >= 0) {
             float t = 0.0f;
-            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
+            for (int w = 0; w < kHelp; ++w) t += red[w];
             a.chi2_part[b] = t;
           }
           help_sync();                                     // red[] may be rewritten
@@ -457,7 +480,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
           help_sync();
           if (htid < kNSum && b >= 0) {
             float t = 0.0f;
-            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
+            for (int w = 0; w < kHelp; ++w) t += red[w * kNSum + htid];
             a.grad_part[((size_t)b * a.md.n_comp + c) * kNSum + htid] = t;
           }
           help_sync();
@@ -493,18 +516,18 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
     }
   } else if (wid < kLastWarp) {
     // ----------------------------------- MMA issue ------------------------------------
-    // (the accumulator row is a template argument so that every address of the issue loop is warp-uniform at
+    // (the accumulator rows are template arguments so that every address of the issue loop is warp-uniform at
     // compile time and stays in uniform registers)
-    static_assert(kMmaWarps == 4 && kTileR == 4, "one accumulator row per MMA warp");
+    static_assert(kMmaWarps == 4, "accumulator rows w, w + 4, ... per MMA warp");
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, Gm::kRingF>(n_items, phases, b0, r0, tD, tA, a.trace);
-    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
-    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    if (wid == 4 + kHelp) fused_mma_role<KP, 0, Gm::kRingF>(n_items, phases, b0, r0, tD, tA, a.trace);
+    else if (wid == 5 + kHelp) fused_mma_role<KP, 1, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
+    else if (wid == 6 + kHelp) fused_mma_role<KP, 2, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
     else fused_mma_role<KP, 3, Gm::kRingF>(n_items, phases, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
-    // in the order of first use: window row y = seq(i) brings tap row y (r = 0) on the low side and
-    // tap row y - 3 (r = 3) on the high side.  Several cutouts per pass share one PSF (the host sees to it).
+    // in the order of first use on its side: window row y = seq(i) brings tap row y (r = 0) on the low side and
+    // tap row y - (kTileR - 1) on the high side.  Several cutouts per pass share one PSF (the host sees to it).
     if (lane == 0) {
       int jc = 0;
       for_each_job(n_items, phases, [&](int item, int ph, int) {
@@ -530,13 +553,17 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_fused(const FusedTcAr
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Cutouts above 128 px: the same engine on SUPER-TILES of 128 lanes (128 x 128 or 64 x 256 / 256 x 64
-// pixels, whichever covers the cutout with the fewest), G through global memory between the forward and
-// the backward kernel as in the FFMA2 tile kernels (k_forward / k_backward).  One shared-memory slot holds
-// the super-tile plus its halo, so the phases of an item run one after the other:
-//   k_tc_tile<KP, TRB, false>  a1 render S on tile + halo -> scale, split -> C1 -> drain M -> a3 residual,
-//                              G to global, chi^2 partial (mode 0: M to global)
-//   k_tc_tile<KP, TRB, true>   G tile + halo from global -> scale, split -> C2 -> drain A -> a5 partial sums
+// Cutouts above 128 px: the same engine on SUPER-TILES of 128 lanes (128 x 128 or 64 x 256 pixels, whichever
+// covers the cutout with the fewest), G through global memory between the forward and the backward kernel
+// as in the FFMA2 tile kernels (k_forward / k_backward).  One shared-memory slot holds the super-tile plus
+// its halo (two do not fit beside the tap-row rings), so an item's input is built while the tensor pipe
+// idles; everything after the convolution, however, runs beside the NEXT item's convolution: the accumulators
+// are double buffered in tensor memory and leave it through a 16 KB transposition buffer, never through the slot.
+//   k_tc_tile<KP, TRB, false>  fill: a1 render S on tile + halo, scale, split | C1 | post: a3 residual, G to
+//                              global, chi^2 partial (mode 0: M to global)
+//   k_tc_tile<KP, TRB, true>   fill: G tile + halo from global, scale, split  | C2 | post: a5 partial sums
+// Helper order: fill(0), fill(1) || post(0) ... : fill(n + 1) waits for the window-row warps to have staged the
+// last row of item n (F_SLOT_FREE), post(n) for its last MMA (F_D_FULL).
 // ---------------------------------------------------------------------------------------------------
 struct TileTcArgs {
   ModelDesc md;
@@ -561,47 +588,53 @@ template <int KP, int TRB> struct TileCfg {
   static constexpr int RW = TW + KP - 1;                      // columns that carry data
   static constexpr int kPitchT = (TW - kTileC + 16 * C::NCH + 31) / 32 * 32;   // + window padding of the last tile column, whole swizzle groups
   static constexpr int kSlotWordsT = RR * kPitchT;
-  static constexpr int kRingT = ((kSmemLimit - 2048 - (size_t)kSlotWordsT * 4) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
-                                    ? kMaxRing : (int)((kSmemLimit - 2048 - (size_t)kSlotWordsT * 4) / (2 * (size_t)C::kTapBytes));
-  static_assert(kRingT >= 5, "tap-row rings");
-  static constexpr size_t kSmem = 1024 + 1024 + (size_t)(2 * kRingT) * C::kTapBytes + (size_t)kSlotWordsT * 4;
+  static constexpr int kPieceWords = 128 * 32;                // transposition buffer: 32 accumulator columns of every lane
+  static constexpr size_t kFixed = kAlignSlack + Roles<kTileHW>::kHeaderBytes + (size_t)kSlotWordsT * 4 + (size_t)kPieceWords * 4;
+  static constexpr int kRingT = ((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
+                                    ? kMaxRing : (int)((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes));
+  static_assert(kRingT >= kTileR + 1, "tap-row rings");
+  static constexpr size_t kSmem = kFixed + (size_t)(2 * kRingT) * C::kTapBytes;
   static_assert(kSmem <= kSmemLimit, "shared memory");
+  static_assert(TW % 32 == 0 && TW >= 32, "rows of the transposition buffer are whole swizzle groups");
 };
 
 template <int KP, int TRB, bool BWD>
-__global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs a) {
+__global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const TileTcArgs a) {
   using C = Cfg<KP>;
   using T = TileCfg<KP, TRB>;
-  constexpr int h = C::h;
+  using Ro = Roles<kTileHW>;
+  constexpr int h = C::h, kHN = Ro::kHN, kHelp = Ro::kHelp;
   extern __shared__ unsigned char smem_raw[];
-  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  unsigned char* base = reinterpret_cast<unsigned char*>(((uintptr_t)smem_raw + (kAlignSlack - 1)) & ~(uintptr_t)(kAlignSlack - 1));
   uint64_t* bars = reinterpret_cast<uint64_t*>(base);
   uint32_t* tmem_base_s = reinterpret_cast<uint32_t*>(base + 512);
   float* red = reinterpret_cast<float*>(base + 528);
-  float* redmax = red + kHelpWarpsTc * kNSum;
-  unsigned char* ring = base + 1024;
+  float* redmax = red + kHelp * kNSum;
+  unsigned char* ring = base + Ro::kHeaderBytes;
   uint32_t* slotw = reinterpret_cast<uint32_t*>(ring + (size_t)(2 * T::kRingT) * C::kTapBytes);
+  uint32_t* piecew = slotw + T::kSlotWordsT;
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelpWarpsTc); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelp); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
     for (int i = 0; i < kNBuf; ++i) { mbar_init(bar(F_A_FULL + i), 4); mbar_init(bar(F_A_EMPTY + i), kMmaWarps); }
-    for (int i = 0; i < 2 * T::kRingT; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), 4); }
+    for (int i = 0; i < 2 * T::kRingT; ++i) { mbar_init(bar(F_B_FULL + i), 1); mbar_init(bar(F_B_EMPTY + i), kTileR); }
+    mbar_init(bar(F_SLOT_FREE), 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  constexpr int kLastWarp = 4 + kHelpWarpsTc + kMmaWarps;
+  constexpr int kLastWarp = Ro::kLastWarp;
   if (wid == kLastWarp) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_base_s)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = tid; i < T::kSlotWordsT; i += kFusedThreadsTc) slotw[i] = 0u;        // padding columns stay zero
+  for (int i = tid; i < T::kSlotWordsT; i += Ro::kThreads) slotw[i] = 0u;        // padding columns stay zero
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tm = __shfl_sync(0xffffffffu, *tmem_base_s, 0);
   const uint32_t tD = tm, tA = tm + 2 * C::kDCols;
-  const uint32_t slot = smem_u32(slotw);
+  const uint32_t slot = smem_u32(slotw), piece = smem_u32(piecew);
 
   // items of this CTA: (galaxy of the list, super-tile), entries blockIdx.x, + gridDim.x, ...
   const int tiles = a.tiles_x * a.tiles_y;
@@ -629,42 +662,29 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
         const int buf = row_count % kNBuf;
         mbar_wait(bar(F_A_EMPTY + buf), ((row_count / kNBuf) & 1) ^ 1);
         fence_after();
-        const int R = 4 * tr + y;                                  // slot row (row 0 = image row i0 - h)
-        const uint32_t rowp = slot + 4u * (uint32_t)(R * T::kPitchT);
-        const int sw = (R >> 2) & 7;
-#pragma unroll
-        for (int kc = 0; kc < C::NCH; ++kc) {
-          uint32_t w[16];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const uint4 v = lds128(rowp + 16u * (uint32_t)((8 * tc + 4 * kc + q) ^ sw));
-            w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
-          }
-          uint32_t hi[8], lo[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            hi[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x5410);
-            lo[j] = __byte_perm(w[2 * j], w[2 * j + 1], 0x7632);
-          }
-          const uint32_t col = tA + (uint32_t)(buf * C::kACols + kc * 16) + lane_base;
-          tmem_st8(col, hi);
-          tmem_st8(col + 8, lo);
-        }
+        const int R = kTileR * tr + y;                             // slot row (row 0 = image row i0 - h)
+        stage_window_row<KP>(slot + 4u * (uint32_t)(R * T::kPitchT), slot, true, (kTileC * tc) >> 2, T::kPitchT / 4, swz_of(R),
+                             tA + (uint32_t)(buf * C::kACols) + lane_base);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(F_A_FULL + buf));
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(F_SLOT_FREE));                 // every window row of the item is in tensor memory
     }
-  } else if (wid < 4 + kHelpWarpsTc) {
+  } else if (wid < 4 + kHelp) {
     // ------------------------------------ helpers -------------------------------------
     const int hw = wid - 4, htid = tid - 128;
     const uint32_t lane_base = (uint32_t)(32 * (hw & 3)) << 16;
     auto px_addr = [&](int R, int c) -> uint32_t { return slot + 4u * (uint32_t)swz(R, c, T::kPitchT); };
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
     constexpr int RW4 = T::RW / 4, kRegionGroups = T::RR * RW4;      // groups of four pixels of the tile + halo
-    constexpr int TW4 = T::TW / 4, kTileGroups = T::TH * TW4;        // ... of the tile itself
+    constexpr int TW4 = T::TW / 4;
+    constexpr int kPieceRows = kRowsPerLd * TRB, kPieceGroups = kPieceRows * TW4;   // a piece = 32 accumulator columns (kRowsPerLd rows) of every tile
+    constexpr int kPieces = C::kDCols / 32;
     const float inv_rw4 = 1.0f / (float)RW4;
+    float inv_sc[2] = {1.0f, 1.0f};
 
     auto scale_and_split = [&](float amax) -> float {
       for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
@@ -672,7 +692,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
       help_sync();
       float mx = redmax[0];
 #pragma unroll
-      for (int w = 1; w < kHelpWarpsTc; ++w) mx = fmaxf(mx, redmax[w]);
+      for (int w = 1; w < kHelp; ++w) mx = fmaxf(mx, redmax[w]);
       const float sc = pow2_scale(mx);
 #pragma unroll 2
       for (int idx = htid; idx < kRegionGroups; idx += kHN) {
@@ -686,16 +706,14 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
       return 1.0f / sc;
     };
 
-    for (int it = 0; it < n_items; ++it) {
-      const int s = it & 1;
+    // ---- the slot of item `it`: S (forward) or G (backward) on the tile + halo, zero outside the cutout
+    auto fill = [&](int it) {
       int b, tile;
       item_of(it, b, tile);
       const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
       const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;          // tile origin in the cutout
       const size_t img = (size_t)(b >= 0 ? b : 0) * a.H * a.W;
       float amax = 0.0f;
-
-      // ---- fill the slot: S (forward) or G (backward) on the tile + halo, zero outside the cutout
       if (!BWD) {
         const CompConst* ccb = a.cc + (size_t)(b >= 0 ? b : 0) * a.md.n_comp;
         for (int c = 0; c < a.md.n_comp; ++c) {
@@ -722,6 +740,7 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
         }
       } else {
         const float* gsrc = a.gbuf + img;
+#pragma unroll 4
         for (int idx = htid; idx < kRegionGroups; idx += kHN) {
           const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
           const int i = i0 - h + R, j = j0 - h + x;
@@ -734,64 +753,88 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
         }
       }
       if (!isfinite(amax)) amax = 0.0f;
-      const float inv_sc = scale_and_split(amax);
+      inv_sc[it & 1] = scale_and_split(amax);
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(F_IN_FULL + s));
+      if (lane == 0) mbar_arrive(bar(F_IN_FULL + (it & 1)));
+    };
 
-      // ---- drain the accumulators into the (now free) slot, top-left aligned: pixel (R, c) of the tile
+    // accumulator columns 32 p .. 32 p + 31 of every lane -> the transposition buffer as a (kRowsPerLd TRB) x TW
+    // sub-image: buffer row kRowsPerLd tr + rr = tile row tr, accumulator row kRowsPerLd p + rr; 16-byte chunks
+    // XOR-swizzled with tr
+    auto piece_in = [&](int s, int p, float inv) {
+      if ((hw >> 2) == (p & 3)) {                          // one warp per lane quarter
+        const int m = 32 * (hw & 3) + lane, tr = m % TRB, tc = m / TRB;
+        uint32_t v[32];
+        tmem_ld32(tD + (uint32_t)(s * C::kDCols + 32 * p) + lane_base, v);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int row = kRowsPerLd * tr + (4 * k) / kTileC, ch = (kTileC / 4) * tc + ((4 * k) % kTileC) / 4;
+          sts128(piece + 4u * (uint32_t)(row * T::TW + ((ch ^ (tr & 7)) << 2)),
+                 make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
+                            __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
+        }
+      }
+      help_sync();
+    };
+    // group idx of piece p: buffer address, and its pixel (R, x) of the tile
+    auto piece_px = [&](int p, int idx, int& R, int& x) -> uint32_t {
+      const int row = idx / TW4, ch = idx - row * TW4;
+      const int tr = row / kRowsPerLd;
+      R = kTileR * tr + kRowsPerLd * p + (row - kRowsPerLd * tr);
+      x = ch << 2;
+      return piece + 4u * (uint32_t)(row * T::TW + ((ch ^ (tr & 7)) << 2));
+    };
+
+    // ---- everything after the convolution of item `it`, beside the convolution of item it + 1
+    auto post = [&](int it) {
+      const int s = it & 1;
+      int b, tile;
+      item_of(it, b, tile);
+      const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
+      const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;
+      const size_t img = (size_t)(b >= 0 ? b : 0) * a.H * a.W;
       mbar_wait(bar(F_D_FULL + s), (it >> 1) & 1);
       fence_after();
-      {
-        const float inv = inv_sc * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
-        const int q = hw & 3, r_first = 2 * (hw >> 2);
-        const int m = 32 * q + lane, tr = m % TRB, tc = m / TRB;
-#pragma unroll 1
-        for (int r = r_first; r < r_first + 2; ++r) {
-          uint32_t v[32];
-          tmem_ld32(tD + (uint32_t)(s * C::kDCols + r * kTileC) + lane_base, v);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-          for (int k = 0; k < 8; ++k)
-            sts128(px_addr(4 * tr + r, kTileC * tc + 4 * k), make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
-                                           __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
-        }
-        fence_before();
-        help_sync();
-      }
-
+      const float inv = inv_sc[s] * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
       if (!BWD) {
-        // ---- a3 on the tile: residual, chi^2 partial, G to global (mode 0: M to global)
+        // a3 on the tile: residual, chi^2 partial, G to global (mode 0: M to global)
         float chi2 = 0.0f;
-        if (b >= 0) {
-          auto one = [&](float mm, float d, float sg, bool used) -> float {
-            float w = rcp_fast(sg * sg), rho = d - mm;
-            w = used ? w : 0.0f;
-            rho = used ? rho : 0.0f;
-            const float t = w * rho;
-            chi2 = fmaf(t, rho, chi2);
-            return -2.0f * t;
-          };
+        auto one = [&](float mm, float d, float sg, bool used) -> float {
+          float w = rcp_fast(sg * sg), rho = d - mm;
+          w = used ? w : 0.0f;
+          rho = used ? rho : 0.0f;
+          const float t = w * rho;
+          chi2 = fmaf(t, rho, chi2);
+          return -2.0f * t;
+        };
+        for (int p = 0; p < kPieces; ++p) {
+          piece_in(s, p, inv);
+          if (b >= 0) {
 #pragma unroll 2
-          for (int idx = htid; idx < kTileGroups; idx += kHN) {
-            const int R = idx / TW4, x = (idx - R * TW4) << 2;
-            const int i = i0 + R, j = j0 + x;
-            if (i >= a.H || j >= a.W) continue;
-            const size_t o = img + (size_t)i * a.W + j;
-            const uint4 m4 = lds128(px_addr(R, x));
-            if (a.mode == 0) {
-              *reinterpret_cast<float4*>(a.out + o) = make_float4(__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w));
-            } else {
-              const float4 d4 = *reinterpret_cast<const float4*>(a.data + o), s4 = *reinterpret_cast<const float4*>(a.sigma + o);
-              uchar4 k4 = make_uchar4(1, 1, 1, 1);
-              if (a.mask) k4 = *reinterpret_cast<const uchar4*>(a.mask + o);
-              float4 g;
-              g.x = one(__uint_as_float(m4.x), d4.x, s4.x, k4.x != 0);
-              g.y = one(__uint_as_float(m4.y), d4.y, s4.y, k4.y != 0);
-              g.z = one(__uint_as_float(m4.z), d4.z, s4.z, k4.z != 0);
-              g.w = one(__uint_as_float(m4.w), d4.w, s4.w, k4.w != 0);
-              if (a.mode == 2) *reinterpret_cast<float4*>(a.gbuf + o) = g;
+            for (int idx = htid; idx < kPieceGroups; idx += kHN) {
+              int R, x;
+              const uint32_t pa = piece_px(p, idx, R, x);
+              const int i = i0 + R, j = j0 + x;
+              if (i >= a.H || j >= a.W) continue;
+              const size_t o = img + (size_t)i * a.W + j;
+              const uint4 m4 = lds128(pa);
+              if (a.mode == 0) {
+                *reinterpret_cast<float4*>(a.out + o) = make_float4(__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w));
+              } else {
+                const float4 d4 = *reinterpret_cast<const float4*>(a.data + o), s4 = *reinterpret_cast<const float4*>(a.sigma + o);
+                uchar4 k4 = make_uchar4(1, 1, 1, 1);
+                if (a.mask) k4 = *reinterpret_cast<const uchar4*>(a.mask + o);
+                float4 g;
+                g.x = one(__uint_as_float(m4.x), d4.x, s4.x, k4.x != 0);
+                g.y = one(__uint_as_float(m4.y), d4.y, s4.y, k4.y != 0);
+                g.z = one(__uint_as_float(m4.z), d4.z, s4.z, k4.z != 0);
+                g.w = one(__uint_as_float(m4.w), d4.w, s4.w, k4.w != 0);
+                if (a.mode == 2) *reinterpret_cast<float4*>(a.gbuf + o) = g;
+              }
             }
           }
+          help_sync();                                     // the buffer may be rewritten
         }
         if (a.mode != 0) {
           chi2 = warp_sum(chi2);
@@ -799,40 +842,45 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
           help_sync();
           if (htid == 0 && b >= 0) {
             float t = 0.0f;
-            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w];
+            for (int w = 0; w < kHelp; ++w) t += red[w];
             a.chi2_part[(size_t)b * tiles + tile] = t;
           }
+          help_sync();
         }
-        help_sync();                                       // every read of the slot is done before the next fill
       } else {
-        // ---- a5 on the tile: the partial sums of every component from A
+        // a5 on the tile: the partial sums of every component from A (the pieces are drained once per component)
         for (int c = 0; c < a.md.n_comp; ++c) {
           float sm[kNSum];
 #pragma unroll
           for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
-          if (b >= 0) {
-            const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
-            const bool box = a.md.box[c] != 0;
-            dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-              GradAcc<KIND> acc;
-              acc.init();
-              for (int idx = htid; idx < kTileGroups; idx += kHN) {
-                const int R = idx / TW4, x = (idx - R * TW4) << 2;
-                const int i = i0 + R, j = j0 + x;
-                if (i >= a.H || j >= a.W) continue;
-                const uint4 q = lds128(px_addr(R, x));
-                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
-                if (box) {
+          const CompConst cc = a.cc[(size_t)(b >= 0 ? b : 0) * a.md.n_comp + c];
+          const bool box = a.md.box[c] != 0;
+          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+            GradAcc<KIND> acc;
+            acc.init();
+            for (int p = 0; p < kPieces; ++p) {
+              piece_in(s, p, inv);
+              if (b >= 0) {
+                for (int idx = htid; idx < kPieceGroups; idx += kHN) {
+                  int R, x;
+                  const uint32_t pa = piece_px(p, idx, R, x);
+                  const int i = i0 + R, j = j0 + x;
+                  if (i >= a.H || j >= a.W) continue;
+                  const uint4 q = lds128(pa);
+                  const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+                  if (box) {
 #pragma unroll
-                  for (int k = 0; k < 4; ++k)
-                    grad_accumulate<KIND>(cc, true, seed[k], (float)(j + k) + 0.5f, (float)a.H - 0.5f - (float)i, sm);
-                } else {
-                  grad_add4<KIND>(acc, cc, seed, (float)j + 0.5f, (float)a.H - 0.5f - (float)i);
+                    for (int k = 0; k < 4; ++k)
+                      grad_accumulate<KIND>(cc, true, seed[k], (float)(j + k) + 0.5f, (float)a.H - 0.5f - (float)i, sm);
+                  } else {
+                    grad_add4<KIND>(acc, cc, seed, (float)j + 0.5f, (float)a.H - 0.5f - (float)i);
+                  }
                 }
               }
-              if (!box) { acc.finish(cc, sm); sm[8] = sm[2]; }
-            });
-          }
+              help_sync();
+            }
+            if (b >= 0 && !box) { acc.finish(cc, sm); sm[8] = sm[2]; }
+          });
 #pragma unroll
           for (int k = 0; k < kNSum; ++k) {
             const float v = warp_sum(sm[k]);
@@ -841,19 +889,28 @@ __global__ void __launch_bounds__(kFusedThreadsTc, 1) k_tc_tile(const TileTcArgs
           help_sync();
           if (htid < kNSum && b >= 0) {
             float t = 0.0f;
-            for (int w = 0; w < kHelpWarpsTc; ++w) t += red[w * kNSum + htid];
+            for (int w = 0; w < kHelp; ++w) t += red[w * kNSum + htid];
             a.grad_part[(((size_t)b * tiles + tile) * a.md.n_comp + c) * kNSum + htid] = t;
           }
           help_sync();
         }
       }
+      fence_before();
+    };
+
+    for (int it = 0; it <= n_items; ++it) {
+      if (it < n_items) {
+        if (it > 0) mbar_wait(bar(F_SLOT_FREE), (it - 1) & 1);
+        fill(it);
+      }
+      if (it > 0) post(it - 1);
     }
   } else if (wid < kLastWarp) {
     // ----------------------------------- MMA issue ------------------------------------
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelpWarpsTc) fused_mma_role<KP, 0, T::kRingT>(n_items, 1, b0, r0, tD, tA);
-    else if (wid == 5 + kHelpWarpsTc) fused_mma_role<KP, 1, T::kRingT>(n_items, 1, b0, r0, tD, tA);
-    else if (wid == 6 + kHelpWarpsTc) fused_mma_role<KP, 2, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    if (wid == 4 + kHelp) fused_mma_role<KP, 0, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 5 + kHelp) fused_mma_role<KP, 1, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    else if (wid == 6 + kHelp) fused_mma_role<KP, 2, T::kRingT>(n_items, 1, b0, r0, tD, tA);
     else fused_mma_role<KP, 3, T::kRingT>(n_items, 1, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
