@@ -217,6 +217,7 @@ class Bench:
         self.stream = torch.cuda.current_stream()
         self.workers = min(16, os.cpu_count() or 1)
         gm.gm_init()
+        gm.gm_set_option(gm.GM_OPT_TENSOR, 1 if args.engine == "tensor" else 0)
         # the roofline denominator, measured in this process: a pure FFMA2 kernel (gm.h)
         self.peak_measured = gm.gm_measure_fp32_peak(10)
         pk, self.pk_src = peaks()
@@ -644,6 +645,7 @@ def run_ours(args):
                                    "gm_fit per cutout side, one after the other") if len(buckets) > 1 else None,
                        "parallelism": f"dp{bn.world} (galaxies dealt by pixel count, no collective in the loop, "
                                       "final all-gather of params/chi2)" if bn.world > 1 else "single GPU",
+                       "engine": args.engine,
                        "l2": "flushed between steps (256 MiB write)",
                        "inputs": "seeded synthetic SDSS-like (gen/configs.py), resident in HBM"},
             "galaxies_fitted_per_s": rec["galaxies_fitted_per_s"], "fit_summary": rec["fit_summary"],
@@ -706,6 +708,9 @@ def main():
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sub-records (C1, C3, C4, P1)")
     ap.add_argument("--per-galaxy-psf", action="store_true",
                     help="pass the PSF as [B,K,K] (the paper's data layout, P:45)")
+    ap.add_argument("--engine", default="tensor", choices=["tensor", "ffma2"],
+                    help="convolution engine: tcgen05 tensor cores (default, where the shape allows) or the FP32 FFMA2 "
+                         "loops only (gm_set_option(GM_OPT_TENSOR, 0)): the same workload on the engine of round 1")
     ap.add_argument("--stream-batches", type=int, default=0,
                     help="also stream this many batches through two streams (C4: 65,536 galaxies = 32 x 2048)")
     args = ap.parse_args()
