@@ -446,7 +446,9 @@ class Bench:
             for name in kern:
                 kern[name]["share_of_step"] = kinds[name][0] / t_ms if world == 1 else None
         if dom:
-            big = max(buckets, key=lambda k: k["B"] * k["H"] * k["W"])
+            # the largest bucket that runs the dominant kernel (with several buckets, the one its captures are keyed on)
+            ran = [k for k in buckets if dom in (k.get("serial") or {dom: None})]
+            big = max(ran or buckets, key=lambda k: k["B"] * k["H"] * k["W"])
             px_bytes = 9 if big["dev"][2] is not None else 8
             tensor = dom.startswith("tc_")
             peak = self.peak_tensor if tensor else self.peak_measured

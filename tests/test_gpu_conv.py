@@ -6,6 +6,7 @@ import torch
 
 import oracle
 import paper_2404_07780_b200 as gm
+from gen import models
 from gen.psf import gaussian_psf, moffat_psf
 from gpu_util import assert_pixels, dev
 
@@ -91,3 +92,35 @@ def test_tensor_engine_precision_and_dynamic_range():
 def test_tensor_engine_refuses_other_sizes():
     with pytest.raises(gm.GmError):
         gm.gm_conv(torch.zeros(2, 64, 64, device="cuda"), torch.ones(5, 5, device="cuda"), engine=gm.GM_CONV_TENSOR)
+
+
+def test_phase_trace_hook_records_every_phase():
+    """gm_trace_set (include/gm.h): CTA 0 of k_tc_fused appends one record per phase boundary; the hook is
+    off by default and switches off again with None."""
+    import torch
+    rng = np.random.default_rng(7)
+    model = models.single_sersic()
+    B, H, K = 300, 128, 25                                   # three cutouts for CTA 0 of 148
+    par = np.tile(np.array([[64.3, 63.1, 1.0, 6.0, 2.0, 0.7, 0.4]], dtype=np.float32), (B, 1))
+    psf = np.zeros((K, K), dtype=np.float32); psf[K // 2, K // 2] = 1.0
+    data = rng.normal(size=(B, H, H)).astype(np.float32); sigma = np.ones_like(data)
+    d = lambda a: torch.from_numpy(a).cuda()
+    buf = torch.zeros(gm.binding.TRACE_ROLES * gm.binding.TRACE_CAP, dtype=torch.int64, device="cuda")
+    gm.gm_trace_set(buf)
+    try:
+        gm.gm_loss_grad(model, d(par), d(data), d(sigma), None, d(psf))
+        torch.cuda.synchronize()
+    finally:
+        gm.gm_trace_set(None)
+    rec = buf.cpu().numpy().view(np.uint64).reshape(gm.binding.TRACE_ROLES, gm.binding.TRACE_CAP)
+    helper = [int(x) for x in rec[0] if x]; mma = [int(x) for x in rec[1] if x]
+    tags = [x >> 56 for x in helper]
+    # 3 cutouts: produce begin/end, drain wait/begin twice, residual begin/end, gradient begin/end each
+    assert tags.count(1) == 3 and tags.count(2) == 3 and tags.count(5) == 3 and tags.count(7) == 3 and tags.count(8) == 3
+    assert len(mma) == 2 * 2 * 3                             # job begin / end of two convolutions per cutout
+    clk = [x & ((1 << 48) - 1) for x in helper]
+    assert all(b >= a for a, b in zip(clk, clk[1:]))         # one thread writes the list in program order
+    again = torch.zeros_like(buf)
+    gm.gm_loss_grad(model, d(par), d(data), d(sigma), None, d(psf))
+    torch.cuda.synchronize()
+    assert int(again.abs().sum().item()) == 0
