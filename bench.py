@@ -230,14 +230,14 @@ class Bench:
     def mma_inflation(name, k):
         """MMA flops the tensor-core kernels issue per algorithmic convolution flop (1 for the FFMA2 kernels).
         One pass = 128 lanes of 4 x 32 output pixels; per pass and convolution KT tap rows x 4 accumulator rows x
-        NCH 16-column chunks x 3 split terms MMAs of 128 x 32 x 16 (gm_tc.cuh)."""
+        3 split terms x (NCH - 2 MMAs of 128 x 32 x 16 + 2 of 128 x 16 x 16 for the two edge chunks) (gm_tc.cuh)."""
         if not name.startswith("tc_"):
             return 1.0
         K, H, W = k["K"], k["H"], k["W"]
         KT = next(t for t in (9, 17, 25, 33, 41) if t >= K)
         TR, TC = 4, 32                                                    # kTileR, kTileC of gm_tc.cuh
         nch = (TC + KT - 1 + 15) // 16
-        per_pass = KT * TR * nch * 3 * (2.0 * 128 * TC * 16)
+        per_pass = KT * TR * 3 * ((nch - 2) * (2.0 * 128 * TC * 16) + 2 * (2.0 * 128 * (TC // 2) * 16))
         if name == "tc_fused":
             passes = {64: 0.25, 96: 1.0, 128: 1.0}[H]                     # per cutout
         else:

@@ -92,7 +92,7 @@ template <int KP, int R0, int RING>
 __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t bars, uint32_t ring_addr, uint32_t tD, uint32_t tA,
                                                unsigned long long* trace = nullptr) {
   using C = Cfg<KP>;
-  constexpr uint32_t idesc = instr_desc(128, kTileC);
+  constexpr uint32_t idesc = instr_desc(128, kTileC), idesc_half = instr_desc(128, kTileC / 2);
   constexpr uint32_t desc_hi = (uint32_t)(smem_desc(0, C::NR * 16, 128) >> 32);
   constexpr uint32_t desc_lo0 = (uint32_t)(smem_desc(0, C::NR * 16, 128) & 0xffffffffu);
   auto bar = [&](int i) -> uint32_t { return bars + 8u * (uint32_t)i; };
@@ -119,13 +119,20 @@ __device__ __forceinline__ void fused_mma_role(int n_items, int phases, uint32_t
         fence_after();
         const uint32_t dcol = tD + (uint32_t)(s * C::kDCols + (R0 + kMmaWarps * rr) * kTileC);
         const uint32_t lo0 = desc_lo0 + ((ring_addr + (uint32_t)(slot * C::kTapBytes)) >> 4);
+        // chunk 0 reaches only the lower half of the output columns (j <= c) and the last chunk only the upper half
+        // (j >= c - K + 1 >= kTileC / 2): those two run as N = kTileC / 2 MMAs; a full chunk goes first and overwrites
+        static_assert(C::NCH >= 3 && 16 * (C::NCH - 1) - (KP - 1) >= kTileC / 2 && kTileC / 2 >= 16, "half-width edge chunks");
 #pragma unroll
-        for (int kc = 0; kc < C::NCH; ++kc) {
-          const uint32_t b_hi = lo0 + (uint32_t)(16 * (C::NCH - 1 - kc));
+        for (int q = 0; q < C::NCH; ++q) {
+          const int kc = q < C::NCH - 2 ? q + 1 : (q == C::NCH - 2 ? 0 : C::NCH - 1);       // 1 .. NCH-2, then 0, then NCH-1
+          const bool lower = kc == 0, upper = kc == C::NCH - 1;
+          const uint32_t b_hi = lo0 + (uint32_t)(16 * (C::NCH - 1 - kc) + (upper ? kTileC / 2 : 0));
           const uint32_t b_lo = b_hi + (uint32_t)(2 * C::NR);
-          mma_f16_ts2(dcol, acol + kc * 16, b_hi, desc_hi, idesc, kc ? 1u : ((started >> rr) & 1u));   // hi * hi (the first MMA overwrites)
-          mma_f16_ts2(dcol, acol + kc * 16 + 8, b_hi, desc_hi, idesc, 1);                                // lo * hi
-          mma_f16_ts2(dcol, acol + kc * 16, b_lo, desc_hi, idesc, 1);                                    // hi * lo
+          const uint32_t dc = dcol + (upper ? kTileC / 2 : 0);
+          const uint32_t id = (lower || upper) ? idesc_half : idesc;
+          mma_f16_ts2(dc, acol + kc * 16, b_hi, desc_hi, id, q ? 1u : ((started >> rr) & 1u));          // hi * hi (the first MMA overwrites)
+          mma_f16_ts2(dc, acol + kc * 16 + 8, b_hi, desc_hi, id, 1);                   // lo * hi
+          mma_f16_ts2(dc, acol + kc * 16, b_lo, desc_hi, id, 1);                       // hi * lo
         }
         started |= 1u << rr;
         mma_commit(bar(F_B_EMPTY + slot));
