@@ -98,6 +98,34 @@ def test_multi_tile_and_ragged(H, W, K):
     assert_grad(grad, og)
 
 
+# ---- tensor-core super-tile kernels: several super-tiles per cutout, ragged in both directions, both shapes ----
+@pytest.mark.parametrize("H,W,K,per_psf", [(200, 264, 25, False),      # 2 x 3 super-tiles of 128 x 128, ragged
+                                           (132, 520, 41, False),      # 64 x 256 super-tiles (3 x 3), ragged
+                                           (260, 132, 25, True),       # one PSF per galaxy
+                                           (129, 128, 41, False)])     # one row beyond a single pass
+def test_tensor_super_tiles_ragged(H, W, K, per_psf):
+    model = models.bulge_disk()
+    B = 3                                                    # fewer items than CTAs, more than one per galaxy
+    par, data, sigma, mask, psf = synth(model, B, H, W, K, seed=3 * H + W + K, per_galaxy_psf=per_psf)
+    assert gm.gm_get_option(gm.GM_OPT_TENSOR) == 1
+    img = gm.gm_render(model, dev(par), H, W, dev(psf))
+    n_tc = gm.gm_last_launch_count()
+    assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+    # the FFMA2 engine on the same inputs: another launch sequence (this call did take the tensor-core path), same answers
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)
+    try:
+        img2 = gm.gm_render(model, dev(par), H, W, dev(psf))
+        n_ff = gm.gm_last_launch_count()
+    finally:
+        gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
+    assert n_tc != n_ff
+    assert_pixels(img2.cpu().numpy(), oracle.render(model, par, H, W, psf))
+
+
 def test_psf_orientation_not_flipped_or_transposed():
     # a delta PSF off centre must shift the model the way the oracle does
     model = models.single_sersic()
