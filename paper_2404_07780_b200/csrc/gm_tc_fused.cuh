@@ -157,6 +157,9 @@ __device__ __forceinline__ void stage_window_row(uint32_t rowp, uint32_t zero, b
     uint32_t w[16];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
+      // window columns beyond kTileC + KP - 2 meet only zero taps (chunk padding): zeros, no shared-memory read
+      // (the shared-memory pipe is what this engine runs out of first, and these warps are its largest client)
+      if (16 * kc + 4 * q >= kTileC + KP - 1) { w[4 * q] = w[4 * q + 1] = w[4 * q + 2] = w[4 * q + 3] = 0u; continue; }
       const int ch = chunk0 + 4 * kc + q;
       const uint4 v = lds128((row_ok && (unsigned)ch < (unsigned)n_chunks) ? rowp + 16u * (uint32_t)(ch ^ sw) : zero);
       w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
