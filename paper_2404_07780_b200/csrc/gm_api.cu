@@ -711,6 +711,8 @@ struct Workspace {
   int *calm, *frozen, *live, *n_live;
   uint8_t *tc_fwd, *tc_adj;  // E_a tables of the tensor-core path (128 x 128 cutouts only)
   float* tc_scale;
+  float* tc_gmax;            // [B, tiles] largest |G| per super-tile (forward -> backward kernel)
+  float* tc_sbuf;            // scratch of the forward super-tile kernel: one tile + halo of S per CTA
   size_t total;
 };
 
@@ -777,6 +779,8 @@ static Workspace carve(void* base, const ModelDesc& md, const gm_batch* bt, int 
   w.tc_fwd = (uint8_t*)take(tcb);
   w.tc_adj = (uint8_t*)take(tcb);
   w.tc_scale = (float*)take(tck ? n_psf * 4 : 0);
+  w.tc_gmax = (float*)take(tck == 2 ? B * tiles * 4 : 0);
+  w.tc_sbuf = (float*)take(tck == 2 ? (size_t)tc::kTileMaxCtas * tc::kTileScratchFloats * 4 : 0);
   w.total = off;
   return w;
 }
@@ -1138,8 +1142,9 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.md = pl.md; a.B = bt->B; a.H = bt->H; a.W = bt->W; a.tiles_x = pl.tc_tx; a.tiles_y = pl.tc_ty; a.mode = mode;
     a.cc = pl.ws.cc; a.btab = pl.ws.tc_fwd; a.btab_stride = stride; a.bscale = pl.ws.tc_scale;
     a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
-    a.out = out; a.gbuf = pl.ws.G; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+    a.out = out; a.gbuf = pl.ws.G; a.sbuf = pl.ws.tc_sbuf; a.gmax_part = pl.ws.tc_gmax; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
+    a.trace = g_trace.load();
     int pi = prof_begin(GM_PROF_TC_FORWARD, st);
     rc = tc::launch_tile(pl.KT, a, pl.tc_trb, 0, pl.caps.n_sm, st, &err);
     prof_end(pi, st);

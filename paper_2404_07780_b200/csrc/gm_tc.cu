@@ -84,7 +84,8 @@ template <int TRB, bool BWD>
 static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
   GM_TRY(set_smem_once((const void*)k_tc_tile<KP, TRB, BWD>, (int)TileCfg<KP, TRB>::kSmem));
   const long long items = (long long)a.B * a.tiles_x * a.tiles_y;
-  const int grid = items < n_sm ? (int)items : n_sm;
+  int grid = items < n_sm ? (int)items : n_sm;
+  if (grid > kTileMaxCtas) grid = kTileMaxCtas;            // the forward kernel's scratch is sized for that many
   k_tc_tile<KP, TRB, BWD><<<grid, Roles<kTileHW>::kThreads, TileCfg<KP, TRB>::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;

@@ -585,10 +585,16 @@ struct TileTcArgs {
   const float* data; const float* sigma; const uint8_t* mask;
   float* out;                // mode 0: model image
   float* gbuf;               // [B,H,W] back-seed G: written by the forward kernel, read by the backward kernel
+  float* sbuf;               // forward kernel: [gridDim.x][kTileScratchFloats] scratch, S of a CTA's next item (L2 resident)
   float* chi2_part;          // [B, tiles]
+  float* gmax_part;          // [B, tiles] largest |G| of a tile: forward kernel (mode 2) -> backward kernel
   float* grad_part;          // [B, tiles, n_comp, kNSum]
   const int* frozen; const int* live; const int* n_live;
+  unsigned long long* trace; // gm_trace_set (CTA 0), or nullptr
 };
+
+constexpr int kTileMaxCtas = 160;            // the super-tile kernels launch at most this many CTAs (one per SM)
+constexpr int kTileScratchFloats = 32768;    // >= (tile + halo) pixels of any super-tile: 104 x 296 at K = 41
 
 template <int KP, int TRB> struct TileCfg {
   using C = Cfg<KP>;
@@ -598,14 +604,19 @@ template <int KP, int TRB> struct TileCfg {
   static constexpr int RW = TW + KP - 1;                      // columns that carry data
   static constexpr int kPitchT = (TW - kTileC + 16 * C::NCH + 31) / 32 * 32;   // + window padding of the last tile column, whole swizzle groups
   static constexpr int kSlotWordsT = RR * kPitchT;
-  static constexpr int kPieceWords = 128 * 32;                // transposition buffer: 32 accumulator columns of every lane
-  static constexpr size_t kFixed = kAlignSlack + Roles<kTileHW>::kHeaderBytes + (size_t)kSlotWordsT * 4 + (size_t)kPieceWords * 4;
+  // transposition buffer of the accumulators: all 128 columns of every lane (the whole tile, 64 KB) where that
+  // leaves the tap-row rings at least 6 slots each (K = 25), else 32 columns at a time (16 KB, four rounds)
+  static constexpr size_t kFixedBase = kAlignSlack + Roles<kTileHW>::kHeaderBytes + (size_t)kSlotWordsT * 4;
+  static constexpr int kLdPerPiece = (kSmemLimit - kFixedBase - (size_t)C::kDCols * 128 * 4) / (2 * (size_t)C::kTapBytes) >= 6 ? C::kDCols / 32 : 1;
+  static constexpr int kPieceWords = 128 * 32 * kLdPerPiece;
+  static constexpr size_t kFixed = kFixedBase + (size_t)kPieceWords * 4;
   static constexpr int kRingT = ((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes)) >= (size_t)kMaxRing
                                     ? kMaxRing : (int)((kSmemLimit - kFixed) / (2 * (size_t)C::kTapBytes));
   static_assert(kRingT >= kTileR + 1, "tap-row rings");
   static constexpr size_t kSmem = kFixed + (size_t)(2 * kRingT) * C::kTapBytes;
   static_assert(kSmem <= kSmemLimit, "shared memory");
   static_assert(TW % 32 == 0 && TW >= 32, "rows of the transposition buffer are whole swizzle groups");
+  static_assert(RR * ((RW / 4) * 4) <= kTileScratchFloats, "scratch of the forward kernel");
 };
 
 template <int KP, int TRB, bool BWD>
@@ -691,32 +702,73 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
     auto help_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(kHN) : "memory"); };
     constexpr int RW4 = T::RW / 4, kRegionGroups = T::RR * RW4;      // groups of four pixels of the tile + halo
     constexpr int TW4 = T::TW / 4;
-    constexpr int kPieceRows = kRowsPerLd * TRB, kPieceGroups = kPieceRows * TW4;   // a piece = 32 accumulator columns (kRowsPerLd rows) of every tile
-    constexpr int kPieces = C::kDCols / 32;
+    constexpr int kLdPP = T::kLdPerPiece;                                          // 32-column loads per piece
+    constexpr int kPieceRows = kRowsPerLd * kLdPP * TRB, kPieceGroups = kPieceRows * TW4;   // a piece = 32 kLdPP accumulator columns of every tile
+    constexpr int kPieces = C::kDCols / (32 * kLdPP);
     const float inv_rw4 = 1.0f / (float)RW4;
     float inv_sc[2] = {1.0f, 1.0f};
+    Tracer tr;                                           // tags: TR_PRODUCE = fill / render ahead, TR_RESIDUAL / TR_GRADIENT = post
+    tr.init(a.trace, TR_HELPER, htid == 0);
 
-    auto scale_and_split = [&](float amax) -> float {
+    // ---- forward kernel: S of item `it` on the tile + halo (zero outside the cutout) -> this CTA's scratch in global
+    // memory (L2), as fp32.  Runs beside the convolution of item it - 1, so that the slot, the one thing the tensor
+    // pipe waits for, is filled by a single load-scale-split pass.  Returns the largest magnitude (every thread the same).
+    float* const scratch = BWD ? nullptr : a.sbuf + (size_t)blockIdx.x * kTileScratchFloats;
+    auto render_ahead = [&](int it) -> float {
+      int b, tile;
+      item_of(it, b, tile);
+      const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
+      const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;          // tile origin in the cutout
+      const CompConst* ccb = a.cc + (size_t)(b >= 0 ? b : 0) * a.md.n_comp;
+      float amax = 0.0f;
+      for (int c = 0; c < a.md.n_comp; ++c) {
+        const CompConst cc = ccb[c];
+        const bool box = a.md.box[c] != 0;
+        const bool first = c == 0, last = c == a.md.n_comp - 1;
+        dispatch_kind(a.md.kind[c], [&]<int KIND>() {
+          for (int idx = htid; idx < kRegionGroups; idx += kHN) {
+            const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
+            const int i = i0 - h + R, j = j0 - h + x;
+            float4* dst = reinterpret_cast<float4*>(scratch) + idx;
+            float v[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) {        // W % 4 == 0: whole group in or out
+              value4<KIND, kFastForward>(cc, box, (float)j + 0.5f, (float)a.H - 0.5f - (float)i, v);   // R:G1
+              if (!first) {                                                  // this thread's own earlier store
+                const float4 q = __ldcg(dst);
+                v[0] += q.x; v[1] += q.y; v[2] += q.z; v[3] += q.w;
+              }
+              if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
+            }
+            __stcg(dst, make_float4(v[0], v[1], v[2], v[3]));
+          }
+        });
+      }
+      if (!isfinite(amax)) amax = 0.0f;
       for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
       if (lane == 0) redmax[hw] = amax;
-      help_sync();
+      help_sync();                                       // also: every store of the scratch is visible to the CTA
       float mx = redmax[0];
 #pragma unroll
       for (int w = 1; w < kHelp; ++w) mx = fmaxf(mx, redmax[w]);
-      const float sc = pow2_scale(mx);
-#pragma unroll 2
+      help_sync();                                       // redmax may be rewritten
+      return mx;
+    };
+    // scratch -> slot: scale by the power of two of `amax`, split into (hi, lo) halves; the input of item `it` is ready
+    auto fill_from_scratch = [&](int it, float amax) {
+      const float sc = pow2_scale(amax);
+#pragma unroll 4
       for (int idx = htid; idx < kRegionGroups; idx += kHN) {
         const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
-        const uint32_t p = px_addr(R, x);
-        const uint4 v = lds128(p);
-        sts128(p, make_uint4(split_pack(__uint_as_float(v.x) * sc), split_pack(__uint_as_float(v.y) * sc),
-                             split_pack(__uint_as_float(v.z) * sc), split_pack(__uint_as_float(v.w) * sc)));
+        const float4 v = __ldcg(reinterpret_cast<const float4*>(scratch) + idx);
+        sts128(px_addr(R, x), make_uint4(split_pack(v.x * sc), split_pack(v.y * sc), split_pack(v.z * sc), split_pack(v.w * sc)));
       }
-      help_sync();
-      return 1.0f / sc;
+      inv_sc[it & 1] = 1.0f / sc;
+      help_sync();                                       // the scratch may be rewritten (render_ahead of the next item)
+      if (lane == 0) mbar_arrive(bar(F_IN_FULL + (it & 1)));
     };
 
-    // ---- the slot of item `it`: S (forward) or G (backward) on the tile + halo, zero outside the cutout
+    // ---- backward kernel: the slot of item `it`: G on the tile + halo from global memory, zero outside the cutout;
+    // one pass: the scale comes from the tile maxima the forward kernel left (this tile and its neighbours)
     auto fill = [&](int it) {
       int b, tile;
       item_of(it, b, tile);
@@ -724,46 +776,23 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
       const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;          // tile origin in the cutout
       const size_t img = (size_t)(b >= 0 ? b : 0) * a.H * a.W;
       float amax = 0.0f;
-      if (!BWD) {
-        const CompConst* ccb = a.cc + (size_t)(b >= 0 ? b : 0) * a.md.n_comp;
-        for (int c = 0; c < a.md.n_comp; ++c) {
-          const CompConst cc = ccb[c];
-          const bool box = a.md.box[c] != 0;
-          const bool first = c == 0, last = c == a.md.n_comp - 1;
-          dispatch_kind(a.md.kind[c], [&]<int KIND>() {
-            for (int idx = htid; idx < kRegionGroups; idx += kHN) {
-              const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
-              const int i = i0 - h + R, j = j0 - h + x;
-              const uint32_t p = px_addr(R, x);
-              float v[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-              if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) {        // W % 4 == 0: whole group in or out
-                value4<KIND, kFastForward>(cc, box, (float)j + 0.5f, (float)a.H - 0.5f - (float)i, v);   // R:G1
-                if (!first) {
-                  const uint4 q = lds128(p);
-                  v[0] += __uint_as_float(q.x); v[1] += __uint_as_float(q.y); v[2] += __uint_as_float(q.z); v[3] += __uint_as_float(q.w);
-                }
-                if (last) amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v[0]), fabsf(v[1]))), fmaxf(fabsf(v[2]), fabsf(v[3])));
-              }
-              sts128(p, make_uint4(__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3])));
-            }
-          });
-        }
-      } else {
-        const float* gsrc = a.gbuf + img;
-#pragma unroll 4
-        for (int idx = htid; idx < kRegionGroups; idx += kHN) {
-          const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
-          const int i = i0 - h + R, j = j0 - h + x;
-          float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) {
-            v = *reinterpret_cast<const float4*>(gsrc + (size_t)i * a.W + j);
-            amax = fmaxf(fmaxf(amax, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
-          }
-          sts128(px_addr(R, x), make_uint4(__float_as_uint(v.x), __float_as_uint(v.y), __float_as_uint(v.z), __float_as_uint(v.w)));
-        }
+      if (b >= 0) {
+        for (int ty = max(tile_y - 1, 0); ty <= min(tile_y + 1, a.tiles_y - 1); ++ty)
+          for (int tx = max(tile_x - 1, 0); tx <= min(tile_x + 1, a.tiles_x - 1); ++tx)
+            amax = fmaxf(amax, a.gmax_part[(size_t)b * tiles + ty * a.tiles_x + tx]);
       }
       if (!isfinite(amax)) amax = 0.0f;
-      inv_sc[it & 1] = scale_and_split(amax);
+      const float sc = pow2_scale(amax);
+      const float* gsrc = a.gbuf + img;
+#pragma unroll 4
+      for (int idx = htid; idx < kRegionGroups; idx += kHN) {
+        const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
+        const int i = i0 - h + R, j = j0 - h + x;
+        float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (b >= 0 && (unsigned)i < (unsigned)a.H && (unsigned)j < (unsigned)a.W) v = *reinterpret_cast<const float4*>(gsrc + (size_t)i * a.W + j);
+        sts128(px_addr(R, x), make_uint4(split_pack(v.x * sc), split_pack(v.y * sc), split_pack(v.z * sc), split_pack(v.w * sc)));
+      }
+      inv_sc[it & 1] = 1.0f / sc;
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(F_IN_FULL + (it & 1)));
     };
@@ -772,14 +801,17 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
     // sub-image: buffer row kRowsPerLd tr + rr = tile row tr, accumulator row kRowsPerLd p + rr; 16-byte chunks
     // XOR-swizzled with tr
     auto piece_in = [&](int s, int p, float inv) {
-      if ((hw >> 2) == (p & 3)) {                          // one warp per lane quarter
+      const int g = hw >> 2;                               // one warp per lane quarter and load
+      if (kLdPP > 1 || g == (p & 3)) {
+        const int ld = kLdPP > 1 ? g : p;                  // which 32 columns of the lane
         const int m = 32 * (hw & 3) + lane, tr = m % TRB, tc = m / TRB;
         uint32_t v[32];
-        tmem_ld32(tD + (uint32_t)(s * C::kDCols + 32 * p) + lane_base, v);
+        tmem_ld32(tD + (uint32_t)(s * C::kDCols + 32 * ld) + lane_base, v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          const int row = kRowsPerLd * tr + (4 * k) / kTileC, ch = (kTileC / 4) * tc + ((4 * k) % kTileC) / 4;
+          const int row = kRowsPerLd * kLdPP * tr + kRowsPerLd * (kLdPP > 1 ? ld : 0) + (4 * k) / kTileC;
+          const int ch = (kTileC / 4) * tc + ((4 * k) % kTileC) / 4;
           sts128(piece + 4u * (uint32_t)(row * T::TW + ((ch ^ (tr & 7)) << 2)),
                  make_uint4(__float_as_uint(__uint_as_float(v[4 * k]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 1]) * inv),
                             __float_as_uint(__uint_as_float(v[4 * k + 2]) * inv), __float_as_uint(__uint_as_float(v[4 * k + 3]) * inv)));
@@ -790,8 +822,8 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
     // group idx of piece p: buffer address, and its pixel (R, x) of the tile
     auto piece_px = [&](int p, int idx, int& R, int& x) -> uint32_t {
       const int row = idx / TW4, ch = idx - row * TW4;
-      const int tr = row / kRowsPerLd;
-      R = kTileR * tr + kRowsPerLd * p + (row - kRowsPerLd * tr);
+      const int tr = row / (kRowsPerLd * kLdPP);
+      R = kTileR * tr + kRowsPerLd * kLdPP * p + (row - kRowsPerLd * kLdPP * tr);
       x = ch << 2;
       return piece + 4u * (uint32_t)(row * T::TW + ((ch ^ (tr & 7)) << 2));
     };
@@ -806,6 +838,7 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
       const size_t img = (size_t)(b >= 0 ? b : 0) * a.H * a.W;
       mbar_wait(bar(F_D_FULL + s), (it >> 1) & 1);
       fence_after();
+      tr.ev(TR_JOB, it);                                   // the accumulators of the item are complete
       const float inv = inv_sc[s] * a.bscale[(a.btab_stride && b >= 0) ? b : 0];
       if (!BWD) {
         // a3 on the tile: residual, chi^2 partial, G to global (mode 0: M to global)
@@ -818,10 +851,11 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
           chi2 = fmaf(t, rho, chi2);
           return -2.0f * t;
         };
+        float gmax = 0.0f;
         for (int p = 0; p < kPieces; ++p) {
           piece_in(s, p, inv);
           if (b >= 0) {
-#pragma unroll 2
+#pragma unroll 4
             for (int idx = htid; idx < kPieceGroups; idx += kHN) {
               int R, x;
               const uint32_t pa = piece_px(p, idx, R, x);
@@ -840,6 +874,7 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
                 g.y = one(__uint_as_float(m4.y), d4.y, s4.y, k4.y != 0);
                 g.z = one(__uint_as_float(m4.z), d4.z, s4.z, k4.z != 0);
                 g.w = one(__uint_as_float(m4.w), d4.w, s4.w, k4.w != 0);
+                gmax = fmaxf(fmaxf(gmax, fmaxf(fabsf(g.x), fabsf(g.y))), fmaxf(fabsf(g.z), fabsf(g.w)));
                 if (a.mode == 2) *reinterpret_cast<float4*>(a.gbuf + o) = g;
               }
             }
@@ -848,12 +883,16 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
         }
         if (a.mode != 0) {
           chi2 = warp_sum(chi2);
-          if (lane == 0) red[hw] = chi2;
+          for (int o2 = 16; o2 > 0; o2 >>= 1) gmax = fmaxf(gmax, __shfl_xor_sync(0xffffffffu, gmax, o2));
+          if (lane == 0) { red[hw] = chi2; redmax[hw] = gmax; }
           help_sync();
           if (htid == 0 && b >= 0) {
-            float t = 0.0f;
-            for (int w = 0; w < kHelp; ++w) t += red[w];
+            float t = 0.0f, mx = 0.0f;
+            for (int w = 0; w < kHelp; ++w) { t += red[w]; mx = fmaxf(mx, redmax[w]); }
             a.chi2_part[(size_t)b * tiles + tile] = t;
+            // the largest back-seed of the tile: the backward kernel scales its input by the maximum over the tile and
+            // its neighbours, an upper bound of the maximum over tile + halo, and so needs no pass of its own for it
+            if (a.mode == 2) a.gmax_part[(size_t)b * tiles + tile] = mx;
           }
           help_sync();
         }
@@ -908,17 +947,35 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
       fence_before();
     };
 
-    for (int it = 0; it <= n_items; ++it) {
-      if (it < n_items) {
-        if (it > 0) mbar_wait(bar(F_SLOT_FREE), (it - 1) & 1);
-        fill(it);
+    if constexpr (!BWD) {
+      float amax_next = n_items > 0 ? render_ahead(0) : 0.0f;
+      for (int it = 0; it <= n_items; ++it) {
+        if (it < n_items) {
+          tr.ev(TR_DRAIN_WAIT, it);
+          if (it > 0) mbar_wait(bar(F_SLOT_FREE), (it - 1) & 1);
+          tr.ev(TR_DRAIN, it);
+          fill_from_scratch(it, amax_next);                // the convolution of item `it` starts
+          tr.ev(TR_PRODUCE_END, it);
+        }
+        if (it > 0) { tr.ev(TR_RESIDUAL, it - 1); post(it - 1); tr.ev(TR_RESIDUAL_END, it - 1); }
+        if (it + 1 < n_items) { tr.ev(TR_PRODUCE, it + 1); amax_next = render_ahead(it + 1); }
       }
-      if (it > 0) post(it - 1);
+    } else {
+      for (int it = 0; it <= n_items; ++it) {
+        if (it < n_items) {
+          tr.ev(TR_DRAIN_WAIT, it);
+          if (it > 0) mbar_wait(bar(F_SLOT_FREE), (it - 1) & 1);
+          tr.ev(TR_PRODUCE, it);
+          fill(it);
+          tr.ev(TR_PRODUCE_END, it);
+        }
+        if (it > 0) { tr.ev(TR_GRADIENT, it - 1); post(it - 1); tr.ev(TR_GRADIENT_END, it - 1); }
+      }
     }
   } else if (wid < kLastWarp) {
     // ----------------------------------- MMA issue ------------------------------------
     const uint32_t b0 = smem_u32(bars), r0 = smem_u32(ring);
-    if (wid == 4 + kHelp) fused_mma_role<KP, 0, T::kRingT>(n_items, 1, b0, r0, tD, tA);
+    if (wid == 4 + kHelp) fused_mma_role<KP, 0, T::kRingT>(n_items, 1, b0, r0, tD, tA, a.trace);
     else if (wid == 5 + kHelp) fused_mma_role<KP, 1, T::kRingT>(n_items, 1, b0, r0, tD, tA);
     else if (wid == 6 + kHelp) fused_mma_role<KP, 2, T::kRingT>(n_items, 1, b0, r0, tD, tA);
     else fused_mma_role<KP, 3, T::kRingT>(n_items, 1, b0, r0, tD, tA);
