@@ -92,16 +92,11 @@ static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaErr
 }
 
 int GM_CAT(launch_tile_tc_, GM_TC_K)(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err) {
-#if GM_TC_K == 25 || GM_TC_K == 41
   switch (trb) {
     case 128 / kTileR: return bwd ? launch_tile_t<128 / kTileR, true>(a, n_sm, st, err) : launch_tile_t<128 / kTileR, false>(a, n_sm, st, err);   // 128 x 128
     case 64 / kTileR: return bwd ? launch_tile_t<64 / kTileR, true>(a, n_sm, st, err) : launch_tile_t<64 / kTileR, false>(a, n_sm, st, err);      // 64 x 256
     default: return GM_ENOTSUP;
   }
-#else
-  (void)a; (void)trb; (void)bwd; (void)n_sm; (void)st; (void)err;
-  return GM_ENOTSUP;                        // the super-tile kernels are built for the PSF sides of the configs (25, 41)
-#endif
 }
 
 }  // namespace tc
