@@ -209,6 +209,9 @@ __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const
   uint32_t* slots = reinterpret_cast<uint32_t*>(ring + (size_t)(2 * Gm::kRingF) * C::kTapBytes);
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
+  // a CTA without work (late iterations of a fit with early stop: a few live galaxies, 148 CTAs) leaves at once, before
+  // it allocates tensor memory or zeroes 130 KB of slots: it would hold the SM against the other buckets' kernels
+  if ((int)blockIdx.x >= (a.live ? *a.n_live : a.B)) return;
   // warp index through a lane-0 broadcast: warp-uniform for the compiler (uniform registers in the role code)
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
@@ -636,6 +639,7 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
   uint32_t* piecew = slotw + T::kSlotWordsT;
   auto bar = [&](int i) -> uint32_t { return smem_u32(bars + i); };
 
+  if ((long long)blockIdx.x >= (long long)(a.live ? *a.n_live : a.B) * a.tiles_x * a.tiles_y) return;   // no item for this CTA
   const int tid = threadIdx.x, wid = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
   if (tid == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(bar(F_IN_FULL + i), kHelp); mbar_init(bar(F_D_FULL + i), kMmaWarps); }
