@@ -469,6 +469,9 @@ class Bench:
                 "fp32_peak_nominal": self.peak_nominal,
                 # whole-step view: the same flops against the step time (small kernels and gaps included)
                 "step_frac": (conv_flops / (ms_per_step * 1e-3) / 1e12) / peak}
+            if early and len(buckets) > 1:
+                rec["roofline"]["note"] = ("whole fit with early stop: most of the iterations run the few galaxies that have not "
+                                           "converged yet (latency, not throughput); per_config holds the same kernels at full batch")
             if tensor:
                 # what the tensor pipe is asked to do for those flops: 3 fp16 MMAs per product (hi*hi + lo*hi + hi*lo)
                 # on Toeplitz band blocks: issued MMA flops / the same time / the same peak
