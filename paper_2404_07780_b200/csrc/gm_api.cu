@@ -1025,12 +1025,10 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
       pl->ct_stream = st;
     }
   }
-  // Tensor-core path (gm_tc_fused.cuh): 128 x 128 cutouts whose components all go through the PSF.  It
+  // Tensor-core path (gm_tc_fused.cuh), where the shape of the batch allows it (tc_kind).  It
   // needs the E_a tables of the PSF(s), forward and adjoint; the FFMA2 taps above stay available for the
   // Jacobian columns of the covariance row.
   pl->tc = g_opt[GM_OPT_TENSOR].load() != 0 ? tc_kind(bt, &pl->KT) : 0;
-  for (int c = 0; c < pl->md.n_comp && pl->tc; ++c)
-    if (pl->md.conv[c] == 0) pl->tc = 0;
   if (pl->tc) {
     const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma;
     if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = 0;              // 128-bit row accesses
@@ -1131,6 +1129,9 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.btab_fwd = pl.ws.tc_fwd; a.btab_adj = pl.ws.tc_adj; a.btab_stride = stride; a.bscale = pl.ws.tc_scale;
     a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
     a.out = out; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+    a.any_unconv = 0;
+    for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
+    a.gseed = pl.ws.G;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
     a.trace = g_trace.load();
     const int pi = prof_begin(GM_PROF_TC_FUSED, st);
@@ -1142,7 +1143,10 @@ static int dispatch_tc(const Plan& pl, const gm_batch* bt, int mode, float* out,
     a.md = pl.md; a.B = bt->B; a.H = bt->H; a.W = bt->W; a.tiles_x = pl.tc_tx; a.tiles_y = pl.tc_ty; a.mode = mode;
     a.cc = pl.ws.cc; a.btab = pl.ws.tc_fwd; a.btab_stride = stride; a.bscale = pl.ws.tc_scale;
     a.data = bt->data; a.sigma = bt->sigma; a.mask = bt->mask;
-    a.out = out; a.gbuf = pl.ws.G; a.sbuf = pl.ws.tc_sbuf; a.gmax_part = pl.ws.tc_gmax; a.chi2_part = pl.ws.chi2_part; a.grad_part = pl.ws.grad_part;
+    a.out = out; a.gbuf = pl.ws.G; a.sbuf = pl.ws.tc_sbuf; a.gmax_part = pl.ws.tc_gmax; a.chi2_part = pl.ws.chi2_part;
+    a.any_unconv = 0;
+    for (int c = 0; c < pl.md.n_comp; ++c) a.any_unconv |= (pl.md.conv[c] == 0);
+    a.grad_part = pl.ws.grad_part;
     a.frozen = ls.frozen; a.live = ls.live; a.n_live = ls.n_live;
     a.trace = g_trace.load();
     int pi = prof_begin(GM_PROF_TC_FORWARD, st);

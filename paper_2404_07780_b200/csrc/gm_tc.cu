@@ -59,15 +59,19 @@ int GM_CAT(launch_conv_tc_, GM_TC_K)(const ConvArgs& a, int n_sm, cudaStream_t s
 }
 
 // a1 .. a5 of square cutouts of 64, 96 or 128 pixels in one launch
-template <int SIDE>
-static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+template <int SIDE, bool UNCONV>
+static int launch_fused_u(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
   using Gm = FusedGeomTc<KP, SIDE>;
-  GM_TRY(set_smem_once((const void*)k_tc_fused<KP, SIDE>, (int)Gm::kSmem));
+  GM_TRY(set_smem_once((const void*)k_tc_fused<KP, SIDE, UNCONV>, (int)Gm::kSmem));
   const int passes = (a.B + Gm::G - 1) / Gm::G;
   const int grid = passes < n_sm ? passes : n_sm;
-  k_tc_fused<KP, SIDE><<<grid, Roles<kFusedHW>::kThreads, Gm::kSmem, st>>>(a);
+  k_tc_fused<KP, SIDE, UNCONV><<<grid, Roles<kFusedHW>::kThreads, Gm::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;
+}
+template <int SIDE>
+static int launch_fused_t(const FusedTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  return a.any_unconv ? launch_fused_u<SIDE, true>(a, n_sm, st, err) : launch_fused_u<SIDE, false>(a, n_sm, st, err);
 }
 
 int GM_CAT(launch_fused_tc_, GM_TC_K)(const FusedTcArgs& a, int side, int n_sm, cudaStream_t st, cudaError_t* err) {
@@ -80,15 +84,19 @@ int GM_CAT(launch_fused_tc_, GM_TC_K)(const FusedTcArgs& a, int side, int n_sm, 
 }
 
 // larger cutouts, super-tiles of trb x (128 / trb) tiles; bwd = 0: forward kernel, 1: backward kernel
-template <int TRB, bool BWD>
-static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
-  GM_TRY(set_smem_once((const void*)k_tc_tile<KP, TRB, BWD>, (int)TileCfg<KP, TRB>::kSmem));
+template <int TRB, bool BWD, bool UNCONV>
+static int launch_tile_u(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  GM_TRY(set_smem_once((const void*)k_tc_tile<KP, TRB, BWD, UNCONV>, (int)TileCfg<KP, TRB>::kSmem));
   const long long items = (long long)a.B * a.tiles_x * a.tiles_y;
   int grid = items < n_sm ? (int)items : n_sm;
   if (grid > kTileMaxCtas) grid = kTileMaxCtas;            // the forward kernel's scratch is sized for that many
-  k_tc_tile<KP, TRB, BWD><<<grid, Roles<kTileHW>::kThreads, TileCfg<KP, TRB>::kSmem, st>>>(a);
+  k_tc_tile<KP, TRB, BWD, UNCONV><<<grid, Roles<kTileHW>::kThreads, TileCfg<KP, TRB>::kSmem, st>>>(a);
   GM_TRY(cudaGetLastError());
   return GM_OK;
+}
+template <int TRB, bool BWD>
+static int launch_tile_t(const TileTcArgs& a, int n_sm, cudaStream_t st, cudaError_t* err) {
+  return a.any_unconv ? launch_tile_u<TRB, BWD, true>(a, n_sm, st, err) : launch_tile_u<TRB, BWD, false>(a, n_sm, st, err);
 }
 
 int GM_CAT(launch_tile_tc_, GM_TC_K)(const TileTcArgs& a, int trb, int bwd, int n_sm, cudaStream_t st, cudaError_t* err) {

@@ -45,6 +45,8 @@ struct FusedTcArgs {
   const float* bscale;       // [n_psf] 1 / (power-of-two scale of the PSF)
   const float* data; const float* sigma; const uint8_t* mask;
   float* out;                // mode 0: model image [B,128,128]
+  int any_unconv;            // the model has components that do not go through the PSF (R:C3; the sky is one)
+  float* gseed;              // [B,SIDE,SIDE] back-seed G for the gradient of those components (mode 2 with any_unconv)
   float* chi2_part;          // [B]
   float* grad_part;          // [B, n_comp, kNSum]
   const int* frozen;
@@ -193,7 +195,9 @@ template <int KP, int SIDE> struct FusedGeomTc {
   static_assert(kSmem <= kSmemLimit, "shared memory");
 };
 
-template <int KP, int SIDE>
+// UNCONV: the model has components that do not go through the PSF (a variant of its own: the extra tests in the
+// helper loops cost 12 % at K = 25, where the helper warps bind)
+template <int KP, int SIDE, bool UNCONV>
 __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const FusedTcArgs a) {
   using C = Cfg<KP>;
   using Gm = FusedGeomTc<KP, SIDE>;
@@ -324,10 +328,16 @@ __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const
         float amax = 0.0f;
         if (b >= 0) {
           const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+          int c_first = -1, c_last = -1;                   // the components that go through the PSF
+          for (int c = 0; c < a.md.n_comp; ++c)
+            if (!UNCONV || a.md.conv[c]) { if (c_first < 0) c_first = c; c_last = c; }
+          if (c_first < 0)                                 // none: S = 0, the model is the unconvolved part alone
+            for (int idx = htid; idx < kGroups; idx += kHN) sts128(px_addr(cut, idx / W4, (idx % W4) << 2), make_uint4(0u, 0u, 0u, 0u));
           for (int c = 0; c < a.md.n_comp; ++c) {
+            if (UNCONV && !a.md.conv[c]) continue;
             const CompConst cc = ccb[c];
             const bool box = a.md.box[c] != 0;
-            const bool first = c == 0, last = c == a.md.n_comp - 1;
+            const bool first = c == c_first, last = c == c_last;
             dispatch_kind(a.md.kind[c], [&]<int KIND>() {
               for (int idx = htid; idx < kGroups; idx += kHN) {
                 const int R = idx / W4, x = (idx % W4) << 2;
@@ -397,9 +407,28 @@ __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const
         float chi2 = 0.0f, amax = 0.0f;
         if (b >= 0) {
           const size_t img = (size_t)b * SIDE * SIDE;
+          // components that do not go through the PSF are added to the convolved image here (R:C3), pixel by pixel
+          const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+          auto add_unconv = [&](uint4& m4, int idx) {
+            const int R = idx / W4, x = (idx % W4) << 2;
+            const float y = (float)SIDE - 0.5f - (float)R;
+            float m[4] = {__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w)};
+            for (int c = 0; c < a.md.n_comp; ++c) {
+              if (a.md.conv[c]) continue;
+              const CompConst cc = ccb[c];
+              const int kind = a.md.kind[c];
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry<false>(cc, a.md.box[c] != 0, (float)(x + k) + 0.5f, y).r);
+                m[k] = fmaf(cc.amp, U, m[k]);
+              }
+            }
+            m4 = make_uint4(__float_as_uint(m[0]), __float_as_uint(m[1]), __float_as_uint(m[2]), __float_as_uint(m[3]));
+          };
           if (a.mode == 0) {
             for (int idx = htid; idx < kGroups; idx += kHN) {
-              const uint4 v = lds128(px_addr(cut, idx / W4, (idx % W4) << 2));
+              uint4 v = lds128(px_addr(cut, idx / W4, (idx % W4) << 2));
+              if (UNCONV) add_unconv(v, idx);
               *reinterpret_cast<float4*>(a.out + img + 4 * (size_t)idx) =
                   make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
             }
@@ -425,13 +454,19 @@ __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const
                 const float4 d4 = dptr[idx], s4 = sptr[idx];
                 uchar4 k4 = make_uchar4(1, 1, 1, 1);
                 if (MASKED) k4 = kptr[idx];
-                const uint4 m4 = lds128(p);
+                uint4 m4 = lds128(p);
+                if (UNCONV) add_unconv(m4, idx);
                 uint4 gv;
                 gv.x = __float_as_uint(one(__uint_as_float(m4.x), d4.x, s4.x, !MASKED || k4.x != 0));
                 gv.y = __float_as_uint(one(__uint_as_float(m4.y), d4.y, s4.y, !MASKED || k4.y != 0));
                 gv.z = __float_as_uint(one(__uint_as_float(m4.z), d4.z, s4.z, !MASKED || k4.z != 0));
                 gv.w = __float_as_uint(one(__uint_as_float(m4.w), d4.w, s4.w, !MASKED || k4.w != 0));
-                if (with_grad) sts128(p, gv);
+                if (with_grad) {
+                  sts128(p, gv);
+                  if (UNCONV)                             // their gradient needs G itself, not PSF * G
+                    *reinterpret_cast<float4*>(a.gseed + img + 4 * (size_t)idx) =
+                        make_float4(__uint_as_float(gv.x), __uint_as_float(gv.y), __uint_as_float(gv.z), __uint_as_float(gv.w));
+                }
               }
             };
             if (a.mask) pass.template operator()<true>();
@@ -466,14 +501,20 @@ __global__ void __launch_bounds__(Roles<kFusedHW>::kThreads, 1) k_tc_fused(const
           for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
           if (b >= 0) {
             const CompConst cc = a.cc[(size_t)b * a.md.n_comp + c];
-            const bool box = a.md.box[c] != 0;
+            const bool box = a.md.box[c] != 0, conv = !UNCONV || a.md.conv[c] != 0;
             dispatch_kind(a.md.kind[c], [&]<int KIND>() {
               GradAcc<KIND> acc;
               acc.init();
               for (int idx = htid; idx < kGroups; idx += kHN) {
                 const int R = idx / W4, x = (idx % W4) << 2;
-                const uint4 q = lds128(px_addr(cut, R, x));
-                const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+                float seed[4];
+                if (conv) {                                // A = PSF * G, in the slot
+                  const uint4 q = lds128(px_addr(cut, R, x));
+                  seed[0] = __uint_as_float(q.x); seed[1] = __uint_as_float(q.y); seed[2] = __uint_as_float(q.z); seed[3] = __uint_as_float(q.w);
+                } else {                                   // G itself (written by this CTA's residual pass)
+                  const float4 q = __ldcg(reinterpret_cast<const float4*>(a.gseed + (size_t)b * SIDE * SIDE) + idx);
+                  seed[0] = q.x; seed[1] = q.y; seed[2] = q.z; seed[3] = q.w;
+                }
                 if (box) {                                 // Eq. 2 with B != 0: per-pixel geometry
 #pragma unroll
                   for (int k = 0; k < 4; ++k)
@@ -590,6 +631,7 @@ struct TileTcArgs {
   float* gbuf;               // [B,H,W] back-seed G: written by the forward kernel, read by the backward kernel
   float* sbuf;               // forward kernel: [gridDim.x][kTileScratchFloats] scratch, S of a CTA's next item (L2 resident)
   float* chi2_part;          // [B, tiles]
+  int any_unconv;            // the model has components that do not go through the PSF
   float* gmax_part;          // [B, tiles] largest |G| of a tile: forward kernel (mode 2) -> backward kernel
   float* grad_part;          // [B, tiles, n_comp, kNSum]
   const int* frozen; const int* live; const int* n_live;
@@ -622,7 +664,7 @@ template <int KP, int TRB> struct TileCfg {
   static_assert(RR * ((RW / 4) * 4) <= kTileScratchFloats, "scratch of the forward kernel");
 };
 
-template <int KP, int TRB, bool BWD>
+template <int KP, int TRB, bool BWD, bool UNCONV>
 __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const TileTcArgs a) {
   using C = Cfg<KP>;
   using T = TileCfg<KP, TRB>;
@@ -725,10 +767,16 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
       const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;          // tile origin in the cutout
       const CompConst* ccb = a.cc + (size_t)(b >= 0 ? b : 0) * a.md.n_comp;
       float amax = 0.0f;
+      int c_first = -1, c_last = -1;                       // the components that go through the PSF
+      for (int c = 0; c < a.md.n_comp; ++c)
+        if (!UNCONV || a.md.conv[c]) { if (c_first < 0) c_first = c; c_last = c; }
+      if (c_first < 0)                                     // none: S = 0
+        for (int idx = htid; idx < kRegionGroups; idx += kHN) __stcg(reinterpret_cast<float4*>(scratch) + idx, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
       for (int c = 0; c < a.md.n_comp; ++c) {
+        if (UNCONV && !a.md.conv[c]) continue;
         const CompConst cc = ccb[c];
         const bool box = a.md.box[c] != 0;
-        const bool first = c == 0, last = c == a.md.n_comp - 1;
+        const bool first = c == c_first, last = c == c_last;
         dispatch_kind(a.md.kind[c], [&]<int KIND>() {
           for (int idx = htid; idx < kRegionGroups; idx += kHN) {
             const int R = (int)(((float)idx + 0.5f) * inv_rw4), x = (idx - R * RW4) << 2;
@@ -866,7 +914,23 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
               const int i = i0 + R, j = j0 + x;
               if (i >= a.H || j >= a.W) continue;
               const size_t o = img + (size_t)i * a.W + j;
-              const uint4 m4 = lds128(pa);
+              uint4 m4 = lds128(pa);
+              if (UNCONV) {                                // components that do not go through the PSF (R:C3)
+                const CompConst* ccb = a.cc + (size_t)b * a.md.n_comp;
+                const float y = (float)a.H - 0.5f - (float)i;
+                float m[4] = {__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w)};
+                for (int c = 0; c < a.md.n_comp; ++c) {
+                  if (a.md.conv[c]) continue;
+                  const CompConst cc = ccb[c];
+                  const int kind = a.md.kind[c];
+#pragma unroll
+                  for (int k = 0; k < 4; ++k) {
+                    const float U = (kind == GM_SKY) ? 1.0f : profile_value(kind, cc, geometry<false>(cc, a.md.box[c] != 0, (float)(j + k) + 0.5f, y).r);
+                    m[k] = fmaf(cc.amp, U, m[k]);
+                  }
+                }
+                m4 = make_uint4(__float_as_uint(m[0]), __float_as_uint(m[1]), __float_as_uint(m[2]), __float_as_uint(m[3]));
+              }
               if (a.mode == 0) {
                 *reinterpret_cast<float4*>(a.out + o) = make_float4(__uint_as_float(m4.x), __uint_as_float(m4.y), __uint_as_float(m4.z), __uint_as_float(m4.w));
               } else {
@@ -907,7 +971,7 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
 #pragma unroll
           for (int k = 0; k < kNSum; ++k) sm[k] = 0.0f;
           const CompConst cc = a.cc[(size_t)(b >= 0 ? b : 0) * a.md.n_comp + c];
-          const bool box = a.md.box[c] != 0;
+          const bool box = a.md.box[c] != 0, conv = !UNCONV || a.md.conv[c] != 0;
           dispatch_kind(a.md.kind[c], [&]<int KIND>() {
             GradAcc<KIND> acc;
             acc.init();
@@ -919,8 +983,14 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
                   const uint32_t pa = piece_px(p, idx, R, x);
                   const int i = i0 + R, j = j0 + x;
                   if (i >= a.H || j >= a.W) continue;
-                  const uint4 q = lds128(pa);
-                  const float seed[4] = {__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), __uint_as_float(q.w)};
+                  float seed[4];
+                  if (conv) {                                // A = PSF * G, from the accumulators
+                    const uint4 q = lds128(pa);
+                    seed[0] = __uint_as_float(q.x); seed[1] = __uint_as_float(q.y); seed[2] = __uint_as_float(q.z); seed[3] = __uint_as_float(q.w);
+                  } else {                                   // G itself
+                    const float4 q = *reinterpret_cast<const float4*>(a.gbuf + img + (size_t)i * a.W + j);
+                    seed[0] = q.x; seed[1] = q.y; seed[2] = q.z; seed[3] = q.w;
+                  }
                   if (box) {
 #pragma unroll
                     for (int k = 0; k < 4; ++k)

@@ -126,6 +126,29 @@ def test_tensor_super_tiles_ragged(H, W, K, per_psf):
     assert_pixels(img2.cpu().numpy(), oracle.render(model, par, H, W, psf))
 
 
+# ---- tensor-core kernels with components that do not go through the PSF (point source, sky; R:C3) ----
+@pytest.mark.parametrize("H,W,K,per_psf", [(128, 128, 9, False), (96, 96, 15, True), (64, 64, 25, False),
+                                           (200, 264, 9, False), (132, 520, 25, True)])
+def test_tensor_engine_with_unconvolved_components(H, W, K, per_psf):
+    model = models.all_profiles()                            # six laws, tied parameters, an unconvolved source, the sky
+    assert any(c["convolve"] == 0 for c in model["components"])
+    par, data, sigma, mask, psf = synth(model, 3, H, W, K, seed=7 * H + W + K, per_galaxy_psf=per_psf)
+    img = gm.gm_render(model, dev(par), H, W, dev(psf))
+    n_tc = gm.gm_last_launch_count()
+    assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
+    chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
+    oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
+    assert_chi2(chi2, oc)
+    assert_grad(grad, og)
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # the FFMA2 engine launches another sequence
+    try:
+        gm.gm_render(model, dev(par), H, W, dev(psf))
+        n_ff = gm.gm_last_launch_count()
+    finally:
+        gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
+    assert n_tc != n_ff
+
+
 def test_psf_orientation_not_flipped_or_transposed():
     # a delta PSF off centre must shift the model the way the oracle does
     model = models.single_sersic()
