@@ -162,7 +162,7 @@ int gm_init(void* cuda_stream);
 /* Process-wide switches, for tests and measurements (value 0 / 1, default 1 each):
  *   GM_OPT_FUSED       cutouts up to 128 x 128 take the single fused kernel; 0: tile kernels
  *   GM_OPT_CONST_TAPS  a batch-wide PSF is read from the constant bank; 0: shared memory
- *   GM_OPT_TENSOR      both convolutions run on the
+ *   GM_OPT_TENSOR      with a PSF of more than 9 x 9 taps both convolutions run on the
  *                      tensor cores (fp16 hi/lo split of the fp32 operands, see gm_conv): square cutouts
  *                      of 64 (shared PSF), 96 or 128 pixels in one fused kernel, cutouts above 128 pixels
  *                      with W a multiple of 4 in super-tiles; every other shape and 0: the FP32 (FFMA2)

@@ -729,16 +729,22 @@ static void tc_tile_geom(int H, int W, int* trb, int* tx, int* ty) {
 }
 
 // which tensor-core path the SHAPE of the batch allows (the model and the options decide later):
-// 1 = k_tc_fused (square cutouts of 64, 96, 128 px), 2 = k_tc_tile (larger, W a multiple of 4, PSF side with tile kernels), 0 = none;
+// 1 = k_tc_fused (square cutouts of 64, 96, 128 px), 2 = k_tc_tile (larger or of another shape, W a multiple of 4), 0 = none;
 // *KT = padded PSF side of that engine
 static int tc_kind(const gm_batch* bt, int* KT) {
   *KT = tc::padded_side(bt->K);
   if (*KT < 0) return 0;
+  // up to 9 x 9 taps the FFMA2 engine is as fast or faster (measured, profiles/r02_tc_engine.md section 6: the tensor-core
+  // kernels' render / residual / gradient phases no longer hide behind so short a convolution)
+  if (bt->K <= 9) return 0;
   if (bt->H == bt->W && (bt->H == 64 || bt->H == 96 || bt->H == 128)) {
     // several 64 px cutouts share the lanes of one pass, and with them one PSF
     return (bt->H == 64 && bt->psf_stride != 0) ? 0 : 1;
   }
-  if ((bt->H > tc::kSide || bt->W > tc::kSide) && (bt->W & 3) == 0 && tc::has_tile_kernels(*KT)) return 2;
+  // the super-tile kernels also take the other shapes up to 128 px (100 x 100, 128 x 96, ...) when the cutout fills
+  // at least 96 x 96 pixels of a 128-lane pass; below that the FFMA2 engine wastes less
+  const bool large = bt->H > tc::kSide || bt->W > tc::kSide || (long long)bt->H * bt->W >= 96 * 96;
+  if (large && (bt->W & 3) == 0 && tc::has_tile_kernels(*KT)) return 2;
   return 0;
 }
 

@@ -102,7 +102,10 @@ def test_multi_tile_and_ragged(H, W, K):
 @pytest.mark.parametrize("H,W,K,per_psf", [(200, 264, 25, False),      # 2 x 3 super-tiles of 128 x 128, ragged
                                            (132, 520, 41, False),      # 64 x 256 super-tiles (3 x 3), ragged
                                            (260, 132, 25, True),       # one PSF per galaxy
-                                           (129, 128, 41, False)])     # one row beyond a single pass
+                                           (129, 128, 41, False),      # one row beyond a single pass
+                                           (100, 100, 25, False),      # one ragged super-tile: shapes up to 128 px that
+                                           (128, 96, 15, True),        # are not 64 / 96 / 128 squares
+                                           (72, 256, 15, False)])
 def test_tensor_super_tiles_ragged(H, W, K, per_psf):
     model = models.bulge_disk()
     B = 3                                                    # fewer items than CTAs, more than one per galaxy
@@ -127,8 +130,8 @@ def test_tensor_super_tiles_ragged(H, W, K, per_psf):
 
 
 # ---- tensor-core kernels with components that do not go through the PSF (point source, sky; R:C3) ----
-@pytest.mark.parametrize("H,W,K,per_psf", [(128, 128, 9, False), (96, 96, 15, True), (64, 64, 25, False),
-                                           (200, 264, 9, False), (132, 520, 25, True)])
+@pytest.mark.parametrize("H,W,K,per_psf", [(128, 128, 11, False), (96, 96, 15, True), (64, 64, 25, False),
+                                           (200, 264, 17, False), (132, 520, 25, True)])
 def test_tensor_engine_with_unconvolved_components(H, W, K, per_psf):
     model = models.all_profiles()                            # six laws, tied parameters, an unconvolved source, the sky
     assert any(c["convolve"] == 0 for c in model["components"])
