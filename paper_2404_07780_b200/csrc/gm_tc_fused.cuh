@@ -1055,8 +1055,43 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
     else fused_mma_role<KP, 3, T::kRingT>(n_items, 1, b0, r0, tD, tA);
   } else {
     // ------------------------------- tap-row producer --------------------------------
-    if (lane == 0) {
-      for (int it = 0; it < n_items; ++it) {
+    // (forward kernel: its idle lanes first ask the L2 for D, sigma and the mask of the item, which the residual
+    // pass reads one convolution later: that pass waits on global memory)
+    for (int it = 0; it < n_items; ++it) {
+      if (!BWD && a.mode != 0) {
+        int b, tile;
+        item_of(it, b, tile);
+        if (b >= 0) {
+          const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
+          const int i0 = tile_y * T::TH, j0 = tile_x * T::TW;
+          const size_t img = (size_t)b * a.H * a.W;
+          constexpr int kLines = T::TW / 32;                       // 128-byte lines of floats per tile row
+          for (int e = lane; e < T::TH * kLines; e += 32) {
+            const int i = i0 + e / kLines, j = j0 + (e % kLines) * 32;
+            if (i >= a.H || j >= a.W) continue;
+            const size_t o = img + (size_t)i * a.W + j;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + o));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.sigma + o));
+            if (a.mask && (e % kLines) % 4 == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.mask + o));
+          }
+        }
+      }
+      if (BWD && it + 1 < n_items) {                        // backward kernel: G of the NEXT item's tile + halo
+        int b, tile;
+        item_of(it + 1, b, tile);
+        if (b >= 0) {
+          const int tile_y = tile / a.tiles_x, tile_x = tile - tile_y * a.tiles_x;
+          const int i0 = tile_y * T::TH - h, j0 = tile_x * T::TW - h;
+          const size_t img = (size_t)b * a.H * a.W;
+          constexpr int kLines = (T::RW + 31) / 32 + 1;            // 128-byte lines that a row of the region may touch
+          for (int e = lane; e < T::RR * kLines; e += 32) {
+            const int i = i0 + e / kLines, j = ((j0 < 0 ? 0 : j0) & ~31) + (e % kLines) * 32;
+            if ((unsigned)i >= (unsigned)a.H || j >= a.W || j > j0 + T::RW) continue;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.gbuf + img + (size_t)i * a.W + j));
+          }
+        }
+      }
+      if (lane == 0) {
         int b, tile;
         item_of(it, b, tile);
         const uint8_t* tab = a.btab + (size_t)(b >= 0 ? b : 0) * a.btab_stride;
@@ -1071,6 +1106,7 @@ __global__ void __launch_bounds__(Roles<kTileHW>::kThreads, 1) k_tc_tile(const T
           bulk_g2s(smem_u32(ring + (size_t)sl * C::kTapBytes), tab + (size_t)ta * C::kTapBytes, C::kTapBytes, bar(F_B_FULL + sl));
         }
       }
+      __syncwarp();
     }
   }
   fence_before();
