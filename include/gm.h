@@ -68,7 +68,8 @@ typedef enum {
                         slot index out of range, non-positive size               */
   GM_ENOTSUP = -2,   /* valid request that this build has no kernel for          */
   GM_ECUDA = -3,     /* CUDA launch / runtime error (see gm_last_cuda_error)      */
-  GM_EWORKSPACE = -4 /* workspace NULL, misaligned or too small                   */
+  GM_EWORKSPACE = -4,/* workspace NULL, misaligned or too small                   */
+  GM_ETOOLARGE = -5  /* problem larger than the built-in scratch of a *_static call */
 } gm_status;
 
 /* radial laws: Sec. 4.1, 4.2.1 - 4.2.6 */
@@ -265,6 +266,37 @@ typedef struct {
 int gm_bootstrap_counts(const gm_batch* batch, const gm_boot_opts* boot, int32_t r,
                         int32_t* counts, void* workspace, size_t workspace_bytes,
                         void* cuda_stream);
+
+/* gm_bootstrap_counts for callers that CANNOT ALLOCATE device memory and so have no workspace to
+ * pass: code that runs inside a host application which hands it a fixed set of buffers (a plug-in,
+ * a pipeline stage), services that fix their memory plan at start-up (real-time, embedded, or
+ * running beside a framework that has claimed the whole GPU), and threads for which an allocation
+ * could stall or deadlock (another library's callback, a lock the allocator also wants).  Same
+ * arguments as gm_bootstrap_counts minus the workspace, same kernels, bit for bit the same counts;
+ * the caller still provides the mask (input) and `counts` (output, dev [B,H,W] int32).
+ *   - Scratch is an array compiled into the library (`static __device__`, 256-byte aligned,
+ *     4 * (GM_STATIC_MAX_PIXELS + GM_STATIC_MAX_B) bytes = about 4.02 MB).  Every GPU on which the
+ *     library's device code is loaded holds it until the process exits, used or not.
+ *   - Limits: B <= GM_STATIC_MAX_B and B * H * W <= GM_STATIC_MAX_PIXELS (e.g. 64 cutouts of
+ *     128 x 128, 16 of 256 x 256).  Anything larger returns GM_ETOOLARGE before any launch or
+ *     write; split the batch (id_offset keeps the draws of a galaxy independent of the split) or
+ *     call gm_bootstrap_counts with a workspace.
+ *   - The call itself makes no cudaMalloc / cudaFree / pool allocation and calls no library routine
+ *     that does: two kernels and one cudaMemsetAsync of `counts` on `cuda_stream`, asynchronous.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with
+ *     that device current; the calling thread's current device is the one used) and keeps it.  Make
+ *     that first call during set-up, before any stream capture begins on that device.
+ *   - All calls on a device share the one array and it keeps what the last call wrote.  Nothing in it
+ *     has to start at zero (each call rewrites every entry it later reads; `counts` is cleared by
+ *     the call), but two calls whose kernels may overlap on the GPU -- different streams without an
+ *     event between them, or several host threads -- RACE on it and give wrong counts.  Issue
+ *     them on one stream, or order them yourself.
+ * Errors: GM_EINVAL (NULL pointer, r < 0, non-positive size), GM_ETOOLARGE, GM_ECUDA,
+ * GM_ENOTSUP (device ordinal >= 64). */
+#define GM_STATIC_MAX_PIXELS (1 << 20)   /* B * H * W of one gm_bootstrap_counts_static call  */
+#define GM_STATIC_MAX_B      4096        /* galaxies of one gm_bootstrap_counts_static call    */
+int gm_bootstrap_counts_static(const gm_batch* batch, const gm_boot_opts* boot, int32_t r,
+                               int32_t* counts, void* cuda_stream);
 
 /* M refits, every one started from `params` (dev [B,P], not modified) with `opts`.
  * sigma_boot: dev [B,P].  mean: dev [B,P] or NULL.  samples: dev [M,B,P] fitted

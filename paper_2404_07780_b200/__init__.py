@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     gm_trace_set,
     gm_bootstrap,
     gm_bootstrap_counts,
+    gm_bootstrap_counts_static,
     gm_conv,
     gm_fit,
     gm_fit_host,

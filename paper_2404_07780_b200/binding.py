@@ -90,6 +90,8 @@ def _lib():
         bo = C.POINTER(_BootOpts)
         L.gm_bootstrap_workspace_bytes.restype = sz; L.gm_bootstrap_workspace_bytes.argtypes = [mp, bp, C.c_int32]
         L.gm_bootstrap_counts.restype = i; L.gm_bootstrap_counts.argtypes = [bp, bo, C.c_int32, vp, vp, sz, vp]
+        L.gm_bootstrap_counts_static.restype = i
+        L.gm_bootstrap_counts_static.argtypes = [bp, bo, C.c_int32, vp, vp]
         L.gm_bootstrap.restype = i; L.gm_bootstrap.argtypes = [mp, bp, vp, op, bo, vp, vp, vp, vp, sz, vp]
         L.gm_uncertainty_workspace_bytes.restype = sz; L.gm_uncertainty_workspace_bytes.argtypes = [mp, bp]
         L.gm_uncertainty.restype = i; L.gm_uncertainty.argtypes = [mp, bp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -414,6 +416,31 @@ def gm_bootstrap_counts(B, H, W, mask, seed, r, id_offset=0, stream=None):
     _check(rc, "gm_bootstrap_counts")
     counts._gm_ws = ws
     return counts
+
+
+STATIC_MAX_PIXELS, STATIC_MAX_B = 1 << 20, 4096       # GM_STATIC_MAX_PIXELS, GM_STATIC_MAX_B
+
+
+@_on_stream
+def gm_bootstrap_counts_static(B, H, W, mask, seed, r, id_offset=0, out=None, stream=None):
+    """gm_bootstrap_counts without a workspace, for callers that may not allocate device memory
+    (plug-ins given fixed buffers, services with a memory plan fixed at start-up, threads where an
+    allocation could deadlock).  The scratch is an array built into libgm.so, so B <= STATIC_MAX_B and
+    B*H*W <= STATIC_MAX_PIXELS, else GmError(GM_ETOOLARGE).  Pass `out` (int32 CUDA tensor [B,H,W]) and
+    this wrapper allocates nothing either; without it the result tensor comes from torch.  Calls share
+    the one array: keep them on one stream (or ordered by events), never overlapping.  Make the first
+    call on a device during set-up, before any stream capture.  Asynchronous."""
+    dev = mask.device if mask is not None else (out.device if out is not None else torch.device("cuda"))
+    b = _Batch(B, H, W, 1, None, None, _dev(mask, torch.uint8, "mask"), None, 0)
+    o = _BootOpts(1, int(seed), int(id_offset))
+    if out is None:
+        out = torch.empty((B, H, W), dtype=torch.int32, device=dev)
+    elif (not out.is_cuda or out.dtype != torch.int32 or not out.is_contiguous()
+          or tuple(out.shape) != (B, H, W)):
+        raise ValueError("out: contiguous int32 CUDA tensor [B,H,W]")
+    rc = _lib().gm_bootstrap_counts_static(C.byref(b), C.byref(o), int(r), out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "gm_bootstrap_counts_static")
+    return out
 
 
 @_on_stream

@@ -1691,6 +1691,72 @@ int gm_bootstrap(const gm_model* model, const gm_batch* bt, const float* params,
 
 }  // extern "C"
 
+// ---- gm_bootstrap_counts_static: the same multiplicities for callers that cannot allocate ----
+// Some users of this library own no allocator on the device: a plug-in handed a fixed set of
+// buffers by its host application, a real-time or embedded service that fixes its memory plan at
+// start-up, or a thread that runs while an allocation would stall or deadlock the process (inside
+// another library's callback, under a lock the allocator also takes).  gm_bootstrap_counts needs a
+// scratch list (the used-pixel table and one count per galaxy) that somebody must provide; here it
+// lives in the library image itself, so the caller passes only the mask in and the counts out.
+//
+// The array below is device memory that every GPU which loads libgm.so reserves until the process
+// exits (about 4.02 MB: GM_STATIC_MAX_PIXELS ints for the list, GM_STATIC_MAX_B ints for the per
+// galaxy totals, plus alignment).  In HOST code its name is only a handle for the runtime, not a
+// device address, so the address the kernels get comes from cudaGetSymbolAddress, looked up once
+// per device with that device current and cached.
+namespace gm {
+constexpr size_t kStaticListBytes = (size_t)GM_STATIC_MAX_PIXELS * 4;                 // used[], 256-byte multiple
+constexpr size_t kStaticBytes = kStaticListBytes + (size_t)GM_STATIC_MAX_B * 4;
+static_assert(kStaticListBytes % 256 == 0, "the per-galaxy totals start on a 256-byte boundary");
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mu;
+static void* g_static_ptr[kStaticMaxDevices] = {};      // device address of g_static_scratch, per device ordinal
+
+// Address of the scratch array on the CURRENT device (set-up on the first call there).
+static int static_scratch(void** out) {
+  int dev = -1;
+  GM_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return GM_ENOTSUP;
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    GM_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p || ((uintptr_t)p & 255)) return GM_EWORKSPACE;
+    g_static_ptr[dev] = p;
+  }
+  *out = g_static_ptr[dev];
+  return GM_OK;
+}
+}  // namespace gm
+
+extern "C" {
+
+int gm_bootstrap_counts_static(const gm_batch* bt, const gm_boot_opts* bo, int32_t r, int32_t* counts,
+                               void* cuda_stream) {
+  t_launches = 0;
+  if (!bt || !bo || !counts || r < 0) return GM_EINVAL;
+  if (bt->B < 1 || bt->H < 1 || bt->W < 1) return GM_EINVAL;
+  const size_t B = bt->B, N = (size_t)bt->H * bt->W;
+  if (B > (size_t)GM_STATIC_MAX_B || N > (size_t)GM_STATIC_MAX_PIXELS || B * N > (size_t)GM_STATIC_MAX_PIXELS)
+    return GM_ETOOLARGE;                                     // nothing launched, nothing touched
+  void* base = nullptr;
+  int rc = static_scratch(&base);
+  if (rc != GM_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // Layout: used[B*N] at 0, n_used[B] at kStaticListBytes.  Both are written by k_used_list before
+  // k_boot_draw reads them (used[] only up to n_used[b] per galaxy, and not at all without a
+  // mask), so what an earlier call left behind is never read and nothing here needs clearing;
+  // the one buffer that must start at zero is the OUTPUT, which boot_counts clears on `st`.
+  int* used = (int*)base;
+  int* n_used = (int*)((char*)base + kStaticListBytes);
+  if ((rc = boot_used(bt, used, n_used, st)) != GM_OK) return rc;
+  return boot_counts(bt, bo, r, used, n_used, counts, st);
+}
+
+}  // extern "C"
+
 extern "C" {
 
 // ---- host-buffer variants ----------------------------------------------------
@@ -1878,6 +1944,7 @@ const char* gm_strerror(int status) {
     case GM_ENOTSUP: return "not supported by this build";
     case GM_ECUDA: return "CUDA error (see gm_last_cuda_error_string)";
     case GM_EWORKSPACE: return "workspace missing, misaligned or too small";
+    case GM_ETOOLARGE: return "larger than the built-in scratch of this *_static entry point (see GM_STATIC_MAX_*)";
     default: return "unknown status";
   }
 }
