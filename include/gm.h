@@ -25,14 +25,16 @@
  *   - All images are row-major, [B,H,W] contiguous, float32; row 0 is the TOP row
  *     (largest y).  Angles are radians, lengths pixels, amplitudes intensities.
  *   - Device entry points are asynchronous on `cuda_stream` (a cudaStream_t; NULL =
- *     the legacy default stream), allocate nothing, and never synchronise, from the first
- *     call on.  Scratch comes from the caller: `workspace` (dev, 256-byte aligned) of at
+ *     the legacy default stream), allocate nothing, and never synchronise (gm_init excepted),
+ *     from the first call on.  Scratch comes from the caller: `workspace` (dev, 256-byte aligned) of at
  *     least gm_workspace_bytes(model, batch) bytes.
  *   - Process-wide state the library keeps (all of it derived, none of it observable in
  *     results): the nu_n interpolation table, filled once per device by a kernel on the
  *     stream of gm_init or of the first compute call (calls on other streams are made to
- *     wait for that kernel through an event until it has completed; call gm_init before
- *     capturing a CUDA graph); a 59 KB constant-bank pool per PSF side that holds the
+ *     wait for that kernel through an event until it has completed; gm_init itself returns
+ *     only after the table is complete, so call it before capturing a CUDA graph -- a compute
+ *     call that finds the table missing or still in flight on a stream that is being
+ *     captured returns GM_EINVAL and enqueues nothing); a 59 KB constant-bank pool per PSF side that holds the
  *     paired taps of a batch-wide PSF (psf_stride == 0) for the duration of a call -- a
  *     region is filled by a device-to-device copy on the call's stream and handed back
  *     through an event on that stream, a later call on the same stream (same
@@ -56,7 +58,7 @@
 extern "C" {
 #endif
 
-#define GM_VERSION   200     /* major*10000 + minor*100 + patch */
+#define GM_VERSION   300     /* major*10000 + minor*100 + patch */
 #define GM_MAX_COMP  8       /* components per model                               */
 #define GM_MAX_PAR   32      /* entries of the per-galaxy parameter vector          */
 #define GM_MAX_K     41      /* PSF side (odd); the paper's PSFs are 41x41   */
@@ -157,7 +159,9 @@ enum { GM_FIT_OK = 0, GM_FIT_CONVERGED = 1, GM_FIT_NONFINITE = 2 };
 /* ---- device entry points (asynchronous) ---------------------------------- */
 
 /* Optional: build the per-device tables on `cuda_stream` now instead of inside the first
- * compute call (asynchronous; idempotent).  Needed only before CUDA graph capture. */
+ * compute call.  Idempotent.  The one device entry point that WAITS: it returns after its
+ * (microseconds long) table kernel has completed, so a stream capture may begin right after it;
+ * needed only before CUDA graph capture.  GM_EINVAL when `cuda_stream` is already capturing. */
 int gm_init(void* cuda_stream);
 
 /* Process-wide switches, for tests and measurements (value 0 / 1, default 1 each):
@@ -168,8 +172,10 @@ int gm_init(void* cuda_stream);
  *                      of 64 (shared PSF), 96 or 128 pixels in one fused kernel, cutouts above 128 pixels
  *                      with W a multiple of 4 in super-tiles; every other shape and 0: the FP32 (FFMA2)
  *                      convolution
- * The first two give bit for bit the same results; GM_OPT_TENSOR changes the convolution arithmetic
- * (pixels agree to a few 1e-6 relative, inside every documented tolerance).  gm_set_option returns
+ * The first two give bit for bit the same results; GM_OPT_TENSOR changes the convolution arithmetic:
+ * its error is ABSOLUTE, a few 1e-7 of the cutout's brightest pixel (one power-of-two scale per cutout,
+ * see gm_conv), i.e. a few 1e-6 relative on pixels within two decades of the maximum and no significant
+ * bits below about 1e-7 of it; inside every documented tolerance.  gm_set_option returns
  * GM_EINVAL for an unknown option, gm_get_option -1. */
 enum { GM_OPT_FUSED = 0, GM_OPT_CONST_TAPS = 1, GM_OPT_TENSOR = 2, GM_OPT_COUNT_ = 3 };
 int gm_set_option(int option, int value);
@@ -177,7 +183,10 @@ int gm_get_option(int option);
 
 /* Bytes of device scratch gm_render / gm_loss_grad / gm_fit need for this model
  * and batch shape (B, H, W, K, psf_stride -- one PSF or B of them -- and the model are
- * read; the pointers are not).  0 on invalid input. */
+ * read; the pointers are not).  0 on invalid input.  Sized by shape alone, for whichever engine may run:
+ * with one PSF per galaxy (psf_stride != 0) it holds the tap tables of every galaxy for both engines
+ * (forward and adjoint each), which dominates the total -- 0.53 MB per galaxy at K = 41 (0.27 MB at
+ * K = 25), 4.4 GB for 8,289 galaxies; a batch-wide PSF costs one set.  A call fills only the tables of the engine it runs. */
 size_t gm_workspace_bytes(const gm_model* model, const gm_batch* batch);
 
 /* Render the model image M (App. C "initial_model").
@@ -315,10 +324,14 @@ int gm_bootstrap(const gm_model* model, const gm_batch* batch, const float* para
  *   GM_CONV_FFMA2   the FP32 direct convolution of the fit path (packed FFMA2 loop); any H, W, odd
  *                   K <= GM_MAX_K
  *   GM_CONV_TENSOR  tcgen05 tensor cores: every fp32 operand is scaled by an exact power of two and
- *                   split into two fp16 halves (22 significant bits), three MMAs per product accumulate
+ *                   split into two fp16 halves (22 bits of the SCALED value: one scale per cutout taken
+ *                   from its largest |pixel|, so a pixel 2^-k below the maximum keeps 22 - k bits and anything
+ *                   below 2^-24 of the scaled range is flushed to zero), three MMAs per product accumulate
  *                   hi*hi + lo*hi + hi*lo in fp32 in tensor memory (the dropped lo*lo term is 2^-22
  *                   relative); Toeplitz band blocks of the PSF stream through shared memory.  H = W = 128
- *                   only (GM_ENOTSUP otherwise); inputs must be finite.
+ *                   only (GM_ENOTSUP otherwise); inputs must be finite.  batch->data and out must be
+ *                   16-byte aligned (the kernel moves 128-bit rows): GM_EINVAL otherwise, nothing launched;
+ *                   GM_CONV_FFMA2 takes any 4-byte aligned view.
  * batch: B, H, W, K, psf, psf_stride are read and batch->data is the INPUT image, dev [B,H,W].
  * out: dev [B,H,W].  workspace: gm_conv_workspace_bytes(engine, batch).  Asynchronous. */
 enum { GM_CONV_FFMA2 = 0, GM_CONV_TENSOR = 1 };
@@ -344,6 +357,14 @@ int gm_fit_host(const gm_model* model, const gm_batch* host_batch, float* params
 int gm_fit_multi_host(const gm_model* model, int32_t n_batches, const gm_batch* host_batches,
                       float* const* params, const gm_fit_opts* opts, float* const* chi2_out,
                       int32_t* const* iters_used, int32_t* const* status);
+
+/* Extended chi^2 log-likelihood, Eq. 17:
+ *   ln L = -(k/2) ln 2 - ln Gamma(k/2) + (k/2 - 1) ln chi2 - chi2/2,
+ * k = n_used[b] - n_free: "the number of pixels ... not included in the mask" minus "the number of model
+ * fit parameters".  A per-galaxy scalar after a fit, so a HOST helper (fp64, no CUDA call):
+ * chi2 host [B] (as copied back from gm_fit / gm_loss_grad), n_used host [B], loglike host [B].
+ * Entries with k < 1 or chi2 <= 0 or non-finite chi2 get NaN.  GM_EINVAL for NULL / B < 1 / n_free < 0. */
+int gm_loglike(int32_t B, const float* chi2, const int32_t* n_used, int32_t n_free, double* loglike);
 
 /* ---- misc ------------------------------------------------------------------ */
 const char* gm_strerror(int status);

@@ -25,6 +25,7 @@ from .binding import (  # noqa: F401
     gm_fit_multi,
     gm_fit_multi_host,
     gm_last_launch_count,
+    gm_loglike,
     gm_loss_grad,
     gm_loss_grad_host,
     gm_profile_enable,

@@ -98,6 +98,7 @@ def _lib():
         L.gm_render_host.restype = i; L.gm_render_host.argtypes = [mp, bp, vp, vp]
         L.gm_loss_grad_host.restype = i; L.gm_loss_grad_host.argtypes = [mp, bp, vp, vp, vp]
         L.gm_fit_host.restype = i; L.gm_fit_host.argtypes = [mp, bp, vp, op, vp, vp, vp]
+        L.gm_loglike.restype = i; L.gm_loglike.argtypes = [C.c_int32, vp, vp, C.c_int32, vp]
         L.gm_strerror.restype = C.c_char_p; L.gm_strerror.argtypes = [i]
         L.gm_version.restype = i; L.gm_version.argtypes = []
         L.gm_last_cuda_error.restype = i; L.gm_last_cuda_error.argtypes = []
@@ -225,6 +226,18 @@ def _opts_struct(opts: dict, P: int):
 # ---- entry points (same names as include/gm.h) ---------------------------------
 def gm_version() -> int:
     return _lib().gm_version()
+
+
+def gm_loglike(chi2, n_used, n_free: int):
+    """ln L of Eq. 17 per galaxy, k = n_used - n_free.  Host helper: chi2 [B] (numpy or a
+    tensor, copied to the host), n_used [B] int; returns float64 numpy [B] (NaN where k < 1 or chi2 <= 0)."""
+    c = np.ascontiguousarray(chi2.detach().cpu().numpy() if isinstance(chi2, torch.Tensor) else chi2, dtype=np.float32)
+    n = np.ascontiguousarray(n_used.detach().cpu().numpy() if isinstance(n_used, torch.Tensor) else n_used, dtype=np.int32)
+    if c.ndim != 1 or n.shape != c.shape:
+        raise ValueError("chi2 and n_used: one entry per galaxy")
+    out = np.empty(c.shape[0], dtype=np.float64)
+    _check(_lib().gm_loglike(c.shape[0], c.ctypes.data, n.ctypes.data, int(n_free), out.ctypes.data), "gm_loglike")
+    return out
 
 
 def gm_strerror(status: int) -> str:

@@ -149,7 +149,10 @@ __global__ void k_nu_table() {
   g_nu_table[i] = make_double2(nu, dnu * n);             // (nu, d nu / d ln n)
 }
 
-static int ensure_nu_table(cudaStream_t st) {
+// wait: gm_init -- return only once the table is complete (phase 2), so that a stream capture may
+// begin right after it.  A call that finds the table missing or in flight while `st` is being captured
+// is refused (GM_EINVAL): the fill kernel and the wait on its event belong outside the graph.
+static int ensure_nu_table(cudaStream_t st, bool wait = false) {
   struct State { int phase = 0; cudaEvent_t ev = nullptr; unsigned long long sid = 0; };   // 0 none, 1 in flight, 2 done
   static std::mutex mu;
   static State state[64];
@@ -159,16 +162,24 @@ static int ensure_nu_table(cudaStream_t st) {
   std::lock_guard<std::mutex> lk(mu);
   State& s = state[dev];
   if (s.phase == 2) return GM_OK;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  GM_CUDA(cudaStreamIsCapturing(st, &cap));
+  if (cap != cudaStreamCaptureStatusNone) return GM_EINVAL;
   unsigned long long sid = 0;
   GM_CUDA(cudaStreamGetId(st, &sid));
   if (s.phase == 0) {
+    if (!s.ev) GM_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));   // kept for a retry if what follows fails
     k_nu_table<<<(kNuTableN + 1 + 127) / 128, 128, 0, st>>>();
     GM_CUDA(cudaGetLastError());
     ++t_launches;
-    GM_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
     GM_CUDA(cudaEventRecord(s.ev, st));
     s.sid = sid;
     s.phase = 1;
+    if (!wait) return GM_OK;
+  }
+  if (wait) {
+    GM_CUDA(cudaEventSynchronize(s.ev));
+    s.phase = 2;
     return GM_OK;
   }
   const cudaError_t q = cudaEventQuery(s.ev);
@@ -986,8 +997,11 @@ static bool make_fused_geom(int H, int W, int KP, bool shared_taps, size_t smem_
 
 // early_stop: the call is a fit whose galaxies stop one by one (tol > 0), so the number of live
 // galaxies shrinks during the call.
+// want: which engines the caller will run besides what the shape selects (see the body)
+enum : unsigned { kPlanAuto = 0u, kPlanFfma2 = 1u, kPlanNoTensor = 2u };
 static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, void* workspace,
-                     size_t workspace_bytes, cudaStream_t st, Plan* pl, bool early_stop = false) {
+                     size_t workspace_bytes, cudaStream_t st, Plan* pl, bool early_stop = false,
+                     unsigned want = kPlanAuto) {
   int rc = validate(model, bt, need_data, &pl->md);
   if (rc != GM_OK) return rc;
   pl->KP = padded_K(bt->K);
@@ -998,6 +1012,8 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   pl->ws = carve(workspace, pl->md, bt, pl->KP, pl->tg);
   if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < pl->ws.total) return GM_EWORKSPACE;
   if ((rc = device_caps(&pl->caps)) != GM_OK) return rc;
+  // before the first launch of the call: refuses a capturing stream while the nu_n table is missing
+  if ((rc = ensure_nu_table(st)) != GM_OK) return rc;
   pl->fused = bt->H <= 128 && bt->W <= 128 && g_opt[GM_OPT_FUSED].load() != 0 &&
               make_fused_geom(bt->H, bt->W, pl->KP, bt->psf_stride == 0, pl->caps.smem_optin, &pl->fg,
                               &pl->fused_variant);
@@ -1005,19 +1021,31 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
   // the tile count of the tile geometry, so that must be one as well (it is for every H, W <= 128
   // today; checked here so that a change of make_geom cannot silently break the sums)
   if (pl->fused && pl->tiles != 1) pl->fused = false;
+  // Tensor-core path (gm_tc_fused.cuh), where the shape of the batch allows it (tc_kind) and the caller
+  // does not rule it out.  Decided first: each engine's tables are built only if that engine will run.
+  pl->tc = ((want & kPlanNoTensor) == 0 && g_opt[GM_OPT_TENSOR].load() != 0) ? tc_kind(bt, &pl->KT) : 0;
+  if (pl->tc) {
+    const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma;
+    if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = 0;              // 128-bit row accesses
+  }
+  // FFMA2 engine: padded PSF, paired taps and (batch-wide PSF) a region of the constant-bank pool.  Skipped
+  // when the tensor path runs every evaluation of the call, so that the region stays free for a concurrent
+  // FFMA2 bucket (gm_fit_multi) and two launches are saved; kPlanFfma2 = the caller also runs FFMA2 kernels
+  // (the Jacobian columns of J^T W J).
   pl->psf = bt->psf;
   pl->psf_stride = bt->psf_stride;
-  if (pl->KP != bt->K) {
+  pl->taps_fwd = pl->taps_adj = nullptr;
+  pl->taps_stride = 0;
+  if (!pl->tc || (want & kPlanFfma2)) {
     const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
-    const long long n = (long long)n_psf * pl->KP * pl->KP;
-    k_pad_psf<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, pl->KP, pl->ws.psf_pad);
-    ++t_launches;
-    GM_CUDA(cudaGetLastError());
-    pl->psf = pl->ws.psf_pad;
-    pl->psf_stride = bt->psf_stride == 0 ? 0 : (long long)pl->KP * pl->KP;
-  }
-  {
-    const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
+    if (pl->KP != bt->K) {
+      const long long n = (long long)n_psf * pl->KP * pl->KP;
+      k_pad_psf<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bt->psf, bt->psf_stride, n_psf, bt->K, pl->KP, pl->ws.psf_pad);
+      ++t_launches;
+      GM_CUDA(cudaGetLastError());
+      pl->psf = pl->ws.psf_pad;
+      pl->psf_stride = bt->psf_stride == 0 ? 0 : (long long)pl->KP * pl->KP;
+    }
     const int per = (pl->KP + 1) * (pl->KP + 1);
     const long long n = (long long)n_psf * 2 * per;
     k_make_taps<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pl->psf, pl->psf_stride, n_psf, pl->KP, pl->ws.taps);
@@ -1031,14 +1059,7 @@ static int make_plan(const gm_model* model, const gm_batch* bt, bool need_data, 
       pl->ct_stream = st;
     }
   }
-  // Tensor-core path (gm_tc_fused.cuh), where the shape of the batch allows it (tc_kind).  It
-  // needs the E_a tables of the PSF(s), forward and adjoint; the FFMA2 taps above stay available for the
-  // Jacobian columns of the covariance row.
-  pl->tc = g_opt[GM_OPT_TENSOR].load() != 0 ? tc_kind(bt, &pl->KT) : 0;
-  if (pl->tc) {
-    const uintptr_t bits = (uintptr_t)bt->data | (uintptr_t)bt->sigma;
-    if ((bits & 15) || ((uintptr_t)bt->mask & 3)) pl->tc = 0;              // 128-bit row accesses
-  }
+  // the E_a tables of the PSF(s), forward and adjoint
   if (pl->tc) {
     cudaError_t err = cudaSuccess;
     const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
@@ -1286,10 +1307,12 @@ int gm_render(const gm_model* model, const gm_batch* bt, const float* params, fl
   if (!params || !model_out) return GM_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   Plan pl;
-  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
+  // the tensor kernels store 128-bit rows: an output view off a 16-byte boundary takes the FFMA2 engine
+  const unsigned want = ((uintptr_t)model_out & 15) ? kPlanNoTensor : kPlanAuto;
+  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl, false, want);
   if (rc != GM_OK) return rc;
   if ((rc = run_prologue(pl, bt->B, params, nullptr, st)) != GM_OK) return rc;
-  if (pl.tc && (((uintptr_t)model_out & 15) == 0)) return dispatch_tc(pl, bt, 0, model_out, LiveSet{}, st);
+  if (pl.tc) return dispatch_tc(pl, bt, 0, model_out, LiveSet{}, st);
   if (pl.fused)
     return dispatch_fused(pl.KP, fused_args(pl, bt, 0, model_out, LiveSet{}), pl.fused_variant, pl.caps.n_sm,
                           pl.caps.smem_optin, st);
@@ -1303,7 +1326,7 @@ int gm_loss_grad(const gm_model* model, const gm_batch* bt, const float* params,
   if (!params || !chi2) return GM_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   Plan pl;
-  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl);
+  int rc = make_plan(model, bt, true, workspace, workspace_bytes, st, &pl, false, jtj ? kPlanFfma2 : kPlanAuto);
   if (rc != GM_OK) return rc;
   UncWorkspace uw{};
   if (jtj) {
@@ -1359,6 +1382,9 @@ int gm_conv(int engine, int adjoint, const gm_batch* bt, float* out, void* works
   const int n_psf = bt->psf_stride == 0 ? 1 : bt->B;
   if (engine == GM_CONV_TENSOR) {
     if (bt->H != 128 || bt->W != 128) return GM_ENOTSUP;
+    // k_tc_conv reads and writes whole float4 rows: a view that starts off a 16-byte boundary would fault
+    // (and leave the context with a sticky error), so it is refused here, before anything is launched
+    if (((uintptr_t)bt->data | (uintptr_t)out) & 15) return GM_EINVAL;
     const int KP = tc::padded_side(bt->K);
     uint8_t* tab = (uint8_t*)workspace;
     float* bscale = (float*)((char*)workspace + align_up((size_t)n_psf * tc::table_bytes(KP), 256));
@@ -1415,7 +1441,7 @@ int gm_uncertainty(const gm_model* model, const gm_batch* bt, const float* param
   if (!params || !sigma_p || !bt || !bt->sigma) return GM_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   Plan pl;
-  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl);
+  int rc = make_plan(model, bt, false, workspace, workspace_bytes, st, &pl, false, kPlanNoTensor);   // J columns: FFMA2 only
   if (rc != GM_OK) return rc;
   const UncWorkspace uw = carve_unc(workspace, pl.ws.total, pl.md, bt);
   if (workspace_bytes < uw.total) return GM_EWORKSPACE;
@@ -1973,7 +1999,7 @@ int gm_profile_read(double* ms, int64_t* count) {
 
 int gm_init(void* cuda_stream) {
   t_launches = 0;
-  return ensure_nu_table((cudaStream_t)cuda_stream);
+  return ensure_nu_table((cudaStream_t)cuda_stream, /*wait=*/true);
 }
 
 int gm_set_option(int option, int value) {
@@ -2021,6 +2047,21 @@ int gm_measure_fp32_peak(int repeats, double* tflops, void* cuda_stream) {
   // per thread and loop trip: kPeakAcc FFMA2 = 2 * kPeakAcc multiply-adds = 4 * kPeakAcc flop
   const double flop = (double)repeats * grid * 256.0 * iters * kPeakAcc * 4.0;
   *tflops = flop / ((double)ms * 1e-3) / 1e12;
+  return GM_OK;
+}
+
+// Eq. 17, k = used pixels - fitted parameters; host arithmetic in fp64
+int gm_loglike(int32_t B, const float* chi2, const int32_t* n_used, int32_t n_free, double* loglike) {
+  if (!chi2 || !n_used || !loglike || B < 1 || n_free < 0) return GM_EINVAL;
+  for (int32_t b = 0; b < B; ++b) {
+    const double x = (double)chi2[b];
+    const double half_k = 0.5 * ((double)n_used[b] - (double)n_free);
+    if (!(half_k >= 0.5) || !(x > 0.0) || !std::isfinite(x)) {
+      loglike[b] = std::numeric_limits<double>::quiet_NaN();
+      continue;
+    }
+    loglike[b] = (half_k - 1.0) * std::log(x) - 0.5 * x - half_k * 0.6931471805599453094 - std::lgamma(half_k);
+  }
   return GM_OK;
 }
 

@@ -46,9 +46,11 @@ struct Geo { float u, vq, r; };
 // SFU forms.  FAST = MUFU.LG2 / MUFU.EX2 approximations (absolute error 2^-22 in the logarithm,
 // 2 ulp in the exponential): used by the gradient pass and, with kFastForward (the default,
 // gm_kernels.cuh), by every pass that produces a pixel of M as well -- gm_render included.
-// Accuracy contract of a rendered pixel: relative error below 1e-5 wherever the profile has
-// not underflowed (nu t < 30), derived in DESIGN.md section 6 and checked by
-// test_render_accuracy_high_n_wings.  !FAST = log2f / exp2f of the CUDA math library
+// Accuracy contract of a rendered, UNCONVOLVED pixel: relative error below 2e-5 wherever the profile
+// has not underflowed (nu t < 30; worst measured 1.3e-5 at that edge for n = 0.5, where the fp32
+// rounding of the exponent adds to the lg2 term), derived in DESIGN.md section 6 and checked by
+// tests/test_gpu_parity.py::test_render_accuracy_high_n_wings.  (After the tensor-core convolution the
+// error is absolute, relative to the cutout's maximum: include/gm.h, GM_OPT_TENSOR.)  !FAST = log2f / exp2f of the CUDA math library
 // (<= 2 ulp), selected for all pixel values by -DGM_PRECISE_FORWARD.
 template <bool FAST> __device__ __forceinline__ float lg2(float x) {
   if (FAST) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }

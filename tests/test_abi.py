@@ -87,3 +87,23 @@ def test_binding_refuses_cpu_tensors():
     from gen import models
     with pytest.raises(TypeError):
         gm.gm_render(models.single_sersic(), torch.zeros(2, 7), 16, 16, torch.zeros(5, 5))
+
+
+def test_loglike_eq17_host_helper():
+    """gm_loglike (Eq. 17; k of P:204) against scipy's chi^2 log-density: a host helper, no GPU."""
+    import numpy as np
+    from scipy import stats
+    import paper_2404_07780_b200 as gm
+    chi2 = np.array([3.5, 16000.0, 14321.7, 1e-3, 0.0, np.inf, 50.0], dtype=np.float32)
+    n_used = np.array([12, 16384, 14746, 9, 100, 100, 7], dtype=np.int32)
+    out = gm.gm_loglike(chi2, n_used, 7)
+    k = n_used.astype(np.float64) - 7
+    for b in range(4):
+        # ln Gamma(k/2) ~ 6e4 at k = 16377: fp64 rounding of the cancelling terms is ~1e-11 absolute
+        assert out[b] == pytest.approx(stats.chi2.logpdf(float(chi2[b]), k[b]), rel=1e-12, abs=1e-9)
+    assert np.isnan(out[4]) and np.isnan(out[5]) and np.isnan(out[6])      # chi2 = 0, inf, k = 0
+    # the mode of the chi^2 density is k - 2: ln L falls off on either side of it
+    m = gm.gm_loglike(np.array([98.0, 90.0, 106.0], dtype=np.float32), np.array([107] * 3, dtype=np.int32), 7)
+    assert m[0] > m[1] and m[0] > m[2]
+    with pytest.raises(gm.GmError):
+        gm.gm_loglike(chi2, n_used, -1)

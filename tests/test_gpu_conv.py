@@ -94,6 +94,28 @@ def test_tensor_engine_refuses_other_sizes():
         gm.gm_conv(torch.zeros(2, 64, 64, device="cuda"), torch.ones(5, 5, device="cuda"), engine=gm.GM_CONV_TENSOR)
 
 
+def test_tensor_engine_refuses_misaligned_views():
+    """gm.h, gm_conv: the tensor engine moves 128-bit rows, so an image or output view that starts 4 bytes off
+    a 16-byte boundary is GM_EINVAL before any launch (no fault, no sticky error); the FFMA2 engine takes it."""
+    img = images(3, 128, 128, seed=2)
+    psf = asymmetric(15, seed=3)
+    flat = torch.zeros(3 * 128 * 128 + 1, device="cuda")
+    view = flat[1:].view(3, 128, 128)
+    view.copy_(dev(img))
+    assert view.data_ptr() % 16 == 4
+    with pytest.raises(gm.GmError) as e:
+        gm.gm_conv(view, dev(psf), engine=gm.GM_CONV_TENSOR)
+    assert e.value.status == -1
+    oflat = torch.zeros(3 * 128 * 128 + 1, device="cuda")
+    with pytest.raises(gm.GmError) as e:
+        gm.gm_conv(dev(img), dev(psf), engine=gm.GM_CONV_TENSOR, out=oflat[1:].view(3, 128, 128))
+    assert e.value.status == -1
+    torch.cuda.synchronize()                                  # the context is still healthy
+    ref = np.stack([oracle.conv2d_same(img[b], psf) for b in range(3)])
+    assert_pixels(gm.gm_conv(view, dev(psf), engine=gm.GM_CONV_FFMA2).cpu().numpy(), ref)
+    assert_pixels(gm.gm_conv(dev(img), dev(psf), engine=gm.GM_CONV_TENSOR).cpu().numpy(), ref)
+
+
 def test_phase_trace_hook_records_every_phase():
     """gm_trace_set (include/gm.h): CTA 0 of k_tc_fused appends one record per phase boundary; the hook is
     off by default and switches off again with None."""

@@ -31,6 +31,18 @@ def synth(model, B, H, W, K, seed, masked=True, per_galaxy_psf=False):
     return par, data, sigma, mask, psf
 
 
+def render_and_engine(model, par, H, W, psf):
+    """gm_render with the launch-timing hook on -> (image, families of heavy kernels that ran: 'tensor' / 'ffma2')."""
+    gm.gm_profile_enable(1)
+    try:
+        img = gm.gm_render(model, dev(par), H, W, dev(psf))
+        torch.cuda.synchronize()
+        kinds = gm.gm_profile_read()
+    finally:
+        gm.gm_profile_enable(0)
+    return img, {"tensor" if name.startswith("tc_") else "ffma2" for name, (_, n) in kinds.items() if n > 0}
+
+
 def run_loss_grad(model, par, data, sigma, mask, psf):
     chi2, grad = gm.gm_loss_grad(model, dev(par), dev(data), dev(sigma), dev(mask), dev(psf))
     torch.cuda.synchronize()
@@ -111,21 +123,20 @@ def test_tensor_super_tiles_ragged(H, W, K, per_psf):
     B = 3                                                    # fewer items than CTAs, more than one per galaxy
     par, data, sigma, mask, psf = synth(model, B, H, W, K, seed=3 * H + W + K, per_galaxy_psf=per_psf)
     assert gm.gm_get_option(gm.GM_OPT_TENSOR) == 1
-    img = gm.gm_render(model, dev(par), H, W, dev(psf))
-    n_tc = gm.gm_last_launch_count()
+    img, fam = render_and_engine(model, par, H, W, psf)
+    assert fam == {"tensor"}                                 # this call did take the tensor-core path
     assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
     chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
     oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
     assert_chi2(chi2, oc)
     assert_grad(grad, og)
-    # the FFMA2 engine on the same inputs: another launch sequence (this call did take the tensor-core path), same answers
+    # the FFMA2 engine on the same inputs: other kernels, same answers
     gm.gm_set_option(gm.GM_OPT_TENSOR, 0)
     try:
-        img2 = gm.gm_render(model, dev(par), H, W, dev(psf))
-        n_ff = gm.gm_last_launch_count()
+        img2, fam2 = render_and_engine(model, par, H, W, psf)
     finally:
         gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
-    assert n_tc != n_ff
+    assert fam2 == {"ffma2"}
     assert_pixels(img2.cpu().numpy(), oracle.render(model, par, H, W, psf))
 
 
@@ -136,20 +147,19 @@ def test_tensor_engine_with_unconvolved_components(H, W, K, per_psf):
     model = models.all_profiles()                            # six laws, tied parameters, an unconvolved source, the sky
     assert any(c["convolve"] == 0 for c in model["components"])
     par, data, sigma, mask, psf = synth(model, 3, H, W, K, seed=7 * H + W + K, per_galaxy_psf=per_psf)
-    img = gm.gm_render(model, dev(par), H, W, dev(psf))
-    n_tc = gm.gm_last_launch_count()
+    img, fam = render_and_engine(model, par, H, W, psf)
+    assert fam == {"tensor"}
     assert_pixels(img.cpu().numpy(), oracle.render(model, par, H, W, psf))
     chi2, grad = run_loss_grad(model, par, data, sigma, mask, psf)
     oc, og = oracle.loss_grad(model, par, data, sigma, mask, psf)
     assert_chi2(chi2, oc)
     assert_grad(grad, og)
-    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # the FFMA2 engine launches another sequence
+    gm.gm_set_option(gm.GM_OPT_TENSOR, 0)                    # the FFMA2 engine runs other kernels
     try:
-        gm.gm_render(model, dev(par), H, W, dev(psf))
-        n_ff = gm.gm_last_launch_count()
+        _, fam2 = render_and_engine(model, par, H, W, psf)
     finally:
         gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
-    assert n_tc != n_ff
+    assert fam2 == {"ffma2"}
 
 
 def test_psf_orientation_not_flipped_or_transposed():
@@ -302,3 +312,33 @@ def test_host_entry_points():
     c_h, g_h = gm.gm_loss_grad_host(model, b["start"], b["data"], b["sigma"], None, b["psf"])
     c_d, g_d = run_loss_grad(model, b["start"], b["data"], b["sigma"], None, b["psf"])
     assert np.array_equal(c_h, c_d) and np.array_equal(g_h, g_d)
+
+
+# ---- accuracy contract of a rendered pixel (gm_device.cuh) ----------------
+@pytest.mark.parametrize("tensor", [1, 0])
+def test_render_accuracy_high_n_wings(tensor):
+    """Unconvolved Sersic pixels are within 2e-5 relative of the oracle wherever the profile has not underflowed
+    (nu t < 30, t = (r / re)^(1/n)): five times tighter than the pixel tolerance, far out in the wings of low-n
+    profiles and through the steep cores of high-n ones, where the SFU error of lg2 and the fp32 rounding of the
+    exponent are amplified by nu t (worst measured: 1.3e-5 at the nu t -> 30 edge of an n = 0.5 profile)."""
+    model = models.one_component("sersic", convolve=0)              # [xc, yc, theta, q, Ie, re, n]
+    H = W = 128
+    rows = [(n, re, q) for n in (0.5, 1.0, 2.0, 4.0, 6.0, 8.0) for re, q in ((2.0, 0.9), (9.5, 0.35))]
+    par = np.array([[64.37, 63.21, 0.3 + 0.2 * k, q, 3.0, re, n] for k, (n, re, q) in enumerate(rows)], dtype=np.float32)
+    psf = gaussian_psf(15, 3.0).astype(np.float32)
+    gm.gm_set_option(gm.GM_OPT_TENSOR, tensor)
+    try:
+        img = gm.gm_render(model, dev(par), H, W, dev(psf)).cpu().numpy().astype(np.float64)
+    finally:
+        gm.gm_set_option(gm.GM_OPT_TENSOR, 1)
+    ref = oracle.render(model, par, H, W, psf)
+    covered = 0
+    for k, (n, re, q) in enumerate(rows):
+        nu = oracle.sersic_nu(float(np.float32(n)))
+        live = ref[k] > 3.0 * math.exp(nu - 30.0)                  # I = Ie exp(-nu (t - 1)): nu t < 30
+        rel = np.abs(img[k] - ref[k])[live] / ref[k][live]
+        assert rel.max() < 2e-5, (n, re, q, rel.max())
+        covered += int(live.sum())
+        if n <= 1.0 and re == 2.0:
+            assert not live.all()                                  # the low-n wings do reach the underflow edge
+    assert covered > 0.7 * len(rows) * H * W
