@@ -189,9 +189,23 @@ def cpu_baseline(cfg):
     t0 = time.perf_counter()
     oracle.fit(b["model"], b["start"], b["data"], b["sigma"], b["mask"], b["psf"], opts)
     dt = time.perf_counter() - t0
-    return {"value": n_gal * b["H"] * b["W"] * n_iter / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{n_gal} galaxies x {n_iter} iterations of {cfg.name}'s {b['H']}x{b['W']} bucket (K={b['K']}), "
-                      f"{dt:.1f} s, OpenMP over galaxies"}
+    out = {"value": n_gal * b["H"] * b["W"] * n_iter / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"{n_gal} galaxies x {n_iter} iterations of {cfg.name}'s {b['H']}x{b['W']} bucket (K={b['K']}), "
+                     f"{dt:.1f} s, OpenMP over galaxies"}
+    # the oracle "at 1 thread and at all cores" -- one galaxy of the same sample on one thread, ~5 s
+    n1 = int(min(max(5.0 / max(t_eval / max(n_gal / cores, 1.0), 1e-3), 2), n_iter))
+    o1 = configs.fit_options(b["model"], b["H"], b["W"], n1)
+    oracle.set_num_threads(1)
+    try:
+        t0 = time.perf_counter()
+        oracle.fit(b["model"], b["start"][:1], b["data"][:1], b["sigma"][:1], None if b["mask"] is None else b["mask"][:1],
+                   b["psf"], o1)
+        d1 = time.perf_counter() - t0
+    finally:
+        oracle.set_num_threads(cores)
+    out["one_thread"] = {"value": b["H"] * b["W"] * n1 / d1, "unit": UNIT, "cores": 1,
+                         "sample": f"1 galaxy x {n1} iterations of the same bucket, {d1:.1f} s"}
+    return out
 
 
 # ---------------------------------------------------------------------------------
@@ -509,6 +523,20 @@ class Bench:
                           "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                           "api": ("gm_fit_multi_host" if len(buckets) > 1 else "gm_fit_host") +
                                  " (host buffers; device allocation + H2D + fit + D2H inside the call)"}
+            # the copy rate of this box, measured on its own: the step's pinned host inputs -> their device buffers
+            a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record(self.stream)
+            with torch.cuda.stream(self.stream):
+                nb = 0
+                for k in buckets:
+                    for h, dv in zip(k["host"], k["dev"]):
+                        if h is not None:
+                            dv.copy_(h, non_blocking=True); nb += h.numel() * h.element_size()
+            z.record(self.stream)
+            torch.cuda.synchronize()
+            rec["e2e"]["h2d_gbs"] = nb / (a.elapsed_time(z) * 1e-3) / 1e9
+            rec["e2e"]["h2d_ms_alone"] = a.elapsed_time(z)
         rec["_outs"] = outs
         return rec
 
@@ -684,10 +712,40 @@ def run_ours(args):
                       "traffic": rf.get("traffic"), "kernels": rf.get("kernels")})
             if key == "C1":
                 r["loss_grad"] = bn.loss_grad_line(bk[0])
+            if key == "C4_batch2048":
+                # BASELINE C4 is "streamed in batches": a short leg of it (4 of the 32 batches) in the default line
+                r["streamed"] = bn.streamed(bk[0], 4)
             per[key] = r
             del bk
             torch.cuda.empty_cache()
         line["per_config"] = per
+        # the same facts, compact, inside a key every reader of the line keeps: enough to recompute each `frac`
+        def _compact(r):
+            e = r.get("e2e") or {}
+            c = {"ms_per_step": r.get("ms_per_step"), "value": r.get("value"), "workload": r.get("workload"),
+                 "kernel": r.get("kernel"), "frac": r.get("frac"), "peak": r.get("peak"),
+                 "achieved_tflops": r.get("achieved_tflops"), "mma_issued_frac": r.get("mma_issued_frac"),
+                 "step_frac": r.get("step_frac"), "kernels": r.get("kernels"), "gpu_launches": r.get("gpu_launches"),
+                 "e2e_ms": e.get("ms_per_step"), "h2d_bytes": e.get("h2d_bytes_per_step"), "h2d_gbs": e.get("h2d_gbs"),
+                 "h2d_ms_alone": e.get("h2d_ms_alone")}
+            if r.get("loss_grad"):
+                c["loss_grad"] = {k: r["loss_grad"].get(k) for k in ("value", "ms_per_call", "tflops")}
+            if r.get("streamed"):
+                c["streamed"] = {k: r["streamed"].get(k) for k in ("batches", "galaxies", "seconds", "galaxies_fitted_per_s",
+                                                                   "value", "h2d_bytes_per_batch")}
+            return c
+        if line.get("roofline") is not None:
+            line["roofline"]["per_config"] = {k: _compact(r) for k, r in per.items()}
+    if line.get("roofline") is not None and line.get("buckets"):
+        line["roofline"]["per_bucket"] = line["buckets"]
+    e2e = line.get("e2e")
+    if e2e and e2e.get("ms_per_step"):
+        # what the host-buffer call adds to the device-timed fit, and the copy rate that implies if all of it were
+        # the H2D copy (a lower bound of the achieved rate; run-to-run noise of the fit is inside it)
+        e2e["overhead_ms"] = e2e["ms_per_step"] - line["ms_per_step"]
+        e2e["overhead_note"] = ("e2e minus the device-timed step; smaller than h2d_ms_alone where gm_fit_multi_host overlaps one "
+                                "bucket's copy with another bucket's fit, and because the device-timed steps run back to back "
+                                "under the power cap (plus an L2 flush each) while the host steps idle the SMs during copies")
     if bn.world == 1 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(cfg)
     print(json.dumps(line))

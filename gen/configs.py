@@ -195,8 +195,11 @@ def _noise_one(cfg: Config, g: int, M: np.ndarray, Ie: float):
     return D, sigma, mask
 
 
-def make_batch(cid: int, galaxies, render, side: int | None = None, workers: int = 1) -> dict:
+def make_batch(cid: int, galaxies, render, side: int | None = None, workers: int = 1, **overrides) -> dict:
     """Inputs for the given galaxy indices of config ``cid`` (one cutout side).
+
+    ``overrides`` replace fields of the config (``K=41``, ``psf_kind="moffat3.5"`` ...): the same
+    recipe on another shape, e.g. C0's constant-sigma noise on 128 px cutouts under a 41 x 41 PSF.
 
     ``render(model, params_f32[B,P], H, W, psf_f32) -> ndarray[B,H,W]`` supplies the
     noiseless model.  For C2, ``side`` selects the size bucket; galaxies whose
@@ -204,6 +207,9 @@ def make_batch(cid: int, galaxies, render, side: int | None = None, workers: int
     threads (every galaxy has its own generator, so the result does not depend on it).
     """
     cfg = CONFIGS[cid]
+    if overrides:
+        from dataclasses import replace
+        cfg = replace(cfg, **overrides)
     galaxies = list(galaxies)
     if len(cfg.sides) > 1:
         assert side is not None

@@ -42,8 +42,12 @@ def test_c2_every_bucket_through_fit_multi_early_stop_masked():
     stopped = 0
     for (b, opts), g in zip(buckets, outs):
         assert b["mask"] is not None and opts["tol"] > 0 and opts["n_iter"] == 500
-        ok, dt = fp.stop_decision_ok(g, fp.oracle_fit(b, opts, want_trace=True), opts)
+        own = fp.oracle_fit(b, opts, want_trace=True)
+        ok, dt = fp.stop_decision_ok(g, own, opts)
         assert ok, f"C2/{b['H']}px: the GPU stopped a galaxy while the oracle's chi^2 still moved; |d iterations| = {dt}"
+        # (3) against the oracle's own stop: iteration counts within MAX_STOP_SHIFT, end points the same fit within
+        # the looser bounds of fit_parity.py (the two runs legitimately end tens of iterations apart)
+        fp.assert_close_to_own_stop(f"C2/{b['H']}px", b, g, own, dt)
         o = fp.oracle_fit_at_iters(b, opts, g["iters_used"])
         j = fp.judge(b, g, o)
         # profiles/r02_parity.md (120-galaxy sample): 0.966 .. 1.000 per bucket; the 8 .. 19 galaxies per bucket of
